@@ -1,0 +1,164 @@
+"""ctypes front end of oracle/concordia_oracle.c (TEST INFRASTRUCTURE ONLY).
+
+Every function here only marshals numpy buffers into the plain-C oracle; none of
+the method's arithmetic lives in Python.  Citations are in concordia_oracle.c.
+"""
+import ctypes
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+ORC_OK = 0
+ORC_ERR_INVALID = -1
+ORC_ERR_LOG_FULL = -4
+ORC_ERR_CORRUPT = -5
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "concordia_oracle.c")
+_SO = os.path.join(_HERE, "libconcordia_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the C oracle with gcc (building the checker is not using it)."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        tmp = _SO + ".tmp.%d" % os.getpid()
+        subprocess.run(["gcc", "-O2", "-std=c11", "-shared", "-fPIC", "-pthread", "-o", tmp, _SRC], check=True)
+        os.replace(tmp, _SO)
+    return _SO
+
+
+class _CRegion(ctypes.Structure):
+    _fields_ = [("region_id", ctypes.c_uint32), ("page_bytes", ctypes.c_uint32), ("bytes", ctypes.c_uint64),
+                ("base", ctypes.c_void_p), ("shadow", ctypes.c_void_p)]
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        u8p, u32p, u64p = ctypes.c_void_p, ctypes.c_void_p, ctypes.POINTER(ctypes.c_uint64)
+        lib.orc_crc32c.restype = ctypes.c_uint32
+        lib.orc_crc32c.argtypes = [u8p, ctypes.c_uint64]
+        lib.orc_crc32c_bitwise.restype = ctypes.c_uint32
+        lib.orc_crc32c_bitwise.argtypes = [u8p, ctypes.c_uint64]
+        lib.orc_scan.restype = ctypes.c_uint64
+        lib.orc_scan.argtypes = [u8p, u8p, ctypes.c_uint64, ctypes.c_uint64, u8p]
+        lib.orc_scan_mt.restype = ctypes.c_uint64
+        lib.orc_scan_mt.argtypes = [u8p, u8p, ctypes.c_uint64, ctypes.c_uint64, u8p, ctypes.c_uint32]
+        lib.orc_checkpoint.restype = ctypes.c_int32
+        lib.orc_checkpoint.argtypes = [u8p, u8p, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint32, ctypes.c_uint64,
+                                       u8p, ctypes.c_uint64, u64p, u32p, u64p, u64p]
+        lib.orc_apply.restype = ctypes.c_int32
+        lib.orc_apply.argtypes = [u8p, ctypes.c_uint64, ctypes.POINTER(_CRegion), ctypes.c_uint32, u64p, u64p]
+        lib.orc_write_epoch.restype = ctypes.c_int32
+        lib.orc_write_epoch.argtypes = [u8p, ctypes.c_uint64, u64p, ctypes.c_uint32, ctypes.c_uint64,
+                                        ctypes.c_uint64, ctypes.c_uint64, u32p, ctypes.c_uint64, u8p]
+        _lib = lib
+    return _lib
+
+
+def _u8(a) -> np.ndarray:
+    """View any C-contiguous numpy array (or bytes-like) as a flat uint8 array, no copy."""
+    if isinstance(a, (bytes, bytearray, memoryview)):
+        a = np.frombuffer(a, dtype=np.uint8)
+    a = np.asarray(a)
+    if not a.flags["C_CONTIGUOUS"]:
+        raise ValueError("oracle buffers must be C-contiguous")
+    return a.reshape(-1).view(np.uint8)
+
+
+def _ptr(a: np.ndarray) -> int:
+    return a.ctypes.data
+
+
+def crc32c(data) -> int:
+    d = _u8(data)
+    return int(_load().orc_crc32c(_ptr(d), d.size))
+
+
+def crc32c_bitwise(data) -> int:
+    d = _u8(data)
+    return int(_load().orc_crc32c_bitwise(_ptr(d), d.size))
+
+
+def scan(cur, shadow, page_bytes: int) -> np.ndarray:
+    """dirty[p] flags (uint8) -- PAPER.md:L261."""
+    c, s = _u8(cur), _u8(shadow)
+    assert c.size == s.size and page_bytes > 0
+    n_pages = (c.size + page_bytes - 1) // page_bytes
+    dirty = np.zeros(n_pages, dtype=np.uint8)
+    _load().orc_scan(_ptr(c), _ptr(s), c.size, page_bytes, _ptr(dirty))
+    return dirty
+
+
+def scan_mt(cur, shadow, page_bytes: int, n_threads: int) -> np.ndarray:
+    c, s = _u8(cur), _u8(shadow)
+    assert c.size == s.size and page_bytes > 0
+    n_pages = (c.size + page_bytes - 1) // page_bytes
+    dirty = np.zeros(n_pages, dtype=np.uint8)
+    _load().orc_scan_mt(_ptr(c), _ptr(s), c.size, page_bytes, _ptr(dirty), n_threads)
+    return dirty
+
+
+def checkpoint(cur, shadow, page_bytes: int, region_id: int, epoch: int, log, W: int):
+    """One delta checkpoint.  shadow and log are modified in place.
+
+    Returns (status, D, bytes_appended, W_after); D is the ascending uint32 dirty list
+    (also returned on LOG_FULL, where nothing was written).
+    """
+    c, s, lg = _u8(cur), _u8(shadow), _u8(log)
+    assert c.size == s.size
+    assert s.flags["WRITEABLE"] and lg.flags["WRITEABLE"]
+    n_pages = (c.size + page_bytes - 1) // page_bytes
+    D = np.zeros(max(n_pages, 1), dtype=np.uint32)
+    w = ctypes.c_uint64(W)
+    k = ctypes.c_uint64(0)
+    nb = ctypes.c_uint64(0)
+    st = _load().orc_checkpoint(_ptr(c), _ptr(s), c.size, page_bytes, region_id, epoch,
+                                _ptr(lg), lg.size, ctypes.byref(w), _ptr(D), ctypes.byref(k), ctypes.byref(nb))
+    return int(st), D[: k.value].copy(), int(nb.value), int(w.value)
+
+
+@dataclass
+class Region:
+    region_id: int
+    page_bytes: int
+    base: np.ndarray            # uint8 view, modified in place by apply_log
+    shadow: np.ndarray = None   # optional
+
+
+def apply_log(log, nbytes: int, regions):
+    """Replay log[:nbytes] into the regions.  Returns (status, applied, consumed)."""
+    lg = _u8(log)
+    assert nbytes <= lg.size
+    arr = (_CRegion * max(len(regions), 1))()
+    keep = []
+    for i, r in enumerate(regions):
+        b = _u8(r.base)
+        assert b.flags["WRITEABLE"]
+        keep.append(b)
+        sh = 0
+        if r.shadow is not None:
+            s = _u8(r.shadow)
+            assert s.size == b.size and s.flags["WRITEABLE"]
+            keep.append(s)
+            sh = _ptr(s)
+        arr[i] = _CRegion(r.region_id, r.page_bytes, b.size, _ptr(b), sh)
+    applied = ctypes.c_uint64(0)
+    consumed = ctypes.c_uint64(0)
+    st = _load().orc_apply(_ptr(lg), nbytes, arr, len(regions), ctypes.byref(applied), ctypes.byref(consumed))
+    return int(st), int(applied.value), int(consumed.value)
+
+
+def write_epoch(log, W: int, region_id: int, epoch: int, region_bytes: int, page_bytes: int, pages, payloads):
+    """Append one committed epoch of caller-given page records.  Returns (status, W_after)."""
+    lg = _u8(log)
+    pg = np.ascontiguousarray(pages, dtype=np.uint32)
+    pl = _u8(payloads)
+    w = ctypes.c_uint64(W)
+    st = _load().orc_write_epoch(_ptr(lg), lg.size, ctypes.byref(w), region_id, epoch, region_bytes, page_bytes,
+                                 _ptr(pg), pg.size, _ptr(pl))
+    return int(st), int(w.value)
