@@ -1,0 +1,216 @@
+/*
+ * concordia.h -- C ABI of libconcordia.so: GPU-side delta checkpointing of registered
+ * regions on one NVIDIA B200 (sm_100a).
+ *
+ * The operations are those of Concordia (arxiv 2606.23521; citations are lines of
+ * /root/reference/PAPER.md as used in SURVEY.md / DESIGN.md):
+ *   - region registration              PAPER.md:L193 (region specification), L217 (registered regions)
+ *   - delta checkpoint                 PAPER.md:L219, L259-264 (4-stage pipeline: dirty discovery ->
+ *                                      record construction -> append + commit -> shadow update)
+ *   - append-only log discipline       PAPER.md:L221 (header, payloads, commit marker, publish epoch;
+ *                                      recovery ignores an uncommitted suffix)
+ *   - recovery applier                 PAPER.md:L156-158 (TASK_RESTORE), L227, L445
+ *   - ring buffer + persistent worker  PAPER.md:L119, L125-160 (listings), L247-249 (host-mapped
+ *                                      memory, release/acquire), Table 1 L166-175 (host API)
+ *
+ * Conventions
+ *   - Plain C, no exceptions across the boundary.  Every call returns an int32_t status:
+ *     CC_OK (0) or a negative CC_ERR_*; on error there are no partial side effects unless
+ *     stated.  cc_poll returns CC_PENDING (1) while a task is still running.
+ *   - OWNERSHIP: the caller owns, and keeps alive, every buffer it passes (live region,
+ *     shadow, workspace, log buffer, apply scratch, result structs).  The library borrows the
+ *     pointers.  It allocates its own small control blocks in cc_init / cc_worker_start only
+ *     and never allocates or frees device memory while the worker is running
+ *     (cudaMalloc / cudaDeviceSynchronize can deadlock under a resident kernel).
+ *   - "device" pointers are CUDA device memory of the context's GPU.  "pinned host" pointers
+ *     are page-locked, device-mapped host memory (cudaHostAlloc / torch pin_memory; with UVA
+ *     the same address is valid on both sides).  A log buffer and a cc_result
+ *     may be either; regions, shadows, workspaces and apply scratch are device memory.
+ *   - Streams are cudaStream_t passed as void* (0 = the legacy default stream).
+ *   - One host thread per context at a time (cc_submit is single-producer).
+ *   - No CPU fallback exists: if no CUDA device is usable cc_init fails with CC_ERR_CUDA.
+ *
+ * On-log record format (the paper lists the fields, PAPER.md:L85,
+ * L219, not their widths).  All integers little-endian, no padding:
+ *   page record   : { u32 region_id; u32 page_idx; u32 len; u32 crc32c(payload) } + len payload bytes
+ *   commit record : { 0xFFFFFFFF; 0xFFFFFFFF; 16; crc32c(payload) } + { u64 epoch; u32 region_id; u32 k }
+ *   CRC32C        : Castagnoli, reflected 0x82F63B78, init 0xFFFFFFFF, xorout 0xFFFFFFFF.
+ * One checkpoint of one region appends its k dirty pages in ascending page order followed by
+ * one commit record, or nothing at all when k == 0.
+ */
+#ifndef CONCORDIA_H
+#define CONCORDIA_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CC_OK 0
+#define CC_PENDING 1
+#define CC_ERR_INVALID (-1)        /* bad argument / alignment / size */
+#define CC_ERR_NOT_REGISTERED (-2)
+#define CC_ERR_EXISTS (-3)
+#define CC_ERR_LOG_FULL (-4)       /* checkpoint: W + need > capacity; nothing appended, shadow untouched */
+#define CC_ERR_CORRUPT (-5)        /* apply: a structure or CRC check failed; committed prefix before it applied */
+#define CC_ERR_RING_FULL (-6)
+#define CC_ERR_WORKER (-7)         /* worker not running / running when it must not be / heartbeat stale */
+#define CC_ERR_CUDA (-8)           /* a CUDA call failed: cc_last_cuda_error() */
+#define CC_ERR_TIMEOUT (-9)
+#define CC_ERR_SCRATCH (-10)       /* apply: log holds more records/epochs than the attached scratch; nothing applied */
+
+#define CC_MAX_REGIONS 64
+#define CC_COMMIT_ID 0xFFFFFFFFu
+#define CC_RECORD_HEADER_BYTES 16u
+#define CC_COMMIT_RECORD_BYTES 32u
+
+/* cc_region_desc.flags */
+#define CC_REG_SNAPSHOT_NOW 1u     /* shadow := base at registration (first delta is relative to now) */
+
+typedef struct cc_ctx cc_ctx;
+
+typedef struct {
+    uint32_t ring_capacity;    /* slots, power of two, 0 = 256 (256 x 64 B) */
+    uint32_t worker_blocks;    /* persistent worker CTAs, 0 = as many as are co-resident with worker_threads */
+    uint32_t worker_threads;   /* threads per worker CTA ("tpb" of Table 1), multiple of 32, 0 = 512 */
+    uint32_t backoff_ns;       /* idle poll back-off of the worker (set_yield_every analogue, L172), 0 = 500 */
+    uint64_t max_lifetime_ns;  /* worker exits by itself after this long (safety net), 0 = 600 s */
+} cc_config;
+
+typedef struct {
+    uint32_t region_id;        /* 1 ... 0xFFFFFFFE */
+    uint32_t page_bytes;       /* P: multiple of 16 (benchmarks: 4096 / 16384 / 65536) */
+    uint64_t bytes;            /* N: multiple of 16, > 0; the last page may be short; ceil(N/P) <= 2^31 */
+    void*    base;             /* live region, device, 16-byte aligned */
+    void*    shadow;           /* last-committed copy, device, N bytes, 16-byte aligned, caller-allocated */
+    void*    workspace;        /* device, 256-byte aligned, >= cc_workspace_bytes(N, P); zeroed by the call */
+    uint64_t workspace_bytes;
+    uint32_t flags;            /* CC_REG_* */
+    uint32_t reserved;
+} cc_region_desc;
+
+/* Completion / result record, exactly 64 bytes.  Written by the GPU. */
+typedef struct {
+    uint64_t seq_done;         /* worker path: task seq + 1, release-stored LAST; host-launched path: 1 */
+    uint64_t n_dirty;          /* checkpoint: k;  apply: page records applied (duplicates counted) */
+    uint64_t bytes;            /* checkpoint: bytes appended;  apply: bytes consumed (end of last applied commit) */
+    uint64_t log_offset_after; /* checkpoint: log write offset W after the call;  apply: same as bytes */
+    uint64_t epoch;            /* checkpoint: the epoch passed in;  apply: number of epochs applied */
+    int32_t  status;           /* CC_OK / CC_ERR_LOG_FULL / CC_ERR_CORRUPT / CC_ERR_SCRATCH / ... */
+    uint32_t flags;            /* task kind echoed back */
+    uint64_t t_start_ns;       /* %globaltimer when the GPU started the operation */
+    uint64_t t_end_ns;         /* %globaltimer when it finished */
+} cc_result;
+
+/* Task descriptor, exactly 64 bytes ("64-128 bytes including operator ID, tensor
+ * pointers, dimensions, and control flags"; L148-159 kinds, epoch, seq). */
+#define CC_TASK_NOP 0u
+#define CC_TASK_DELTA_CKPT 1u      /* region_id, epoch */
+#define CC_TASK_RESTORE 2u         /* arg0 = log pointer, arg1 = nbytes */
+#define CC_TASK_LOG_RESET 3u       /* W := 0 */
+#define CC_TASK_TEST_MUTATE 4u     /* bench/test only: region_id; arg0 = n_mut, arg1 = A (odd), arg2 = h:
+                                      for j < n_mut: page (j*A + h) mod n_pages, byte (h + j) mod len_p, ^= 0x5A */
+#define CC_TASK_EXIT 255u
+typedef struct {
+    uint32_t kind;
+    uint32_t region_id;
+    uint32_t flags;
+    uint32_t version;          /* carried, unused (the paper's operator-table version) */
+    uint64_t seq;              /* assigned by cc_submit */
+    uint64_t epoch;
+    uint64_t arg0, arg1, arg2, arg3;
+} cc_task;
+
+/* ---- lifecycle (Table 1: init / shutdown) --------------------------------------- */
+
+/* Create a context on CUDA device `device`.  cfg may be NULL (all defaults). */
+int32_t cc_init(cc_ctx** out, int32_t device, const cc_config* cfg);
+/* Stop the worker if it runs, free the library's control blocks.  Caller buffers are untouched. */
+int32_t cc_shutdown(cc_ctx* ctx);
+/* Last cudaError_t seen by this context (0 = none). */
+int32_t cc_last_cuda_error(cc_ctx* ctx);
+/* Number of kernels this context has launched so far (host-launched path + worker launches). */
+uint64_t cc_kernel_launches(cc_ctx* ctx);
+
+/* ---- regions ------------------------------------------------------- */
+
+/* Device workspace a region of N bytes with pages of P bytes needs (0 if the pair is invalid). */
+uint64_t cc_workspace_bytes(uint64_t bytes, uint32_t page_bytes);
+/* Register a region.  Synchronous (zeroes the workspace, optionally snapshots the shadow, on an
+ * internal stream, and waits).  Only while the worker is stopped (CC_ERR_WORKER otherwise). */
+int32_t cc_register_region(cc_ctx* ctx, const cc_region_desc* desc);
+int32_t cc_unregister_region(cc_ctx* ctx, uint32_t region_id);
+
+/* ---- log placement ("AOF log placement") ------------------------------------ */
+
+/* Attach the append-only log: log_buf (device or pinned host, 16-byte aligned), capacity bytes.
+ * committed_off (pinned host or device, 8 bytes, may be NULL) receives the committed write
+ * offset with a system-scope release store after every commit record.  W := 0.
+ * Only while the worker is stopped. */
+int32_t cc_log_attach(cc_ctx* ctx, void* log_buf, uint64_t capacity, uint64_t* committed_off);
+/* W := 0 (synchronous; only while the worker is stopped -- use CC_TASK_LOG_RESET otherwise). */
+int32_t cc_log_reset(cc_ctx* ctx);
+
+/* ---- host-launched path -------------------------------------------------------------------- */
+
+/* Delta-checkpoint one region: scan live vs shadow per page, compact the
+ * dirty page indices in ascending order, append k page records + one commit record at the log
+ * write offset, refresh the shadow of the dirty pages, publish the committed offset.
+ * ASYNCHRONOUS on `stream`: kernels only, no host round trip between them.  `out` (pinned host
+ * or device, 64 bytes, may be NULL) is valid once the stream has reached this point.
+ * k == 0 appends nothing.  If the records do not fit: out->status = CC_ERR_LOG_FULL, nothing is
+ * appended and the shadow is untouched.  The return value covers argument / launch errors only.
+ * The region must not be written while the call is in flight (boundaries are
+ * quiescent).  The ascending dirty list of the last checkpoint stays readable in the workspace
+ * (cc_dirty_list). */
+int32_t cc_checkpoint_delta(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out);
+
+/* Scan + compaction only (steps a1-a2), for measurement: fills the dirty list, appends nothing,
+ * leaves the shadow alone.  out->n_dirty = k. */
+int32_t cc_scan_only(cc_ctx* ctx, uint32_t region_id, void* stream, cc_result* out);
+
+/* Device pointer to the u32 ascending dirty page list of the region's last scan and to its
+ * u32 count (valid after the stream reached the end of that call). */
+int32_t cc_dirty_list(cc_ctx* ctx, uint32_t region_id, const uint32_t** d_list, const uint32_t** d_count);
+
+/* Attach device scratch for the applier: room for the record / epoch tables of a log with at most
+ * max_records page records and max_records commit records; cc_apply_scratch_bytes gives the size.
+ * Only while the worker is stopped. */
+uint64_t cc_apply_scratch_bytes(uint64_t max_records);
+int32_t cc_apply_attach(cc_ctx* ctx, void* scratch, uint64_t scratch_bytes);
+
+/* Recovery applier: parse log[0, nbytes) (device or pinned host,
+ * 16-byte aligned), validate structure and CRC32C of every record, and for every committed epoch
+ * before the first failed check, in log order, write each page record's payload into its
+ * region's live page and shadow page (a page present several times ends with its last record).
+ * Running out of bytes is "torn": status CC_OK, the committed prefix is applied.  A failed check
+ * is CC_ERR_CORRUPT: the committed prefix before the bad epoch is applied, nothing after.
+ * ASYNCHRONOUS on `stream`; result fields as documented in cc_result. */
+int32_t cc_apply_log(cc_ctx* ctx, const void* log, uint64_t nbytes, void* stream, cc_result* out);
+
+/* ---- ring buffer + persistent worker ------------------- */
+
+/* Launch the persistent worker kernel (cooperative, stays resident) on an internal non-blocking
+ * stream.  Everything (regions, log, apply scratch) must be registered/attached before. */
+int32_t cc_worker_start(cc_ctx* ctx);
+/* Submit CC_TASK_EXIT, wait for the kernel to leave (up to 10 s), CC_ERR_TIMEOUT otherwise. */
+int32_t cc_worker_stop(cc_ctx* ctx);
+/* Table 1 worker_alive(): 1 if the worker runs and its heartbeat advanced within 1 s, else 0. */
+int32_t cc_worker_alive(cc_ctx* ctx);
+/* Table 1 peek_queue(): head = tasks completed, tail = tasks submitted. */
+int32_t cc_peek_queue(cc_ctx* ctx, uint64_t* head, uint64_t* tail);
+/* Copy *task into the next ring slot and publish it with a store-release;
+ * no CUDA call.  Non-blocking: CC_ERR_RING_FULL when `capacity` tasks are outstanding.
+ * *seq_out (may be NULL) = the sequence number to poll / wait on. */
+int32_t cc_submit(cc_ctx* ctx, const cc_task* task, uint64_t* seq_out);
+/* CC_OK and *out filled when task `seq` has completed; CC_PENDING otherwise.  A completion slot
+ * is reused `capacity` submissions later: poll before then. */
+int32_t cc_poll(cc_ctx* ctx, uint64_t seq, cc_result* out);
+/* Spin (host) until done or timeout_ns elapsed (CC_ERR_TIMEOUT). */
+int32_t cc_wait(cc_ctx* ctx, uint64_t seq, uint64_t timeout_ns, cc_result* out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CONCORDIA_H */

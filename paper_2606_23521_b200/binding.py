@@ -1,0 +1,303 @@
+"""Thin ctypes binding of libconcordia.so -- argument marshalling only.
+
+Every step of the path (scan, compaction, gather + CRC32C, commit, shadow update, apply, ring
+worker) runs in the CUDA kernels behind the C ABI of include/concordia.h.  PyTorch is used for
+device memory, pinned memory and streams.  There is no CPU fallback: importing works without a
+GPU (so that the symbol table can be checked), but creating a Context without the library or
+without a CUDA device raises.
+"""
+import ctypes
+import os
+
+import torch
+
+from . import build as _build
+
+CC_OK = 0
+CC_PENDING = 1
+CC_ERR_INVALID = -1
+CC_ERR_NOT_REGISTERED = -2
+CC_ERR_EXISTS = -3
+CC_ERR_LOG_FULL = -4
+CC_ERR_CORRUPT = -5
+CC_ERR_RING_FULL = -6
+CC_ERR_WORKER = -7
+CC_ERR_CUDA = -8
+CC_ERR_TIMEOUT = -9
+CC_ERR_SCRATCH = -10
+
+CC_REG_SNAPSHOT_NOW = 1
+
+CC_TASK_NOP = 0
+CC_TASK_DELTA_CKPT = 1
+CC_TASK_RESTORE = 2
+CC_TASK_LOG_RESET = 3
+CC_TASK_TEST_MUTATE = 4
+CC_TASK_EXIT = 255
+
+EXPORTS = [
+    "cc_init", "cc_shutdown", "cc_last_cuda_error", "cc_kernel_launches", "cc_workspace_bytes",
+    "cc_register_region", "cc_unregister_region", "cc_log_attach", "cc_log_reset", "cc_checkpoint_delta",
+    "cc_scan_only", "cc_dirty_list", "cc_apply_scratch_bytes", "cc_apply_attach", "cc_apply_log",
+    "cc_worker_start", "cc_worker_stop", "cc_worker_alive", "cc_peek_queue", "cc_submit", "cc_poll", "cc_wait",
+]
+
+
+class cc_config(ctypes.Structure):
+    _fields_ = [("ring_capacity", ctypes.c_uint32), ("worker_blocks", ctypes.c_uint32),
+                ("worker_threads", ctypes.c_uint32), ("backoff_ns", ctypes.c_uint32),
+                ("max_lifetime_ns", ctypes.c_uint64)]
+
+
+class cc_region_desc(ctypes.Structure):
+    _fields_ = [("region_id", ctypes.c_uint32), ("page_bytes", ctypes.c_uint32), ("bytes", ctypes.c_uint64),
+                ("base", ctypes.c_void_p), ("shadow", ctypes.c_void_p), ("workspace", ctypes.c_void_p),
+                ("workspace_bytes", ctypes.c_uint64), ("flags", ctypes.c_uint32), ("reserved", ctypes.c_uint32)]
+
+
+class cc_result(ctypes.Structure):
+    _fields_ = [("seq_done", ctypes.c_uint64), ("n_dirty", ctypes.c_uint64), ("bytes", ctypes.c_uint64),
+                ("log_offset_after", ctypes.c_uint64), ("epoch", ctypes.c_uint64), ("status", ctypes.c_int32),
+                ("flags", ctypes.c_uint32), ("t_start_ns", ctypes.c_uint64), ("t_end_ns", ctypes.c_uint64)]
+
+    def as_dict(self):
+        return {f: getattr(self, f) for f, _ in self._fields_}
+
+
+class cc_task(ctypes.Structure):
+    _fields_ = [("kind", ctypes.c_uint32), ("region_id", ctypes.c_uint32), ("flags", ctypes.c_uint32),
+                ("version", ctypes.c_uint32), ("seq", ctypes.c_uint64), ("epoch", ctypes.c_uint64),
+                ("arg0", ctypes.c_uint64), ("arg1", ctypes.c_uint64), ("arg2", ctypes.c_uint64),
+                ("arg3", ctypes.c_uint64)]
+
+
+assert ctypes.sizeof(cc_result) == 64 and ctypes.sizeof(cc_task) == 64
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def load_library():
+    """dlopen libconcordia.so (building it if the sources are newer) and declare the signatures."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build()
+    lib = ctypes.CDLL(path)
+    vp, u32, u64, i32 = ctypes.c_void_p, ctypes.c_uint32, ctypes.c_uint64, ctypes.c_int32
+    P = ctypes.POINTER
+    sig = {
+        "cc_init": (i32, [P(vp), i32, P(cc_config)]),
+        "cc_shutdown": (i32, [vp]),
+        "cc_last_cuda_error": (i32, [vp]),
+        "cc_kernel_launches": (u64, [vp]),
+        "cc_workspace_bytes": (u64, [u64, u32]),
+        "cc_register_region": (i32, [vp, P(cc_region_desc)]),
+        "cc_unregister_region": (i32, [vp, u32]),
+        "cc_log_attach": (i32, [vp, vp, u64, vp]),
+        "cc_log_reset": (i32, [vp]),
+        "cc_checkpoint_delta": (i32, [vp, u32, u64, vp, vp]),
+        "cc_scan_only": (i32, [vp, u32, vp, vp]),
+        "cc_dirty_list": (i32, [vp, u32, P(vp), P(vp)]),
+        "cc_apply_scratch_bytes": (u64, [u64]),
+        "cc_apply_attach": (i32, [vp, vp, u64]),
+        "cc_apply_log": (i32, [vp, vp, u64, vp, vp]),
+        "cc_worker_start": (i32, [vp]),
+        "cc_worker_stop": (i32, [vp]),
+        "cc_worker_alive": (i32, [vp]),
+        "cc_peek_queue": (i32, [vp, P(u64), P(u64)]),
+        "cc_submit": (i32, [vp, P(cc_task), P(u64)]),
+        "cc_poll": (i32, [vp, u64, P(cc_result)]),
+        "cc_wait": (i32, [vp, u64, u64, P(cc_result)]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(lib, name)
+        fn.restype = res
+        fn.argtypes = args
+    _lib = lib
+    return lib
+
+
+class ConcordiaError(RuntimeError):
+    def __init__(self, call, code, cuda=0):
+        super().__init__("%s failed: status %d (cuda error %d)" % (call, code, cuda))
+        self.code = code
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+class Result:
+    """A 64-byte cc_result in pinned host memory that the GPU writes."""
+
+    def __init__(self):
+        self.buf = torch.zeros(64, dtype=torch.uint8, pin_memory=True)
+        self.ptr = self.buf.data_ptr()
+
+    def clear(self):
+        self.buf.zero_()
+
+    def read(self) -> cc_result:
+        return cc_result.from_buffer_copy(self.buf.numpy().tobytes())
+
+
+class Context:
+    """One libconcordia context on one CUDA device.  Same names as the C ABI, minus the cc_ prefix."""
+
+    def __init__(self, device: int = 0, ring_capacity: int = 0, worker_blocks: int = 0, worker_threads: int = 0,
+                 backoff_ns: int = 0, max_lifetime_ns: int = 0):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2606_23521_b200 needs a CUDA device (sm_100a); there is no CPU fallback")
+        self.lib = load_library()
+        self.device = device
+        cfg = cc_config(ring_capacity, worker_blocks, worker_threads, backoff_ns, max_lifetime_ns)
+        h = ctypes.c_void_p()
+        rc = self.lib.cc_init(ctypes.byref(h), device, ctypes.byref(cfg))
+        if rc != CC_OK:
+            raise ConcordiaError("cc_init", rc)
+        self.h = h
+        self._keep = {}     # region_id -> tensors we must keep alive
+        self._log = None
+        self._committed = None
+        self._scratch = None
+
+    # -- helpers
+    def _check(self, call, rc):
+        if rc < 0:
+            raise ConcordiaError(call, rc, self.lib.cc_last_cuda_error(self.h))
+        return rc
+
+    def kernel_launches(self) -> int:
+        return int(self.lib.cc_kernel_launches(self.h))
+
+    def workspace_bytes(self, nbytes: int, page_bytes: int) -> int:
+        return int(self.lib.cc_workspace_bytes(nbytes, page_bytes))
+
+    # -- regions
+    def register_region(self, region_id: int, base: torch.Tensor, page_bytes: int, shadow: torch.Tensor = None,
+                        snapshot_now: bool = True):
+        """base/shadow: contiguous CUDA tensors of equal byte size.  Allocates shadow and workspace with
+        torch if not given.  Returns the shadow tensor (uint8 view)."""
+        assert base.is_cuda and base.is_contiguous()
+        nbytes = base.numel() * base.element_size()
+        if shadow is None:
+            shadow = torch.empty(nbytes, dtype=torch.uint8, device=base.device)
+        assert shadow.is_cuda and shadow.is_contiguous() and shadow.numel() * shadow.element_size() == nbytes
+        wsb = self.workspace_bytes(nbytes, page_bytes)
+        if wsb == 0:
+            raise ConcordiaError("cc_workspace_bytes", CC_ERR_INVALID)
+        ws = torch.empty(wsb + 256, dtype=torch.uint8, device=base.device)
+        off = (-ws.data_ptr()) % 256
+        d = cc_region_desc(region_id, page_bytes, nbytes, base.data_ptr(), shadow.data_ptr(), ws.data_ptr() + off,
+                           wsb, CC_REG_SNAPSHOT_NOW if snapshot_now else 0, 0)
+        self._check("cc_register_region", self.lib.cc_register_region(self.h, ctypes.byref(d)))
+        self._keep[region_id] = (base, shadow, ws)
+        return shadow
+
+    def unregister_region(self, region_id: int):
+        self._check("cc_unregister_region", self.lib.cc_unregister_region(self.h, region_id))
+        self._keep.pop(region_id, None)
+
+    # -- log
+    def log_attach(self, log: torch.Tensor, committed_off: torch.Tensor = None):
+        """log: uint8 tensor, CUDA or pinned host.  committed_off: pinned int64[1] (optional)."""
+        assert log.dtype == torch.uint8 and log.is_contiguous() and (log.is_cuda or log.is_pinned())
+        cptr = None
+        if committed_off is not None:
+            assert committed_off.numel() * committed_off.element_size() >= 8
+            cptr = ctypes.c_void_p(committed_off.data_ptr())
+        self._check("cc_log_attach", self.lib.cc_log_attach(self.h, log.data_ptr(), log.numel(), cptr))
+        self._log, self._committed = log, committed_off
+
+    def log_reset(self):
+        self._check("cc_log_reset", self.lib.cc_log_reset(self.h))
+
+    # -- host-launched path
+    def checkpoint_delta(self, region_id: int, epoch: int, result: Result = None, stream=None):
+        self._check("cc_checkpoint_delta", self.lib.cc_checkpoint_delta(
+            self.h, region_id, epoch, _stream_ptr(stream), ctypes.c_void_p(result.ptr) if result else None))
+
+    def scan_only(self, region_id: int, result: Result = None, stream=None):
+        self._check("cc_scan_only", self.lib.cc_scan_only(
+            self.h, region_id, _stream_ptr(stream), ctypes.c_void_p(result.ptr) if result else None))
+
+    def dirty_list(self, region_id: int) -> torch.Tensor:
+        """Ascending dirty page indices of the last scan as an int64 CPU tensor (synchronises)."""
+        dl, dc = ctypes.c_void_p(), ctypes.c_void_p()
+        self._check("cc_dirty_list", self.lib.cc_dirty_list(self.h, region_id, ctypes.byref(dl), ctypes.byref(dc)))
+        base, _, ws = self._keep[region_id]
+        torch.cuda.current_stream().synchronize()
+        ws_off = dc.value - ws.data_ptr()
+        k = int(ws[ws_off:ws_off + 4].view(torch.int32).item())
+        d_off = dl.value - ws.data_ptr()
+        return ws[d_off:d_off + 4 * k].view(torch.int32).to(torch.int64).cpu()
+
+    def apply_attach(self, max_records: int, device=None):
+        nb = int(self.lib.cc_apply_scratch_bytes(max_records))
+        if nb == 0:
+            raise ConcordiaError("cc_apply_scratch_bytes", CC_ERR_INVALID)
+        s = torch.empty(nb + 256, dtype=torch.uint8, device=device or torch.device("cuda", self.device))
+        off = (-s.data_ptr()) % 256
+        self._check("cc_apply_attach", self.lib.cc_apply_attach(self.h, s.data_ptr() + off, nb))
+        self._scratch = s
+
+    def apply_log(self, log: torch.Tensor, nbytes: int, result: Result = None, stream=None):
+        assert log.dtype == torch.uint8 and log.is_contiguous() and (log.is_cuda or log.is_pinned())
+        assert nbytes <= log.numel()
+        self._check("cc_apply_log", self.lib.cc_apply_log(
+            self.h, log.data_ptr(), nbytes, _stream_ptr(stream), ctypes.c_void_p(result.ptr) if result else None))
+
+    # -- ring + persistent worker
+    def worker_start(self):
+        # everything the worker touches is allocated; make sure nothing of ours is still queued
+        torch.cuda.synchronize(self.device)
+        self._check("cc_worker_start", self.lib.cc_worker_start(self.h))
+
+    def worker_stop(self):
+        self._check("cc_worker_stop", self.lib.cc_worker_stop(self.h))
+
+    def worker_alive(self) -> bool:
+        return self.lib.cc_worker_alive(self.h) == 1
+
+    def peek_queue(self):
+        h, t = ctypes.c_uint64(), ctypes.c_uint64()
+        self._check("cc_peek_queue", self.lib.cc_peek_queue(self.h, ctypes.byref(h), ctypes.byref(t)))
+        return h.value, t.value
+
+    def submit(self, kind: int, region_id: int = 0, epoch: int = 0, arg0: int = 0, arg1: int = 0, arg2: int = 0,
+               arg3: int = 0) -> int:
+        """Returns the sequence number, or raises ConcordiaError(CC_ERR_RING_FULL)."""
+        t = cc_task(kind, region_id, 0, 0, 0, epoch, arg0, arg1, arg2, arg3)
+        seq = ctypes.c_uint64()
+        self._check("cc_submit", self.lib.cc_submit(self.h, ctypes.byref(t), ctypes.byref(seq)))
+        return seq.value
+
+    def poll(self, seq: int):
+        r = cc_result()
+        rc = self._check("cc_poll", self.lib.cc_poll(self.h, seq, ctypes.byref(r)))
+        return None if rc == CC_PENDING else r
+
+    def wait(self, seq: int, timeout_s: float = 10.0) -> cc_result:
+        r = cc_result()
+        self._check("cc_wait", self.lib.cc_wait(self.h, seq, int(timeout_s * 1e9), ctypes.byref(r)))
+        return r
+
+    def shutdown(self):
+        if self.h:
+            rc = self.lib.cc_shutdown(self.h)
+            self.h = None
+            self._keep.clear()
+            if rc < 0:
+                raise ConcordiaError("cc_shutdown", rc)
+
+    def __del__(self):
+        try:
+            self.shutdown()
+        except Exception:
+            pass

@@ -1,0 +1,288 @@
+// cc_apply.cuh -- a6, the recovery applier ("fn.apply(aof_read(epoch))", L221
+// "Recovery ignores any suffix without a commit marker", L227 "replays ... committed AOF suffix").
+//
+// The sequential definition (walk record by record; hold page records pending until their commit
+// validates; apply epochs in log order) is reproduced exactly by five data-parallel phases:
+//   parse    one block walks the headers.  Inside an epoch all full-page records of a region
+//            have the same stride 16+P, so the block reads blockDim headers speculatively per
+//            step and accepts the leading run that is structurally valid; commit records, short
+//            tail pages and region changes are handled one at a time.  The walk stops at the
+//            first torn or structurally invalid record, exactly where the definition stops.
+//   validate every 4 KiB payload segment is CRC'd by a warp; a record whose CRC differs lowers
+//            first_bad_rec (atomicMin).  The last block then resolves the committed prefix:
+//            the epochs whose records all precede the first failed check.
+//   latest   atomicMax(latest[page], rec+1) over the committed records (last record wins).
+//   scatter  a segment is copied into the live page and the shadow only if its record is the
+//            page's latest.
+//   cleanup  latest[] back to zero; result written.
+#pragma once
+#include "cc_common.cuh"
+#include "cc_crc.cuh"
+
+struct cc_apply_tabs {      // carved out of the attached scratch
+    cc_rec* recs;
+    cc_epoch_ent* epochs;
+    u32* rec_acc;           // per-record CRC accumulator
+    u32* rec_cnt;           // per-record finished segments
+    u32* seg_begin;         // per-record first segment number (+ one trailing total)
+    u64 max_records;
+};
+
+__device__ __forceinline__ int cc_find_slot(const cc_dev* dev, u32 rid) {
+    for (int s = 0; s < CC_MAX_REGIONS; s++)
+        if (dev->region_used[s] && dev->regions[s].region_id == rid) return s;
+    return -1;
+}
+
+#define CC_PA_STOP 0u
+#define CC_PA_NEXT 1u
+#define CC_PA_RUN 2u
+
+__device__ __forceinline__ void cc_apply_parse_phase(cc_dev* dev, const cc_apply_tabs& T, const u8* log, u64 n) {
+    __shared__ u64 s_off;
+    __shared__ u32 s_action, s_slot, s_first_fail, s_nrecs, s_nepochs, s_pending, s_pend_rid, s_mixed, s_segs;
+    cc_apply_state* A = &dev->apply;
+    const u32 tid = threadIdx.x, nthr = blockDim.x;
+    if (tid == 0) {
+        s_off = 0; s_nrecs = 0; s_nepochs = 0; s_pending = 0; s_pend_rid = 0; s_mixed = 0; s_segs = 0;
+        A->struct_fail = 0; A->scratch_overflow = 0; A->first_bad_rec = 0xFFFFFFFFu; A->validate_done = 0;
+        A->n_commit_recs = 0; A->n_commit_epochs = 0; A->consumed = 0; A->status = CC_OK; A->final_done = 0;
+        A->t_start_ns = globaltimer_ns();
+    }
+    __syncthreads();
+    for (;;) {
+        if (tid == 0) {
+            u32 action = CC_PA_STOP;
+            const u64 off = s_off;
+            do {
+                if (n - off < CC_RECORD_HEADER_BYTES) break;                               // torn
+                const uint4 h = ld_v4(reinterpret_cast<const uint4*>(log + off));
+                if ((u64)h.z > n - off - CC_RECORD_HEADER_BYTES) break;                    // torn
+                if (h.x == CC_COMMIT_ID) {
+                    bool ok = (h.y == CC_COMMIT_ID) && (h.z == 16u);
+                    if (ok) {
+                        const uint4 pl = ld_v4(reinterpret_cast<const uint4*>(log + off + 16));
+                        u32 pay[4] = {pl.x, pl.y, pl.z, pl.w};
+                        ok = crc_serial(&dev->crc, reinterpret_cast<const u8*>(pay), 16) == h.w;
+                        ok = ok && (pl.w == s_pending) && !s_mixed && (s_pending == 0 || s_pend_rid == pl.z);
+                    }
+                    if (!ok) { A->struct_fail = 1; break; }
+                    if (s_nepochs >= T.max_records) { A->scratch_overflow = 1; break; }
+                    T.epochs[s_nepochs].off_after = off + CC_COMMIT_RECORD_BYTES;
+                    T.epochs[s_nepochs].rec_end = s_nrecs;
+                    s_nepochs++;
+                    s_pending = 0; s_mixed = 0;
+                    s_off = off + CC_COMMIT_RECORD_BYTES;
+                    action = CC_PA_NEXT;
+                    break;
+                }
+                const int slot = cc_find_slot(dev, h.x);
+                if (slot < 0) { A->struct_fail = 1; break; }
+                const cc_region_dev& r = dev->regions[slot];
+                if ((u64)h.y >= r.n_pages || (u64)h.z != page_len_dev(r, h.y)) { A->struct_fail = 1; break; }
+                if (s_pending != 0 && s_pend_rid != h.x) s_mixed = 1;
+                s_pend_rid = h.x;
+                s_slot = (u32)slot;
+                s_first_fail = nthr;
+                action = CC_PA_RUN;
+            } while (0);
+            s_action = action;
+        }
+        __syncthreads();
+        const u32 action = s_action;
+        if (action == CC_PA_STOP) break;
+        if (action == CC_PA_RUN) {
+            const cc_region_dev& r = dev->regions[s_slot];
+            const u64 P = r.page_bytes;
+            const u64 stride = P + CC_RECORD_HEADER_BYTES;
+            const u64 off_t = s_off + (u64)tid * stride;
+            uint4 h = make_uint4(0, 0, 0, 0);
+            bool ok = (off_t + CC_RECORD_HEADER_BYTES <= n);
+            if (ok) {
+                h = ld_v4(reinterpret_cast<const uint4*>(log + off_t));
+                ok = ((u64)h.z <= n - off_t - CC_RECORD_HEADER_BYTES) && (h.x == r.region_id) &&
+                     ((u64)h.y < r.n_pages) && ((u64)h.z == page_len_dev(r, h.y));
+            }
+            // a short (tail) page is valid but breaks the stride: it may only END a run
+            const bool full = ok && ((u64)h.z == P);
+            if (!ok) atomicMin(&s_first_fail, tid);
+            else if (!full) atomicMin(&s_first_fail, tid + 1);
+            __syncthreads();
+            u32 run = s_first_fail < nthr ? s_first_fail : nthr;      // >= 1: thread 0 re-checked record 0
+            const u32 base = s_nrecs;
+            const bool overflow = (u64)base + run > T.max_records;
+            if (!overflow && tid < run) {
+                cc_rec rec;
+                rec.off = off_t; rec.page_idx = h.y; rec.len = h.z; rec.crc = h.w;
+                rec.slot = s_slot; rec.epoch_idx = s_nepochs; rec.pad = 0;
+                T.recs[base + tid] = rec;
+                T.rec_acc[base + tid] = 0;
+                T.rec_cnt[base + tid] = 0;
+                T.seg_begin[base + tid] = s_segs + tid * r.spp;        // only the run's last record can be short
+            }
+            __syncthreads();
+            if (tid == 0) {
+                if (overflow) { A->scratch_overflow = 1; s_action = CC_PA_STOP; }
+                else {
+                    const cc_rec& last = T.recs[base + run - 1];
+                    s_off = last.off + CC_RECORD_HEADER_BYTES + last.len;
+                    s_nrecs = base + run;
+                    s_pending += run;
+                    s_segs += (run - 1) * r.spp + (last.len + CC_SEG_BYTES - 1) / CC_SEG_BYTES;
+                }
+            }
+            __syncthreads();
+            if (s_action == CC_PA_STOP) break;
+        }
+    }
+    if (tid == 0) {
+        A->n_recs = s_nrecs;
+        A->n_epochs = s_nepochs;
+        T.seg_begin[s_nrecs] = s_segs;          // table has max_records + 1 entries
+        __threadfence();
+    }
+}
+
+// warp-cooperative search: largest rec with seg_begin[rec] <= item, rec in [0, n)
+__device__ __forceinline__ u32 cc_find_rec(const u32* seg_begin, u32 n, u32 item, u32 lane) {
+    u32 lo = 0, hi = n;
+    while (hi - lo > 1) {
+        const u32 step = (hi - lo + 31) / 32;
+        const u32 idx = lo + lane * step;
+        const bool le = (idx < hi) && (seg_begin[idx] <= item);
+        const u32 cnt = __popc(__ballot_sync(0xFFFFFFFFu, le));     // >= 1 (lane 0)
+        lo = lo + (cnt - 1) * step;
+        hi = min(lo + step, hi);
+    }
+    return lo;
+}
+
+__device__ __forceinline__ void cc_apply_validate_phase(cc_dev* dev, const cc_apply_tabs& T, cc_crc_smem* cs,
+                                                        const u8* log, cc_grid g, bool init_tables) {
+    constexpr int U = 8;
+    cc_apply_state* A = &dev->apply;
+    const u32 n_recs = A->n_recs;
+    const u32 lane = threadIdx.x & 31u;
+    if (n_recs != 0 && !A->scratch_overflow) {
+        if (init_tables) cc_crc_smem_init(cs, &dev->crc);
+        const u32 n_items = T.seg_begin[n_recs];
+        for (u32 item = g.warp(); item < n_items; item += g.nwarps()) {
+            const u32 ri = cc_find_rec(T.seg_begin, n_recs, item, lane);
+            const cc_rec rec = T.recs[ri];
+            const u32 c = item - T.seg_begin[ri];
+            const u64 so = (u64)c * CC_SEG_BYTES;
+            const u64 rem = rec.len - so;
+            const u32 seg_len = (u32)(rem < CC_SEG_BYTES ? rem : CC_SEG_BYTES);
+            const u32 nv = seg_len >> 4;
+            const u32 nseg = (rec.len + CC_SEG_BYTES - 1) / CC_SEG_BYTES;
+            const uint4* src = reinterpret_cast<const uint4*>(log + rec.off + CC_RECORD_HEADER_BYTES + so);
+            uint4 v[U];
+#pragma unroll
+            for (int u = 0; u < U; u++) {
+                const u32 j = lane + 32 * u;
+                v[u] = (j < nv) ? ld_v4(src + j) : make_uint4(0, 0, 0, 0);
+            }
+            const u32 contrib = crc_segment_warp<U>(cs, &dev->crc, v, nv, rem - seg_len, lane);
+            if (lane == 0) {
+                u32 acc = contrib;
+                bool finish = true;
+                if (nseg > 1) {
+                    atomicXor(&T.rec_acc[ri], contrib);
+                    __threadfence();
+                    finish = (atomicAdd(&T.rec_cnt[ri], 1u) == nseg - 1);
+                    if (finish) { __threadfence(); acc = atomicExch(&T.rec_acc[ri], 0u); }
+                }
+                if (finish && crc_finalize(&dev->crc, acc, rec.len) != rec.crc) atomicMin(&A->first_bad_rec, ri);
+            }
+        }
+    }
+    // last block resolves the committed prefix
+    __shared__ u32 s_last;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(&A->validate_done, 1u) == g.nblocks - 1) ? 1u : 0u;
+    __syncthreads();
+    if (s_last && threadIdx.x == 0) {
+        __threadfence();
+        const u32 f = A->first_bad_rec;           // 0xFFFFFFFF if every CRC matched
+        const u32 ne = A->n_epochs;
+        u32 lo = 0, hi = ne;                      // epochs are ordered by rec_end: count those with rec_end <= f
+        while (lo < hi) {
+            const u32 mid = (lo + hi) >> 1;
+            if (T.epochs[mid].rec_end <= f) lo = mid + 1; else hi = mid;
+        }
+        int32_t st = CC_OK;
+        if (f != 0xFFFFFFFFu || A->struct_fail) st = CC_ERR_CORRUPT;
+        u32 E = lo;
+        if (A->scratch_overflow) { st = CC_ERR_SCRATCH; E = 0; }
+        A->n_commit_epochs = E;
+        A->n_commit_recs = E ? T.epochs[E - 1].rec_end : 0;
+        A->consumed = E ? T.epochs[E - 1].off_after : 0;
+        A->status = st;
+        A->validate_done = 0;
+        __threadfence();
+    }
+}
+
+__device__ __forceinline__ void cc_apply_latest_phase(cc_dev* dev, const cc_apply_tabs& T, cc_grid g) {
+    const u32 n = dev->apply.n_commit_recs;
+    for (u32 i = g.block * blockDim.x + threadIdx.x; i < n; i += g.nblocks * blockDim.x) {
+        const cc_rec rec = T.recs[i];
+        atomicMax(&dev->regions[rec.slot].latest[rec.page_idx], i + 1);
+    }
+}
+
+__device__ __forceinline__ void cc_apply_scatter_phase(cc_dev* dev, const cc_apply_tabs& T, const u8* log, cc_grid g) {
+    constexpr int U = 8;
+    const u32 n = dev->apply.n_commit_recs;
+    if (n == 0) return;
+    const u32 lane = threadIdx.x & 31u;
+    const u32 n_items = T.seg_begin[n];
+    for (u32 item = g.warp(); item < n_items; item += g.nwarps()) {
+        const u32 ri = cc_find_rec(T.seg_begin, n, item, lane);
+        const cc_rec rec = T.recs[ri];
+        const cc_region_dev& r = dev->regions[rec.slot];
+        if (r.latest[rec.page_idx] != ri + 1) continue;              // an earlier duplicate: a later record wins
+        const u32 c = item - T.seg_begin[ri];
+        const u64 so = (u64)c * CC_SEG_BYTES;
+        const u64 rem = rec.len - so;
+        const u32 nv = (u32)(rem < CC_SEG_BYTES ? rem : CC_SEG_BYTES) >> 4;
+        const uint4* src = reinterpret_cast<const uint4*>(log + rec.off + CC_RECORD_HEADER_BYTES + so);
+        const u64 dst_off = (u64)rec.page_idx * r.page_bytes + so;
+        uint4* d0 = reinterpret_cast<uint4*>(r.base + dst_off);
+        uint4* d1 = reinterpret_cast<uint4*>(r.shadow + dst_off);
+        uint4 v[U];
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            const u32 j = lane + 32 * u;
+            if (j < nv) v[u] = ld_v4(src + j);
+        }
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            const u32 j = lane + 32 * u;
+            if (j < nv) { st_stream(d0 + j, v[u]); st_stream(d1 + j, v[u]); }
+        }
+    }
+}
+
+__device__ __forceinline__ void cc_apply_cleanup_phase(cc_dev* dev, const cc_apply_tabs& T, cc_grid g, cc_result* out,
+                                                       u32 kind) {
+    cc_apply_state* A = &dev->apply;
+    const u32 n = A->n_commit_recs;
+    for (u32 i = g.block * blockDim.x + threadIdx.x; i < n; i += g.nblocks * blockDim.x) {
+        const cc_rec rec = T.recs[i];
+        dev->regions[rec.slot].latest[rec.page_idx] = 0;
+    }
+    if (g.block == 0 && threadIdx.x == 0 && out) {
+        out->n_dirty = n;
+        out->bytes = A->consumed;
+        out->log_offset_after = A->consumed;
+        out->epoch = A->n_commit_epochs;
+        out->status = A->status;
+        out->flags = kind;
+        out->t_start_ns = A->t_start_ns;
+        out->t_end_ns = globaltimer_ns();
+        __threadfence_system();
+        st_release_sys_u64(&out->seq_done, 1ull);
+    }
+}

@@ -1,0 +1,323 @@
+// cc_ckpt.cuh -- the checkpoint direction: a1 scan, a2 compaction, a3-a5 gather + CRC + commit +
+// shadow update.  Device functions over a virtual grid so that the
+// host-launched kernels and the persistent worker run the very same code.
+#pragma once
+#include "cc_common.cuh"
+#include "cc_crc.cuh"
+
+// ------------------------------------------------------------------------- a1: scan --
+// dirty[p] = any byte of cur page p differs from shadow page p.
+// Work item = one 4 KiB segment of one page, handled by one warp: each lane issues 8 + 8
+// independent 16-byte streaming loads (cur, shadow), XOR/ORs them, the warp votes, and lane 0
+// sets the page's bit in the bitmap only if the segment differs.  The bitmap is all-zero on
+// entry (the compaction clears what it consumes).
+template <int U>
+__device__ __forceinline__ void cc_scan_phase(const cc_region_dev& r, cc_grid g) {
+    const u32 lane = threadIdx.x & 31u;
+    if (g.block == 0 && threadIdx.x == 0) {
+        r.hdr->t_start_ns = globaltimer_ns();
+        r.hdr->ticket = 0;
+        r.hdr->run_id = r.hdr->run_id + 1;
+    }
+    constexpr u32 SEGV = 32u * U;            // vectors per item
+    constexpr u32 SEGB = SEGV * 16u;         // bytes per item
+    const u32 P = r.page_bytes;
+    const u32 spp = (P + SEGB - 1) / SEGB;
+    const u64 n_items = r.n_pages * (u64)spp;
+    const bool pow2 = (spp & (spp - 1)) == 0;
+    const u32 sh = 31 - __clz(spp);
+    const bool uniform = (r.bytes % P == 0) && (P % SEGB == 0);
+    const u64 stride = g.nwarps();
+    for (u64 item = g.warp(); item < n_items; item += stride) {
+        u64 p;
+        u32 s;
+        if (pow2) { p = item >> sh; s = (u32)(item & (spp - 1)); }
+        else { p = item / spp; s = (u32)(item - p * spp); }
+        const u64 start = p * (u64)P + (u64)s * SEGB;
+        const uint4* a = reinterpret_cast<const uint4*>(r.base + start);
+        const uint4* b = reinterpret_cast<const uint4*>(r.shadow + start);
+        u32 acc = 0;
+        if (uniform) {
+            uint4 va[U], vb[U];
+#pragma unroll
+            for (int u = 0; u < U; u++) va[u] = ld_stream(a + lane + 32 * u);
+#pragma unroll
+            for (int u = 0; u < U; u++) vb[u] = ld_stream(b + lane + 32 * u);
+#pragma unroll
+            for (int u = 0; u < U; u++)
+                acc |= (va[u].x ^ vb[u].x) | (va[u].y ^ vb[u].y) | (va[u].z ^ vb[u].z) | (va[u].w ^ vb[u].w);
+        } else {
+            const u64 plen = page_len_dev(r, p);
+            const u64 so = (u64)s * SEGB;
+            if (so >= plen) continue;
+            const u64 rem = plen - so;
+            const u32 nv = (u32)((rem < SEGB ? rem : SEGB) >> 4);
+#pragma unroll
+            for (int u = 0; u < U; u++) {
+                const u32 j = lane + 32 * u;
+                if (j < nv) {
+                    uint4 x = ld_stream(a + j), y = ld_stream(b + j);
+                    acc |= (x.x ^ y.x) | (x.y ^ y.y) | (x.z ^ y.z) | (x.w ^ y.w);
+                }
+            }
+        }
+        if (__any_sync(0xFFFFFFFFu, acc != 0) && lane == 0)
+            atomicOr(&r.bitmap[p >> 5], 1u << (p & 31));
+    }
+}
+
+// ------------------------------------------------------------------ a2: compaction --
+// Ascending list D[0..k) of set bits of the bitmap and k ("dirty page
+// descriptors").  Single pass: tiles of 1024 bitmap words are handed out by ticket (so a tile's
+// predecessors have always started), each tile publishes its popcount and resolves its exclusive
+// prefix by decoupled look-back over run-tagged status words.  The bitmap words are cleared as
+// they are consumed.  The block that owns the last tile also writes the plan of the gather:
+// record count, byte need, log-full decision (all-or-nothing, reading #10).
+#define CC_LB_AGG 1ull
+#define CC_LB_INC 2ull
+__device__ __forceinline__ u64 lb_pack(u32 run, u64 flag, u32 val) { return ((u64)run << 34) | (flag << 32) | val; }
+
+#define CC_MODE_CHECKPOINT 0u
+#define CC_MODE_SCAN_ONLY 1u
+
+// Only the first CC_COMPACT_THREADS threads of a block work (the worker's blocks may be wider);
+// every thread takes part in the barriers.
+__device__ __forceinline__ void cc_compact_phase(const cc_region_dev& r, cc_log_dev* log, u32 mode, u64 epoch,
+                                                 cc_result* out) {
+    __shared__ u32 s_ticket, s_excl, s_last_dirty;
+    __shared__ u32 s_warp[CC_COMPACT_THREADS / 32];
+    const u32 tid = threadIdx.x, lane = tid & 31u, wid = tid >> 5;
+    const u32 run = r.hdr->run_id & 0x3FFFFFFFu;
+    const u32 nt = (u32)((r.n_words + CC_COMPACT_TILE_WORDS - 1) / CC_COMPACT_TILE_WORDS);
+    const u32 nwarp = CC_COMPACT_THREADS / 32;
+    const bool active = tid < CC_COMPACT_THREADS;
+    for (;;) {
+        if (tid == 0) { s_ticket = atomicAdd(&r.hdr->ticket, 1u); s_last_dirty = 0; }
+        __syncthreads();
+        const u32 t = s_ticket;
+        if (t >= nt) break;
+        // each thread owns CC_COMPACT_WORDS_PER_THREAD consecutive words per 'row' of blockDim threads
+        u32 cnt = 0;
+        constexpr u32 words_per_thread = CC_COMPACT_WORDS_PER_THREAD;
+        const u64 w0 = (u64)t * CC_COMPACT_TILE_WORDS + (u64)tid * words_per_thread;
+        u32 wv[words_per_thread] = {0, 0, 0, 0};
+        if (active) {
+            uint4 q = *reinterpret_cast<const uint4*>(&r.bitmap[w0]);   // bitmap is padded to whole tiles
+            wv[0] = q.x; wv[1] = q.y; wv[2] = q.z; wv[3] = q.w;
+            if (q.x | q.y | q.z | q.w) *reinterpret_cast<uint4*>(&r.bitmap[w0]) = make_uint4(0, 0, 0, 0);
+            cnt = __popc(q.x) + __popc(q.y) + __popc(q.z) + __popc(q.w);
+        }
+        // block exclusive scan of cnt
+        u32 inc = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            u32 n = __shfl_up_sync(0xFFFFFFFFu, inc, o);
+            if (lane >= o) inc += n;
+        }
+        if (lane == 31 && active) s_warp[wid] = inc;
+        __syncthreads();
+        u32 warp_base = 0, total = 0;
+        for (u32 i = 0; i < nwarp; i++) {
+            u32 v = s_warp[i];
+            if (i < wid) warp_base += v;
+            total += v;
+        }
+        if (tid == 0) {
+            u32 excl = 0;
+            if (t == 0) {
+                st_release_gpu_u64(&r.lb_status[0], lb_pack(run, CC_LB_INC, total));
+            } else {
+                st_release_gpu_u64(&r.lb_status[t], lb_pack(run, CC_LB_AGG, total));
+                int j = (int)t - 1;
+                while (j >= 0) {
+                    u64 s = ld_acquire_gpu_u64(&r.lb_status[j]);
+                    if ((u32)(s >> 34) != run || ((s >> 32) & 3ull) == 0) { __nanosleep(20); continue; }
+                    excl += (u32)s;
+                    if (((s >> 32) & 3ull) == CC_LB_INC) break;
+                    j--;
+                }
+                st_release_gpu_u64(&r.lb_status[t], lb_pack(run, CC_LB_INC, excl + total));
+            }
+            s_excl = excl;
+        }
+        __syncthreads();
+        u32 pos = s_excl + warp_base + (inc - cnt);
+#pragma unroll
+        for (u32 i = 0; i < words_per_thread; i++) {
+            u32 w = wv[i];
+            const u64 pbase = (w0 + i) << 5;
+            while (w) {
+                const u32 bit = __ffs(w) - 1;
+                w &= w - 1;
+                const u64 page = pbase + bit;
+                r.D[pos++] = (u32)page;
+                if (page == r.n_pages - 1) s_last_dirty = 1;
+            }
+        }
+        __syncthreads();
+        if (t == nt - 1 && tid == 0) {
+            const u32 k = s_excl + total;
+            cc_ws_hdr* h = r.hdr;
+            h->k = k;
+            h->epoch = epoch;
+            u64 need = (u64)k * (CC_RECORD_HEADER_BYTES + (u64)r.page_bytes) + CC_COMMIT_RECORD_BYTES;
+            if (s_last_dirty) need -= (u64)r.page_bytes - page_len_dev(r, r.n_pages - 1);
+            const u64 W = log->W;
+            int32_t st = CC_OK;
+            u32 k_eff = 0;
+            if (mode == CC_MODE_CHECKPOINT && k != 0) {
+                if (log->buf == nullptr || W + need > log->capacity) st = CC_ERR_LOG_FULL;
+                else k_eff = k;
+            }
+            h->k_eff = k_eff;
+            h->status = st;
+            h->W_start = W;
+            h->need = k_eff ? need : 0;
+            h->gather_done = 0;
+            if (mode == CC_MODE_SCAN_ONLY && out) {
+                out->n_dirty = k;
+                out->bytes = 0;
+                out->log_offset_after = W;
+                out->epoch = epoch;
+                out->status = CC_OK;
+                out->flags = CC_TASK_NOP;
+                out->t_start_ns = h->t_start_ns;
+                out->t_end_ns = globaltimer_ns();
+                __threadfence_system();
+                st_release_sys_u64(&out->seq_done, 1ull);
+            }
+            __threadfence();
+        }
+        __syncthreads();
+    }
+}
+
+// ------------------------------------------------- a3-a5: gather + CRC + commit + shadow --
+// For record i < k_eff: header {region_id, D[i], len, crc32c(payload)} + payload at
+// W_start + i*(16+P), and shadow[page] := cur[page] (L264).  One warp moves
+// one 4 KiB segment: the bytes are read ONCE into registers and the log payload, the shadow and
+// the CRC all come from that one read.  The warp that completes a record's last segment writes
+// its header.  Every block fences its stores at system scope and counts itself done; the last
+// block appends the commit record, fences, publishes the committed offset with a system-scope
+// release store (L263: "a commit marker publishes the epoch only after all bytes are visible")
+// and fills the result.
+__device__ __forceinline__ void st_u32x4(u8* p, u32 a, u32 b, u32 c, u32 d) {
+    uint4 v = make_uint4(a, b, c, d);
+    st_stream(reinterpret_cast<uint4*>(p), v);
+}
+
+__device__ __forceinline__ void cc_gather_phase(const cc_region_dev& r, cc_dev* dev, cc_crc_smem* cs, cc_grid g,
+                                                cc_result* out, u32 kind, bool init_tables) {
+    constexpr int U = 8;
+    cc_ws_hdr* h = r.hdr;
+    cc_log_dev* log = &dev->log;
+    const u32 k_eff = h->k_eff;
+    const u32 lane = threadIdx.x & 31u;
+    const u32 P = r.page_bytes;
+    const u64 W0 = h->W_start;
+    // warps take items round-robin, so a block has work iff its first warp index is < n_items
+    if (k_eff != 0 && (u64)g.block * (blockDim.x >> 5) < (u64)k_eff * r.spp) {
+        if (init_tables) cc_crc_smem_init(cs, &dev->crc);
+        const u32 spp = r.spp;
+        const u64 n_items = (u64)k_eff * spp;
+        const u64 rec_stride = (u64)P + CC_RECORD_HEADER_BYTES;
+        const u64 stride = g.nwarps();
+        for (u64 item = g.warp(); item < n_items; item += stride) {
+            u32 i, c;
+            if (r.spp_shift >= 0) { i = (u32)(item >> r.spp_shift); c = (u32)(item & (spp - 1)); }
+            else { i = (u32)(item / spp); c = (u32)(item - (u64)i * spp); }
+            const u32 p = r.D[i];
+            const u64 plen = page_len_dev(r, p);
+            const u64 so = (u64)c * CC_SEG_BYTES;
+            if (so >= plen) continue;
+            const u64 rem = plen - so;
+            const u32 seg_len = (u32)(rem < CC_SEG_BYTES ? rem : CC_SEG_BYTES);
+            const u32 nv = seg_len >> 4;
+            const u64 after = rem - seg_len;
+            const u32 nseg = (u32)((plen + CC_SEG_BYTES - 1) / CC_SEG_BYTES);
+            const u64 src_off = (u64)p * P + so;
+            const uint4* src = reinterpret_cast<const uint4*>(r.base + src_off);
+            uint4* dsh = reinterpret_cast<uint4*>(r.shadow + src_off);
+            u8* rec = log->buf + W0 + (u64)i * rec_stride;
+            uint4* dlog = reinterpret_cast<uint4*>(rec + CC_RECORD_HEADER_BYTES + so);
+            uint4 v[U];
+            if (nv == CC_SEG_VECS) {
+#pragma unroll
+                for (int u = 0; u < U; u++) v[u] = ld_stream(src + lane + 32 * u);
+#pragma unroll
+                for (int u = 0; u < U; u++) st_stream(dlog + lane + 32 * u, v[u]);
+#pragma unroll
+                for (int u = 0; u < U; u++) st_stream(dsh + lane + 32 * u, v[u]);
+            } else {
+#pragma unroll
+                for (int u = 0; u < U; u++) {
+                    const u32 j = lane + 32 * u;
+                    if (j < nv) {
+                        v[u] = ld_stream(src + j);
+                        st_stream(dlog + j, v[u]);
+                        st_stream(dsh + j, v[u]);
+                    } else {
+                        v[u] = make_uint4(0, 0, 0, 0);
+                    }
+                }
+            }
+            const u32 contrib = crc_segment_warp<U>(cs, &dev->crc, v, nv, after, lane);
+            if (lane == 0) {
+                u32 acc;
+                bool finish;
+                if (nseg == 1) { acc = contrib; finish = true; }
+                else {
+                    atomicXor(&r.rec_crc[i], contrib);
+                    __threadfence();
+                    finish = (atomicAdd(&r.rec_done[i], 1u) == nseg - 1);
+                    acc = 0;
+                    if (finish) {
+                        __threadfence();
+                        acc = atomicExch(&r.rec_crc[i], 0u);
+                        r.rec_done[i] = 0;
+                    }
+                }
+                if (finish) st_u32x4(rec, r.region_id, p, (u32)plen, crc_finalize(&dev->crc, acc, plen));
+            }
+        }
+    }
+    // ---- completion: last block commits ----
+    __shared__ u32 s_last;
+    __threadfence_system();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence_system();
+        s_last = (atomicAdd(&h->gather_done, 1u) == g.nblocks - 1) ? 1u : 0u;
+    }
+    __syncthreads();
+    if (s_last && threadIdx.x == 0) {
+        __threadfence_system();
+        u64 W_after = W0;
+        if (k_eff != 0) {
+            u8* c = log->buf + W0 + h->need - CC_COMMIT_RECORD_BYTES;
+            const u64 epoch = h->epoch;
+            u32 pay[4] = {(u32)epoch, (u32)(epoch >> 32), r.region_id, k_eff};
+            const u32 crc = crc_serial(&dev->crc, reinterpret_cast<const u8*>(pay), 16);
+            st_u32x4(c + 16, pay[0], pay[1], pay[2], pay[3]);
+            st_u32x4(c, CC_COMMIT_ID, CC_COMMIT_ID, 16u, crc);
+            W_after = W0 + h->need;
+            __threadfence_system();
+            if (log->committed_off) st_release_sys_u64(log->committed_off, W_after);
+            log->W = W_after;
+        }
+        h->gather_done = 0;
+        if (out) {
+            out->n_dirty = h->k;
+            out->bytes = h->need;
+            out->log_offset_after = W_after;
+            out->epoch = h->epoch;
+            out->status = h->status;
+            out->flags = kind;
+            out->t_start_ns = h->t_start_ns;
+            out->t_end_ns = globaltimer_ns();
+            __threadfence_system();
+            st_release_sys_u64(&out->seq_done, 1ull);
+        }
+        __threadfence();
+    }
+}

@@ -1,0 +1,180 @@
+// cc_common.cuh -- device-side data structures and PTX helpers of libconcordia (sm_100a).
+// Part of the CUDA path; shares nothing with oracle/.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+#include "../../include/concordia.h"
+
+typedef uint8_t u8;
+typedef uint32_t u32;
+typedef uint64_t u64;
+
+#define CC_SEG_BYTES 4096u        // one warp item: 32 lanes x 8 x 16 B
+#define CC_SEG_VECS 256u          // 16-byte vectors per segment
+#define CC_COMPACT_THREADS 256
+#define CC_COMPACT_WORDS_PER_THREAD 4
+#define CC_COMPACT_TILE_WORDS (CC_COMPACT_THREADS * CC_COMPACT_WORDS_PER_THREAD)   // 1024 words = 32768 pages
+
+// Per-region control block in the workspace (device memory).
+struct cc_ws_hdr {
+    u32 k;              // dirty pages of the last scan
+    u32 k_eff;          // records the gather must write (0 on log-full / scan-only)
+    int32_t status;     // CC_OK / CC_ERR_LOG_FULL
+    u32 ticket;         // compaction tile ticket
+    u32 run_id;         // compaction look-back tag
+    u32 gather_done;    // warps/blocks finished (last-block pattern)
+    u32 pad0, pad1;
+    u64 W_start;        // log offset at which this checkpoint's records start
+    u64 need;           // bytes this checkpoint appends
+    u64 t_start_ns;
+    u64 epoch;
+};
+
+// Device-visible region descriptor.
+struct cc_region_dev {
+    u8* base;
+    u8* shadow;
+    u64 bytes;
+    u64 n_pages;
+    u32 page_bytes;
+    u32 region_id;
+    u32 spp;            // 4 KiB segments per page = ceil(P / 4096)
+    int32_t spp_shift;  // log2(spp) if power of two else -1
+    u64 n_words;        // bitmap words
+    u32* bitmap;        // n_words (+ padding to a multiple of 4) u32, all zero between calls
+    u32* D;             // n_pages u32: ascending dirty list
+    u32* rec_crc;       // n_pages u32: per-record CRC accumulators, all zero between calls
+    u32* rec_done;      // n_pages u32: per-record finished-segment counters, all zero between calls
+    u64* lb_status;     // compaction look-back status, one per tile
+    u32* latest;        // n_pages u32: applier last-wins table, all zero between calls
+    cc_ws_hdr* hdr;
+};
+
+struct cc_log_dev {
+    u8* buf;
+    u64 capacity;
+    u64 W;                  // running write offset (device-resident so that async calls chain)
+    u64* committed_off;     // host-visible published offset (may be null)
+};
+
+// Applier tables (in the attached scratch).
+struct cc_rec {             // 32 bytes
+    u64 off;                // offset of the record header in the log
+    u32 page_idx;
+    u32 len;
+    u32 crc;
+    u32 slot;               // region slot
+    u32 epoch_idx;
+    u32 pad;
+};
+struct cc_epoch_ent {       // 16 bytes
+    u64 off_after;
+    u32 rec_end;            // records [.., rec_end) belong to epochs <= this one
+    u32 pad;
+};
+struct cc_apply_state {
+    u32 n_recs;
+    u32 n_epochs;
+    u32 struct_fail;        // 1 if the parse stopped on a failed structural check
+    u32 scratch_overflow;
+    u32 first_bad_rec;      // min index of a record failing CRC (init 0xFFFFFFFF)
+    u32 validate_done;
+    u32 n_commit_recs;      // records in applied epochs
+    u32 n_commit_epochs;
+    u64 consumed;
+    u64 t_start_ns;
+    int32_t status;
+    u32 final_done;
+};
+
+struct cc_crc_tables {
+    u32 t0[256];            // byte table of the reflected polynomial
+    u32 s512[4][256];       // multiply by x^(8*512) mod G, one table per register byte
+    u32 lane_mul[32];       // x^(8*16*(31-lane))
+    u32 seg_mul[65];        // x^(8*4096*m), m = 0..64
+    u32 xp[48];             // x^(8*2^j), j = 0..47
+};
+
+struct cc_dev {
+    cc_region_dev regions[CC_MAX_REGIONS];
+    u32 region_used[CC_MAX_REGIONS];
+    cc_log_dev log;
+    cc_crc_tables crc;
+    // applier
+    cc_rec* recs;
+    cc_epoch_ent* epochs;
+    u64 max_records;
+    cc_apply_state apply;
+    // grid barrier + worker doorbell
+    u32 bar_count;
+    u32 bar_gen;
+    u64 doorbell;
+    cc_task cur_task;
+    u32 worker_exit;
+};
+
+// ------------------------------------------------------------------ PTX helpers --
+
+__device__ __forceinline__ uint4 ld_stream(const uint4* p) {
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+// Plain (coherent) 16-byte load: log buffers may live in host memory and may have been
+// written by another kernel moments ago; no non-coherent path.
+__device__ __forceinline__ uint4 ld_v4(const uint4* p) {
+    uint4 r;
+    asm volatile("ld.global.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ void st_stream(uint4* p, const uint4& v) {
+    asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};"
+                 :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+__device__ __forceinline__ u64 globaltimer_ns() {
+    u64 t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ u64 ld_acquire_gpu_u64(const u64* p) {
+    u64 v;
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_gpu_u64(u64* p, u64 v) {
+    asm volatile("st.release.gpu.global.u64 [%0], %1;" :: "l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ u32 ld_acquire_gpu_u32(const u32* p) {
+    u32 v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ u64 ld_acquire_sys_u64(const u64* p) {
+    u64 v;
+    asm volatile("ld.acquire.sys.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_sys_u64(u64* p, u64 v) {
+    asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ u32 ld_relaxed_sys_u32(const u32* p) {
+    u32 v;
+    asm volatile("ld.relaxed.sys.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
+__device__ __forceinline__ u64 page_len_dev(const cc_region_dev& r, u64 p) {
+    u64 rest = r.bytes - p * (u64)r.page_bytes;
+    return rest < r.page_bytes ? rest : (u64)r.page_bytes;
+}
+
+// Virtual grid: the same device code runs as a host-launched kernel (blockIdx/gridDim) and
+// inside the persistent worker.
+struct cc_grid {
+    u32 block, nblocks;
+    __device__ __forceinline__ u32 warp() const { return block * (blockDim.x >> 5) + (threadIdx.x >> 5); }
+    __device__ __forceinline__ u32 nwarps() const { return nblocks * (blockDim.x >> 5); }
+};
+__device__ __forceinline__ cc_grid cc_hw_grid() { return cc_grid{blockIdx.x, gridDim.x}; }

@@ -1,0 +1,139 @@
+// cc_crc.cuh -- CRC32C (Castagnoli, reflected 0x82F63B78) for the CUDA path.
+//
+// A GPU has no CRC instruction, so a page's CRC is assembled from independent pieces using
+// the linearity of the CRC register over GF(2):
+//   raw(M, init)      = register after feeding M starting from init (no final XOR)
+//   raw(A||B, 0)      = raw(A, 0) * x^(8|B|)  XOR  raw(B, 0)          (mod G)
+//   raw(M, ~0)        = raw(M, 0) XOR (~0) * x^(8|M|)
+//   CRC32C(M)         = raw(M, ~0) XOR ~0
+// A warp handles one 4 KiB segment: lane l owns the 16-byte vectors l, l+32, ..., l+224.  It
+// runs the byte-table loop over each vector from 0 (8 independent chains -> ILP), folds them with
+// Horner steps of x^(8*512), multiplies by its lane constant x^(8*16*(31-l)), the warp XORs the
+// lanes together, and lane 0 multiplies by the segment constant x^(8*bytes after the segment).
+// The byte table is replicated per lane in shared memory (entry*32 + lane) so the random
+// lookups of the 32 lanes never collide on a bank.
+#pragma once
+#include "cc_common.cuh"
+
+#define CC_CRC_POLY 0x82F63B78u
+
+// ---- GF(2)[x] / G arithmetic in the reflected representation (bit 31 = x^0) ----
+__host__ __device__ __forceinline__ u32 gf_mulx(u32 b) { return (b >> 1) ^ ((b & 1u) ? CC_CRC_POLY : 0u); }
+
+__host__ __device__ inline u32 gf_mul(u32 a, u32 b) {
+    u32 p = 0;
+#pragma unroll 8
+    for (int i = 0; i < 32; i++) {
+        p ^= (a & (0x80000000u >> i)) ? b : 0u;
+        b = gf_mulx(b);
+    }
+    return p;
+}
+
+// x^(8*nbytes) using the table xp[j] = x^(8*2^j)
+__host__ __device__ inline u32 gf_xpow_bytes(const u32* xp, u64 nbytes) {
+    u32 r = 0x80000000u;
+    for (int j = 0; nbytes != 0 && j < 48; j++, nbytes >>= 1)
+        if (nbytes & 1) r = gf_mul(r, xp[j]);
+    return r;
+}
+
+// ---- host: build all constant tables ----
+static inline void cc_crc_build_tables(cc_crc_tables* t) {
+    for (u32 i = 0; i < 256; i++) {
+        u32 c = i;
+        for (int b = 0; b < 8; b++) c = gf_mulx(c);
+        t->t0[i] = c;
+    }
+    u32 x8 = 0x80000000u;
+    for (int b = 0; b < 8; b++) x8 = gf_mulx(x8);
+    t->xp[0] = x8;
+    for (int j = 1; j < 48; j++) t->xp[j] = gf_mul(t->xp[j - 1], t->xp[j - 1]);
+    u32 s512 = gf_xpow_bytes(t->xp, 512);
+    for (int b = 0; b < 4; b++)
+        for (u32 v = 0; v < 256; v++) t->s512[b][v] = gf_mul(v << (8 * b), s512);
+    for (u32 l = 0; l < 32; l++) t->lane_mul[l] = gf_xpow_bytes(t->xp, 16ull * (31 - l));
+    for (u32 m = 0; m <= 64; m++) t->seg_mul[m] = gf_xpow_bytes(t->xp, 4096ull * m);
+}
+
+// ---- device: shared-memory tables ----
+struct cc_crc_smem {
+    u32 t0[256 * 32];       // lane-replicated byte table: t0[entry*32 + lane]
+    u32 s512[4 * 256];
+};
+
+__device__ __forceinline__ void cc_crc_smem_init(cc_crc_smem* s, const cc_crc_tables* g) {
+    for (u32 i = threadIdx.x; i < 256 * 32; i += blockDim.x) s->t0[i] = g->t0[i >> 5];
+    for (u32 i = threadIdx.x; i < 4 * 256; i += blockDim.x) s->s512[i] = (&g->s512[0][0])[i];
+    __syncthreads();
+}
+
+// raw register update over one 32-bit word (4 bytes, memory order = little endian)
+__device__ __forceinline__ u32 crc_word(const u32* t0_lane, u32 crc, u32 w) {
+    crc ^= w;
+#pragma unroll
+    for (int i = 0; i < 4; i++) crc = t0_lane[(crc & 0xFFu) << 5] ^ (crc >> 8);
+    return crc;
+}
+
+__device__ __forceinline__ u32 crc_vec16(const u32* t0_lane, const uint4& v) {
+    u32 c = crc_word(t0_lane, 0u, v.x);
+    c = crc_word(t0_lane, c, v.y);
+    c = crc_word(t0_lane, c, v.z);
+    c = crc_word(t0_lane, c, v.w);
+    return c;
+}
+
+__device__ __forceinline__ u32 crc_shift512(const u32* s512, u32 v) {
+    return s512[v & 0xFFu] ^ s512[256 + ((v >> 8) & 0xFFu)] ^ s512[512 + ((v >> 16) & 0xFFu)] ^ s512[768 + (v >> 24)];
+}
+
+// Warp-level raw CRC contribution of one segment of nv (<= 256) 16-byte vectors held as
+// v[u] = vector (lane + 32u); `after` = bytes of the message that follow this segment.
+// Returns (in every lane) raw(segment, 0) * x^(8*after).
+template <int U>
+__device__ __forceinline__ u32 crc_segment_warp(const cc_crc_smem* s, const cc_crc_tables* g, const uint4 (&v)[U],
+                                                u32 nv, u64 after, u32 lane) {
+    const u32* t0_lane = s->t0 + lane;
+    u32 acc = 0;
+    u32 part[U];
+    if (nv == 32u * U) {
+#pragma unroll
+        for (int u = 0; u < U; u++) part[u] = crc_vec16(t0_lane, v[u]);     // independent chains
+#pragma unroll
+        for (int u = 0; u < U; u++) acc = (u ? crc_shift512(s->s512, acc) : 0u) ^ part[u];
+        acc = gf_mul(acc, g->lane_mul[lane]);
+    } else {
+        int last = -1;
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            if (lane + 32u * u < nv) {
+                acc = crc_shift512(s->s512, acc) ^ crc_vec16(t0_lane, v[u]);
+                last = u;
+            }
+        }
+        if (last >= 0) {
+            u32 j_last = lane + 32u * (u32)last;
+            acc = gf_mul(acc, gf_xpow_bytes(g->xp, 16ull * (nv - 1 - j_last)));
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc ^= __shfl_xor_sync(0xFFFFFFFFu, acc, o);
+    if (after != 0) {
+        u32 m = ((after & 4095u) == 0 && (after >> 12) <= 64) ? g->seg_mul[after >> 12] : gf_xpow_bytes(g->xp, after);
+        acc = gf_mul(acc, m);
+    }
+    return acc;
+}
+
+// Finalise: XOR of all segment contributions -> CRC32C of a len-byte message.
+__device__ __forceinline__ u32 crc_finalize(const cc_crc_tables* g, u32 acc, u64 len) {
+    return acc ^ gf_mul(0xFFFFFFFFu, gf_xpow_bytes(g->xp, len)) ^ 0xFFFFFFFFu;
+}
+
+// Serial CRC32C of a few bytes (commit payload), single thread, global table.
+__device__ inline u32 crc_serial(const cc_crc_tables* g, const u8* p, u32 n) {
+    u32 c = 0xFFFFFFFFu;
+    for (u32 i = 0; i < n; i++) c = g->t0[(c ^ p[i]) & 0xFFu] ^ (c >> 8);
+    return c ^ 0xFFFFFFFFu;
+}

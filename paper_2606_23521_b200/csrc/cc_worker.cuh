@@ -1,0 +1,184 @@
+// cc_worker.cuh -- a7: the persistent worker kernel and its host-mapped ring (PAPER.md:L119,
+// L139-160 dispatch loop, L247-249 host-mapped memory + release/acquire protocol).
+//
+// Differences from the paper's worker, and why:
+//   - many co-resident blocks (cooperative launch) instead of 1 block x 128 threads: one block
+//     cannot move HBM bandwidth; FIFO, one task at a time across the whole grid because
+//     checkpoint / restore order is semantic (reading #15);
+//   - block 0 / thread 0 is the only thread that touches host memory: it polls the tail word,
+//     copies the 64-byte descriptor to device memory and rings a device-memory doorbell that the
+//     other blocks spin on (L2-resident); task phases are separated by a grid barrier;
+//   - static switch instead of a JIT-filled function-pointer table.
+#pragma once
+#include "cc_common.cuh"
+#include "cc_ckpt.cuh"
+#include "cc_apply.cuh"
+
+struct cc_ring_dev {            // all pointers are pinned, device-mapped host memory
+    cc_task* slots;             // capacity x 64 B
+    cc_result* results;         // capacity x 64 B
+    u64* tail;                  // host -> device: tasks submitted (store-release by the host)
+    u64* completed;             // device -> host: tasks completed
+    u64* heartbeat;             // device -> host: %globaltimer of the last poll
+    u32 capacity;
+    u32 backoff_ns;
+    u64 max_lifetime_ns;
+};
+
+__device__ __forceinline__ void cc_grid_barrier(cc_dev* dev, u32 nblocks, u32& gen) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(&dev->bar_count, 1u) == nblocks - 1) {
+            atomicExch(&dev->bar_count, 0u);
+            __threadfence();
+            atomicAdd(&dev->bar_gen, 1u);
+        } else {
+            while (ld_acquire_gpu_u32(&dev->bar_gen) == gen) __nanosleep(40);
+        }
+        __threadfence();
+    }
+    gen++;
+    __syncthreads();
+}
+
+__device__ __forceinline__ void cc_task_mutate(const cc_region_dev& r, const cc_task& t, cc_grid g) {
+    const u64 n_mut = t.arg0, A = t.arg1, h = t.arg2;
+    for (u64 j = (u64)g.block * blockDim.x + threadIdx.x; j < n_mut; j += (u64)g.nblocks * blockDim.x) {
+        const u64 page = (j * A + h) % r.n_pages;
+        const u64 off = (h + j) % page_len_dev(r, page);
+        r.base[page * r.page_bytes + off] ^= 0x5A;
+    }
+}
+
+#define CC_WORKER_MAX_THREADS 512
+
+__global__ void __launch_bounds__(CC_WORKER_MAX_THREADS, 1)
+cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cc_crc_smem* cs = reinterpret_cast<cc_crc_smem*>(smem_raw);
+    __shared__ __align__(16) cc_task s_task;
+    const cc_grid g = cc_hw_grid();
+    u32 gen = ld_acquire_gpu_u32(&dev->bar_gen);
+    u64 head = 0;
+    const u64 t0 = globaltimer_ns();
+    cc_crc_smem_init(cs, &dev->crc);
+
+    for (;;) {
+        // ---- leader: poll the host-mapped tail, fetch the descriptor, ring the doorbell ----
+        if (g.block == 0 && threadIdx.x == 0) {
+            bool expired = false;
+            u32 spins = 0;
+            while (ld_acquire_sys_u64(ring.tail) <= head) {
+                const u64 now = globaltimer_ns();
+                if ((spins++ & 15u) == 0) *reinterpret_cast<volatile u64*>(ring.heartbeat) = now;
+                if (now - t0 > ring.max_lifetime_ns) { expired = true; break; }
+                __nanosleep(ring.backoff_ns);
+            }
+            cc_task t;
+            if (expired) {
+                t.kind = CC_TASK_EXIT; t.region_id = 0; t.flags = 1; t.version = 0; t.seq = ~0ull;
+                t.epoch = 0; t.arg0 = t.arg1 = t.arg2 = t.arg3 = 0;
+            } else {
+                const volatile uint4* src = reinterpret_cast<const volatile uint4*>(&ring.slots[head & (ring.capacity - 1)]);
+                uint4 q[4];
+#pragma unroll
+                for (int i = 0; i < 4; i++) { q[i].x = src[i].x; q[i].y = src[i].y; q[i].z = src[i].z; q[i].w = src[i].w; }
+                t = *reinterpret_cast<cc_task*>(q);
+            }
+            dev->cur_task = t;
+            __threadfence();
+            st_release_gpu_u64(&dev->doorbell, head + 1);
+        }
+        // ---- everyone: wait for the doorbell ----
+        if (threadIdx.x == 0) {
+            while (ld_acquire_gpu_u64(&dev->doorbell) <= head) __nanosleep(ring.backoff_ns);
+            __threadfence();
+            const uint4* ct = reinterpret_cast<const uint4*>(&dev->cur_task);
+            uint4* st = reinterpret_cast<uint4*>(&s_task);
+#pragma unroll
+            for (int i = 0; i < 4; i++) st[i] = __ldcg(ct + i);
+        }
+        __syncthreads();
+        const cc_task task = s_task;
+        const u64 t_start = globaltimer_ns();
+        if (task.kind == CC_TASK_EXIT) break;
+
+        int32_t status = CC_OK;
+        int slot = -1;
+        if (task.kind == CC_TASK_DELTA_CKPT || task.kind == CC_TASK_TEST_MUTATE) {
+            slot = cc_find_slot(dev, task.region_id);
+            if (slot < 0) status = CC_ERR_NOT_REGISTERED;
+        }
+        if (status == CC_OK) {
+            switch (task.kind) {
+            case CC_TASK_DELTA_CKPT: {
+                const cc_region_dev& r = dev->regions[slot];
+                cc_scan_phase<8>(r, g);
+                cc_grid_barrier(dev, g.nblocks, gen);
+                cc_compact_phase(r, &dev->log, CC_MODE_CHECKPOINT, task.epoch, nullptr);
+                cc_grid_barrier(dev, g.nblocks, gen);
+                cc_gather_phase(r, dev, cs, g, nullptr, task.kind, false);
+                break;
+            }
+            case CC_TASK_RESTORE: {
+                const u8* log = reinterpret_cast<const u8*>(task.arg0);
+                if (g.block == 0) cc_apply_parse_phase(dev, tabs, log, task.arg1);
+                cc_grid_barrier(dev, g.nblocks, gen);
+                cc_apply_validate_phase(dev, tabs, cs, log, g, false);
+                cc_grid_barrier(dev, g.nblocks, gen);
+                cc_apply_latest_phase(dev, tabs, g);
+                cc_grid_barrier(dev, g.nblocks, gen);
+                cc_apply_scatter_phase(dev, tabs, log, g);
+                cc_grid_barrier(dev, g.nblocks, gen);
+                cc_apply_cleanup_phase(dev, tabs, g, nullptr, task.kind);
+                break;
+            }
+            case CC_TASK_TEST_MUTATE:
+                cc_task_mutate(dev->regions[slot], task, g);
+                break;
+            case CC_TASK_LOG_RESET:
+                if (g.block == 0 && threadIdx.x == 0) {
+                    dev->log.W = 0;
+                    if (dev->log.committed_off) st_release_sys_u64(dev->log.committed_off, 0ull);
+                }
+                break;
+            default:
+                break;
+            }
+        }
+        // ---- end of task: everyone done, leader publishes the completion ----
+        cc_grid_barrier(dev, g.nblocks, gen);
+        if (g.block == 0 && threadIdx.x == 0) {
+            cc_result* out = &ring.results[task.seq & (ring.capacity - 1)];
+            u64 n_dirty = 0, bytes = 0, off_after = dev->log.W, ep = task.epoch;
+            if (status == CC_OK && task.kind == CC_TASK_DELTA_CKPT) {
+                const cc_ws_hdr* h = dev->regions[slot].hdr;
+                n_dirty = h->k; bytes = h->need; status = h->status;
+            } else if (status == CC_OK && task.kind == CC_TASK_RESTORE) {
+                const cc_apply_state* A = &dev->apply;
+                n_dirty = A->n_commit_recs; bytes = A->consumed; off_after = A->consumed;
+                ep = A->n_commit_epochs; status = A->status;
+            }
+            out->n_dirty = n_dirty; out->bytes = bytes; out->log_offset_after = off_after; out->epoch = ep;
+            out->status = status; out->flags = task.kind;
+            out->t_start_ns = t_start; out->t_end_ns = globaltimer_ns();
+            __threadfence_system();
+            st_release_sys_u64(&out->seq_done, task.seq + 1);
+            st_release_sys_u64(ring.completed, task.seq + 1);
+        }
+        head++;
+    }
+    // exit: the leader acknowledges the EXIT task (if it came from the host) and stamps the heartbeat
+    if (g.block == 0 && threadIdx.x == 0) {
+        const cc_task t = s_task;
+        if (t.seq != ~0ull) {
+            cc_result* out = &ring.results[t.seq & (ring.capacity - 1)];
+            out->n_dirty = 0; out->bytes = 0; out->log_offset_after = dev->log.W; out->epoch = 0;
+            out->status = CC_OK; out->flags = CC_TASK_EXIT; out->t_start_ns = globaltimer_ns(); out->t_end_ns = out->t_start_ns;
+            __threadfence_system();
+            st_release_sys_u64(&out->seq_done, t.seq + 1);
+            st_release_sys_u64(ring.completed, t.seq + 1);
+        }
+    }
+}

@@ -1,0 +1,544 @@
+// concordia.cu -- libconcordia.so: kernels (thin __global__ wrappers over the device phases)
+// and the C ABI of include/concordia.h.  sm_100a only.  No CPU fallback: every step of the path
+// runs in the kernels below; the host code only validates arguments, keeps the region table and
+// launches.
+#include <atomic>
+#include <chrono>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "cc_common.cuh"
+#include "cc_crc.cuh"
+#include "cc_ckpt.cuh"
+#include "cc_apply.cuh"
+#include "cc_worker.cuh"
+
+static_assert(sizeof(cc_result) == 64, "cc_result must be 64 bytes");
+static_assert(sizeof(cc_task) == 64, "cc_task must be 64 bytes");
+static_assert(sizeof(cc_rec) == 32, "cc_rec must be 32 bytes");
+
+// ------------------------------------------------------------------------ kernels --
+
+#define CC_SCAN_THREADS 256
+#define CC_GATHER_THREADS 256
+#define CC_APPLY_THREADS 256
+#define CC_PARSE_THREADS 1024
+
+__global__ void __launch_bounds__(CC_SCAN_THREADS) cc_scan_kernel(const cc_dev* dev, int slot) {
+    cc_scan_phase<8>(dev->regions[slot], cc_hw_grid());
+}
+
+__global__ void __launch_bounds__(CC_COMPACT_THREADS) cc_compact_kernel(cc_dev* dev, int slot, u32 mode, u64 epoch,
+                                                                        cc_result* out) {
+    cc_compact_phase(dev->regions[slot], &dev->log, mode, epoch, out);
+}
+
+__global__ void __launch_bounds__(CC_GATHER_THREADS) cc_gather_kernel(cc_dev* dev, int slot, cc_result* out) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cc_gather_phase(dev->regions[slot], dev, reinterpret_cast<cc_crc_smem*>(smem_raw), cc_hw_grid(), out,
+                    CC_TASK_DELTA_CKPT, true);
+}
+
+__global__ void __launch_bounds__(CC_PARSE_THREADS) cc_apply_parse_kernel(cc_dev* dev, cc_apply_tabs tabs, const u8* log, u64 n) {
+    cc_apply_parse_phase(dev, tabs, log, n);
+}
+
+__global__ void __launch_bounds__(CC_APPLY_THREADS) cc_apply_validate_kernel(cc_dev* dev, cc_apply_tabs tabs, const u8* log) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cc_apply_validate_phase(dev, tabs, reinterpret_cast<cc_crc_smem*>(smem_raw), log, cc_hw_grid(), true);
+}
+
+__global__ void __launch_bounds__(CC_APPLY_THREADS) cc_apply_latest_kernel(cc_dev* dev, cc_apply_tabs tabs) {
+    cc_apply_latest_phase(dev, tabs, cc_hw_grid());
+}
+
+__global__ void __launch_bounds__(CC_APPLY_THREADS) cc_apply_scatter_kernel(cc_dev* dev, cc_apply_tabs tabs, const u8* log) {
+    cc_apply_scatter_phase(dev, tabs, log, cc_hw_grid());
+}
+
+__global__ void __launch_bounds__(CC_APPLY_THREADS) cc_apply_cleanup_kernel(cc_dev* dev, cc_apply_tabs tabs, cc_result* out) {
+    cc_apply_cleanup_phase(dev, tabs, cc_hw_grid(), out, CC_TASK_RESTORE);
+}
+
+// --------------------------------------------------------------------- host context --
+
+struct cc_host_region {
+    bool used;
+    cc_region_desc desc;
+    cc_region_dev dev;
+};
+
+struct cc_ctx {
+    int device;
+    cc_config cfg;
+    int sm_count;
+    cc_dev* d_dev;
+    cudaStream_t internal;
+    cc_host_region regions[CC_MAX_REGIONS];
+    bool log_attached;
+    cc_apply_tabs tabs;
+    bool apply_attached;
+    int last_cuda;
+    uint64_t launches;
+    int scan_bps, gather_bps, validate_bps;     // blocks per SM from the occupancy API
+    // ring + worker (pinned host)
+    cc_task* ring_slots;
+    cc_result* ring_results;
+    u64* ring_words;            // [0] tail, [8] completed, [16] heartbeat (one cache line apart)
+    u64 submitted;
+    bool worker_running;
+    cudaStream_t worker_stream;
+    cudaEvent_t worker_done;
+    u32 worker_blocks_used;
+};
+
+#define CC_CUDA(ctx, call)                                     \
+    do {                                                       \
+        cudaError_t e__ = (call);                              \
+        if (e__ != cudaSuccess) {                              \
+            (ctx)->last_cuda = (int)e__;                       \
+            return CC_ERR_CUDA;                                \
+        }                                                      \
+    } while (0)
+
+static inline uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
+
+static int find_slot(cc_ctx* ctx, uint32_t id) {
+    for (int s = 0; s < CC_MAX_REGIONS; s++)
+        if (ctx->regions[s].used && ctx->regions[s].desc.region_id == id) return s;
+    return -1;
+}
+
+struct cc_ws_layout {
+    uint64_t hdr, bitmap, D, rec_crc, rec_done, latest, lb, total;
+    uint64_t n_pages, n_words, n_tiles;
+};
+
+static bool ws_layout(uint64_t bytes, uint32_t P, cc_ws_layout* L) {
+    if (P == 0 || (P & 15u) || bytes == 0 || (bytes & 15ull)) return false;
+    uint64_t n_pages = (bytes + P - 1) / P;
+    if (n_pages > (1ull << 31)) return false;
+    L->n_pages = n_pages;
+    L->n_words = (n_pages + 31) / 32;
+    L->n_tiles = (L->n_words + CC_COMPACT_TILE_WORDS - 1) / CC_COMPACT_TILE_WORDS;
+    uint64_t o = 0;
+    L->hdr = o; o += 256;
+    L->bitmap = o; o += align_up(L->n_tiles * CC_COMPACT_TILE_WORDS * 4, 256);
+    L->D = o; o += align_up(n_pages * 4, 256);
+    L->rec_crc = o; o += align_up(n_pages * 4, 256);
+    L->rec_done = o; o += align_up(n_pages * 4, 256);
+    L->latest = o; o += align_up(n_pages * 4, 256);
+    L->lb = o; o += align_up(L->n_tiles * 8, 256);
+    L->total = o;
+    return true;
+}
+
+// ------------------------------------------------------------------------ lifecycle --
+
+extern "C" int32_t cc_init(cc_ctx** out, int32_t device, const cc_config* cfg) {
+    if (!out) return CC_ERR_INVALID;
+    *out = nullptr;
+    cc_ctx* ctx = new (std::nothrow) cc_ctx();
+    if (!ctx) return CC_ERR_INVALID;
+    memset(ctx, 0, sizeof(*ctx));
+    ctx->device = device;
+    if (cfg) ctx->cfg = *cfg;
+    if (ctx->cfg.ring_capacity == 0) ctx->cfg.ring_capacity = 256;
+    if (ctx->cfg.worker_threads == 0) ctx->cfg.worker_threads = CC_WORKER_MAX_THREADS;
+    if (ctx->cfg.backoff_ns == 0) ctx->cfg.backoff_ns = 500;
+    if (ctx->cfg.max_lifetime_ns == 0) ctx->cfg.max_lifetime_ns = 600ull * 1000000000ull;
+    const uint32_t cap = ctx->cfg.ring_capacity;
+    if ((cap & (cap - 1)) || ctx->cfg.worker_threads > CC_WORKER_MAX_THREADS || (ctx->cfg.worker_threads & 31u) ||
+        ctx->cfg.worker_threads < CC_COMPACT_THREADS) {
+        delete ctx;
+        return CC_ERR_INVALID;
+    }
+    cudaError_t e = cudaSetDevice(device);
+    cudaDeviceProp prop;
+    if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, device);
+    if (e == cudaSuccess && prop.major < 10) e = cudaErrorNoKernelImageForDevice;   // sm_100a code only
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->d_dev, sizeof(cc_dev));
+    if (e != cudaSuccess) {
+        fprintf(stderr, "libconcordia: cc_init failed: %s (no CPU fallback exists)\n", cudaGetErrorString(e));
+        delete ctx;
+        return CC_ERR_CUDA;
+    }
+    ctx->sm_count = prop.multiProcessorCount;
+    cc_dev* h = (cc_dev*)calloc(1, sizeof(cc_dev));
+    cc_crc_build_tables(&h->crc);
+    e = cudaMemcpy(ctx->d_dev, h, sizeof(cc_dev), cudaMemcpyHostToDevice);
+    free(h);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->internal, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->worker_stream, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->worker_done, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->scan_bps, cc_scan_kernel, CC_SCAN_THREADS, 0);
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->gather_bps, cc_gather_kernel, CC_GATHER_THREADS, sizeof(cc_crc_smem));
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->validate_bps, cc_apply_validate_kernel, CC_APPLY_THREADS, sizeof(cc_crc_smem));
+    // ring + completion slots + control words: pinned, device-mapped host memory
+    if (e == cudaSuccess) e = cudaHostAlloc((void**)&ctx->ring_slots, (size_t)cap * sizeof(cc_task), cudaHostAllocMapped | cudaHostAllocPortable);
+    if (e == cudaSuccess) e = cudaHostAlloc((void**)&ctx->ring_results, (size_t)cap * sizeof(cc_result), cudaHostAllocMapped | cudaHostAllocPortable);
+    if (e == cudaSuccess) e = cudaHostAlloc((void**)&ctx->ring_words, 256, cudaHostAllocMapped | cudaHostAllocPortable);
+    if (e != cudaSuccess) {
+        fprintf(stderr, "libconcordia: cc_init failed: %s\n", cudaGetErrorString(e));
+        ctx->last_cuda = (int)e;
+        cc_shutdown(ctx);
+        return CC_ERR_CUDA;
+    }
+    memset(ctx->ring_slots, 0, (size_t)cap * sizeof(cc_task));
+    memset(ctx->ring_results, 0, (size_t)cap * sizeof(cc_result));
+    memset(ctx->ring_words, 0, 256);
+    if (ctx->scan_bps < 1) ctx->scan_bps = 1;
+    if (ctx->gather_bps < 1) ctx->gather_bps = 1;
+    if (ctx->validate_bps < 1) ctx->validate_bps = 1;
+    *out = ctx;
+    return CC_OK;
+}
+
+extern "C" int32_t cc_shutdown(cc_ctx* ctx) {
+    if (!ctx) return CC_ERR_INVALID;
+    cudaSetDevice(ctx->device);
+    int32_t rc = CC_OK;
+    if (ctx->worker_running) rc = cc_worker_stop(ctx);
+    if (rc == CC_OK) {   // never free under a resident kernel
+        if (ctx->d_dev) cudaFree(ctx->d_dev);
+        if (ctx->ring_slots) cudaFreeHost(ctx->ring_slots);
+        if (ctx->ring_results) cudaFreeHost(ctx->ring_results);
+        if (ctx->ring_words) cudaFreeHost(ctx->ring_words);
+        if (ctx->internal) cudaStreamDestroy(ctx->internal);
+        if (ctx->worker_stream) cudaStreamDestroy(ctx->worker_stream);
+        if (ctx->worker_done) cudaEventDestroy(ctx->worker_done);
+    }
+    delete ctx;
+    return rc;
+}
+
+extern "C" int32_t cc_last_cuda_error(cc_ctx* ctx) { return ctx ? ctx->last_cuda : 0; }
+extern "C" uint64_t cc_kernel_launches(cc_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+// -------------------------------------------------------------------------- regions --
+
+extern "C" uint64_t cc_workspace_bytes(uint64_t bytes, uint32_t page_bytes) {
+    cc_ws_layout L;
+    return ws_layout(bytes, page_bytes, &L) ? L.total : 0;
+}
+
+extern "C" int32_t cc_register_region(cc_ctx* ctx, const cc_region_desc* d) {
+    if (!ctx || !d) return CC_ERR_INVALID;
+    if (ctx->worker_running) return CC_ERR_WORKER;
+    cc_ws_layout L;
+    if (d->region_id == 0 || d->region_id == CC_COMMIT_ID || !ws_layout(d->bytes, d->page_bytes, &L)) return CC_ERR_INVALID;
+    if (!d->base || !d->shadow || !d->workspace || ((uintptr_t)d->base & 15) || ((uintptr_t)d->shadow & 15) ||
+        ((uintptr_t)d->workspace & 255) || d->workspace_bytes < L.total)
+        return CC_ERR_INVALID;
+    if (find_slot(ctx, d->region_id) >= 0) return CC_ERR_EXISTS;
+    int slot = -1;
+    for (int s = 0; s < CC_MAX_REGIONS; s++)
+        if (!ctx->regions[s].used) { slot = s; break; }
+    if (slot < 0) return CC_ERR_INVALID;
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    // Legacy default stream: ordered after whatever the caller queued on blocking streams.
+    CC_CUDA(ctx, cudaMemsetAsync(d->workspace, 0, L.total, 0));
+    if (d->flags & CC_REG_SNAPSHOT_NOW) CC_CUDA(ctx, cudaMemcpyAsync(d->shadow, d->base, d->bytes, cudaMemcpyDeviceToDevice, 0));
+    cc_region_dev r;
+    memset(&r, 0, sizeof(r));
+    u8* ws = (u8*)d->workspace;
+    r.base = (u8*)d->base;
+    r.shadow = (u8*)d->shadow;
+    r.bytes = d->bytes;
+    r.n_pages = L.n_pages;
+    r.page_bytes = d->page_bytes;
+    r.region_id = d->region_id;
+    r.spp = (d->page_bytes + CC_SEG_BYTES - 1) / CC_SEG_BYTES;
+    r.spp_shift = -1;
+    if ((r.spp & (r.spp - 1)) == 0) { r.spp_shift = 0; while ((1u << r.spp_shift) < r.spp) r.spp_shift++; }
+    r.n_words = L.n_words;
+    r.hdr = (cc_ws_hdr*)(ws + L.hdr);
+    r.bitmap = (u32*)(ws + L.bitmap);
+    r.D = (u32*)(ws + L.D);
+    r.rec_crc = (u32*)(ws + L.rec_crc);
+    r.rec_done = (u32*)(ws + L.rec_done);
+    r.latest = (u32*)(ws + L.latest);
+    r.lb_status = (u64*)(ws + L.lb);
+    const u32 one = 1;
+    CC_CUDA(ctx, cudaMemcpyAsync(&ctx->d_dev->regions[slot], &r, sizeof(r), cudaMemcpyHostToDevice, 0));
+    CC_CUDA(ctx, cudaMemcpyAsync(&ctx->d_dev->region_used[slot], &one, sizeof(one), cudaMemcpyHostToDevice, 0));
+    CC_CUDA(ctx, cudaStreamSynchronize(0));
+    ctx->regions[slot].used = true;
+    ctx->regions[slot].desc = *d;
+    ctx->regions[slot].dev = r;
+    return CC_OK;
+}
+
+extern "C" int32_t cc_unregister_region(cc_ctx* ctx, uint32_t region_id) {
+    if (!ctx) return CC_ERR_INVALID;
+    if (ctx->worker_running) return CC_ERR_WORKER;
+    int slot = find_slot(ctx, region_id);
+    if (slot < 0) return CC_ERR_NOT_REGISTERED;
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    const u32 zero = 0;
+    CC_CUDA(ctx, cudaMemcpyAsync(&ctx->d_dev->region_used[slot], &zero, sizeof(zero), cudaMemcpyHostToDevice, 0));
+    CC_CUDA(ctx, cudaStreamSynchronize(0));
+    ctx->regions[slot].used = false;
+    return CC_OK;
+}
+
+// ------------------------------------------------------------------------------ log --
+
+extern "C" int32_t cc_log_attach(cc_ctx* ctx, void* log_buf, uint64_t capacity, uint64_t* committed_off) {
+    if (!ctx || !log_buf || ((uintptr_t)log_buf & 15) || capacity < CC_COMMIT_RECORD_BYTES) return CC_ERR_INVALID;
+    if (ctx->worker_running) return CC_ERR_WORKER;
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    cc_log_dev l;
+    l.buf = (u8*)log_buf;
+    l.capacity = capacity;
+    l.W = 0;
+    l.committed_off = committed_off;
+    CC_CUDA(ctx, cudaMemcpyAsync(&ctx->d_dev->log, &l, sizeof(l), cudaMemcpyHostToDevice, 0));
+    CC_CUDA(ctx, cudaStreamSynchronize(0));
+    ctx->log_attached = true;
+    return CC_OK;
+}
+
+extern "C" int32_t cc_log_reset(cc_ctx* ctx) {
+    if (!ctx || !ctx->log_attached) return CC_ERR_INVALID;
+    if (ctx->worker_running) return CC_ERR_WORKER;
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    const u64 zero = 0;
+    CC_CUDA(ctx, cudaMemcpyAsync(&ctx->d_dev->log.W, &zero, sizeof(zero), cudaMemcpyHostToDevice, 0));
+    CC_CUDA(ctx, cudaStreamSynchronize(0));
+    return CC_OK;
+}
+
+// ------------------------------------------------------------- host-launched path --
+
+static int32_t launch_scan_compact(cc_ctx* ctx, int slot, u32 mode, uint64_t epoch, cudaStream_t st, cc_result* out) {
+    const cc_region_dev& r = ctx->regions[slot].dev;
+    const uint64_t n_items = r.n_pages * (uint64_t)r.spp;
+    const uint64_t wpb = CC_SCAN_THREADS / 32;
+    uint64_t g1 = (n_items + wpb - 1) / wpb;
+    const uint64_t cap1 = (uint64_t)ctx->sm_count * ctx->scan_bps;
+    if (g1 > cap1) g1 = cap1;
+    cc_scan_kernel<<<(unsigned)g1, CC_SCAN_THREADS, 0, st>>>(ctx->d_dev, slot);
+    const uint64_t n_tiles = (r.n_words + CC_COMPACT_TILE_WORDS - 1) / CC_COMPACT_TILE_WORDS;
+    uint64_t g2 = n_tiles < (uint64_t)ctx->sm_count * 4 ? n_tiles : (uint64_t)ctx->sm_count * 4;
+    cc_compact_kernel<<<(unsigned)g2, CC_COMPACT_THREADS, 0, st>>>(ctx->d_dev, slot, mode, epoch, out);
+    ctx->launches += 2;
+    CC_CUDA(ctx, cudaGetLastError());
+    return CC_OK;
+}
+
+extern "C" int32_t cc_checkpoint_delta(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out) {
+    if (!ctx) return CC_ERR_INVALID;
+    int slot = find_slot(ctx, region_id);
+    if (slot < 0) return CC_ERR_NOT_REGISTERED;
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    int32_t rc = launch_scan_compact(ctx, slot, CC_MODE_CHECKPOINT, epoch, st, nullptr);
+    if (rc != CC_OK) return rc;
+    const unsigned g3 = (unsigned)(ctx->sm_count * ctx->gather_bps);
+    cc_gather_kernel<<<g3, CC_GATHER_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, slot, out);
+    ctx->launches += 1;
+    CC_CUDA(ctx, cudaGetLastError());
+    return CC_OK;
+}
+
+extern "C" int32_t cc_scan_only(cc_ctx* ctx, uint32_t region_id, void* stream, cc_result* out) {
+    if (!ctx) return CC_ERR_INVALID;
+    int slot = find_slot(ctx, region_id);
+    if (slot < 0) return CC_ERR_NOT_REGISTERED;
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    return launch_scan_compact(ctx, slot, CC_MODE_SCAN_ONLY, 0, (cudaStream_t)stream, out);
+}
+
+extern "C" int32_t cc_dirty_list(cc_ctx* ctx, uint32_t region_id, const uint32_t** d_list, const uint32_t** d_count) {
+    if (!ctx) return CC_ERR_INVALID;
+    int slot = find_slot(ctx, region_id);
+    if (slot < 0) return CC_ERR_NOT_REGISTERED;
+    if (d_list) *d_list = ctx->regions[slot].dev.D;
+    if (d_count) *d_count = &ctx->regions[slot].dev.hdr->k;
+    return CC_OK;
+}
+
+extern "C" uint64_t cc_apply_scratch_bytes(uint64_t max_records) {
+    if (max_records == 0 || max_records > 0xFFFFFFF0ull) return 0;
+    return align_up(max_records * sizeof(cc_rec), 256) + align_up(max_records * sizeof(cc_epoch_ent), 256) +
+           2 * align_up(max_records * 4, 256) + align_up((max_records + 1) * 4, 256);
+}
+
+extern "C" int32_t cc_apply_attach(cc_ctx* ctx, void* scratch, uint64_t scratch_bytes) {
+    if (!ctx || !scratch || ((uintptr_t)scratch & 255)) return CC_ERR_INVALID;
+    if (ctx->worker_running) return CC_ERR_WORKER;
+    // largest max_records whose tables fit
+    uint64_t lo = 0, hi = scratch_bytes / 32 + 1;
+    while (lo + 1 < hi) {
+        uint64_t mid = (lo + hi) / 2;
+        uint64_t need = cc_apply_scratch_bytes(mid);
+        if (need != 0 && need <= scratch_bytes) lo = mid; else hi = mid;
+    }
+    if (lo == 0) return CC_ERR_INVALID;
+    const uint64_t m = lo;
+    u8* p = (u8*)scratch;
+    cc_apply_tabs T;
+    T.max_records = m;
+    T.recs = (cc_rec*)p; p += align_up(m * sizeof(cc_rec), 256);
+    T.epochs = (cc_epoch_ent*)p; p += align_up(m * sizeof(cc_epoch_ent), 256);
+    T.rec_acc = (u32*)p; p += align_up(m * 4, 256);
+    T.rec_cnt = (u32*)p; p += align_up(m * 4, 256);
+    T.seg_begin = (u32*)p;
+    ctx->tabs = T;
+    ctx->apply_attached = true;
+    return CC_OK;
+}
+
+extern "C" int32_t cc_apply_log(cc_ctx* ctx, const void* log, uint64_t nbytes, void* stream, cc_result* out) {
+    if (!ctx || !log || ((uintptr_t)log & 15)) return CC_ERR_INVALID;
+    if (!ctx->apply_attached) return CC_ERR_INVALID;
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    const u8* lg = (const u8*)log;
+    const unsigned gv = (unsigned)(ctx->sm_count * ctx->validate_bps);
+    const unsigned gs = (unsigned)(ctx->sm_count * 8);
+    cc_apply_parse_kernel<<<1, CC_PARSE_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, lg, nbytes);
+    cc_apply_validate_kernel<<<gv, CC_APPLY_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, ctx->tabs, lg);
+    cc_apply_latest_kernel<<<(unsigned)ctx->sm_count, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs);
+    cc_apply_scatter_kernel<<<gs, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, lg);
+    cc_apply_cleanup_kernel<<<(unsigned)ctx->sm_count, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, out);
+    ctx->launches += 5;
+    CC_CUDA(ctx, cudaGetLastError());
+    return CC_OK;
+}
+
+// ---------------------------------------------------------- ring + persistent worker --
+
+static inline u64 now_ns() {
+    return (u64)std::chrono::duration_cast<std::chrono::nanoseconds>(std::chrono::steady_clock::now().time_since_epoch()).count();
+}
+static inline volatile u64* ring_tail(cc_ctx* c) { return c->ring_words + 0; }
+static inline volatile u64* ring_completed(cc_ctx* c) { return c->ring_words + 8; }
+static inline volatile u64* ring_heartbeat(cc_ctx* c) { return c->ring_words + 16; }
+
+extern "C" int32_t cc_worker_start(cc_ctx* ctx) {
+    if (!ctx) return CC_ERR_INVALID;
+    if (ctx->worker_running) return CC_ERR_WORKER;
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    int coop = 0;
+    CC_CUDA(ctx, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, ctx->device));
+    if (!coop) return CC_ERR_WORKER;
+    const int threads = (int)ctx->cfg.worker_threads;
+    int bps = 0;
+    CC_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, cc_worker_kernel, threads, sizeof(cc_crc_smem)));
+    if (bps < 1) return CC_ERR_WORKER;
+    uint32_t blocks = ctx->cfg.worker_blocks ? ctx->cfg.worker_blocks : (uint32_t)(bps * ctx->sm_count);
+    if (blocks > (uint32_t)(bps * ctx->sm_count)) return CC_ERR_INVALID;   // must all be co-resident (grid barrier)
+    // reset barrier / doorbell state and the host-side ring words
+    struct { u32 bar_count, bar_gen; u64 doorbell; } z = {0, 0, 0};
+    CC_CUDA(ctx, cudaMemcpyAsync(&ctx->d_dev->bar_count, &z.bar_count, 4, cudaMemcpyHostToDevice, 0));
+    CC_CUDA(ctx, cudaMemcpyAsync(&ctx->d_dev->bar_gen, &z.bar_gen, 4, cudaMemcpyHostToDevice, 0));
+    CC_CUDA(ctx, cudaMemcpyAsync(&ctx->d_dev->doorbell, &z.doorbell, 8, cudaMemcpyHostToDevice, 0));
+    CC_CUDA(ctx, cudaStreamSynchronize(0));
+    memset(ctx->ring_results, 0, (size_t)ctx->cfg.ring_capacity * sizeof(cc_result));
+    *ring_tail(ctx) = 0;
+    *ring_completed(ctx) = 0;
+    *ring_heartbeat(ctx) = 0;
+    ctx->submitted = 0;
+    std::atomic_thread_fence(std::memory_order_seq_cst);
+    cc_ring_dev ring;
+    ring.slots = ctx->ring_slots;
+    ring.results = ctx->ring_results;
+    ring.tail = (u64*)ring_tail(ctx);
+    ring.completed = (u64*)ring_completed(ctx);
+    ring.heartbeat = (u64*)ring_heartbeat(ctx);
+    ring.capacity = ctx->cfg.ring_capacity;
+    ring.backoff_ns = ctx->cfg.backoff_ns;
+    ring.max_lifetime_ns = ctx->cfg.max_lifetime_ns;
+    cc_dev* d = ctx->d_dev;
+    cc_apply_tabs tabs = ctx->tabs;
+    if (!ctx->apply_attached) memset(&tabs, 0, sizeof(tabs));
+    void* args[] = {&d, &ring, &tabs};
+    CC_CUDA(ctx, cudaLaunchCooperativeKernel((const void*)cc_worker_kernel, dim3(blocks), dim3(threads), args,
+                                             sizeof(cc_crc_smem), ctx->worker_stream));
+    CC_CUDA(ctx, cudaEventRecord(ctx->worker_done, ctx->worker_stream));
+    ctx->launches += 1;
+    ctx->worker_running = true;
+    ctx->worker_blocks_used = blocks;
+    return CC_OK;
+}
+
+extern "C" int32_t cc_submit(cc_ctx* ctx, const cc_task* task, uint64_t* seq_out) {
+    if (!ctx || !task) return CC_ERR_INVALID;
+    if (!ctx->worker_running) return CC_ERR_WORKER;
+    const u64 seq = ctx->submitted;
+    const u64 done = __atomic_load_n(ctx->ring_words + 8, __ATOMIC_ACQUIRE);
+    if (seq - done >= ctx->cfg.ring_capacity) return CC_ERR_RING_FULL;
+    cc_task* slot = &ctx->ring_slots[seq & (ctx->cfg.ring_capacity - 1)];
+    cc_task t = *task;
+    t.seq = seq;
+    memcpy(slot, &t, sizeof(t));                                         // write(slot, desc)
+    __atomic_store_n(ctx->ring_words + 0, seq + 1, __ATOMIC_RELEASE);    // commit(slot): store-release
+    ctx->submitted = seq + 1;
+    if (seq_out) *seq_out = seq;
+    return CC_OK;
+}
+
+extern "C" int32_t cc_poll(cc_ctx* ctx, uint64_t seq, cc_result* out) {
+    if (!ctx) return CC_ERR_INVALID;
+    if (seq >= ctx->submitted) return CC_ERR_INVALID;
+    cc_result* r = &ctx->ring_results[seq & (ctx->cfg.ring_capacity - 1)];
+    const u64 sd = __atomic_load_n(&r->seq_done, __ATOMIC_ACQUIRE);
+    if (sd != seq + 1) return sd > seq + 1 ? CC_ERR_INVALID : CC_PENDING;   // slot already reused: too late
+    if (out) memcpy(out, r, sizeof(*r));
+    return CC_OK;
+}
+
+extern "C" int32_t cc_wait(cc_ctx* ctx, uint64_t seq, uint64_t timeout_ns, cc_result* out) {
+    const u64 t0 = now_ns();
+    for (;;) {
+        int32_t rc = cc_poll(ctx, seq, out);
+        if (rc != CC_PENDING) return rc;
+        if (now_ns() - t0 > timeout_ns) return CC_ERR_TIMEOUT;
+#if defined(__x86_64__)
+        __builtin_ia32_pause();
+#endif
+    }
+}
+
+extern "C" int32_t cc_peek_queue(cc_ctx* ctx, uint64_t* head, uint64_t* tail) {
+    if (!ctx) return CC_ERR_INVALID;
+    if (head) *head = __atomic_load_n(ctx->ring_words + 8, __ATOMIC_ACQUIRE);
+    if (tail) *tail = ctx->submitted;
+    return CC_OK;
+}
+
+extern "C" int32_t cc_worker_alive(cc_ctx* ctx) {
+    if (!ctx || !ctx->worker_running) return 0;
+    cudaSetDevice(ctx->device);
+    if (cudaEventQuery(ctx->worker_done) != cudaErrorNotReady) return 0;    // kernel has left (or failed)
+    const u64 hb0 = __atomic_load_n(ctx->ring_words + 16, __ATOMIC_ACQUIRE);
+    const u64 t0 = now_ns();
+    while (now_ns() - t0 < 1000000000ull) {
+        if (__atomic_load_n(ctx->ring_words + 16, __ATOMIC_ACQUIRE) != hb0) return 1;
+    }
+    return 0;
+}
+
+extern "C" int32_t cc_worker_stop(cc_ctx* ctx) {
+    if (!ctx) return CC_ERR_INVALID;
+    if (!ctx->worker_running) return CC_ERR_WORKER;
+    cudaSetDevice(ctx->device);
+    cc_task t;
+    memset(&t, 0, sizeof(t));
+    t.kind = CC_TASK_EXIT;
+    const u64 t0 = now_ns();
+    bool sent = false;
+    for (;;) {
+        cudaError_t q = cudaEventQuery(ctx->worker_done);
+        if (q == cudaSuccess) break;
+        if (q != cudaErrorNotReady) { ctx->last_cuda = (int)q; ctx->worker_running = false; return CC_ERR_CUDA; }
+        if (!sent && cc_submit(ctx, &t, nullptr) == CC_OK) sent = true;
+        if (now_ns() - t0 > 10ull * 1000000000ull) return CC_ERR_TIMEOUT;
+    }
+    ctx->worker_running = false;
+    return CC_OK;
+}

@@ -1,0 +1,206 @@
+"""GPU parity: cc_apply_log vs the CPU apply oracle (post-apply region, shadow, counters, status)."""
+import struct
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import synth
+import paper_2606_23521_b200 as cc
+from gpu_util import gpu_checkpoint
+
+pytestmark = pytest.mark.gpu
+
+
+def _gpu_apply(ctx, log_t, nbytes):
+    res = cc.Result()
+    ctx.apply_log(log_t, nbytes, res)
+    torch.cuda.synchronize()
+    r = res.read()
+    assert r.seq_done == 1
+    return r
+
+
+def _two_epoch_setup(P=64, n_pages=12, tail=32):
+    N = (n_pages - 1) * P + tail
+    rng = np.random.default_rng(5)
+    old = rng.integers(0, 256, N, dtype=np.uint8)
+    cur, sh = old.copy(), old.copy()
+    log = np.zeros(4096, dtype=np.uint8)
+    for p in (1, 4, n_pages - 1):
+        cur[p * P + 3] ^= 0x55
+    st, D1, nb1, W = oracle.checkpoint(cur, sh, P, 3, 100, log, 0)
+    for p in (4, 7):
+        cur[p * P + 9] ^= 0xAA
+    st, D2, nb2, W = oracle.checkpoint(cur, sh, P, 3, 101, log, W)
+    return old, log, nb1, nb2, P
+
+
+def _compare(old, log_np, nbytes, P, region_id=3, pinned=False):
+    """Apply log_np[:nbytes] to `old` on both sides and compare everything."""
+    reg_o, sh_o = old.copy(), old.copy()
+    exp = oracle.apply_log(log_np, nbytes, [oracle.Region(region_id, P, reg_o, sh_o)])
+    ctx = cc.Context()
+    reg = torch.from_numpy(old.copy()).cuda()
+    sh = ctx.register_region(region_id, reg, P)
+    ctx.apply_attach(1024)
+    lt = torch.from_numpy(log_np.copy())
+    lt = lt.pin_memory() if pinned else lt.cuda()
+    r = _gpu_apply(ctx, lt, nbytes)
+    assert (r.status, r.n_dirty, r.bytes) == exp, ((r.status, r.n_dirty, r.bytes), exp)
+    assert np.array_equal(reg.cpu().numpy(), reg_o)
+    assert np.array_equal(sh.cpu().numpy(), sh_o)
+    return ctx, reg, sh, r
+
+
+def test_round_trip_idempotent_then_empty_checkpoint():
+    old, log, nb1, nb2, P = _two_epoch_setup()
+    ctx, reg, sh, r = _compare(old, log, nb1 + nb2, P)
+    assert r.epoch == 2
+    lt = torch.from_numpy(log).cuda()
+    before = reg.clone()
+    r = _gpu_apply(ctx, lt, nb1 + nb2)                      # idempotent
+    assert torch.equal(reg, before) and r.n_dirty == 5
+    ctx.log_attach(torch.zeros(4096, dtype=torch.uint8, device="cuda"))
+    r = gpu_checkpoint(ctx, 3, 200)                          # apply refreshed the shadow
+    assert r.n_dirty == 0 and r.bytes == 0
+
+
+def test_truncation_sweep():
+    old, log, nb1, nb2, P = _two_epoch_setup()
+    total = nb1 + nb2
+    ctx = cc.Context()
+    reg = torch.from_numpy(old.copy()).cuda()
+    sh = ctx.register_region(3, reg, P)
+    ctx.apply_attach(64)
+    lt = torch.from_numpy(log).cuda()
+    old_t = torch.from_numpy(old).cuda()
+    for t in list(range(0, total + 1, 7)) + [nb1 - 1, nb1, nb1 + 1, total - 1, total]:
+        reg.copy_(old_t)
+        sh.copy_(old_t)
+        reg_o = old.copy()
+        exp = oracle.apply_log(log, t, [oracle.Region(3, P, reg_o)])
+        r = _gpu_apply(ctx, lt, t)
+        assert (r.status, r.n_dirty, r.bytes) == exp, t
+        assert np.array_equal(reg.cpu().numpy(), reg_o), t
+
+
+@pytest.mark.parametrize("where,idx,val", [("payload1", None, None), ("payload2", None, None),
+                                           ("hdr2", 0, 99), ("hdr2", 4, 10_000), ("hdr2", 8, 48),
+                                           ("hdr2", 12, 0xDEADBEEF), ("hdr2", 8, 1 << 30),
+                                           ("commit_k", None, None), ("commit_region", None, None),
+                                           ("commit_crc", None, None), ("commit_pageidx", None, None),
+                                           ("commit_len", None, None)])
+def test_corruption_cases(where, idx, val):
+    old, log, nb1, nb2, P = _two_epoch_setup()
+    bad = log.copy()
+    c = nb1 + nb2 - 32
+    if where == "payload1":
+        bad[16] ^= 0x80
+    elif where == "payload2":
+        bad[nb1 + 16 + 5] ^= 0x04
+    elif where == "hdr2":
+        bad[nb1 + idx: nb1 + idx + 4] = np.frombuffer(struct.pack("<I", val), dtype=np.uint8)
+    elif where in ("commit_k", "commit_region"):
+        payload = struct.pack("<QII", 101, 3, 3) if where == "commit_k" else struct.pack("<QII", 101, 4, 2)
+        bad[c + 16: c + 32] = np.frombuffer(payload, dtype=np.uint8)
+        bad[c + 12: c + 16] = np.frombuffer(struct.pack("<I", oracle.crc32c(payload)), dtype=np.uint8)
+    elif where == "commit_crc":
+        bad[c + 20] ^= 1
+    elif where == "commit_pageidx":
+        bad[c + 4] = 0
+    else:
+        bad[c + 8] = 32
+    _compare(old, bad, nb1 + nb2, P)
+
+
+def test_config5a_scaled_mixed_pages_duplicates(pinned=False):
+    """Config 5a scaled: three regions (4/16/64 KiB pages) of one arena, log written by the ORACLE's record
+    writer, pages repeat across epochs (last wins).  Log in device memory and in pinned host memory."""
+    arena_bytes = 64 << 20
+    arena = synth.raw_region(arena_bytes, 1005, "cuda")
+    unit = arena_bytes // 8
+    eps = synth.recovery_epochs(arena_bytes, 30, 40, 1005, forced_repeats=10)
+    cap = sum(e.payloads.numel() + 16 * e.pages.numel() + 32 for e in eps)
+    olog = np.zeros(cap, dtype=np.uint8)
+    W = 0
+    views = {rid: (o8 * unit, s8 * unit, P) for rid, o8, s8, P in synth.C5A_REGIONS}
+    for e in eps:
+        o, sz, P = views[e.region_id]
+        st, W = oracle.write_epoch(olog, W, e.region_id, e.epoch, sz, P, e.pages.numpy(), e.payloads.numpy())
+        assert st == 0
+    assert W == cap
+    host = arena.cpu().numpy().copy()
+    regs_o = [oracle.Region(rid, P, host[o:o + sz]) for rid, (o, sz, P) in views.items()]
+    exp = oracle.apply_log(olog, W, regs_o)
+    assert exp[0] == 0 and exp[1] == sum(e.pages.numel() for e in eps)
+
+    for pinned in (False, True):
+        work = arena.clone()
+        ctx = cc.Context()
+        shadows = {}
+        for rid, (o, sz, P) in views.items():
+            shadows[rid] = ctx.register_region(rid, work[o:o + sz], P)
+        ctx.apply_attach(exp[1] + 64)
+        lt = torch.from_numpy(olog)
+        lt = lt.pin_memory() if pinned else lt.cuda()
+        r = _gpu_apply(ctx, lt, W)
+        assert (r.status, r.n_dirty, r.bytes, r.epoch) == (0, exp[1], W, len(eps))
+        assert np.array_equal(work.cpu().numpy(), host)
+        for rid, (o, sz, P) in views.items():
+            assert np.array_equal(shadows[rid].cpu().numpy(), host[o:o + sz])
+
+
+def test_scratch_too_small_applies_nothing():
+    old, log, nb1, nb2, P = _two_epoch_setup()
+    ctx = cc.Context()
+    reg = torch.from_numpy(old.copy()).cuda()
+    ctx.register_region(3, reg, P)
+    ctx.apply_attach(2)
+    r = _gpu_apply(ctx, torch.from_numpy(log).cuda(), nb1 + nb2)
+    assert r.status == cc.CC_ERR_SCRATCH and r.n_dirty == 0 and r.bytes == 0
+    assert np.array_equal(reg.cpu().numpy(), old)
+
+
+def test_checkpoint_then_apply_round_trip_c1():
+    """Config 1 round trip: GPU checkpoint log applied by the GPU applier onto the old snapshot."""
+    P = 4096
+    cur = synth.raw_region(64 << 20, 1001, "cuda")
+    old = cur.clone()
+    pages = synth.mutate_byte_flips(cur, P, 0.01, 1001)
+    ctx = cc.Context()
+    ctx.register_region(1, cur, P, shadow=old.clone(), snapshot_now=False)
+    log = torch.zeros(len(pages) * (16 + P) + 32, dtype=torch.uint8, pin_memory=True)
+    ctx.log_attach(log)
+    r = gpu_checkpoint(ctx, 1, 1)
+    assert r.n_dirty == len(pages) and r.bytes == log.numel()
+    ctx2 = cc.Context()
+    target = old.clone()
+    ctx2.register_region(1, target, P)
+    ctx2.apply_attach(1000)
+    r2 = _gpu_apply(ctx2, log, log.numel())
+    assert (r2.status, r2.n_dirty, r2.bytes) == (0, len(pages), log.numel())
+    assert torch.equal(target, cur)
+    # and the oracle agrees about the same log
+    host = old.cpu().numpy().copy()
+    assert oracle.apply_log(log.numpy(), log.numel(), [oracle.Region(1, P, host)]) == (0, len(pages), log.numel())
+    assert np.array_equal(host, cur.cpu().numpy())
+
+
+def test_long_single_epoch_many_parse_steps():
+    """More records in one epoch than the parser's speculation width, with a short tail page last."""
+    P, n_pages = 64, 3000
+    N = (n_pages - 1) * P + 32
+    cur = synth.raw_region(N, 77, "cuda")
+    old = (~cur).contiguous()
+    olog = np.zeros(n_pages * (16 + P) + 32, dtype=np.uint8)
+    st, D, nb, W = oracle.checkpoint(cur.cpu().numpy(), old.cpu().numpy().copy(), P, 3, 1, olog, 0)
+    assert D.size == n_pages
+    ctx = cc.Context()
+    reg = old.clone()
+    ctx.register_region(3, reg, P)
+    ctx.apply_attach(4000)
+    r = _gpu_apply(ctx, torch.from_numpy(olog).cuda(), nb)
+    assert (r.status, r.n_dirty, r.bytes) == (0, n_pages, nb)
+    assert torch.equal(reg, cur)

@@ -1,0 +1,161 @@
+"""GPU: ring buffer + persistent worker.  Same log bytes as the host-launched path and the oracle;
+FIFO completion; ring-full; wrap-around; liveness."""
+import time
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import synth
+import paper_2606_23521_b200 as cc
+
+pytestmark = pytest.mark.gpu
+
+
+def _mk(P=4096, n_pages=512, cap=8, seed=1006, log_bytes=1 << 22, pinned=True, **kw):
+    cur = synth.raw_region(P * n_pages, seed, "cuda")
+    ctx = cc.Context(ring_capacity=cap, max_lifetime_ns=int(60e9), **kw)
+    sh = ctx.register_region(1, cur, P)
+    log = torch.zeros(log_bytes, dtype=torch.uint8, pin_memory=True) if pinned else \
+        torch.zeros(log_bytes, dtype=torch.uint8, device="cuda")
+    committed = torch.zeros(1, dtype=torch.int64, pin_memory=True)
+    ctx.log_attach(log, committed)
+    ctx.apply_attach(4096)
+    return ctx, cur, sh, log, committed
+
+
+def test_nop_roundtrip_alive_and_stop():
+    ctx, cur, sh, log, committed = _mk()
+    assert not ctx.worker_alive()
+    with pytest.raises(cc.ConcordiaError) as e:
+        ctx.submit(cc.CC_TASK_NOP)
+    assert e.value.code == cc.CC_ERR_WORKER
+    ctx.worker_start()
+    try:
+        assert ctx.worker_alive()
+        seqs = [ctx.submit(cc.CC_TASK_NOP) for _ in range(5)]
+        assert seqs == list(range(5))
+        for s in seqs:
+            r = ctx.wait(s, 5.0)
+            assert r.seq_done == s + 1 and r.status == 0 and r.flags == cc.CC_TASK_NOP
+        h, t = ctx.peek_queue()
+        assert (h, t) == (5, 5)
+        with pytest.raises(cc.ConcordiaError) as e:          # registration only while stopped
+            ctx.log_reset()
+        assert e.value.code == cc.CC_ERR_WORKER
+    finally:
+        ctx.worker_stop()
+    assert not ctx.worker_alive()
+    ctx.log_reset()
+    ctx.shutdown()
+
+
+def test_wraparound_ring_full_and_fifo():
+    ctx, cur, sh, log, committed = _mk(cap=4)
+    ctx.worker_start()
+    try:
+        done = []
+        full_seen = 0
+        submitted = 0
+        while submitted < 40:
+            try:
+                s = ctx.submit(cc.CC_TASK_NOP)
+                submitted += 1
+                done.append(s)
+            except cc.ConcordiaError as e:
+                assert e.code == cc.CC_ERR_RING_FULL
+                full_seen += 1
+                h, t = ctx.peek_queue()
+                ctx.wait(h, 5.0) if h < t else None
+        last_end = 0
+        r = ctx.wait(done[-1], 5.0)
+        assert r.seq_done == 40
+        h, t = ctx.peek_queue()
+        assert (h, t) == (40, 40)
+    finally:
+        ctx.worker_stop()
+    ctx.shutdown()
+
+
+def test_worker_checkpoint_equals_host_launched_and_oracle():
+    """C5b-shaped: MUTATE -> DELTA_CKPT tasks; parity of every task's log bytes on the first tasks."""
+    P, n_pages, n_mut = 4096, 512, 6
+    ctx, cur, sh, log, committed = _mk(P=P, n_pages=n_pages, cap=64)
+    host_cur = cur.cpu().numpy().copy()
+    host_sh = host_cur.copy()
+    olog = np.zeros(log.numel(), dtype=np.uint8)
+    W = 0
+    ctx.worker_start()
+    try:
+        pend = []
+        for task in range(16):
+            pages, h = synth.worker_mutation_pages(task, n_pages, n_mut, 1006)
+            A = 2 * ((1006 * 7919 + 12345) % 100000) + 1
+            ctx.submit(cc.CC_TASK_TEST_MUTATE, region_id=1, arg0=n_mut, arg1=A, arg2=h)
+            s = ctx.submit(cc.CC_TASK_DELTA_CKPT, region_id=1, epoch=1000 + task)
+            for j, p in enumerate(pages):
+                host_cur[p * P + (h + j) % P] ^= 0x5A
+            st, D, nb, W = oracle.checkpoint(host_cur, host_sh, P, 1, 1000 + task, olog, W)
+            pend.append((s, D.size, nb, W))
+        for s, k, nb, w in pend:
+            r = ctx.wait(s, 10.0)
+            assert (r.status, r.n_dirty, r.bytes, r.log_offset_after, r.epoch) == (0, k, nb, w, 1000 + (s // 2))
+            assert r.t_end_ns >= r.t_start_ns
+        assert int(committed.item()) == W
+        assert np.array_equal(log.numpy(), olog)
+        # log reset through the ring, then one more checkpoint lands at offset 0
+        ctx.submit(cc.CC_TASK_LOG_RESET)
+        ctx.submit(cc.CC_TASK_TEST_MUTATE, region_id=1, arg0=1, arg1=1, arg2=7)
+        s = ctx.submit(cc.CC_TASK_DELTA_CKPT, region_id=1, epoch=5)
+        r = ctx.wait(s, 10.0)
+        assert (r.n_dirty, r.bytes, r.log_offset_after) == (1, 16 + P + 32, 16 + P + 32)
+        # unknown region -> NOT_REGISTERED, worker keeps running
+        s = ctx.submit(cc.CC_TASK_DELTA_CKPT, region_id=77, epoch=6)
+        assert ctx.wait(s, 10.0).status == cc.CC_ERR_NOT_REGISTERED
+        assert ctx.worker_alive()
+    finally:
+        ctx.worker_stop()
+    # after the worker has left, the host-launched path continues on the same state
+    torch.cuda.synchronize()
+    assert np.array_equal(sh.cpu().numpy(), cur.cpu().numpy())
+    ctx.shutdown()
+
+
+def test_worker_restore_task():
+    P, n_pages = 4096, 256
+    ctx, cur, sh, log, committed = _mk(P=P, n_pages=n_pages, cap=16, pinned=True)
+    old = cur.clone()
+    for p in (0, 100, 255):
+        cur[p * P + 17] ^= 0x33
+    new = cur.clone()
+    res = cc.Result()
+    ctx.checkpoint_delta(1, 1, res)
+    torch.cuda.synchronize()
+    nb = res.read().bytes
+    assert nb == 3 * (16 + P) + 32
+    cur.copy_(old)
+    sh.copy_(old)
+    torch.cuda.synchronize()
+    ctx.worker_start()
+    try:
+        s = ctx.submit(cc.CC_TASK_RESTORE, arg0=log.data_ptr(), arg1=nb)
+        r = ctx.wait(s, 10.0)
+        assert (r.status, r.n_dirty, r.bytes, r.epoch) == (0, 3, nb, 1)
+    finally:
+        ctx.worker_stop()
+    torch.cuda.synchronize()
+    assert torch.equal(cur, new) and torch.equal(sh, new)
+    ctx.shutdown()
+
+
+def test_worker_lifetime_watchdog():
+    """The worker leaves by itself after max_lifetime_ns (safety net against a lost host)."""
+    cur = synth.raw_region(4096 * 8, 3, "cuda")
+    ctx = cc.Context(ring_capacity=4, max_lifetime_ns=int(0.3e9))
+    ctx.register_region(1, cur, 4096)
+    ctx.worker_start()
+    time.sleep(1.0)
+    assert not ctx.worker_alive()
+    ctx.worker_stop()
+    ctx.shutdown()
