@@ -152,6 +152,10 @@ int32_t cc_log_attach(cc_ctx* ctx, void* log_buf, uint64_t capacity, uint64_t* c
 /* W := 0 (synchronous; only while the worker is stopped -- use CC_TASK_LOG_RESET otherwise). */
 int32_t cc_log_reset(cc_ctx* ctx);
 
+/* W := 0, ASYNCHRONOUS on `stream` (ordered after the checkpoints already queued there): what a log
+ * drainer calls once it has consumed the committed prefix.  Only while the worker is stopped. */
+int32_t cc_log_reset_async(cc_ctx* ctx, void* stream);
+
 /* ---- host-launched path -------------------------------------------------------------------- */
 
 /* Delta-checkpoint one region: scan live vs shadow per page, compact the
@@ -169,6 +173,11 @@ int32_t cc_checkpoint_delta(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, voi
 /* Scan + compaction only (steps a1-a2), for measurement: fills the dirty list, appends nothing,
  * leaves the shadow alone.  out->n_dirty = k. */
 int32_t cc_scan_only(cc_ctx* ctx, uint32_t region_id, void* stream, cc_result* out);
+
+/* Measurement hook: if non-NULL, the next host-launched cc_checkpoint_delta / cc_scan_only calls
+ * record these cudaEvent_t (passed as void*) on the call's stream right after the scan kernel and
+ * right after the compaction kernel.  Pass NULLs to switch it off.  No effect on results. */
+int32_t cc_trace_events(cc_ctx* ctx, void* ev_after_scan, void* ev_after_compact);
 
 /* Device pointer to the u32 ascending dirty page list of the region's last scan and to its
  * u32 count (valid after the stream reached the end of that call). */

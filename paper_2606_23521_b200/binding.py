@@ -37,8 +37,9 @@ CC_TASK_EXIT = 255
 
 EXPORTS = [
     "cc_init", "cc_shutdown", "cc_last_cuda_error", "cc_kernel_launches", "cc_workspace_bytes",
-    "cc_register_region", "cc_unregister_region", "cc_log_attach", "cc_log_reset", "cc_checkpoint_delta",
-    "cc_scan_only", "cc_dirty_list", "cc_apply_scratch_bytes", "cc_apply_attach", "cc_apply_log",
+    "cc_register_region", "cc_unregister_region", "cc_log_attach", "cc_log_reset", "cc_log_reset_async",
+    "cc_checkpoint_delta",
+    "cc_scan_only", "cc_trace_events", "cc_dirty_list", "cc_apply_scratch_bytes", "cc_apply_attach", "cc_apply_log",
     "cc_worker_start", "cc_worker_stop", "cc_worker_alive", "cc_peek_queue", "cc_submit", "cc_poll", "cc_wait",
 ]
 
@@ -99,8 +100,10 @@ def load_library():
         "cc_unregister_region": (i32, [vp, u32]),
         "cc_log_attach": (i32, [vp, vp, u64, vp]),
         "cc_log_reset": (i32, [vp]),
+        "cc_log_reset_async": (i32, [vp, vp]),
         "cc_checkpoint_delta": (i32, [vp, u32, u64, vp, vp]),
         "cc_scan_only": (i32, [vp, u32, vp, vp]),
+        "cc_trace_events": (i32, [vp, vp, vp]),
         "cc_dirty_list": (i32, [vp, u32, P(vp), P(vp)]),
         "cc_apply_scratch_bytes": (u64, [u64]),
         "cc_apply_attach": (i32, [vp, vp, u64]),
@@ -218,6 +221,9 @@ class Context:
     def log_reset(self):
         self._check("cc_log_reset", self.lib.cc_log_reset(self.h))
 
+    def log_reset_async(self, stream=None):
+        self._check("cc_log_reset_async", self.lib.cc_log_reset_async(self.h, _stream_ptr(stream)))
+
     # -- host-launched path
     def checkpoint_delta(self, region_id: int, epoch: int, result: Result = None, stream=None):
         self._check("cc_checkpoint_delta", self.lib.cc_checkpoint_delta(
@@ -226,6 +232,13 @@ class Context:
     def scan_only(self, region_id: int, result: Result = None, stream=None):
         self._check("cc_scan_only", self.lib.cc_scan_only(
             self.h, region_id, _stream_ptr(stream), ctypes.c_void_p(result.ptr) if result else None))
+
+    def trace_events(self, after_scan: "torch.cuda.Event" = None, after_compact: "torch.cuda.Event" = None):
+        """Events (created with enable_timing=True and recorded once, so that the handle exists) that the
+        next host-launched calls record after the scan / compaction kernels; None switches it off."""
+        a = ctypes.c_void_p(after_scan.cuda_event) if after_scan is not None else None
+        b = ctypes.c_void_p(after_compact.cuda_event) if after_compact is not None else None
+        self._check("cc_trace_events", self.lib.cc_trace_events(self.h, a, b))
 
     def dirty_list(self, region_id: int) -> torch.Tensor:
         """Ascending dirty page indices of the last scan as an int64 CPU tensor (synchronises)."""

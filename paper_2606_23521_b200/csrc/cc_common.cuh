@@ -109,7 +109,7 @@ struct cc_dev {
     u32 bar_count;
     u32 bar_gen;
     u64 doorbell;
-    cc_task cur_task;
+    alignas(16) cc_task cur_task;
     u32 worker_exit;
 };
 

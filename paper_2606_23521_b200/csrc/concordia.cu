@@ -92,6 +92,7 @@ struct cc_ctx {
     cudaStream_t worker_stream;
     cudaEvent_t worker_done;
     u32 worker_blocks_used;
+    cudaEvent_t ev_after_scan, ev_after_compact;
 };
 
 #define CC_CUDA(ctx, call)                                     \
@@ -311,6 +312,14 @@ extern "C" int32_t cc_log_reset(cc_ctx* ctx) {
     return CC_OK;
 }
 
+extern "C" int32_t cc_log_reset_async(cc_ctx* ctx, void* stream) {
+    if (!ctx || !ctx->log_attached) return CC_ERR_INVALID;
+    if (ctx->worker_running) return CC_ERR_WORKER;
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    CC_CUDA(ctx, cudaMemsetAsync(&ctx->d_dev->log.W, 0, sizeof(u64), (cudaStream_t)stream));
+    return CC_OK;
+}
+
 // ------------------------------------------------------------- host-launched path --
 
 static int32_t launch_scan_compact(cc_ctx* ctx, int slot, u32 mode, uint64_t epoch, cudaStream_t st, cc_result* out) {
@@ -321,9 +330,11 @@ static int32_t launch_scan_compact(cc_ctx* ctx, int slot, u32 mode, uint64_t epo
     const uint64_t cap1 = (uint64_t)ctx->sm_count * ctx->scan_bps;
     if (g1 > cap1) g1 = cap1;
     cc_scan_kernel<<<(unsigned)g1, CC_SCAN_THREADS, 0, st>>>(ctx->d_dev, slot);
+    if (ctx->ev_after_scan) cudaEventRecord(ctx->ev_after_scan, st);
     const uint64_t n_tiles = (r.n_words + CC_COMPACT_TILE_WORDS - 1) / CC_COMPACT_TILE_WORDS;
     uint64_t g2 = n_tiles < (uint64_t)ctx->sm_count * 4 ? n_tiles : (uint64_t)ctx->sm_count * 4;
     cc_compact_kernel<<<(unsigned)g2, CC_COMPACT_THREADS, 0, st>>>(ctx->d_dev, slot, mode, epoch, out);
+    if (ctx->ev_after_compact) cudaEventRecord(ctx->ev_after_compact, st);
     ctx->launches += 2;
     CC_CUDA(ctx, cudaGetLastError());
     return CC_OK;
@@ -350,6 +361,13 @@ extern "C" int32_t cc_scan_only(cc_ctx* ctx, uint32_t region_id, void* stream, c
     if (slot < 0) return CC_ERR_NOT_REGISTERED;
     CC_CUDA(ctx, cudaSetDevice(ctx->device));
     return launch_scan_compact(ctx, slot, CC_MODE_SCAN_ONLY, 0, (cudaStream_t)stream, out);
+}
+
+extern "C" int32_t cc_trace_events(cc_ctx* ctx, void* ev_after_scan, void* ev_after_compact) {
+    if (!ctx) return CC_ERR_INVALID;
+    ctx->ev_after_scan = (cudaEvent_t)ev_after_scan;
+    ctx->ev_after_compact = (cudaEvent_t)ev_after_compact;
+    return CC_OK;
 }
 
 extern "C" int32_t cc_dirty_list(cc_ctx* ctx, uint32_t region_id, const uint32_t** d_list, const uint32_t** d_count) {

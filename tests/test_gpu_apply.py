@@ -153,14 +153,18 @@ def test_config5a_scaled_mixed_pages_duplicates(pinned=False):
 
 
 def test_scratch_too_small_applies_nothing():
-    old, log, nb1, nb2, P = _two_epoch_setup()
+    P, n_pages = 64, 600
+    cur = synth.raw_region(P * n_pages, 78, "cuda")
+    old = (~cur).contiguous()
+    olog = np.zeros(n_pages * (16 + P) + 32, dtype=np.uint8)
+    st, D, nb, W = oracle.checkpoint(cur.cpu().numpy(), old.cpu().numpy().copy(), P, 3, 1, olog, 0)
     ctx = cc.Context()
-    reg = torch.from_numpy(old.copy()).cuda()
+    reg = old.clone()
     ctx.register_region(3, reg, P)
-    ctx.apply_attach(2)
-    r = _gpu_apply(ctx, torch.from_numpy(log).cuda(), nb1 + nb2)
+    ctx.apply_attach(100)                       # room for ~100 records, the log holds 600
+    r = _gpu_apply(ctx, torch.from_numpy(olog).cuda(), nb)
     assert r.status == cc.CC_ERR_SCRATCH and r.n_dirty == 0 and r.bytes == 0
-    assert np.array_equal(reg.cpu().numpy(), old)
+    assert torch.equal(reg, old)
 
 
 def test_checkpoint_then_apply_round_trip_c1():
