@@ -192,7 +192,11 @@ __device__ __forceinline__ void cc_apply_validate_phase(cc_dev* dev, const cc_ap
                     finish = (atomicAdd(&T.rec_cnt[ri], 1u) == nseg - 1);
                     if (finish) { __threadfence(); acc = atomicExch(&T.rec_acc[ri], 0u); }
                 }
-                if (finish && crc_finalize(&dev->crc, acc, rec.len) != rec.crc) atomicMin(&A->first_bad_rec, ri);
+                if (finish) {
+                    const cc_region_dev& rg = dev->regions[rec.slot];
+                    const u32 it = rec.len == rg.page_bytes ? rg.crc_init_full : rg.crc_init_tail;
+                    if (crc_finalize(acc, it) != rec.crc) atomicMin(&A->first_bad_rec, ri);
+                }
             }
         }
     }

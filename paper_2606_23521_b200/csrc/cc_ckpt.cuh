@@ -277,7 +277,8 @@ __device__ __forceinline__ void cc_gather_phase(const cc_region_dev& r, cc_dev* 
                         r.rec_done[i] = 0;
                     }
                 }
-                if (finish) st_u32x4(rec, r.region_id, p, (u32)plen, crc_finalize(&dev->crc, acc, plen));
+                if (finish) st_u32x4(rec, r.region_id, p, (u32)plen,
+                                     crc_finalize(acc, plen == P ? r.crc_init_full : r.crc_init_tail));
             }
         }
     }

@@ -48,6 +48,8 @@ struct cc_region_dev {
     u64* lb_status;     // compaction look-back status, one per tile
     u32* latest;        // n_pages u32: applier last-wins table, all zero between calls
     cc_ws_hdr* hdr;
+    u32 crc_init_full;  // 0xFFFFFFFF * x^(8*P): the CRC init term of a full page
+    u32 crc_init_tail;  // same for the (possibly short) last page
 };
 
 struct cc_log_dev {
@@ -93,6 +95,8 @@ struct cc_crc_tables {
     u32 lane_mul[32];       // x^(8*16*(31-lane))
     u32 seg_mul[65];        // x^(8*4096*m), m = 0..64
     u32 xp[48];             // x^(8*2^j), j = 0..47
+    u32 lane_nib[8 * 16 * 32];  // (v << 4n) * lane_mul[l] at [(n*16 + v)*32 + l]
+    u32 seg_pow[65 * 32];   // seg_mul[m] * x^i at [m*32 + i]
 };
 
 struct cc_dev {

@@ -8,10 +8,11 @@
 //   CRC32C(M)         = raw(M, ~0) XOR ~0
 // A warp handles one 4 KiB segment: lane l owns the 16-byte vectors l, l+32, ..., l+224.  It
 // runs the byte-table loop over each vector from 0 (8 independent chains -> ILP), folds them with
-// Horner steps of x^(8*512), multiplies by its lane constant x^(8*16*(31-l)), the warp XORs the
-// lanes together, and lane 0 multiplies by the segment constant x^(8*bytes after the segment).
-// The byte table is replicated per lane in shared memory (entry*32 + lane) so the random
-// lookups of the 32 lanes never collide on a bank.
+// Horner steps of x^(8*512), multiplies by its lane constant x^(8*16*(31-l)) (8 nibble-table
+// lookups), the warp XORs the lanes together, and the warp multiplies by the segment constant
+// x^(8*bytes after the segment) with one bit of the product per lane.
+// The byte table and the nibble tables are replicated per lane in shared memory
+// (entry*32 + lane) so the random lookups of the 32 lanes never collide on a bank.
 #pragma once
 #include "cc_common.cuh"
 
@@ -54,38 +55,71 @@ static inline void cc_crc_build_tables(cc_crc_tables* t) {
         for (u32 v = 0; v < 256; v++) t->s512[b][v] = gf_mul(v << (8 * b), s512);
     for (u32 l = 0; l < 32; l++) t->lane_mul[l] = gf_xpow_bytes(t->xp, 16ull * (31 - l));
     for (u32 m = 0; m <= 64; m++) t->seg_mul[m] = gf_xpow_bytes(t->xp, 4096ull * m);
+    // lane_nib[(n*16 + v)*32 + l] = (v << 4n) * lane_mul[l]: multiply by the lane constant in 8 lookups
+    for (u32 n = 0; n < 8; n++)
+        for (u32 v = 0; v < 16; v++)
+            for (u32 l = 0; l < 32; l++) t->lane_nib[(n * 16 + v) * 32 + l] = gf_mul(v << (4 * n), t->lane_mul[l]);
+    // seg_pow[m*32 + i] = seg_mul[m] * x^i: multiply by the segment constant with one term per lane
+    for (u32 m = 0; m <= 64; m++) {
+        u32 b = t->seg_mul[m];
+        for (u32 i = 0; i < 32; i++) { t->seg_pow[m * 32 + i] = b; b = gf_mulx(b); }
+    }
 }
 
 // ---- device: shared-memory tables ----
+// t0 holds the byte table ROTATED LEFT BY 7 and replicated per lane: word (entry*32 + lane), i.e. byte
+// offset entry*128 + lane*4.  The CRC register is kept rotated left by 7 as well ("z"), so the low
+// byte of the register already sits at bits 7..14 = the table's byte offset: one LOP3 forms the
+// address, one funnel shift + one LOP3 form the next state -> 3 ALU + 1 LDS per message byte.
 struct cc_crc_smem {
-    u32 t0[256 * 32];       // lane-replicated byte table: t0[entry*32 + lane]
+    u32 t0[256 * 32];
+    u32 lane_nib[8 * 16 * 32];
     u32 s512[4 * 256];
 };
 
+__device__ __forceinline__ u32 rotl32(u32 x, int n) { return __funnelshift_l(x, x, n); }
+__device__ __forceinline__ u32 rotr32(u32 x, int n) { return __funnelshift_r(x, x, n); }
+
 __device__ __forceinline__ void cc_crc_smem_init(cc_crc_smem* s, const cc_crc_tables* g) {
-    for (u32 i = threadIdx.x; i < 256 * 32; i += blockDim.x) s->t0[i] = g->t0[i >> 5];
+    for (u32 i = threadIdx.x; i < 256 * 32; i += blockDim.x) s->t0[i] = rotl32(g->t0[i >> 5], 7);
+    for (u32 i = threadIdx.x; i < 8 * 16 * 32; i += blockDim.x) s->lane_nib[i] = g->lane_nib[i];
     for (u32 i = threadIdx.x; i < 4 * 256; i += blockDim.x) s->s512[i] = (&g->s512[0][0])[i];
     __syncthreads();
 }
 
-// raw register update over one 32-bit word (4 bytes, memory order = little endian)
-__device__ __forceinline__ u32 crc_word(const u32* t0_lane, u32 crc, u32 w) {
-    crc ^= w;
-#pragma unroll
-    for (int i = 0; i < 4; i++) crc = t0_lane[(crc & 0xFFu) << 5] ^ (crc >> 8);
-    return crc;
+// z' for one message byte already XORed into z
+__device__ __forceinline__ u32 crc_step_z(const char* t0, u32 lane4, u32 z) {
+    const u32 v = *reinterpret_cast<const u32*>(t0 + ((z & 0x7F80u) | lane4));
+    return v ^ (rotr32(z, 8) & 0x7FFFFF80u);
 }
 
-__device__ __forceinline__ u32 crc_vec16(const u32* t0_lane, const uint4& v) {
-    u32 c = crc_word(t0_lane, 0u, v.x);
-    c = crc_word(t0_lane, c, v.y);
-    c = crc_word(t0_lane, c, v.z);
-    c = crc_word(t0_lane, c, v.w);
-    return c;
+// raw register (init 0) over one 16-byte vector, memory order; returns the UNrotated register
+__device__ __forceinline__ u32 crc_vec16(const char* t0, u32 lane4, const uint4& v) {
+    const u32 w[4] = {v.x, v.y, v.z, v.w};
+    u32 z = 0;
+#pragma unroll
+    for (int j = 0; j < 4; j++) {
+        z ^= rotl32(w[j], 7);
+#pragma unroll
+        for (int b = 0; b < 4; b++) z = crc_step_z(t0, lane4, z);
+    }
+    return rotr32(z, 7);
 }
 
 __device__ __forceinline__ u32 crc_shift512(const u32* s512, u32 v) {
     return s512[v & 0xFFu] ^ s512[256 + ((v >> 8) & 0xFFu)] ^ s512[512 + ((v >> 16) & 0xFFu)] ^ s512[768 + (v >> 24)];
+}
+
+// acc * lane_mul[lane] through the lane-replicated nibble tables (conflict-free, 8 lookups)
+__device__ __forceinline__ u32 crc_lane_mul(const cc_crc_smem* s, u32 lane4, u32 acc) {
+    const char* nb = reinterpret_cast<const char*>(s->lane_nib);
+    u32 r = 0;
+#pragma unroll
+    for (int n = 0; n < 8; n++) {
+        const u32 sh = (n * 4 >= 7) ? (acc >> (n * 4 - 7)) : (acc << (7 - n * 4));
+        r ^= *reinterpret_cast<const u32*>(nb + n * 2048 + ((sh & 0x780u) | lane4));
+    }
+    return r;
 }
 
 // Warp-level raw CRC contribution of one segment of nv (<= 256) 16-byte vectors held as
@@ -94,21 +128,22 @@ __device__ __forceinline__ u32 crc_shift512(const u32* s512, u32 v) {
 template <int U>
 __device__ __forceinline__ u32 crc_segment_warp(const cc_crc_smem* s, const cc_crc_tables* g, const uint4 (&v)[U],
                                                 u32 nv, u64 after, u32 lane) {
-    const u32* t0_lane = s->t0 + lane;
+    const char* t0 = reinterpret_cast<const char*>(s->t0);
+    const u32 lane4 = lane << 2;
     u32 acc = 0;
-    u32 part[U];
     if (nv == 32u * U) {
+        u32 part[U];
 #pragma unroll
-        for (int u = 0; u < U; u++) part[u] = crc_vec16(t0_lane, v[u]);     // independent chains
+        for (int u = 0; u < U; u++) part[u] = crc_vec16(t0, lane4, v[u]);     // U independent chains
 #pragma unroll
         for (int u = 0; u < U; u++) acc = (u ? crc_shift512(s->s512, acc) : 0u) ^ part[u];
-        acc = gf_mul(acc, g->lane_mul[lane]);
+        acc = crc_lane_mul(s, lane4, acc);
     } else {
         int last = -1;
 #pragma unroll
         for (int u = 0; u < U; u++) {
             if (lane + 32u * u < nv) {
-                acc = crc_shift512(s->s512, acc) ^ crc_vec16(t0_lane, v[u]);
+                acc = crc_shift512(s->s512, acc) ^ crc_vec16(t0, lane4, v[u]);
                 last = u;
             }
         }
@@ -120,16 +155,22 @@ __device__ __forceinline__ u32 crc_segment_warp(const cc_crc_smem* s, const cc_c
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) acc ^= __shfl_xor_sync(0xFFFFFFFFu, acc, o);
     if (after != 0) {
-        u32 m = ((after & 4095u) == 0 && (after >> 12) <= 64) ? g->seg_mul[after >> 12] : gf_xpow_bytes(g->xp, after);
-        acc = gf_mul(acc, m);
+        if ((after & 4095u) == 0 && (after >> 12) <= 64) {
+            // acc * seg_mul[m]: lane i contributes bit (31-i) of acc times seg_mul[m]*x^i
+            u32 term = ((acc >> (31 - lane)) & 1u) ? g->seg_pow[(u32)(after >> 12) * 32 + lane] : 0u;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) term ^= __shfl_xor_sync(0xFFFFFFFFu, term, o);
+            acc = term;
+        } else {
+            acc = gf_mul(acc, gf_xpow_bytes(g->xp, after));
+        }
     }
     return acc;
 }
 
-// Finalise: XOR of all segment contributions -> CRC32C of a len-byte message.
-__device__ __forceinline__ u32 crc_finalize(const cc_crc_tables* g, u32 acc, u64 len) {
-    return acc ^ gf_mul(0xFFFFFFFFu, gf_xpow_bytes(g->xp, len)) ^ 0xFFFFFFFFu;
-}
+// Finalise: XOR of all segment contributions -> CRC32C.  init_term = 0xFFFFFFFF * x^(8*len), which
+// is precomputed per region for its full and its tail page length.
+__device__ __forceinline__ u32 crc_finalize(u32 acc, u32 init_term) { return acc ^ init_term ^ 0xFFFFFFFFu; }
 
 // Serial CRC32C of a few bytes (commit payload), single thread, global table.
 __device__ inline u32 crc_serial(const cc_crc_tables* g, const u8* p, u32 n) {

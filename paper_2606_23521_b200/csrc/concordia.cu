@@ -174,6 +174,9 @@ extern "C" int32_t cc_init(cc_ctx** out, int32_t device, const cc_config* cfg) {
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->internal, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->worker_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->worker_done, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_apply_validate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_worker_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->scan_bps, cc_scan_kernel, CC_SCAN_THREADS, 0);
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->gather_bps, cc_gather_kernel, CC_GATHER_THREADS, sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->validate_bps, cc_apply_validate_kernel, CC_APPLY_THREADS, sizeof(cc_crc_smem));
@@ -262,6 +265,14 @@ extern "C" int32_t cc_register_region(cc_ctx* ctx, const cc_region_desc* d) {
     r.rec_done = (u32*)(ws + L.rec_done);
     r.latest = (u32*)(ws + L.latest);
     r.lb_status = (u64*)(ws + L.lb);
+    {
+        cc_crc_tables* t = (cc_crc_tables*)malloc(sizeof(cc_crc_tables));
+        cc_crc_build_tables(t);
+        const u64 tail = d->bytes - (L.n_pages - 1) * (u64)d->page_bytes;
+        r.crc_init_full = gf_mul(0xFFFFFFFFu, gf_xpow_bytes(t->xp, d->page_bytes));
+        r.crc_init_tail = gf_mul(0xFFFFFFFFu, gf_xpow_bytes(t->xp, tail));
+        free(t);
+    }
     const u32 one = 1;
     CC_CUDA(ctx, cudaMemcpyAsync(&ctx->d_dev->regions[slot], &r, sizeof(r), cudaMemcpyHostToDevice, 0));
     CC_CUDA(ctx, cudaMemcpyAsync(&ctx->d_dev->region_used[slot], &one, sizeof(one), cudaMemcpyHostToDevice, 0));
