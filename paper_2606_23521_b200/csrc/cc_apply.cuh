@@ -22,8 +22,7 @@
 struct cc_apply_tabs {      // carved out of the attached scratch
     cc_rec* recs;
     cc_epoch_ent* epochs;
-    u32* rec_acc;           // per-record CRC accumulator
-    u32* rec_cnt;           // per-record finished segments
+    u64* rec_state;         // per-record {done-mask or count | CRC accumulator} (crc_record_combine)
     u32* seg_begin;         // per-record first segment number (+ one trailing total)
     u64 max_records;
 };
@@ -116,8 +115,7 @@ __device__ __forceinline__ void cc_apply_parse_phase(cc_dev* dev, const cc_apply
                 rec.off = off_t; rec.page_idx = h.y; rec.len = h.z; rec.crc = h.w;
                 rec.slot = s_slot; rec.epoch_idx = s_nepochs; rec.pad = 0;
                 T.recs[base + tid] = rec;
-                T.rec_acc[base + tid] = 0;
-                T.rec_cnt[base + tid] = 0;
+                T.rec_state[base + tid] = 0;
                 T.seg_begin[base + tid] = s_segs + tid * r.spp;        // only the run's last record can be short
             }
             __syncthreads();
@@ -184,14 +182,8 @@ __device__ __forceinline__ void cc_apply_validate_phase(cc_dev* dev, const cc_ap
             }
             const u32 contrib = crc_segment_warp<U>(cs, &dev->crc, v, nv, rem - seg_len, lane);
             if (lane == 0) {
-                u32 acc = contrib;
-                bool finish = true;
-                if (nseg > 1) {
-                    atomicXor(&T.rec_acc[ri], contrib);
-                    __threadfence();
-                    finish = (atomicAdd(&T.rec_cnt[ri], 1u) == nseg - 1);
-                    if (finish) { __threadfence(); acc = atomicExch(&T.rec_acc[ri], 0u); }
-                }
+                u32 acc = 0;
+                const bool finish = crc_record_combine(&T.rec_state[ri], nseg, c, contrib, &acc);
                 if (finish) {
                     const cc_region_dev& rg = dev->regions[rec.slot];
                     const u32 it = rec.len == rg.page_bytes ? rg.crc_init_full : rg.crc_init_tail;

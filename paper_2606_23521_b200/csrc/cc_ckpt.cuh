@@ -263,20 +263,8 @@ __device__ __forceinline__ void cc_gather_phase(const cc_region_dev& r, cc_dev* 
             }
             const u32 contrib = crc_segment_warp<U>(cs, &dev->crc, v, nv, after, lane);
             if (lane == 0) {
-                u32 acc;
-                bool finish;
-                if (nseg == 1) { acc = contrib; finish = true; }
-                else {
-                    atomicXor(&r.rec_crc[i], contrib);
-                    __threadfence();
-                    finish = (atomicAdd(&r.rec_done[i], 1u) == nseg - 1);
-                    acc = 0;
-                    if (finish) {
-                        __threadfence();
-                        acc = atomicExch(&r.rec_crc[i], 0u);
-                        r.rec_done[i] = 0;
-                    }
-                }
+                u32 acc = 0;
+                const bool finish = crc_record_combine(&r.rec_state[i], nseg, c, contrib, &acc);
                 if (finish) st_u32x4(rec, r.region_id, p, (u32)plen,
                                      crc_finalize(acc, plen == P ? r.crc_init_full : r.crc_init_tail));
             }

@@ -43,8 +43,7 @@ struct cc_region_dev {
     u64 n_words;        // bitmap words
     u32* bitmap;        // n_words (+ padding to a multiple of 4) u32, all zero between calls
     u32* D;             // n_pages u32: ascending dirty list
-    u32* rec_crc;       // n_pages u32: per-record CRC accumulators, all zero between calls
-    u32* rec_done;      // n_pages u32: per-record finished-segment counters, all zero between calls
+    u64* rec_state;     // n_pages u64: per-record {done-mask or count : 32 | CRC accumulator : 32}, zero between calls
     u64* lb_status;     // compaction look-back status, one per tile
     u32* latest;        // n_pages u32: applier last-wins table, all zero between calls
     cc_ws_hdr* hdr;
@@ -162,6 +161,15 @@ __device__ __forceinline__ u64 ld_acquire_sys_u64(const u64* p) {
 }
 __device__ __forceinline__ void st_release_sys_u64(u64* p, u64 v) {
     asm volatile("st.release.sys.global.u64 [%0], %1;" :: "l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ uint4 ld_relaxed_sys_v4(const void* p) {
+    uint4 r;
+    asm volatile("ld.relaxed.sys.global.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p) : "memory");
+    return r;
+}
+__device__ __forceinline__ void st_relaxed_sys_u64(u64* p, u64 v) {
+    asm volatile("st.relaxed.sys.global.u64 [%0], %1;" :: "l"(p), "l"(v) : "memory");
 }
 __device__ __forceinline__ u32 ld_relaxed_sys_u32(const u32* p) {
     u32 v;

@@ -178,3 +178,28 @@ __device__ inline u32 crc_serial(const cc_crc_tables* g, const u8* p, u32 n) {
     for (u32 i = 0; i < n; i++) c = g->t0[(c ^ p[i]) & 0xFFu] ^ (c >> 8);
     return c ^ 0xFFFFFFFFu;
 }
+
+// Combine one segment's CRC contribution into its record's 64-bit state word and tell whether this
+// was the record's last segment.  For nseg <= 32 a single 64-bit atomicXor carries both the
+// contribution (low half) and the segment's done bit (high half), so no fence is needed: the
+// thread that sees every other bit already set is the finisher and the returned old value holds
+// the XOR of all other contributions.  Longer records fall back to XOR + fence + counter.
+// Returns true for the finisher, with *acc = XOR of all contributions; the state word is left zero.
+__device__ __forceinline__ bool crc_record_combine(u64* state, u32 nseg, u32 c, u32 contrib, u32* acc) {
+    if (nseg == 1) { *acc = contrib; return true; }
+    if (nseg <= 32) {
+        const u32 full = nseg == 32 ? 0xFFFFFFFFu : ((1u << nseg) - 1u);
+        const u64 old = atomicXor(reinterpret_cast<unsigned long long*>(state), ((u64)(1u << c) << 32) | contrib);
+        if (((u32)(old >> 32) | (1u << c)) != full) return false;
+        *acc = (u32)old ^ contrib;
+        *state = 0;
+        return true;
+    }
+    atomicXor(reinterpret_cast<unsigned long long*>(state), (u64)contrib);
+    __threadfence();
+    const u64 old = atomicAdd(reinterpret_cast<unsigned long long*>(state), 1ull << 32);
+    if ((u32)(old >> 32) != nseg - 1) return false;
+    __threadfence();
+    *acc = (u32)atomicExch(reinterpret_cast<unsigned long long*>(state), 0ull);
+    return true;
+}

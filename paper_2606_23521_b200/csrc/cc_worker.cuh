@@ -60,39 +60,61 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
     __shared__ __align__(16) cc_task s_task;
     const cc_grid g = cc_hw_grid();
     u32 gen = ld_acquire_gpu_u32(&dev->bar_gen);
-    u64 head = 0;
+    u64 head = 0;       // ring sequence number of the next task (meaningful in the leader thread only)
+    u64 gseq = 0;       // number of grid-wide tasks so far = doorbell value already consumed
     const u64 t0 = globaltimer_ns();
     cc_crc_smem_init(cs, &dev->crc);
 
     for (;;) {
-        // ---- leader: poll the host-mapped tail, fetch the descriptor, ring the doorbell ----
+        // ---- leader: poll the host-mapped tail, fetch descriptors.  NOP and LOG_RESET need no grid:
+        //      the leader completes them on the spot; anything else is handed to all blocks through
+        //      the device-memory doorbell ----
         if (g.block == 0 && threadIdx.x == 0) {
-            bool expired = false;
-            u32 spins = 0;
-            while (ld_acquire_sys_u64(ring.tail) <= head) {
-                const u64 now = globaltimer_ns();
-                if ((spins++ & 15u) == 0) *reinterpret_cast<volatile u64*>(ring.heartbeat) = now;
-                if (now - t0 > ring.max_lifetime_ns) { expired = true; break; }
-                __nanosleep(ring.backoff_ns);
-            }
-            cc_task t;
-            if (expired) {
-                t.kind = CC_TASK_EXIT; t.region_id = 0; t.flags = 1; t.version = 0; t.seq = ~0ull;
-                t.epoch = 0; t.arg0 = t.arg1 = t.arg2 = t.arg3 = 0;
-            } else {
-                const volatile uint4* src = reinterpret_cast<const volatile uint4*>(&ring.slots[head & (ring.capacity - 1)]);
-                uint4 q[4];
+            for (;;) {
+                bool expired = false;
+                u32 spins = 0;
+                while (ld_acquire_sys_u64(ring.tail) <= head) {
+                    const u64 now = globaltimer_ns();
+                    if ((spins++ & 15u) == 0) *reinterpret_cast<volatile u64*>(ring.heartbeat) = now;
+                    if (now - t0 > ring.max_lifetime_ns) { expired = true; break; }
+                    __nanosleep(ring.backoff_ns);
+                }
+                cc_task t;
+                if (expired) {
+                    t.kind = CC_TASK_EXIT; t.region_id = 0; t.flags = 1; t.version = 0; t.seq = ~0ull;
+                    t.epoch = 0; t.arg0 = t.arg1 = t.arg2 = t.arg3 = 0;
+                } else {
+                    // four independent 16-byte system-scope loads (one host-link round trip); they are
+                    // ordered after the acquire of the tail word
+                    const char* src = reinterpret_cast<const char*>(&ring.slots[head & (ring.capacity - 1)]);
+                    uint4 q[4];
 #pragma unroll
-                for (int i = 0; i < 4; i++) { q[i].x = src[i].x; q[i].y = src[i].y; q[i].z = src[i].z; q[i].w = src[i].w; }
-                t = *reinterpret_cast<cc_task*>(q);
+                    for (int i = 0; i < 4; i++) q[i] = ld_relaxed_sys_v4(src + 16 * i);
+                    t = *reinterpret_cast<cc_task*>(q);
+                }
+                if (t.kind == CC_TASK_NOP || t.kind == CC_TASK_LOG_RESET) {
+                    const u64 ts = globaltimer_ns();
+                    if (t.kind == CC_TASK_LOG_RESET) {
+                        dev->log.W = 0;
+                        if (dev->log.committed_off) st_release_sys_u64(dev->log.committed_off, 0ull);
+                    }
+                    cc_result* out = &ring.results[t.seq & (ring.capacity - 1)];
+                    out->n_dirty = 0; out->bytes = 0; out->log_offset_after = dev->log.W; out->epoch = t.epoch;
+                    out->status = CC_OK; out->flags = t.kind; out->t_start_ns = ts; out->t_end_ns = globaltimer_ns();
+                    st_relaxed_sys_u64(ring.completed, t.seq + 1);     // a counter only; results are read through seq_done
+                    st_release_sys_u64(&out->seq_done, t.seq + 1);     // release: every field above is visible first
+                    head++;
+                    continue;
+                }
+                dev->cur_task = t;
+                __threadfence();
+                st_release_gpu_u64(&dev->doorbell, gseq + 1);
+                break;
             }
-            dev->cur_task = t;
-            __threadfence();
-            st_release_gpu_u64(&dev->doorbell, head + 1);
         }
         // ---- everyone: wait for the doorbell ----
         if (threadIdx.x == 0) {
-            while (ld_acquire_gpu_u64(&dev->doorbell) <= head) __nanosleep(ring.backoff_ns);
+            while (ld_acquire_gpu_u64(&dev->doorbell) <= gseq) __nanosleep(ring.backoff_ns < 200 ? ring.backoff_ns : 200);
             __threadfence();
             const uint4* ct = reinterpret_cast<const uint4*>(&dev->cur_task);
             uint4* st = reinterpret_cast<uint4*>(&s_task);
@@ -137,12 +159,6 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
             case CC_TASK_TEST_MUTATE:
                 cc_task_mutate(dev->regions[slot], task, g);
                 break;
-            case CC_TASK_LOG_RESET:
-                if (g.block == 0 && threadIdx.x == 0) {
-                    dev->log.W = 0;
-                    if (dev->log.committed_off) st_release_sys_u64(dev->log.committed_off, 0ull);
-                }
-                break;
             default:
                 break;
             }
@@ -163,11 +179,11 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
             out->n_dirty = n_dirty; out->bytes = bytes; out->log_offset_after = off_after; out->epoch = ep;
             out->status = status; out->flags = task.kind;
             out->t_start_ns = t_start; out->t_end_ns = globaltimer_ns();
-            __threadfence_system();
+            st_relaxed_sys_u64(ring.completed, task.seq + 1);
             st_release_sys_u64(&out->seq_done, task.seq + 1);
-            st_release_sys_u64(ring.completed, task.seq + 1);
         }
         head++;
+        gseq++;
     }
     // exit: the leader acknowledges the EXIT task (if it came from the host) and stamps the heartbeat
     if (g.block == 0 && threadIdx.x == 0) {
@@ -176,9 +192,8 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
             cc_result* out = &ring.results[t.seq & (ring.capacity - 1)];
             out->n_dirty = 0; out->bytes = 0; out->log_offset_after = dev->log.W; out->epoch = 0;
             out->status = CC_OK; out->flags = CC_TASK_EXIT; out->t_start_ns = globaltimer_ns(); out->t_end_ns = out->t_start_ns;
-            __threadfence_system();
+            st_relaxed_sys_u64(ring.completed, t.seq + 1);
             st_release_sys_u64(&out->seq_done, t.seq + 1);
-            st_release_sys_u64(ring.completed, t.seq + 1);
         }
     }
 }

@@ -113,7 +113,7 @@ static int find_slot(cc_ctx* ctx, uint32_t id) {
 }
 
 struct cc_ws_layout {
-    uint64_t hdr, bitmap, D, rec_crc, rec_done, latest, lb, total;
+    uint64_t hdr, bitmap, D, rec_state, latest, lb, total;
     uint64_t n_pages, n_words, n_tiles;
 };
 
@@ -128,8 +128,7 @@ static bool ws_layout(uint64_t bytes, uint32_t P, cc_ws_layout* L) {
     L->hdr = o; o += 256;
     L->bitmap = o; o += align_up(L->n_tiles * CC_COMPACT_TILE_WORDS * 4, 256);
     L->D = o; o += align_up(n_pages * 4, 256);
-    L->rec_crc = o; o += align_up(n_pages * 4, 256);
-    L->rec_done = o; o += align_up(n_pages * 4, 256);
+    L->rec_state = o; o += align_up(n_pages * 8, 256);
     L->latest = o; o += align_up(n_pages * 4, 256);
     L->lb = o; o += align_up(L->n_tiles * 8, 256);
     L->total = o;
@@ -261,8 +260,7 @@ extern "C" int32_t cc_register_region(cc_ctx* ctx, const cc_region_desc* d) {
     r.hdr = (cc_ws_hdr*)(ws + L.hdr);
     r.bitmap = (u32*)(ws + L.bitmap);
     r.D = (u32*)(ws + L.D);
-    r.rec_crc = (u32*)(ws + L.rec_crc);
-    r.rec_done = (u32*)(ws + L.rec_done);
+    r.rec_state = (u64*)(ws + L.rec_state);
     r.latest = (u32*)(ws + L.latest);
     r.lb_status = (u64*)(ws + L.lb);
     {
@@ -393,7 +391,7 @@ extern "C" int32_t cc_dirty_list(cc_ctx* ctx, uint32_t region_id, const uint32_t
 extern "C" uint64_t cc_apply_scratch_bytes(uint64_t max_records) {
     if (max_records == 0 || max_records > 0xFFFFFFF0ull) return 0;
     return align_up(max_records * sizeof(cc_rec), 256) + align_up(max_records * sizeof(cc_epoch_ent), 256) +
-           2 * align_up(max_records * 4, 256) + align_up((max_records + 1) * 4, 256);
+           align_up(max_records * 8, 256) + align_up((max_records + 1) * 4, 256);
 }
 
 extern "C" int32_t cc_apply_attach(cc_ctx* ctx, void* scratch, uint64_t scratch_bytes) {
@@ -413,8 +411,7 @@ extern "C" int32_t cc_apply_attach(cc_ctx* ctx, void* scratch, uint64_t scratch_
     T.max_records = m;
     T.recs = (cc_rec*)p; p += align_up(m * sizeof(cc_rec), 256);
     T.epochs = (cc_epoch_ent*)p; p += align_up(m * sizeof(cc_epoch_ent), 256);
-    T.rec_acc = (u32*)p; p += align_up(m * 4, 256);
-    T.rec_cnt = (u32*)p; p += align_up(m * 4, 256);
+    T.rec_state = (u64*)p; p += align_up(m * 8, 256);
     T.seg_begin = (u32*)p;
     ctx->tabs = T;
     ctx->apply_attached = true;

@@ -29,6 +29,7 @@ def main():
     ap.add_argument("--region-mib", type=int, default=256)
     ap.add_argument("--page", type=int, default=4096)
     ap.add_argument("--dirty", type=float, default=0.01)
+    ap.add_argument("--device-log", action="store_true", help="log buffer in device memory instead of pinned host")
     ap.add_argument("--worker-blocks", type=int, default=0)
     ap.add_argument("--worker-threads", type=int, default=0)
     a = ap.parse_args()
@@ -43,7 +44,10 @@ def main():
                      max_lifetime_ns=int(300e9))
     ctx.register_region(1, cur, P)
     per = n_mut * (16 + P) + 32
-    log = torch.empty(max(1 << 30, 2 * per), dtype=torch.uint8, pin_memory=True)
+    if a.device_log:
+        log = torch.empty(max(1 << 30, 2 * per), dtype=torch.uint8, device="cuda")
+    else:
+        log = torch.empty(max(1 << 30, 2 * per), dtype=torch.uint8, pin_memory=True)
     ctx.log_attach(log)
     lib, h = ctx.lib, ctx.h
     A = 2 * ((1006 * 7919 + 12345) % 100000) + 1
@@ -80,9 +84,12 @@ def main():
             nop_rt.append(t2 - t0)
         # (iii) + (iv): mutate -> checkpoint tasks
         rt, dev_ns, ks = [], [], []
+        used = 0
         for t in range(a.tasks):
-            if t and t % 256 == 0:
+            if used + per > log.numel():
                 ctx.wait(ctx.submit(cc.CC_TASK_LOG_RESET), 30.0)
+                used = 0
+            used += per
             hh = (1006 * 2654435761 + t * 40503) & 0xFFFFFFFF
             ctx.wait(ctx.submit(cc.CC_TASK_TEST_MUTATE, region_id=1, arg0=n_mut, arg1=A, arg2=hh), 30.0)
             ck = cc.cc_task(cc.CC_TASK_DELTA_CKPT, 1, 0, 0, 0, t, 0, 0, 0, 0)
@@ -98,7 +105,7 @@ def main():
         us = lambda xs, q: round(_pct(xs, q) / 1e3, 2)
         out = {
             "config": {"region_MiB": a.region_mib, "page_bytes": P, "dirty_pages_per_task": n_mut, "tasks": a.tasks,
-                       "log": "pinned host", "bytes_per_task": per},
+                       "log": "device" if a.device_log else "pinned host", "bytes_per_task": per},
             "submit_host_cost_us": {"p50": us(submit_ns, 0.5), "p99": us(submit_ns, 0.99)},
             "nop_round_trip_us": {"p50": us(nop_rt, 0.5), "p99": us(nop_rt, 0.99)},
             "checkpoint_task_round_trip_us": {"p50": us(rt, 0.5), "p99": us(rt, 0.99)},
