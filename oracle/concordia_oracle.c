@@ -366,3 +366,121 @@ uint64_t orc_scan_mt(const uint8_t *cur, const uint8_t *shadow, uint64_t N, uint
     }
     return k;
 }
+
+/* ------------------------- allocator-aware discovery --- */
+
+/* The paper's second discovery policy ("the serving runtime exposes the block
+ * table, allocation bitmap, and optional dirty-block/version metadata ... falls back to page
+ * diffing only when such metadata is unavailable"; L257 "Allocator-aware regions ... use
+ * block-table version counters or dirty-block bitmaps supplied by the serving runtime;
+ * Concordia then copies the marked physical pages"; L261 "reads allocator dirty metadata or
+ * compares ..."; L264 "Allocator version counters are advanced"; L266 "discovery is
+ * proportional to the dirty block bitmap").  Readings (#29-#32):
+ *   marked  : packed bitmap, page p = bit (p & 31) of little-endian u32 word p >> 5; bits at
+ *             or beyond n_pages are ignored.
+ *   verify=0: D = marked pages ("copies the marked physical pages"): a marked page is logged
+ *             even when its bytes equal the shadow.
+ *   verify=1: D = marked pages whose bytes differ from the shadow (the mark narrows the diff).
+ *   shadow  : may be NULL with verify=0 (allocator-aware regions need no shadow); when present
+ *             it is refreshed for the pages in D exactly as in orc_checkpoint step 8.
+ *   consume : on ORC_OK every word of `marked` is cleared (the runtime's bitmap is handed back
+ *             empty); on ORC_ERR_LOG_FULL it is left alone so that a retry sees the same marks.
+ * Steps 4-9 (empty epoch, capacity check, records, commit, shadow, publish) are those of
+ * orc_checkpoint, written out again rather than shared. */
+static int marked_bit(const uint8_t *bm, uint64_t p) {
+    uint32_t w = get_u32(bm + 4 * (p >> 5));
+    return (int)((w >> (p & 31u)) & 1u);
+}
+
+static int32_t append_flagged(const uint8_t *cur, uint8_t *shadow, uint64_t N, uint64_t P, uint32_t region_id,
+                              uint64_t epoch, const uint8_t *dirty, uint64_t k, uint8_t *log, uint64_t C,
+                              uint64_t *W, uint64_t *bytes_out) {
+    uint64_t n_pages = (N + P - 1) / P;
+    uint64_t need = ORC_COMMIT_BYTES;
+    for (uint64_t p = 0; p < n_pages; p++)
+        if (dirty[p]) need += ORC_HDR + page_len(N, P, p);
+    if (*W + need > C) return ORC_ERR_LOG_FULL;
+    uint64_t off = *W;
+    for (uint64_t p = 0; p < n_pages; p++) {
+        if (!dirty[p]) continue;
+        uint64_t len = page_len(N, P, p);
+        const uint8_t *src = cur + p * P;
+        put_u32(log + off + 0, region_id);
+        put_u32(log + off + 4, (uint32_t)p);
+        put_u32(log + off + 8, (uint32_t)len);
+        put_u32(log + off + 12, orc_crc32c(src, len));
+        memcpy(log + off + ORC_HDR, src, len);
+        off += ORC_HDR + len;
+    }
+    uint8_t cp[16];
+    put_u64(cp + 0, epoch);
+    put_u32(cp + 8, region_id);
+    put_u32(cp + 12, (uint32_t)k);
+    put_u32(log + off + 0, ORC_COMMIT_ID);
+    put_u32(log + off + 4, ORC_COMMIT_ID);
+    put_u32(log + off + 8, 16u);
+    put_u32(log + off + 12, orc_crc32c(cp, 16));
+    memcpy(log + off + ORC_HDR, cp, 16);
+    off += ORC_COMMIT_BYTES;
+    if (shadow)
+        for (uint64_t p = 0; p < n_pages; p++)
+            if (dirty[p]) memcpy(shadow + p * P, cur + p * P, page_len(N, P, p));
+    *bytes_out = off - *W;
+    *W = off;
+    return ORC_OK;
+}
+
+int32_t orc_checkpoint_marked(const uint8_t *cur, uint8_t *shadow, uint64_t N, uint64_t P,
+                              uint32_t region_id, uint64_t epoch, uint8_t *marked, int verify, int consume,
+                              uint8_t *log, uint64_t C, uint64_t *W,
+                              uint32_t *D_out, uint64_t *k_out, uint64_t *bytes_out) {
+    if (P == 0 || N == 0 || region_id == 0 || region_id == ORC_COMMIT_ID) return ORC_ERR_INVALID;
+    if (verify && !shadow) return ORC_ERR_INVALID;
+    uint64_t n_pages = (N + P - 1) / P;
+    if (n_pages > 0xFFFFFFFEull) return ORC_ERR_INVALID;
+    uint8_t *dirty = (uint8_t *)malloc(n_pages);
+    if (!dirty) return ORC_ERR_INVALID;
+    uint64_t k = 0;
+    for (uint64_t p = 0; p < n_pages; p++) {
+        int d = marked_bit(marked, p);
+        if (d && verify) d = memcmp(cur + p * P, shadow + p * P, page_len(N, P, p)) != 0;
+        dirty[p] = (uint8_t)d;
+        if (d) { if (D_out) D_out[k] = (uint32_t)p; k++; }
+    }
+    *k_out = k;
+    *bytes_out = 0;
+    int32_t st = ORC_OK;
+    if (k != 0) st = append_flagged(cur, shadow, N, P, region_id, epoch, dirty, k, log, C, W, bytes_out);
+    if (st == ORC_OK && consume) memset(marked, 0, 4 * ((n_pages + 31) / 32));
+    free(dirty);
+    return st;
+}
+
+/* Version-counter form of the same policy (L257 "block-table version counters", L264 "Allocator
+ * version counters are advanced"): page p is dirty iff version[p] != committed[p]; after a
+ * successful append committed[p] := version[p] for the pages in D (on LOG_FULL nothing moves). */
+int32_t orc_checkpoint_versions(const uint8_t *cur, uint8_t *shadow, uint64_t N, uint64_t P,
+                                uint32_t region_id, uint64_t epoch, const uint64_t *version, uint64_t *committed,
+                                uint8_t *log, uint64_t C, uint64_t *W,
+                                uint32_t *D_out, uint64_t *k_out, uint64_t *bytes_out) {
+    if (P == 0 || N == 0 || region_id == 0 || region_id == ORC_COMMIT_ID) return ORC_ERR_INVALID;
+    uint64_t n_pages = (N + P - 1) / P;
+    if (n_pages > 0xFFFFFFFEull) return ORC_ERR_INVALID;
+    uint8_t *dirty = (uint8_t *)malloc(n_pages);
+    if (!dirty) return ORC_ERR_INVALID;
+    uint64_t k = 0;
+    for (uint64_t p = 0; p < n_pages; p++) {
+        int d = version[p] != committed[p];
+        dirty[p] = (uint8_t)d;
+        if (d) { if (D_out) D_out[k] = (uint32_t)p; k++; }
+    }
+    *k_out = k;
+    *bytes_out = 0;
+    int32_t st = ORC_OK;
+    if (k != 0) st = append_flagged(cur, shadow, N, P, region_id, epoch, dirty, k, log, C, W, bytes_out);
+    if (st == ORC_OK)
+        for (uint64_t p = 0; p < n_pages; p++)
+            if (dirty[p]) committed[p] = version[p];
+    free(dirty);
+    return st;
+}

@@ -51,6 +51,14 @@ def _load():
         lib.orc_checkpoint.restype = ctypes.c_int32
         lib.orc_checkpoint.argtypes = [u8p, u8p, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint32, ctypes.c_uint64,
                                        u8p, ctypes.c_uint64, u64p, u32p, u64p, u64p]
+        lib.orc_checkpoint_marked.restype = ctypes.c_int32
+        lib.orc_checkpoint_marked.argtypes = [u8p, u8p, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint32,
+                                              ctypes.c_uint64, u8p, ctypes.c_int, ctypes.c_int,
+                                              u8p, ctypes.c_uint64, u64p, u32p, u64p, u64p]
+        lib.orc_checkpoint_versions.restype = ctypes.c_int32
+        lib.orc_checkpoint_versions.argtypes = [u8p, u8p, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint32,
+                                                ctypes.c_uint64, u8p, u8p,
+                                                u8p, ctypes.c_uint64, u64p, u32p, u64p, u64p]
         lib.orc_apply.restype = ctypes.c_int32
         lib.orc_apply.argtypes = [u8p, ctypes.c_uint64, ctypes.POINTER(_CRegion), ctypes.c_uint32, u64p, u64p]
         lib.orc_write_epoch.restype = ctypes.c_int32
@@ -119,6 +127,40 @@ def checkpoint(cur, shadow, page_bytes: int, region_id: int, epoch: int, log, W:
     nb = ctypes.c_uint64(0)
     st = _load().orc_checkpoint(_ptr(c), _ptr(s), c.size, page_bytes, region_id, epoch,
                                 _ptr(lg), lg.size, ctypes.byref(w), _ptr(D), ctypes.byref(k), ctypes.byref(nb))
+    return int(st), D[: k.value].copy(), int(nb.value), int(w.value)
+
+
+def checkpoint_marked(cur, shadow, page_bytes: int, region_id: int, epoch: int, marked, log, W: int,
+                      verify: bool = False, consume: bool = False):
+    """Allocator-aware checkpoint from a packed dirty-page bitmap (uint32 words, numpy, modified in place
+    when consume=True).  shadow may be None when verify=False.  Returns (status, D, bytes_appended, W_after)."""
+    c, lg = _u8(cur), _u8(log)
+    s = None if shadow is None else _u8(shadow)
+    n_pages = (c.size + page_bytes - 1) // page_bytes
+    m = np.asarray(marked)
+    assert m.dtype == np.uint32 and m.flags["C_CONTIGUOUS"] and m.size >= (n_pages + 31) // 32
+    D = np.zeros(max(n_pages, 1), dtype=np.uint32)
+    w, k, nb = ctypes.c_uint64(W), ctypes.c_uint64(0), ctypes.c_uint64(0)
+    st = _load().orc_checkpoint_marked(_ptr(c), None if s is None else _ptr(s), c.size, page_bytes, region_id, epoch,
+                                       _ptr(m), int(verify), int(consume), _ptr(lg), lg.size, ctypes.byref(w),
+                                       _ptr(D), ctypes.byref(k), ctypes.byref(nb))
+    return int(st), D[: k.value].copy(), int(nb.value), int(w.value)
+
+
+def checkpoint_versions(cur, shadow, page_bytes: int, region_id: int, epoch: int, version, committed, log, W: int):
+    """Allocator-aware checkpoint from per-page version counters (uint64 numpy arrays; ``committed`` is
+    advanced in place).  shadow may be None.  Returns (status, D, bytes_appended, W_after)."""
+    c, lg = _u8(cur), _u8(log)
+    s = None if shadow is None else _u8(shadow)
+    n_pages = (c.size + page_bytes - 1) // page_bytes
+    v, cm = np.asarray(version), np.asarray(committed)
+    assert v.dtype == np.uint64 and cm.dtype == np.uint64 and v.size == n_pages == cm.size
+    assert v.flags["C_CONTIGUOUS"] and cm.flags["C_CONTIGUOUS"] and cm.flags["WRITEABLE"]
+    D = np.zeros(max(n_pages, 1), dtype=np.uint32)
+    w, k, nb = ctypes.c_uint64(W), ctypes.c_uint64(0), ctypes.c_uint64(0)
+    st = _load().orc_checkpoint_versions(_ptr(c), None if s is None else _ptr(s), c.size, page_bytes, region_id, epoch,
+                                         _ptr(v), _ptr(cm), _ptr(lg), lg.size, ctypes.byref(w),
+                                         _ptr(D), ctypes.byref(k), ctypes.byref(nb))
     return int(st), D[: k.value].copy(), int(nb.value), int(w.value)
 
 
