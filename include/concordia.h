@@ -67,6 +67,13 @@ extern "C" {
 
 /* cc_region_desc.flags */
 #define CC_REG_SNAPSHOT_NOW 1u     /* shadow := base at registration (first delta is relative to now) */
+#define CC_REG_NO_SHADOW 2u        /* allocator-aware region: `shadow` is NULL, dirty pages come from
+                                      cc_checkpoint_marked / cc_checkpoint_versions only; calls that need the shadow
+                                      (cc_checkpoint_delta, cc_scan_only, CC_MARK_VERIFY) return CC_ERR_INVALID */
+
+/* cc_checkpoint_marked flags */
+#define CC_MARK_VERIFY 1u          /* compare the marked pages with the shadow and log only those that differ */
+#define CC_MARK_CONSUME 2u         /* clear the caller's bitmap once the checkpoint went through (not on LOG_FULL) */
 
 typedef struct cc_ctx cc_ctx;
 
@@ -83,7 +90,8 @@ typedef struct {
     uint32_t page_bytes;       /* P: multiple of 16 (benchmarks: 4096 / 16384 / 65536) */
     uint64_t bytes;            /* N: multiple of 16, > 0; the last page may be short; ceil(N/P) <= 2^31 */
     void*    base;             /* live region, device, 16-byte aligned */
-    void*    shadow;           /* last-committed copy, device, N bytes, 16-byte aligned, caller-allocated */
+    void*    shadow;           /* last-committed copy, device, N bytes, 16-byte aligned, caller-allocated
+                                  (NULL with CC_REG_NO_SHADOW) */
     void*    workspace;        /* device, 256-byte aligned, >= cc_workspace_bytes(N, P); zeroed by the call */
     uint64_t workspace_bytes;
     uint32_t flags;            /* CC_REG_* */
@@ -111,6 +119,8 @@ typedef struct {
 #define CC_TASK_LOG_RESET 3u       /* W := 0 */
 #define CC_TASK_TEST_MUTATE 4u     /* bench/test only: region_id; arg0 = n_mut, arg1 = A (odd), arg2 = h:
                                       for j < n_mut: page (j*A + h) mod n_pages, byte (h + j) mod len_p, ^= 0x5A */
+#define CC_TASK_MARKED_CKPT 5u     /* region_id, epoch; arg0 = dirty bitmap (device), arg1 = CC_MARK_* flags */
+#define CC_TASK_VERSION_CKPT 6u    /* region_id, epoch; arg0 = version[] (device), arg1 = committed[] (device) */
 #define CC_TASK_EXIT 255u
 typedef struct {
     uint32_t kind;
@@ -169,6 +179,28 @@ int32_t cc_log_reset_async(cc_ctx* ctx, void* stream);
  * quiescent).  The ascending dirty list of the last checkpoint stays readable in the workspace
  * (cc_dirty_list). */
 int32_t cc_checkpoint_delta(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out);
+
+/* Allocator-aware delta checkpoint ("reads allocator dirty metadata", L266
+ * "discovery is proportional to the dirty block bitmap"): the dirty set comes from the runtime's
+ * dirty-page bitmap instead of a scan of the whole region.  `dirty_bitmap` is device memory, 4-byte
+ * aligned, ceil(n_pages/32) u32 words; page p is bit (p & 31) of word p >> 5; bits at or beyond
+ * n_pages are ignored.  flags = 0: every marked page is logged ("copies the marked physical pages"),
+ * whether or not its bytes changed.  CC_MARK_VERIFY: only the marked pages are compared with the
+ * shadow and those that differ are logged -- the same log as cc_checkpoint_delta whenever the marks
+ * cover the dirty set.  CC_MARK_CONSUME: the bitmap words are zeroed once the checkpoint went through
+ * (status CC_OK, an empty epoch included); on CC_ERR_LOG_FULL they are left alone.  Everything else
+ * (records, commit, shadow refresh of the logged pages when the region has a shadow, result,
+ * asynchrony) is as in cc_checkpoint_delta. */
+int32_t cc_checkpoint_marked(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, uint32_t* dirty_bitmap,
+                             uint32_t flags, void* stream, cc_result* out);
+
+/* Same, from per-page version counters ("block-table version counters", L264 "Allocator
+ * version counters are advanced"): page p is dirty iff version[p] != committed[p] (both device, u64,
+ * n_pages entries, 8-byte aligned; `committed` is caller-owned state that only this call writes).
+ * After a successful append committed[p] := version[p] for the logged pages; on CC_ERR_LOG_FULL
+ * nothing moves. */
+int32_t cc_checkpoint_versions(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, const uint64_t* version,
+                               uint64_t* committed, void* stream, cc_result* out);
 
 /* Scan + compaction only (steps a1-a2), for measurement: fills the dirty list, appends nothing,
  * leaves the shadow alone.  out->n_dirty = k. */

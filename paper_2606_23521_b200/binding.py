@@ -27,18 +27,23 @@ CC_ERR_TIMEOUT = -9
 CC_ERR_SCRATCH = -10
 
 CC_REG_SNAPSHOT_NOW = 1
+CC_REG_NO_SHADOW = 2
+CC_MARK_VERIFY = 1
+CC_MARK_CONSUME = 2
 
 CC_TASK_NOP = 0
 CC_TASK_DELTA_CKPT = 1
 CC_TASK_RESTORE = 2
 CC_TASK_LOG_RESET = 3
 CC_TASK_TEST_MUTATE = 4
+CC_TASK_MARKED_CKPT = 5
+CC_TASK_VERSION_CKPT = 6
 CC_TASK_EXIT = 255
 
 EXPORTS = [
     "cc_init", "cc_shutdown", "cc_last_cuda_error", "cc_kernel_launches", "cc_workspace_bytes",
     "cc_register_region", "cc_unregister_region", "cc_log_attach", "cc_log_reset", "cc_log_reset_async",
-    "cc_checkpoint_delta",
+    "cc_checkpoint_delta", "cc_checkpoint_marked", "cc_checkpoint_versions",
     "cc_scan_only", "cc_trace_events", "cc_dirty_list", "cc_apply_scratch_bytes", "cc_apply_attach", "cc_apply_log",
     "cc_worker_start", "cc_worker_stop", "cc_worker_alive", "cc_peek_queue", "cc_submit", "cc_poll", "cc_wait",
 ]
@@ -102,6 +107,8 @@ def load_library():
         "cc_log_reset": (i32, [vp]),
         "cc_log_reset_async": (i32, [vp, vp]),
         "cc_checkpoint_delta": (i32, [vp, u32, u64, vp, vp]),
+        "cc_checkpoint_marked": (i32, [vp, u32, u64, vp, u32, vp, vp]),
+        "cc_checkpoint_versions": (i32, [vp, u32, u64, vp, vp, vp, vp]),
         "cc_scan_only": (i32, [vp, u32, vp, vp]),
         "cc_trace_events": (i32, [vp, vp, vp]),
         "cc_dirty_list": (i32, [vp, u32, P(vp), P(vp)]),
@@ -184,21 +191,26 @@ class Context:
 
     # -- regions
     def register_region(self, region_id: int, base: torch.Tensor, page_bytes: int, shadow: torch.Tensor = None,
-                        snapshot_now: bool = True):
+                        snapshot_now: bool = True, no_shadow: bool = False):
         """base/shadow: contiguous CUDA tensors of equal byte size.  Allocates shadow and workspace with
-        torch if not given.  Returns the shadow tensor (uint8 view)."""
+        torch if not given.  Returns the shadow tensor (uint8 view), or None for an allocator-aware
+        region registered with no_shadow=True (CC_REG_NO_SHADOW)."""
         assert base.is_cuda and base.is_contiguous()
         nbytes = base.numel() * base.element_size()
-        if shadow is None:
+        if no_shadow:
+            assert shadow is None
+            snapshot_now = False
+        elif shadow is None:
             shadow = torch.empty(nbytes, dtype=torch.uint8, device=base.device)
-        assert shadow.is_cuda and shadow.is_contiguous() and shadow.numel() * shadow.element_size() == nbytes
+        assert no_shadow or (shadow.is_cuda and shadow.is_contiguous() and shadow.numel() * shadow.element_size() == nbytes)
         wsb = self.workspace_bytes(nbytes, page_bytes)
         if wsb == 0:
             raise ConcordiaError("cc_workspace_bytes", CC_ERR_INVALID)
         ws = torch.empty(wsb + 256, dtype=torch.uint8, device=base.device)
         off = (-ws.data_ptr()) % 256
-        d = cc_region_desc(region_id, page_bytes, nbytes, base.data_ptr(), shadow.data_ptr(), ws.data_ptr() + off,
-                           wsb, CC_REG_SNAPSHOT_NOW if snapshot_now else 0, 0)
+        flags = (CC_REG_SNAPSHOT_NOW if snapshot_now else 0) | (CC_REG_NO_SHADOW if no_shadow else 0)
+        d = cc_region_desc(region_id, page_bytes, nbytes, base.data_ptr(), None if no_shadow else shadow.data_ptr(),
+                           ws.data_ptr() + off, wsb, flags, 0)
         self._check("cc_register_region", self.lib.cc_register_region(self.h, ctypes.byref(d)))
         self._keep[region_id] = (base, shadow, ws)
         return shadow
@@ -228,6 +240,23 @@ class Context:
     def checkpoint_delta(self, region_id: int, epoch: int, result: Result = None, stream=None):
         self._check("cc_checkpoint_delta", self.lib.cc_checkpoint_delta(
             self.h, region_id, epoch, _stream_ptr(stream), ctypes.c_void_p(result.ptr) if result else None))
+
+    def checkpoint_marked(self, region_id: int, epoch: int, dirty_bitmap: torch.Tensor, flags: int = 0,
+                          result: Result = None, stream=None):
+        """dirty_bitmap: CUDA int32/uint32 tensor of ceil(n_pages/32) words (bit p&31 of word p>>5)."""
+        assert dirty_bitmap.is_cuda and dirty_bitmap.is_contiguous() and dirty_bitmap.element_size() == 4
+        self._check("cc_checkpoint_marked", self.lib.cc_checkpoint_marked(
+            self.h, region_id, epoch, dirty_bitmap.data_ptr(), flags, _stream_ptr(stream),
+            ctypes.c_void_p(result.ptr) if result else None))
+
+    def checkpoint_versions(self, region_id: int, epoch: int, version: torch.Tensor, committed: torch.Tensor,
+                            result: Result = None, stream=None):
+        """version / committed: CUDA int64 tensors with one entry per page; committed is advanced in place."""
+        for t in (version, committed):
+            assert t.is_cuda and t.is_contiguous() and t.element_size() == 8
+        self._check("cc_checkpoint_versions", self.lib.cc_checkpoint_versions(
+            self.h, region_id, epoch, version.data_ptr(), committed.data_ptr(), _stream_ptr(stream),
+            ctypes.c_void_p(result.ptr) if result else None))
 
     def scan_only(self, region_id: int, result: Result = None, stream=None):
         self._check("cc_scan_only", self.lib.cc_scan_only(

@@ -256,7 +256,7 @@ __device__ __forceinline__ void cc_apply_scatter_phase(cc_dev* dev, const cc_app
 #pragma unroll
         for (int u = 0; u < U; u++) {
             const u32 j = lane + 32 * u;
-            if (j < nv) { st_stream(d0 + j, v[u]); st_stream(d1 + j, v[u]); }
+            if (j < nv) { st_stream(d0 + j, v[u]); if (r.shadow) st_stream(d1 + j, v[u]); }
         }
     }
 }

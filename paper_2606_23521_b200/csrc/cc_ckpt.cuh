@@ -237,6 +237,7 @@ __device__ __forceinline__ void cc_gather_phase(const cc_region_dev& r, cc_dev* 
             const u32 nseg = (u32)((plen + CC_SEG_BYTES - 1) / CC_SEG_BYTES);
             const u64 src_off = (u64)p * P + so;
             const uint4* src = reinterpret_cast<const uint4*>(r.base + src_off);
+            const bool has_shadow = r.shadow != nullptr;      // allocator-aware regions may have none (cc_mark.cuh)
             uint4* dsh = reinterpret_cast<uint4*>(r.shadow + src_off);
             u8* rec = log->buf + W0 + (u64)i * rec_stride;
             uint4* dlog = reinterpret_cast<uint4*>(rec + CC_RECORD_HEADER_BYTES + so);
@@ -246,8 +247,10 @@ __device__ __forceinline__ void cc_gather_phase(const cc_region_dev& r, cc_dev* 
                 for (int u = 0; u < U; u++) v[u] = ld_stream(src + lane + 32 * u);
 #pragma unroll
                 for (int u = 0; u < U; u++) st_stream(dlog + lane + 32 * u, v[u]);
+                if (has_shadow) {
 #pragma unroll
-                for (int u = 0; u < U; u++) st_stream(dsh + lane + 32 * u, v[u]);
+                    for (int u = 0; u < U; u++) st_stream(dsh + lane + 32 * u, v[u]);
+                }
             } else {
 #pragma unroll
                 for (int u = 0; u < U; u++) {
@@ -255,7 +258,7 @@ __device__ __forceinline__ void cc_gather_phase(const cc_region_dev& r, cc_dev* 
                     if (j < nv) {
                         v[u] = ld_stream(src + j);
                         st_stream(dlog + j, v[u]);
-                        st_stream(dsh + j, v[u]);
+                        if (has_shadow) st_stream(dsh + j, v[u]);
                     } else {
                         v[u] = make_uint4(0, 0, 0, 0);
                     }

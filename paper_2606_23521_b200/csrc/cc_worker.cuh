@@ -12,6 +12,7 @@
 #pragma once
 #include "cc_common.cuh"
 #include "cc_ckpt.cuh"
+#include "cc_mark.cuh"
 #include "cc_apply.cuh"
 
 struct cc_ring_dev {            // all pointers are pinned, device-mapped host memory
@@ -128,9 +129,17 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
 
         int32_t status = CC_OK;
         int slot = -1;
-        if (task.kind == CC_TASK_DELTA_CKPT || task.kind == CC_TASK_TEST_MUTATE) {
+        const bool is_ckpt = task.kind == CC_TASK_DELTA_CKPT || task.kind == CC_TASK_MARKED_CKPT ||
+                             task.kind == CC_TASK_VERSION_CKPT;
+        if (is_ckpt || task.kind == CC_TASK_TEST_MUTATE) {
             slot = cc_find_slot(dev, task.region_id);
             if (slot < 0) status = CC_ERR_NOT_REGISTERED;
+            else if (dev->regions[slot].shadow == nullptr &&
+                     (task.kind == CC_TASK_DELTA_CKPT || (task.kind == CC_TASK_MARKED_CKPT && (task.arg1 & CC_MARK_VERIFY))))
+                status = CC_ERR_INVALID;
+            if (task.kind == CC_TASK_MARKED_CKPT && (task.arg0 == 0 || (task.arg0 & 3))) status = CC_ERR_INVALID;
+            if (task.kind == CC_TASK_VERSION_CKPT && (task.arg0 == 0 || task.arg1 == 0 || ((task.arg0 | task.arg1) & 7)))
+                status = CC_ERR_INVALID;
         }
         if (status == CC_OK) {
             switch (task.kind) {
@@ -141,6 +150,39 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
                 cc_compact_phase(r, &dev->log, CC_MODE_CHECKPOINT, task.epoch, nullptr);
                 cc_grid_barrier(dev, g.nblocks, gen);
                 cc_gather_phase(r, dev, cs, g, nullptr, task.kind, false);
+                break;
+            }
+            case CC_TASK_MARKED_CKPT: {
+                const cc_region_dev& r = dev->regions[slot];
+                u32* marks = reinterpret_cast<u32*>(task.arg0);
+                cc_mark_load_phase(r, marks, g);
+                cc_grid_barrier(dev, g.nblocks, gen);
+                if (task.arg1 & CC_MARK_VERIFY) {
+                    cc_compact_phase(r, &dev->log, CC_MODE_SCAN_ONLY, task.epoch, nullptr);
+                    cc_grid_barrier(dev, g.nblocks, gen);
+                    cc_mark_verify_phase(r, g);
+                    cc_grid_barrier(dev, g.nblocks, gen);
+                }
+                cc_compact_phase(r, &dev->log, CC_MODE_CHECKPOINT, task.epoch, nullptr);
+                cc_grid_barrier(dev, g.nblocks, gen);
+                cc_gather_phase(r, dev, cs, g, nullptr, task.kind, false);
+                if (task.arg1 & CC_MARK_CONSUME) {
+                    cc_grid_barrier(dev, g.nblocks, gen);
+                    cc_mark_finish_phase(r, marks, nullptr, nullptr, g);
+                }
+                break;
+            }
+            case CC_TASK_VERSION_CKPT: {
+                const cc_region_dev& r = dev->regions[slot];
+                const u64* ver = reinterpret_cast<const u64*>(task.arg0);
+                u64* com = reinterpret_cast<u64*>(task.arg1);
+                cc_mark_versions_phase(r, ver, com, g);
+                cc_grid_barrier(dev, g.nblocks, gen);
+                cc_compact_phase(r, &dev->log, CC_MODE_CHECKPOINT, task.epoch, nullptr);
+                cc_grid_barrier(dev, g.nblocks, gen);
+                cc_gather_phase(r, dev, cs, g, nullptr, task.kind, false);
+                cc_grid_barrier(dev, g.nblocks, gen);
+                cc_mark_finish_phase(r, nullptr, ver, com, g);
                 break;
             }
             case CC_TASK_RESTORE: {
@@ -168,7 +210,7 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
         if (g.block == 0 && threadIdx.x == 0) {
             cc_result* out = &ring.results[task.seq & (ring.capacity - 1)];
             u64 n_dirty = 0, bytes = 0, off_after = dev->log.W, ep = task.epoch;
-            if (status == CC_OK && task.kind == CC_TASK_DELTA_CKPT) {
+            if (status == CC_OK && is_ckpt) {
                 const cc_ws_hdr* h = dev->regions[slot].hdr;
                 n_dirty = h->k; bytes = h->need; status = h->status;
             } else if (status == CC_OK && task.kind == CC_TASK_RESTORE) {

@@ -12,6 +12,7 @@
 #include "cc_common.cuh"
 #include "cc_crc.cuh"
 #include "cc_ckpt.cuh"
+#include "cc_mark.cuh"
 #include "cc_apply.cuh"
 #include "cc_worker.cuh"
 
@@ -35,10 +36,26 @@ __global__ void __launch_bounds__(CC_COMPACT_THREADS) cc_compact_kernel(cc_dev* 
     cc_compact_phase(dev->regions[slot], &dev->log, mode, epoch, out);
 }
 
-__global__ void __launch_bounds__(CC_GATHER_THREADS) cc_gather_kernel(cc_dev* dev, int slot, cc_result* out) {
+__global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_gather_kernel(cc_dev* dev, int slot, cc_result* out) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cc_gather_phase(dev->regions[slot], dev, reinterpret_cast<cc_crc_smem*>(smem_raw), cc_hw_grid(), out,
                     CC_TASK_DELTA_CKPT, true);
+}
+
+// allocator-aware discovery (cc_mark.cuh)
+__global__ void __launch_bounds__(256) cc_mark_load_kernel(const cc_dev* dev, int slot, const u32* marks) {
+    cc_mark_load_phase(dev->regions[slot], marks, cc_hw_grid());
+}
+__global__ void __launch_bounds__(256) cc_mark_versions_kernel(const cc_dev* dev, int slot, const u64* version,
+                                                               const u64* committed) {
+    cc_mark_versions_phase(dev->regions[slot], version, committed, cc_hw_grid());
+}
+__global__ void __launch_bounds__(CC_SCAN_THREADS) cc_mark_verify_kernel(const cc_dev* dev, int slot) {
+    cc_mark_verify_phase(dev->regions[slot], cc_hw_grid());
+}
+__global__ void __launch_bounds__(256) cc_mark_finish_kernel(const cc_dev* dev, int slot, u32* marks_to_clear,
+                                                             const u64* version, u64* committed) {
+    cc_mark_finish_phase(dev->regions[slot], marks_to_clear, version, committed, cc_hw_grid());
 }
 
 __global__ void __launch_bounds__(CC_PARSE_THREADS) cc_apply_parse_kernel(cc_dev* dev, cc_apply_tabs tabs, const u8* log, u64 n) {
@@ -232,9 +249,11 @@ extern "C" int32_t cc_register_region(cc_ctx* ctx, const cc_region_desc* d) {
     if (ctx->worker_running) return CC_ERR_WORKER;
     cc_ws_layout L;
     if (d->region_id == 0 || d->region_id == CC_COMMIT_ID || !ws_layout(d->bytes, d->page_bytes, &L)) return CC_ERR_INVALID;
-    if (!d->base || !d->shadow || !d->workspace || ((uintptr_t)d->base & 15) || ((uintptr_t)d->shadow & 15) ||
+    const bool no_shadow = (d->flags & CC_REG_NO_SHADOW) != 0;
+    if (!d->base || !d->workspace || ((uintptr_t)d->base & 15) || ((uintptr_t)d->shadow & 15) ||
         ((uintptr_t)d->workspace & 255) || d->workspace_bytes < L.total)
         return CC_ERR_INVALID;
+    if (no_shadow ? (d->shadow != nullptr || (d->flags & CC_REG_SNAPSHOT_NOW)) : (d->shadow == nullptr)) return CC_ERR_INVALID;
     if (find_slot(ctx, d->region_id) >= 0) return CC_ERR_EXISTS;
     int slot = -1;
     for (int s = 0; s < CC_MAX_REGIONS; s++)
@@ -331,6 +350,17 @@ extern "C" int32_t cc_log_reset_async(cc_ctx* ctx, void* stream) {
 
 // ------------------------------------------------------------- host-launched path --
 
+static int32_t launch_compact(cc_ctx* ctx, int slot, u32 mode, uint64_t epoch, cudaStream_t st, cc_result* out) {
+    const cc_region_dev& r = ctx->regions[slot].dev;
+    const uint64_t n_tiles = (r.n_words + CC_COMPACT_TILE_WORDS - 1) / CC_COMPACT_TILE_WORDS;
+    uint64_t g2 = n_tiles < (uint64_t)ctx->sm_count * 4 ? n_tiles : (uint64_t)ctx->sm_count * 4;
+    cc_compact_kernel<<<(unsigned)g2, CC_COMPACT_THREADS, 0, st>>>(ctx->d_dev, slot, mode, epoch, out);
+    if (ctx->ev_after_compact) cudaEventRecord(ctx->ev_after_compact, st);
+    ctx->launches += 1;
+    CC_CUDA(ctx, cudaGetLastError());
+    return CC_OK;
+}
+
 static int32_t launch_scan_compact(cc_ctx* ctx, int slot, u32 mode, uint64_t epoch, cudaStream_t st, cc_result* out) {
     const cc_region_dev& r = ctx->regions[slot].dev;
     const uint64_t n_items = r.n_pages * (uint64_t)r.spp;
@@ -340,11 +370,76 @@ static int32_t launch_scan_compact(cc_ctx* ctx, int slot, u32 mode, uint64_t epo
     if (g1 > cap1) g1 = cap1;
     cc_scan_kernel<<<(unsigned)g1, CC_SCAN_THREADS, 0, st>>>(ctx->d_dev, slot);
     if (ctx->ev_after_scan) cudaEventRecord(ctx->ev_after_scan, st);
-    const uint64_t n_tiles = (r.n_words + CC_COMPACT_TILE_WORDS - 1) / CC_COMPACT_TILE_WORDS;
-    uint64_t g2 = n_tiles < (uint64_t)ctx->sm_count * 4 ? n_tiles : (uint64_t)ctx->sm_count * 4;
-    cc_compact_kernel<<<(unsigned)g2, CC_COMPACT_THREADS, 0, st>>>(ctx->d_dev, slot, mode, epoch, out);
-    if (ctx->ev_after_compact) cudaEventRecord(ctx->ev_after_compact, st);
-    ctx->launches += 2;
+    ctx->launches += 1;
+    return launch_compact(ctx, slot, mode, epoch, st, out);
+}
+
+static int32_t launch_gather(cc_ctx* ctx, int slot, cudaStream_t st, cc_result* out) {
+    const unsigned g3 = (unsigned)(ctx->sm_count * ctx->gather_bps);
+    cc_gather_kernel<<<g3, CC_GATHER_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, slot, out);
+    ctx->launches += 1;
+    CC_CUDA(ctx, cudaGetLastError());
+    return CC_OK;
+}
+
+static unsigned small_grid(cc_ctx* ctx, uint64_t items, uint64_t per_block) {
+    uint64_t g = (items + per_block - 1) / per_block;
+    const uint64_t cap = (uint64_t)ctx->sm_count * 8;
+    if (g > cap) g = cap;
+    return (unsigned)(g < 1 ? 1 : g);
+}
+
+extern "C" int32_t cc_checkpoint_marked(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, uint32_t* dirty_bitmap,
+                                        uint32_t flags, void* stream, cc_result* out) {
+    if (!ctx || !dirty_bitmap || ((uintptr_t)dirty_bitmap & 3) || (flags & ~(CC_MARK_VERIFY | CC_MARK_CONSUME))) return CC_ERR_INVALID;
+    int slot = find_slot(ctx, region_id);
+    if (slot < 0) return CC_ERR_NOT_REGISTERED;
+    const cc_region_dev& r = ctx->regions[slot].dev;
+    if ((flags & CC_MARK_VERIFY) && !r.shadow) return CC_ERR_INVALID;
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    cc_mark_load_kernel<<<small_grid(ctx, r.n_words, 256), 256, 0, st>>>(ctx->d_dev, slot, dirty_bitmap);
+    ctx->launches += 1;
+    if (flags & CC_MARK_VERIFY) {
+        cudaEvent_t ec = ctx->ev_after_compact;
+        ctx->ev_after_compact = nullptr;                // the trace events bracket discovery as a whole
+        int32_t rc = launch_compact(ctx, slot, CC_MODE_SCAN_ONLY, epoch, st, nullptr);
+        ctx->ev_after_compact = ec;
+        if (rc != CC_OK) return rc;
+        const unsigned gv = (unsigned)(ctx->sm_count * ctx->scan_bps);
+        cc_mark_verify_kernel<<<gv, CC_SCAN_THREADS, 0, st>>>(ctx->d_dev, slot);
+        ctx->launches += 1;
+    }
+    if (ctx->ev_after_scan) cudaEventRecord(ctx->ev_after_scan, st);
+    int32_t rc = launch_compact(ctx, slot, CC_MODE_CHECKPOINT, epoch, st, nullptr);
+    if (rc != CC_OK) return rc;
+    rc = launch_gather(ctx, slot, st, out);
+    if (rc != CC_OK) return rc;
+    if (flags & CC_MARK_CONSUME) {
+        cc_mark_finish_kernel<<<small_grid(ctx, r.n_words, 256), 256, 0, st>>>(ctx->d_dev, slot, dirty_bitmap, nullptr, nullptr);
+        ctx->launches += 1;
+        CC_CUDA(ctx, cudaGetLastError());
+    }
+    return CC_OK;
+}
+
+extern "C" int32_t cc_checkpoint_versions(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, const uint64_t* version,
+                                          uint64_t* committed, void* stream, cc_result* out) {
+    if (!ctx || !version || !committed || ((uintptr_t)version & 7) || ((uintptr_t)committed & 7)) return CC_ERR_INVALID;
+    int slot = find_slot(ctx, region_id);
+    if (slot < 0) return CC_ERR_NOT_REGISTERED;
+    const cc_region_dev& r = ctx->regions[slot].dev;
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    cc_mark_versions_kernel<<<small_grid(ctx, r.n_words, 8), 256, 0, st>>>(ctx->d_dev, slot, version, committed);
+    ctx->launches += 1;
+    if (ctx->ev_after_scan) cudaEventRecord(ctx->ev_after_scan, st);
+    int32_t rc = launch_compact(ctx, slot, CC_MODE_CHECKPOINT, epoch, st, nullptr);
+    if (rc != CC_OK) return rc;
+    rc = launch_gather(ctx, slot, st, out);
+    if (rc != CC_OK) return rc;
+    cc_mark_finish_kernel<<<small_grid(ctx, r.n_pages, 256), 256, 0, st>>>(ctx->d_dev, slot, nullptr, version, committed);
+    ctx->launches += 1;
     CC_CUDA(ctx, cudaGetLastError());
     return CC_OK;
 }
@@ -353,21 +448,19 @@ extern "C" int32_t cc_checkpoint_delta(cc_ctx* ctx, uint32_t region_id, uint64_t
     if (!ctx) return CC_ERR_INVALID;
     int slot = find_slot(ctx, region_id);
     if (slot < 0) return CC_ERR_NOT_REGISTERED;
+    if (!ctx->regions[slot].dev.shadow) return CC_ERR_INVALID;
     CC_CUDA(ctx, cudaSetDevice(ctx->device));
     cudaStream_t st = (cudaStream_t)stream;
     int32_t rc = launch_scan_compact(ctx, slot, CC_MODE_CHECKPOINT, epoch, st, nullptr);
     if (rc != CC_OK) return rc;
-    const unsigned g3 = (unsigned)(ctx->sm_count * ctx->gather_bps);
-    cc_gather_kernel<<<g3, CC_GATHER_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, slot, out);
-    ctx->launches += 1;
-    CC_CUDA(ctx, cudaGetLastError());
-    return CC_OK;
+    return launch_gather(ctx, slot, st, out);
 }
 
 extern "C" int32_t cc_scan_only(cc_ctx* ctx, uint32_t region_id, void* stream, cc_result* out) {
     if (!ctx) return CC_ERR_INVALID;
     int slot = find_slot(ctx, region_id);
     if (slot < 0) return CC_ERR_NOT_REGISTERED;
+    if (!ctx->regions[slot].dev.shadow) return CC_ERR_INVALID;
     CC_CUDA(ctx, cudaSetDevice(ctx->device));
     return launch_scan_compact(ctx, slot, CC_MODE_SCAN_ONLY, 0, (cudaStream_t)stream, out);
 }
