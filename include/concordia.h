@@ -122,6 +122,7 @@ typedef struct {
 #define CC_TASK_MARKED_CKPT 5u     /* region_id, epoch; arg0 = dirty bitmap (device), arg1 = CC_MARK_* flags */
 #define CC_TASK_VERSION_CKPT 6u    /* region_id, epoch; arg0 = version[] (device), arg1 = committed[] (device) */
 #define CC_TASK_EXIT 255u
+#define CC_TASKF_FUSED 1u          /* cc_task.flags, CC_TASK_DELTA_CKPT only: run the fused single pass (cc_checkpoint_delta_fused) */
 typedef struct {
     uint32_t kind;
     uint32_t region_id;
@@ -179,6 +180,15 @@ int32_t cc_log_reset_async(cc_ctx* ctx, void* stream);
  * quiescent).  The ascending dirty list of the last checkpoint stays readable in the workspace
  * (cc_dirty_list). */
 int32_t cc_checkpoint_delta(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out);
+
+/* Same contract, same log bytes, same result as cc_checkpoint_delta, computed by the fused single pass
+ * (DESIGN.md "Fused pass"): one kernel scans the region in page tiles, ranks the dirty pages by
+ * decoupled look-back and -- when the worst case (every page dirty) fits behind the current log write
+ * offset, so that all-or-nothing can be decided up front -- writes each tile's records, CRCs and shadow
+ * right away, overlapping the record writer (and, for a pinned host log, the host-link transfer) with
+ * the scan; otherwise the records are written by the gather kernel afterwards as in
+ * cc_checkpoint_delta.  A short commit kernel follows in both cases. */
+int32_t cc_checkpoint_delta_fused(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out);
 
 /* Allocator-aware delta checkpoint ("reads allocator dirty metadata", L266
  * "discovery is proportional to the dirty block bitmap"): the dirty set comes from the runtime's

@@ -39,11 +39,12 @@ CC_TASK_TEST_MUTATE = 4
 CC_TASK_MARKED_CKPT = 5
 CC_TASK_VERSION_CKPT = 6
 CC_TASK_EXIT = 255
+CC_TASKF_FUSED = 1
 
 EXPORTS = [
     "cc_init", "cc_shutdown", "cc_last_cuda_error", "cc_kernel_launches", "cc_workspace_bytes",
     "cc_register_region", "cc_unregister_region", "cc_log_attach", "cc_log_reset", "cc_log_reset_async",
-    "cc_checkpoint_delta", "cc_checkpoint_marked", "cc_checkpoint_versions",
+    "cc_checkpoint_delta", "cc_checkpoint_delta_fused", "cc_checkpoint_marked", "cc_checkpoint_versions",
     "cc_scan_only", "cc_trace_events", "cc_dirty_list", "cc_apply_scratch_bytes", "cc_apply_attach", "cc_apply_log",
     "cc_worker_start", "cc_worker_stop", "cc_worker_alive", "cc_peek_queue", "cc_submit", "cc_poll", "cc_wait",
 ]
@@ -107,6 +108,7 @@ def load_library():
         "cc_log_reset": (i32, [vp]),
         "cc_log_reset_async": (i32, [vp, vp]),
         "cc_checkpoint_delta": (i32, [vp, u32, u64, vp, vp]),
+        "cc_checkpoint_delta_fused": (i32, [vp, u32, u64, vp, vp]),
         "cc_checkpoint_marked": (i32, [vp, u32, u64, vp, u32, vp, vp]),
         "cc_checkpoint_versions": (i32, [vp, u32, u64, vp, vp, vp, vp]),
         "cc_scan_only": (i32, [vp, u32, vp, vp]),
@@ -241,6 +243,10 @@ class Context:
         self._check("cc_checkpoint_delta", self.lib.cc_checkpoint_delta(
             self.h, region_id, epoch, _stream_ptr(stream), ctypes.c_void_p(result.ptr) if result else None))
 
+    def checkpoint_delta_fused(self, region_id: int, epoch: int, result: Result = None, stream=None):
+        self._check("cc_checkpoint_delta_fused", self.lib.cc_checkpoint_delta_fused(
+            self.h, region_id, epoch, _stream_ptr(stream), ctypes.c_void_p(result.ptr) if result else None))
+
     def checkpoint_marked(self, region_id: int, epoch: int, dirty_bitmap: torch.Tensor, flags: int = 0,
                           result: Result = None, stream=None):
         """dirty_bitmap: CUDA int32/uint32 tensor of ceil(n_pages/32) words (bit p&31 of word p>>5)."""
@@ -313,9 +319,9 @@ class Context:
         return h.value, t.value
 
     def submit(self, kind: int, region_id: int = 0, epoch: int = 0, arg0: int = 0, arg1: int = 0, arg2: int = 0,
-               arg3: int = 0) -> int:
+               arg3: int = 0, flags: int = 0) -> int:
         """Returns the sequence number, or raises ConcordiaError(CC_ERR_RING_FULL)."""
-        t = cc_task(kind, region_id, 0, 0, 0, epoch, arg0, arg1, arg2, arg3)
+        t = cc_task(kind, region_id, flags, 0, 0, epoch, arg0, arg1, arg2, arg3)
         seq = ctypes.c_uint64()
         self._check("cc_submit", self.lib.cc_submit(self.h, ctypes.byref(t), ctypes.byref(seq)))
         return seq.value

@@ -174,6 +174,7 @@ __device__ __forceinline__ void cc_compact_phase(const cc_region_dev& r, cc_log_
             h->W_start = W;
             h->need = k_eff ? need : 0;
             h->gather_done = 0;
+            h->inline_done = 0;
             if (mode == CC_MODE_SCAN_ONLY && out) {
                 out->n_dirty = k;
                 out->bytes = 0;
@@ -216,7 +217,8 @@ __device__ __forceinline__ void cc_gather_phase(const cc_region_dev& r, cc_dev* 
     const u32 P = r.page_bytes;
     const u64 W0 = h->W_start;
     // warps take items round-robin, so a block has work iff its first warp index is < n_items
-    if (k_eff != 0 && (u64)g.block * (blockDim.x >> 5) < (u64)k_eff * r.spp) {
+    // (after a fused pass that already wrote the records -- cc_fused.cuh -- only the commit below is left)
+    if (k_eff != 0 && !h->inline_done && (u64)g.block * (blockDim.x >> 5) < (u64)k_eff * r.spp) {
         if (init_tables) cc_crc_smem_init(cs, &dev->crc);
         const u32 spp = r.spp;
         const u64 n_items = (u64)k_eff * spp;
@@ -298,6 +300,8 @@ __device__ __forceinline__ void cc_gather_phase(const cc_region_dev& r, cc_dev* 
             log->W = W_after;
         }
         h->gather_done = 0;
+        h->fticket = 0;
+        h->frun = h->frun + 1;
         if (out) {
             out->n_dirty = h->k;
             out->bytes = h->need;

@@ -14,6 +14,8 @@ typedef uint64_t u64;
 #define CC_COMPACT_THREADS 256
 #define CC_COMPACT_WORDS_PER_THREAD 4
 #define CC_COMPACT_TILE_WORDS (CC_COMPACT_THREADS * CC_COMPACT_WORDS_PER_THREAD)   // 1024 words = 32768 pages
+#define CC_FUSED_TILE_BYTES (64u * 1024u)    // fused pass: one WARP scans (and gathers) this much of the region per ticket
+#define CC_FUSED_MAX_TP 32u                  // ... but at most this many pages (the tile's dirty mask is one register)
 
 // Per-region control block in the workspace (device memory).
 struct cc_ws_hdr {
@@ -23,11 +25,14 @@ struct cc_ws_hdr {
     u32 ticket;         // compaction tile ticket
     u32 run_id;         // compaction look-back tag
     u32 gather_done;    // warps/blocks finished (last-block pattern)
-    u32 pad0, pad1;
+    u32 fticket;        // fused pass: page-tile ticket (reset by the gather completion, which always follows)
+    u32 frun;           // fused pass: look-back tag (bumped by the gather completion)
     u64 W_start;        // log offset at which this checkpoint's records start
     u64 need;           // bytes this checkpoint appends
     u64 t_start_ns;
     u64 epoch;
+    u32 inline_done;    // fused pass already wrote the records, headers and shadow: the gather only commits
+    u32 pad0;
 };
 
 // Device-visible region descriptor.
@@ -45,6 +50,9 @@ struct cc_region_dev {
     u32* D;             // n_pages u32: ascending dirty list
     u64* rec_state;     // n_pages u64: per-record {done-mask or count : 32 | CRC accumulator : 32}, zero between calls
     u64* lb_status;     // compaction look-back status, one per tile
+    u64* flb_status;    // fused pass look-back status, one per page tile
+    u32 ftile_pages;    // pages per fused warp tile (~64 KiB of region, 1..32 pages)
+    u32 n_ftiles;
     u32* latest;        // n_pages u32: applier last-wins table, all zero between calls
     cc_ws_hdr* hdr;
     u32 crc_init_full;  // 0xFFFFFFFF * x^(8*P): the CRC init term of a full page

@@ -13,6 +13,7 @@
 #include "cc_common.cuh"
 #include "cc_ckpt.cuh"
 #include "cc_mark.cuh"
+#include "cc_fused.cuh"
 #include "cc_apply.cuh"
 
 struct cc_ring_dev {            // all pointers are pinned, device-mapped host memory
@@ -145,9 +146,13 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
             switch (task.kind) {
             case CC_TASK_DELTA_CKPT: {
                 const cc_region_dev& r = dev->regions[slot];
-                cc_scan_phase<8>(r, g);
-                cc_grid_barrier(dev, g.nblocks, gen);
-                cc_compact_phase(r, &dev->log, CC_MODE_CHECKPOINT, task.epoch, nullptr);
+                if (task.flags & CC_TASKF_FUSED) {
+                    cc_fused_phase(r, dev, cs, CC_MODE_CHECKPOINT, task.epoch, false);
+                } else {
+                    cc_scan_phase<8>(r, g);
+                    cc_grid_barrier(dev, g.nblocks, gen);
+                    cc_compact_phase(r, &dev->log, CC_MODE_CHECKPOINT, task.epoch, nullptr);
+                }
                 cc_grid_barrier(dev, g.nblocks, gen);
                 cc_gather_phase(r, dev, cs, g, nullptr, task.kind, false);
                 break;

@@ -13,6 +13,7 @@
 #include "cc_crc.cuh"
 #include "cc_ckpt.cuh"
 #include "cc_mark.cuh"
+#include "cc_fused.cuh"
 #include "cc_apply.cuh"
 #include "cc_worker.cuh"
 
@@ -40,6 +41,11 @@ __global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_gather_kernel(cc_dev*
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cc_gather_phase(dev->regions[slot], dev, reinterpret_cast<cc_crc_smem*>(smem_raw), cc_hw_grid(), out,
                     CC_TASK_DELTA_CKPT, true);
+}
+
+__global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_fused_kernel(cc_dev* dev, int slot, u64 epoch) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cc_fused_phase(dev->regions[slot], dev, reinterpret_cast<cc_crc_smem*>(smem_raw), CC_MODE_CHECKPOINT, epoch, true);
 }
 
 // allocator-aware discovery (cc_mark.cuh)
@@ -99,7 +105,7 @@ struct cc_ctx {
     bool apply_attached;
     int last_cuda;
     uint64_t launches;
-    int scan_bps, gather_bps, validate_bps;     // blocks per SM from the occupancy API
+    int scan_bps, gather_bps, validate_bps, fused_bps;     // blocks per SM from the occupancy API
     // ring + worker (pinned host)
     cc_task* ring_slots;
     cc_result* ring_results;
@@ -130,8 +136,8 @@ static int find_slot(cc_ctx* ctx, uint32_t id) {
 }
 
 struct cc_ws_layout {
-    uint64_t hdr, bitmap, D, rec_state, latest, lb, total;
-    uint64_t n_pages, n_words, n_tiles;
+    uint64_t hdr, bitmap, D, rec_state, latest, lb, flb, total;
+    uint64_t n_pages, n_words, n_tiles, ftile_pages, n_ftiles;
 };
 
 static bool ws_layout(uint64_t bytes, uint32_t P, cc_ws_layout* L) {
@@ -148,6 +154,12 @@ static bool ws_layout(uint64_t bytes, uint32_t P, cc_ws_layout* L) {
     L->rec_state = o; o += align_up(n_pages * 8, 256);
     L->latest = o; o += align_up(n_pages * 4, 256);
     L->lb = o; o += align_up(L->n_tiles * 8, 256);
+    uint64_t tp = CC_FUSED_TILE_BYTES / P;
+    if (tp < 1) tp = 1;
+    if (tp > CC_FUSED_MAX_TP) tp = CC_FUSED_MAX_TP;
+    L->ftile_pages = tp;
+    L->n_ftiles = (n_pages + tp - 1) / tp;
+    L->flb = o; o += align_up(L->n_ftiles * 8, 256);
     L->total = o;
     return true;
 }
@@ -191,6 +203,8 @@ extern "C" int32_t cc_init(cc_ctx** out, int32_t device, const cc_config* cfg) {
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->worker_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->worker_done, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->fused_bps, cc_fused_kernel, CC_GATHER_THREADS, sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_apply_validate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_worker_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->scan_bps, cc_scan_kernel, CC_SCAN_THREADS, 0);
@@ -212,6 +226,7 @@ extern "C" int32_t cc_init(cc_ctx** out, int32_t device, const cc_config* cfg) {
     if (ctx->scan_bps < 1) ctx->scan_bps = 1;
     if (ctx->gather_bps < 1) ctx->gather_bps = 1;
     if (ctx->validate_bps < 1) ctx->validate_bps = 1;
+    if (ctx->fused_bps < 1) ctx->fused_bps = 1;
     *out = ctx;
     return CC_OK;
 }
@@ -282,6 +297,9 @@ extern "C" int32_t cc_register_region(cc_ctx* ctx, const cc_region_desc* d) {
     r.rec_state = (u64*)(ws + L.rec_state);
     r.latest = (u32*)(ws + L.latest);
     r.lb_status = (u64*)(ws + L.lb);
+    r.flb_status = (u64*)(ws + L.flb);
+    r.ftile_pages = (u32)L.ftile_pages;
+    r.n_ftiles = (u32)L.n_ftiles;
     {
         cc_crc_tables* t = (cc_crc_tables*)malloc(sizeof(cc_crc_tables));
         cc_crc_build_tables(t);
@@ -453,6 +471,25 @@ extern "C" int32_t cc_checkpoint_delta(cc_ctx* ctx, uint32_t region_id, uint64_t
     cudaStream_t st = (cudaStream_t)stream;
     int32_t rc = launch_scan_compact(ctx, slot, CC_MODE_CHECKPOINT, epoch, st, nullptr);
     if (rc != CC_OK) return rc;
+    return launch_gather(ctx, slot, st, out);
+}
+
+extern "C" int32_t cc_checkpoint_delta_fused(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out) {
+    if (!ctx) return CC_ERR_INVALID;
+    int slot = find_slot(ctx, region_id);
+    if (slot < 0) return CC_ERR_NOT_REGISTERED;
+    const cc_region_dev& r = ctx->regions[slot].dev;
+    if (!r.shadow) return CC_ERR_INVALID;
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    uint64_t g = (r.n_ftiles + CC_GATHER_THREADS / 32 - 1) / (CC_GATHER_THREADS / 32);
+    const uint64_t cap = (uint64_t)ctx->sm_count * ctx->fused_bps;
+    if (g > cap) g = cap;
+    cc_fused_kernel<<<(unsigned)g, CC_GATHER_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, slot, epoch);
+    ctx->launches += 1;
+    if (ctx->ev_after_scan) cudaEventRecord(ctx->ev_after_scan, st);
+    if (ctx->ev_after_compact) cudaEventRecord(ctx->ev_after_compact, st);
+    CC_CUDA(ctx, cudaGetLastError());
     return launch_gather(ctx, slot, st, out);
 }
 

@@ -30,6 +30,7 @@ def main():
     ap.add_argument("--page", type=int, default=4096)
     ap.add_argument("--dirty", type=float, default=0.01)
     ap.add_argument("--device-log", action="store_true", help="log buffer in device memory instead of pinned host")
+    ap.add_argument("--fused", action="store_true", help="checkpoint tasks run the fused single pass (CC_TASKF_FUSED)")
     ap.add_argument("--worker-blocks", type=int, default=0)
     ap.add_argument("--worker-threads", type=int, default=0)
     a = ap.parse_args()
@@ -60,7 +61,7 @@ def main():
         cur[idx] ^= 0x5A
         torch.cuda.synchronize()
         t0 = time.perf_counter_ns()
-        ctx.checkpoint_delta(1, i, res)
+        (ctx.checkpoint_delta_fused if a.fused else ctx.checkpoint_delta)(1, i, res)
         torch.cuda.synchronize()
         host_launched.append(time.perf_counter_ns() - t0)
         ctx.log_reset()
@@ -92,7 +93,7 @@ def main():
             used += per
             hh = (1006 * 2654435761 + t * 40503) & 0xFFFFFFFF
             ctx.wait(ctx.submit(cc.CC_TASK_TEST_MUTATE, region_id=1, arg0=n_mut, arg1=A, arg2=hh), 30.0)
-            ck = cc.cc_task(cc.CC_TASK_DELTA_CKPT, 1, 0, 0, 0, t, 0, 0, 0, 0)
+            ck = cc.cc_task(cc.CC_TASK_DELTA_CKPT, 1, cc.CC_TASKF_FUSED if a.fused else 0, 0, 0, t, 0, 0, 0, 0)
             t0 = time.perf_counter_ns()
             lib.cc_submit(h, ctypes.byref(ck), ctypes.byref(seq))
             lib.cc_wait(h, seq.value, int(30e9), ctypes.byref(r))
@@ -105,7 +106,8 @@ def main():
         us = lambda xs, q: round(_pct(xs, q) / 1e3, 2)
         out = {
             "config": {"region_MiB": a.region_mib, "page_bytes": P, "dirty_pages_per_task": n_mut, "tasks": a.tasks,
-                       "log": "device" if a.device_log else "pinned host", "bytes_per_task": per},
+                       "log": "device" if a.device_log else "pinned host", "bytes_per_task": per,
+                       "path": "fused single pass" if a.fused else "scan + compact + gather"},
             "submit_host_cost_us": {"p50": us(submit_ns, 0.5), "p99": us(submit_ns, 0.99)},
             "nop_round_trip_us": {"p50": us(nop_rt, 0.5), "p99": us(nop_rt, 0.99)},
             "checkpoint_task_round_trip_us": {"p50": us(rt, 0.5), "p99": us(rt, 0.99)},

@@ -6,16 +6,16 @@ import oracle
 import paper_2606_23521_b200 as cc
 
 
-def gpu_checkpoint(ctx, region_id, epoch, res=None):
+def gpu_checkpoint(ctx, region_id, epoch, res=None, fused=False):
     res = res or cc.Result()
     res.clear()
-    ctx.checkpoint_delta(region_id, epoch, res)
+    (ctx.checkpoint_delta_fused if fused else ctx.checkpoint_delta)(region_id, epoch, res)
     torch.cuda.synchronize()
     return res.read()
 
 
 def check_checkpoint_parity(cur: torch.Tensor, shadow0: torch.Tensor, P: int, region_id=3, epoch=17,
-                            log_capacity=None, pinned_log=False, W0_epochs=0):
+                            log_capacity=None, pinned_log=False, W0_epochs=0, fused=False):
     """cur, shadow0: uint8 CUDA tensors.  Runs one checkpoint on GPU and oracle; compares dirty list,
     log bytes, shadow, result fields.  Returns (ctx, log tensor, result, oracle log numpy, nbytes)."""
     N = cur.numel()
@@ -35,7 +35,7 @@ def check_checkpoint_parity(cur: torch.Tensor, shadow0: torch.Tensor, P: int, re
         glog = torch.zeros(cap, dtype=torch.uint8, device="cuda")
     committed = torch.zeros(1, dtype=torch.int64, pin_memory=True)
     ctx.log_attach(glog, committed)
-    r = gpu_checkpoint(ctx, region_id, epoch)
+    r = gpu_checkpoint(ctx, region_id, epoch, fused=fused)
     assert r.seq_done == 1
     assert r.status == st, (r.status, st)
     assert r.n_dirty == D.size, (r.n_dirty, D.size)

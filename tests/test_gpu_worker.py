@@ -78,8 +78,11 @@ def test_wraparound_ring_full_and_fifo():
     ctx.shutdown()
 
 
-def test_worker_checkpoint_equals_host_launched_and_oracle():
-    """C5b-shaped: MUTATE -> DELTA_CKPT tasks; parity of every task's log bytes on the first tasks."""
+@pytest.mark.parametrize("fused", [False, True])
+def test_worker_checkpoint_equals_host_launched_and_oracle(fused):
+    """C5b-shaped: MUTATE -> DELTA_CKPT tasks; parity of every task's log bytes on the first tasks.
+    fused: the tasks carry CC_TASKF_FUSED (single fused pass inside the worker)."""
+    fl = cc.CC_TASKF_FUSED if fused else 0
     P, n_pages, n_mut = 4096, 512, 6
     ctx, cur, sh, log, committed = _mk(P=P, n_pages=n_pages, cap=64)
     host_cur = cur.cpu().numpy().copy()
@@ -93,7 +96,7 @@ def test_worker_checkpoint_equals_host_launched_and_oracle():
             pages, h = synth.worker_mutation_pages(task, n_pages, n_mut, 1006)
             A = 2 * ((1006 * 7919 + 12345) % 100000) + 1
             ctx.submit(cc.CC_TASK_TEST_MUTATE, region_id=1, arg0=n_mut, arg1=A, arg2=h)
-            s = ctx.submit(cc.CC_TASK_DELTA_CKPT, region_id=1, epoch=1000 + task)
+            s = ctx.submit(cc.CC_TASK_DELTA_CKPT, region_id=1, epoch=1000 + task, flags=fl)
             for j, p in enumerate(pages):
                 host_cur[p * P + (h + j) % P] ^= 0x5A
             st, D, nb, W = oracle.checkpoint(host_cur, host_sh, P, 1, 1000 + task, olog, W)
@@ -107,7 +110,7 @@ def test_worker_checkpoint_equals_host_launched_and_oracle():
         # log reset through the ring, then one more checkpoint lands at offset 0
         ctx.submit(cc.CC_TASK_LOG_RESET)
         ctx.submit(cc.CC_TASK_TEST_MUTATE, region_id=1, arg0=1, arg1=1, arg2=7)
-        s = ctx.submit(cc.CC_TASK_DELTA_CKPT, region_id=1, epoch=5)
+        s = ctx.submit(cc.CC_TASK_DELTA_CKPT, region_id=1, epoch=5, flags=fl)
         r = ctx.wait(s, 10.0)
         assert (r.n_dirty, r.bytes, r.log_offset_after) == (1, 16 + P + 32, 16 + P + 32)
         # unknown region -> NOT_REGISTERED, worker keeps running
