@@ -484,3 +484,145 @@ int32_t orc_checkpoint_versions(const uint8_t *cur, uint8_t *shadow, uint64_t N,
     free(dirty);
     return st;
 }
+
+/* ------------------------------ base snapshot + log compactor --- */
+
+/* Base snapshot ("The initial base snapshot captured all 8,192 pages of the full
+ * region"; L257 "Immutable regions ... are included in the base snapshot but do not keep GPU
+ * shadows"): one committed epoch holding EVERY page of the region, ascending, in the same record
+ * format.  If a shadow is given it becomes a copy of the region (the next delta is relative to the
+ * snapshot).  Same all-or-nothing capacity rule as orc_checkpoint. */
+int32_t orc_snapshot(const uint8_t *cur, uint8_t *shadow, uint64_t N, uint64_t P, uint32_t region_id, uint64_t epoch,
+                     uint8_t *log, uint64_t C, uint64_t *W, uint64_t *k_out, uint64_t *bytes_out) {
+    if (P == 0 || N == 0 || region_id == 0 || region_id == ORC_COMMIT_ID) return ORC_ERR_INVALID;
+    uint64_t n_pages = (N + P - 1) / P;
+    if (n_pages > 0xFFFFFFFEull) return ORC_ERR_INVALID;
+    uint8_t *all = (uint8_t *)malloc(n_pages);
+    if (!all) return ORC_ERR_INVALID;
+    memset(all, 1, n_pages);
+    *k_out = n_pages;
+    *bytes_out = 0;
+    int32_t st = append_flagged(cur, shadow, N, P, region_id, epoch, all, n_pages, log, C, W, bytes_out);
+    free(all);
+    return st;
+}
+
+/* Log compactor ("periodic compaction rewrites the log into a smaller base snapshot plus
+ * recent deltas"; L87 "a background compactor periodically rewrites the log into a consolidated base
+ * snapshot plus a short suffix of deltas"; L221, L266 "bounding replay time").  Readings (DESIGN.md
+ * #33-#36): the input is walked and validated exactly as orc_apply walks it (same torn / corrupt
+ * rules); within its committed prefix the LAST record of every page survives (what a replay would
+ * leave in that page); the output holds, for every region that has a surviving record, in ascending
+ * region_id order, ONE committed epoch: the surviving page records in ascending page order (header
+ * copied: region_id, page_idx, len, crc32c; payload copied) and a commit record carrying the epoch
+ * number of the last input epoch that touched the region and k = number of surviving pages.
+ * A failed check makes the call ORC_ERR_CORRUPT and writes nothing (compaction must not launder a
+ * damaged log); a torn tail is dropped (it holds no committed data); ORC_ERR_LOG_FULL writes nothing.
+ *   *consumed : bytes of the input covered (end of its last committed epoch)
+ *   *n_out    : page records written;  *bytes_out : bytes written at out[0..) */
+int32_t orc_compact_log(const uint8_t *log, uint64_t n, const orc_region *regions, uint32_t n_regions,
+                        uint8_t *out, uint64_t C_out, uint64_t *bytes_out, uint64_t *consumed, uint64_t *n_out) {
+    *bytes_out = 0; *consumed = 0; *n_out = 0;
+    if (n_regions == 0 || n_regions > 4096) return ORC_ERR_INVALID;
+    uint64_t **last = (uint64_t **)calloc(n_regions, sizeof(uint64_t *));   /* header offset + 1 of the last record, 0 = none */
+    uint64_t *last_epoch = (uint64_t *)calloc(n_regions, sizeof(uint64_t));
+    uint64_t pend_cap = 1024, pend_n = 0;
+    uint64_t *pend = (uint64_t *)malloc(pend_cap * sizeof(uint64_t));
+    int32_t status = ORC_OK;
+    for (uint32_t i = 0; i < n_regions; i++) {
+        uint64_t np = (regions[i].bytes + regions[i].page_bytes - 1) / regions[i].page_bytes;
+        last[i] = (uint64_t *)calloc(np, sizeof(uint64_t));
+    }
+    uint64_t off = 0;
+    for (;;) {
+        if (n - off < ORC_HDR) break;
+        const uint8_t *h = log + off;
+        uint32_t rid = get_u32(h + 0), pidx = get_u32(h + 4), len = get_u32(h + 8), crc = get_u32(h + 12);
+        if ((uint64_t)len > n - off - ORC_HDR) break;
+        const uint8_t *payload = h + ORC_HDR;
+        if (rid == ORC_COMMIT_ID) {
+            int ok = (pidx == ORC_COMMIT_ID) && (len == 16u) && (orc_crc32c(payload, 16) == crc);
+            uint32_t c_region = 0;
+            if (ok) {
+                c_region = get_u32(payload + 8);
+                if ((uint64_t)get_u32(payload + 12) != pend_n) ok = 0;
+                for (uint64_t i = 0; ok && i < pend_n; i++)
+                    if (get_u32(log + pend[i]) != c_region) ok = 0;
+            }
+            if (!ok) { status = ORC_ERR_CORRUPT; break; }
+            for (uint64_t i = 0; i < pend_n; i++) {
+                const uint8_t *ph = log + pend[i];
+                uint32_t ri = (uint32_t)(find_region(regions, n_regions, get_u32(ph + 0)) - regions);
+                last[ri][get_u32(ph + 4)] = pend[i] + 1;                /* later records overwrite earlier ones */
+                last_epoch[ri] = (uint64_t)get_u32(payload + 0) | ((uint64_t)get_u32(payload + 4) << 32);
+            }
+            off += ORC_COMMIT_BYTES;
+            *consumed = off;
+            pend_n = 0;
+        } else {
+            const orc_region *r = find_region(regions, n_regions, rid);
+            int ok = (r != NULL);
+            if (ok) {
+                uint64_t n_pages = (r->bytes + r->page_bytes - 1) / r->page_bytes;
+                ok = ((uint64_t)pidx < n_pages) && ((uint64_t)len == page_len(r->bytes, r->page_bytes, pidx)) &&
+                     (orc_crc32c(payload, len) == crc);
+            }
+            if (!ok) { status = ORC_ERR_CORRUPT; break; }
+            if (pend_n == pend_cap) {
+                pend_cap *= 2;
+                pend = (uint64_t *)realloc(pend, pend_cap * sizeof(uint64_t));
+            }
+            pend[pend_n++] = off;
+            off += ORC_HDR + len;
+        }
+    }
+    if (status == ORC_OK) {
+        /* size, then all-or-nothing capacity check */
+        uint64_t need = 0;
+        for (uint32_t i = 0; i < n_regions; i++) {
+            uint64_t np = (regions[i].bytes + regions[i].page_bytes - 1) / regions[i].page_bytes, k = 0;
+            for (uint64_t p = 0; p < np; p++)
+                if (last[i][p]) { need += ORC_HDR + page_len(regions[i].bytes, regions[i].page_bytes, p); k++; }
+            if (k) need += ORC_COMMIT_BYTES;
+        }
+        if (need > C_out) status = ORC_ERR_LOG_FULL;
+        else {
+            uint64_t o = 0;
+            uint32_t prev_id = 0;
+            for (;;) {                                   /* regions in ascending region_id order */
+                uint32_t best = n_regions;
+                for (uint32_t i = 0; i < n_regions; i++)
+                    if (regions[i].region_id > prev_id && (best == n_regions || regions[i].region_id < regions[best].region_id))
+                        best = i;
+                if (best == n_regions) break;
+                prev_id = regions[best].region_id;
+                uint64_t np = (regions[best].bytes + regions[best].page_bytes - 1) / regions[best].page_bytes, k = 0;
+                for (uint64_t p = 0; p < np; p++) {
+                    if (!last[best][p]) continue;
+                    const uint8_t *ph = log + (last[best][p] - 1);
+                    uint32_t plen = get_u32(ph + 8);
+                    memcpy(out + o, ph, ORC_HDR + plen);
+                    o += ORC_HDR + plen;
+                    k++;
+                }
+                if (!k) continue;
+                uint8_t cp[16];
+                put_u64(cp + 0, last_epoch[best]);
+                put_u32(cp + 8, regions[best].region_id);
+                put_u32(cp + 12, (uint32_t)k);
+                put_u32(out + o + 0, ORC_COMMIT_ID);
+                put_u32(out + o + 4, ORC_COMMIT_ID);
+                put_u32(out + o + 8, 16u);
+                put_u32(out + o + 12, orc_crc32c(cp, 16));
+                memcpy(out + o + ORC_HDR, cp, 16);
+                o += ORC_COMMIT_BYTES;
+                *n_out += k;
+            }
+            *bytes_out = o;
+        }
+    }
+    for (uint32_t i = 0; i < n_regions; i++) free(last[i]);
+    free(last); free(last_epoch); free(pend);
+    if (status != ORC_OK) *n_out = 0;
+    return status;
+}

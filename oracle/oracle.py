@@ -59,6 +59,12 @@ def _load():
         lib.orc_checkpoint_versions.argtypes = [u8p, u8p, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint32,
                                                 ctypes.c_uint64, u8p, u8p,
                                                 u8p, ctypes.c_uint64, u64p, u32p, u64p, u64p]
+        lib.orc_snapshot.restype = ctypes.c_int32
+        lib.orc_snapshot.argtypes = [u8p, u8p, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint32, ctypes.c_uint64,
+                                     u8p, ctypes.c_uint64, u64p, u64p, u64p]
+        lib.orc_compact_log.restype = ctypes.c_int32
+        lib.orc_compact_log.argtypes = [u8p, ctypes.c_uint64, ctypes.POINTER(_CRegion), ctypes.c_uint32,
+                                        u8p, ctypes.c_uint64, u64p, u64p, u64p]
         lib.orc_apply.restype = ctypes.c_int32
         lib.orc_apply.argtypes = [u8p, ctypes.c_uint64, ctypes.POINTER(_CRegion), ctypes.c_uint32, u64p, u64p]
         lib.orc_write_epoch.restype = ctypes.c_int32
@@ -193,6 +199,33 @@ def apply_log(log, nbytes: int, regions):
     consumed = ctypes.c_uint64(0)
     st = _load().orc_apply(_ptr(lg), nbytes, arr, len(regions), ctypes.byref(applied), ctypes.byref(consumed))
     return int(st), int(applied.value), int(consumed.value)
+
+
+def snapshot(cur, shadow, page_bytes: int, region_id: int, epoch: int, log, W: int):
+    """Base snapshot: every page of the region as one committed epoch.  shadow (may be None) := cur.
+    Returns (status, k, bytes_appended, W_after)."""
+    c, lg = _u8(cur), _u8(log)
+    s = None if shadow is None else _u8(shadow)
+    w, k, nb = ctypes.c_uint64(W), ctypes.c_uint64(0), ctypes.c_uint64(0)
+    st = _load().orc_snapshot(_ptr(c), None if s is None else _ptr(s), c.size, page_bytes, region_id, epoch,
+                              _ptr(lg), lg.size, ctypes.byref(w), ctypes.byref(k), ctypes.byref(nb))
+    return int(st), int(k.value), int(nb.value), int(w.value)
+
+
+def compact_log(log, nbytes: int, regions, out):
+    """Rewrite the committed prefix of log[:nbytes] into `out`: one epoch per region (ascending region id), the last
+    record of every page, ascending pages.  Only region_id / page_bytes / size of `regions` are used.
+    Returns (status, bytes_out, consumed, n_records_out)."""
+    lg, o = _u8(log), _u8(out)
+    assert nbytes <= lg.size and o.flags["WRITEABLE"]
+    arr = (_CRegion * max(len(regions), 1))()
+    for i, r in enumerate(regions):
+        b = _u8(r.base)
+        arr[i] = _CRegion(r.region_id, r.page_bytes, b.size, _ptr(b), 0)
+    nb, consumed, n_out = ctypes.c_uint64(0), ctypes.c_uint64(0), ctypes.c_uint64(0)
+    st = _load().orc_compact_log(_ptr(lg), nbytes, arr, len(regions), _ptr(o), o.size, ctypes.byref(nb),
+                                 ctypes.byref(consumed), ctypes.byref(n_out))
+    return int(st), int(nb.value), int(consumed.value), int(n_out.value)
 
 
 def write_epoch(log, W: int, region_id: int, epoch: int, region_bytes: int, page_bytes: int, pages, payloads):
