@@ -121,6 +121,8 @@ typedef struct {
                                       for j < n_mut: page (j*A + h) mod n_pages, byte (h + j) mod len_p, ^= 0x5A */
 #define CC_TASK_MARKED_CKPT 5u     /* region_id, epoch; arg0 = dirty bitmap (device), arg1 = CC_MARK_* flags */
 #define CC_TASK_VERSION_CKPT 6u    /* region_id, epoch; arg0 = version[] (device), arg1 = committed[] (device) */
+#define CC_TASK_SNAPSHOT 7u        /* region_id, epoch: base snapshot (cc_snapshot_region) */
+#define CC_TASK_COMPACT_LOG 8u     /* arg0 = input log, arg1 = its bytes, arg2 = output log, arg3 = output capacity */
 #define CC_TASK_EXIT 255u
 #define CC_TASKF_FUSED 1u          /* cc_task.flags, CC_TASK_DELTA_CKPT only: run the fused single pass (cc_checkpoint_delta_fused) */
 typedef struct {
@@ -211,6 +213,30 @@ int32_t cc_checkpoint_marked(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, ui
  * nothing moves. */
 int32_t cc_checkpoint_versions(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, const uint64_t* version,
                                uint64_t* committed, void* stream, cc_result* out);
+
+/* Base snapshot ("The initial base snapshot captured all 8,192 pages of the full region";
+ * L257: immutable regions "are included in the base snapshot but do not keep GPU shadows"): append EVERY
+ * page of the region, ascending, as one committed epoch in the same record format -- no discovery pass.
+ * A region with a shadow gets shadow := base (the next delta is relative to the snapshot).  Same
+ * all-or-nothing CC_ERR_LOG_FULL rule, result and asynchrony as cc_checkpoint_delta. */
+int32_t cc_snapshot_region(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out);
+
+/* Log compactor ("a background compactor periodically rewrites the log into a
+ * consolidated base snapshot plus a short suffix of deltas", L221, L266 "bounding replay time").
+ * in_log[0, in_bytes) is parsed and validated exactly as cc_apply_log does (same torn / corrupt rules;
+ * needs the scratch of cc_apply_attach).  Within its committed prefix the LAST record of every page
+ * survives; out_log (device or pinned host, 16-byte aligned, must not overlap in_log) receives, for
+ * every region with a surviving record, in ascending region_id order, ONE committed epoch: the
+ * surviving page records in ascending page order and a commit record carrying the epoch number of
+ * the last input epoch that touched the region.  Replaying out_log leaves every registered region in
+ * the state that replaying in_log leaves it in.  Regions and the attached log are not touched.
+ * Result: status CC_OK, n_dirty = page records written, bytes = bytes written at out_log[0..),
+ * log_offset_after = input bytes covered (end of its last committed epoch), epoch = regions written.
+ * CC_ERR_CORRUPT (a failed check anywhere in the input), CC_ERR_SCRATCH and CC_ERR_LOG_FULL
+ * (out_capacity too small) write nothing.  ASYNCHRONOUS on `stream`.  The per-region dirty lists
+ * (cc_dirty_list) are overwritten. */
+int32_t cc_compact_log(cc_ctx* ctx, const void* in_log, uint64_t in_bytes, void* out_log, uint64_t out_capacity,
+                       void* stream, cc_result* out);
 
 /* Scan + compaction only (steps a1-a2), for measurement: fills the dirty list, appends nothing,
  * leaves the shadow alone.  out->n_dirty = k. */

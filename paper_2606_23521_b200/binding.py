@@ -38,6 +38,8 @@ CC_TASK_LOG_RESET = 3
 CC_TASK_TEST_MUTATE = 4
 CC_TASK_MARKED_CKPT = 5
 CC_TASK_VERSION_CKPT = 6
+CC_TASK_SNAPSHOT = 7
+CC_TASK_COMPACT_LOG = 8
 CC_TASK_EXIT = 255
 CC_TASKF_FUSED = 1
 
@@ -45,7 +47,7 @@ EXPORTS = [
     "cc_init", "cc_shutdown", "cc_last_cuda_error", "cc_kernel_launches", "cc_workspace_bytes",
     "cc_register_region", "cc_unregister_region", "cc_log_attach", "cc_log_reset", "cc_log_reset_async",
     "cc_checkpoint_delta", "cc_checkpoint_delta_fused", "cc_checkpoint_marked", "cc_checkpoint_versions",
-    "cc_scan_only", "cc_trace_events", "cc_dirty_list", "cc_apply_scratch_bytes", "cc_apply_attach", "cc_apply_log",
+    "cc_snapshot_region", "cc_compact_log", "cc_scan_only", "cc_trace_events", "cc_dirty_list", "cc_apply_scratch_bytes", "cc_apply_attach", "cc_apply_log",
     "cc_worker_start", "cc_worker_stop", "cc_worker_alive", "cc_peek_queue", "cc_submit", "cc_poll", "cc_wait",
 ]
 
@@ -111,6 +113,8 @@ def load_library():
         "cc_checkpoint_delta_fused": (i32, [vp, u32, u64, vp, vp]),
         "cc_checkpoint_marked": (i32, [vp, u32, u64, vp, u32, vp, vp]),
         "cc_checkpoint_versions": (i32, [vp, u32, u64, vp, vp, vp, vp]),
+        "cc_snapshot_region": (i32, [vp, u32, u64, vp, vp]),
+        "cc_compact_log": (i32, [vp, vp, u64, vp, u64, vp, vp]),
         "cc_scan_only": (i32, [vp, u32, vp, vp]),
         "cc_trace_events": (i32, [vp, vp, vp]),
         "cc_dirty_list": (i32, [vp, u32, P(vp), P(vp)]),
@@ -262,6 +266,18 @@ class Context:
             assert t.is_cuda and t.is_contiguous() and t.element_size() == 8
         self._check("cc_checkpoint_versions", self.lib.cc_checkpoint_versions(
             self.h, region_id, epoch, version.data_ptr(), committed.data_ptr(), _stream_ptr(stream),
+            ctypes.c_void_p(result.ptr) if result else None))
+
+    def snapshot_region(self, region_id: int, epoch: int, result: Result = None, stream=None):
+        self._check("cc_snapshot_region", self.lib.cc_snapshot_region(
+            self.h, region_id, epoch, _stream_ptr(stream), ctypes.c_void_p(result.ptr) if result else None))
+
+    def compact_log(self, in_log: torch.Tensor, in_bytes: int, out_log: torch.Tensor, result: Result = None, stream=None):
+        for t in (in_log, out_log):
+            assert t.dtype == torch.uint8 and t.is_contiguous() and (t.is_cuda or t.is_pinned())
+        assert in_bytes <= in_log.numel()
+        self._check("cc_compact_log", self.lib.cc_compact_log(
+            self.h, in_log.data_ptr(), in_bytes, out_log.data_ptr(), out_log.numel(), _stream_ptr(stream),
             ctypes.c_void_p(result.ptr) if result else None))
 
     def scan_only(self, region_id: int, result: Result = None, stream=None):

@@ -59,14 +59,19 @@ __device__ __forceinline__ void cc_apply_parse_phase(cc_dev* dev, const cc_apply
                 if ((u64)h.z > n - off - CC_RECORD_HEADER_BYTES) break;                    // torn
                 if (h.x == CC_COMMIT_ID) {
                     bool ok = (h.y == CC_COMMIT_ID) && (h.z == 16u);
+                    uint4 pl = make_uint4(0, 0, 0, 0);
                     if (ok) {
-                        const uint4 pl = ld_v4(reinterpret_cast<const uint4*>(log + off + 16));
+                        pl = ld_v4(reinterpret_cast<const uint4*>(log + off + 16));
                         u32 pay[4] = {pl.x, pl.y, pl.z, pl.w};
                         ok = crc_serial(&dev->crc, reinterpret_cast<const u8*>(pay), 16) == h.w;
                         ok = ok && (pl.w == s_pending) && !s_mixed && (s_pending == 0 || s_pend_rid == pl.z);
                     }
                     if (!ok) { A->struct_fail = 1; break; }
                     if (s_nepochs >= T.max_records) { A->scratch_overflow = 1; break; }
+                    if (s_pending != 0) {                   // for the log compactor: last epoch number per region
+                        const int cs = cc_find_slot(dev, pl.z);
+                        if (cs >= 0) dev->compactor.region_epoch[cs] = (u64)pl.x | ((u64)pl.y << 32);
+                    }
                     T.epochs[s_nepochs].off_after = off + CC_COMMIT_RECORD_BYTES;
                     T.epochs[s_nepochs].rec_end = s_nrecs;
                     s_nepochs++;

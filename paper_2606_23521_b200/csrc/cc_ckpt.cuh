@@ -80,6 +80,31 @@ __device__ __forceinline__ u64 lb_pack(u32 run, u64 flag, u32 val) { return ((u6
 #define CC_MODE_CHECKPOINT 0u
 #define CC_MODE_SCAN_ONLY 1u
 
+// The plan of the record writer, written once k is final (one thread): record count, byte need,
+// all-or-nothing log-full decision (reading #10), start offset.  last_dirty: the region's (possibly
+// short) last page is among the k pages.  inline_done: the records are already in place (fused pass).
+__device__ __forceinline__ void cc_plan_checkpoint(const cc_region_dev& r, const cc_log_dev* log, u32 mode, u64 epoch, u32 k,
+                                                   bool last_dirty, bool inline_done) {
+    cc_ws_hdr* h = r.hdr;
+    h->k = k;
+    h->epoch = epoch;
+    u64 need = (u64)k * (CC_RECORD_HEADER_BYTES + (u64)r.page_bytes) + CC_COMMIT_RECORD_BYTES;
+    if (last_dirty) need -= (u64)r.page_bytes - page_len_dev(r, r.n_pages - 1);
+    const u64 W = log->W;
+    int32_t st = CC_OK;
+    u32 k_eff = 0;
+    if (mode == CC_MODE_CHECKPOINT && k != 0) {
+        if (log->buf == nullptr || W + need > log->capacity) st = CC_ERR_LOG_FULL;
+        else k_eff = k;
+    }
+    h->k_eff = k_eff;
+    h->status = st;
+    h->W_start = W;
+    h->need = k_eff ? need : 0;
+    h->gather_done = 0;
+    h->inline_done = inline_done ? 1u : 0u;
+}
+
 // Only the first CC_COMPACT_THREADS threads of a block work (the worker's blocks may be wider);
 // every thread takes part in the barriers.
 __device__ __forceinline__ void cc_compact_phase(const cc_region_dev& r, cc_log_dev* log, u32 mode, u64 epoch,
@@ -158,23 +183,8 @@ __device__ __forceinline__ void cc_compact_phase(const cc_region_dev& r, cc_log_
         if (t == nt - 1 && tid == 0) {
             const u32 k = s_excl + total;
             cc_ws_hdr* h = r.hdr;
-            h->k = k;
-            h->epoch = epoch;
-            u64 need = (u64)k * (CC_RECORD_HEADER_BYTES + (u64)r.page_bytes) + CC_COMMIT_RECORD_BYTES;
-            if (s_last_dirty) need -= (u64)r.page_bytes - page_len_dev(r, r.n_pages - 1);
-            const u64 W = log->W;
-            int32_t st = CC_OK;
-            u32 k_eff = 0;
-            if (mode == CC_MODE_CHECKPOINT && k != 0) {
-                if (log->buf == nullptr || W + need > log->capacity) st = CC_ERR_LOG_FULL;
-                else k_eff = k;
-            }
-            h->k_eff = k_eff;
-            h->status = st;
-            h->W_start = W;
-            h->need = k_eff ? need : 0;
-            h->gather_done = 0;
-            h->inline_done = 0;
+            cc_plan_checkpoint(r, log, mode, epoch, k, s_last_dirty != 0, false);
+            const u64 W = h->W_start;
             if (mode == CC_MODE_SCAN_ONLY && out) {
                 out->n_dirty = k;
                 out->bytes = 0;
@@ -190,6 +200,16 @@ __device__ __forceinline__ void cc_compact_phase(const cc_region_dev& r, cc_log_
             __threadfence();
         }
         __syncthreads();
+    }
+}
+
+// Base snapshot ("The initial base snapshot captured all 8,192 pages"):
+// every page is a record -- D = 0..n_pages-1, no discovery at all; the gather below does the rest.
+__device__ __forceinline__ void cc_snapshot_plan_phase(const cc_region_dev& r, const cc_log_dev* log, u64 epoch, cc_grid g) {
+    for (u64 i = (u64)g.block * blockDim.x + threadIdx.x; i < r.n_pages; i += (u64)g.nblocks * blockDim.x) r.D[i] = (u32)i;
+    if (g.block == 0 && threadIdx.x == 0) {
+        r.hdr->t_start_ns = globaltimer_ns();
+        cc_plan_checkpoint(r, log, CC_MODE_CHECKPOINT, epoch, (u32)r.n_pages, true, false);
     }
 }
 

@@ -96,6 +96,15 @@ struct cc_apply_state {
     u32 final_done;
 };
 
+// Log compactor state (cc_compactor.cuh).
+struct cc_compactor_state {
+    u64 region_epoch[CC_MAX_REGIONS];   // epoch number of the last input epoch that touched the region
+    u64 bytes_out;
+    u64 n_out;
+    int32_t status;
+    u32 n_regions_out;
+};
+
 struct cc_crc_tables {
     u32 t0[256];            // byte table of the reflected polynomial
     u32 s512[4][256];       // multiply by x^(8*512) mod G, one table per register byte
@@ -116,6 +125,7 @@ struct cc_dev {
     cc_epoch_ent* epochs;
     u64 max_records;
     cc_apply_state apply;
+    cc_compactor_state compactor;
     // grid barrier + worker doorbell
     u32 bar_count;
     u32 bar_gen;

@@ -1,0 +1,157 @@
+// cc_compactor.cuh -- log compactor ("periodic compaction rewrites the log
+// into a smaller base snapshot plus recent deltas", L87, L221, L266 "bounding replay time").
+//
+// Input: a log (device or pinned host).  It is parsed and validated by the applier's own phases
+// (cc_apply.cuh: same torn / corrupt rules).  Then, instead of scattering into the regions:
+//   mark     latest[page] = last committed record of the page (atomicMax, as in the applier) and the
+//            page's bit in its region's dirty bitmap
+//   rank     the ordered compaction of cc_ckpt.cuh over every region's bitmap -> ascending page list
+//   plan     one thread: regions in ascending region_id order get their output offsets; all-or-nothing
+//            capacity check
+//   copy     warp per 4 KiB segment: surviving record -> output log at its final place; the header
+//            (region, page, len, crc) is copied from the validated input record, no CRC is recomputed;
+//            one commit record per region with the epoch number of the last input epoch that touched it
+//   cleanup  latest[] back to zero; result
+// A failed check (CC_ERR_CORRUPT) or a too small scratch writes nothing: compaction must not launder a
+// damaged log.  A torn tail holds no committed data and is dropped.
+#pragma once
+#include "cc_common.cuh"
+#include "cc_ckpt.cuh"
+#include "cc_apply.cuh"
+
+__device__ __forceinline__ bool cc_compactor_ok(const cc_dev* dev) { return dev->apply.status == CC_OK; }
+
+__device__ __forceinline__ void cc_compactor_mark_phase(cc_dev* dev, const cc_apply_tabs& T, cc_grid g) {
+    if (g.block == 0 && threadIdx.x < CC_MAX_REGIONS && dev->region_used[threadIdx.x]) {
+        cc_ws_hdr* h = dev->regions[threadIdx.x].hdr;       // open a compaction run on every region
+        h->ticket = 0;
+        h->run_id = h->run_id + 1;
+    }
+    if (!cc_compactor_ok(dev)) return;
+    const u32 n = dev->apply.n_commit_recs;
+    for (u32 i = g.block * blockDim.x + threadIdx.x; i < n; i += g.nblocks * blockDim.x) {
+        const cc_rec rec = T.recs[i];
+        const cc_region_dev& r = dev->regions[rec.slot];
+        atomicMax(&r.latest[rec.page_idx], i + 1);
+        atomicOr(&r.bitmap[rec.page_idx >> 5], 1u << (rec.page_idx & 31));
+    }
+}
+
+__device__ __forceinline__ void cc_compactor_rank_phase(cc_dev* dev) {
+    for (int s = 0; s < CC_MAX_REGIONS; s++)
+        if (dev->region_used[s]) cc_compact_phase(dev->regions[s], &dev->log, CC_MODE_SCAN_ONLY, 0, nullptr);
+}
+
+// One thread.  hdr->W_start of every region := its offset in the output; hdr->need := its bytes.
+__device__ __forceinline__ void cc_compactor_plan_phase(cc_dev* dev, u64 out_capacity) {
+    cc_compactor_state* C = &dev->compactor;
+    u64 o = 0, n_out = 0;
+    u32 n_reg = 0;
+    if (cc_compactor_ok(dev)) {
+        u32 prev = 0;
+        for (;;) {
+            int best = -1;
+            for (int s = 0; s < CC_MAX_REGIONS; s++)
+                if (dev->region_used[s] && dev->regions[s].region_id > prev &&
+                    (best < 0 || dev->regions[s].region_id < dev->regions[best].region_id))
+                    best = s;
+            if (best < 0) break;
+            const cc_region_dev& r = dev->regions[best];
+            prev = r.region_id;
+            const u32 k = r.hdr->k;
+            u64 need = 0;
+            if (k) {
+                need = (u64)k * ((u64)r.page_bytes + CC_RECORD_HEADER_BYTES) + CC_COMMIT_RECORD_BYTES;
+                if (r.D[k - 1] == (u32)(r.n_pages - 1)) need -= (u64)r.page_bytes - page_len_dev(r, r.n_pages - 1);
+                n_reg++;
+            }
+            r.hdr->W_start = o;
+            r.hdr->need = need;
+            o += need;
+            n_out += k;
+        }
+    }
+    int32_t st = dev->apply.status;
+    if (st == CC_OK && o > out_capacity) st = CC_ERR_LOG_FULL;
+    C->status = st;
+    C->bytes_out = st == CC_OK ? o : 0;
+    C->n_out = st == CC_OK ? n_out : 0;
+    C->n_regions_out = st == CC_OK ? n_reg : 0;
+    __threadfence();
+}
+
+__device__ __forceinline__ void cc_compactor_copy_phase(cc_dev* dev, const cc_apply_tabs& T, const u8* in, u8* out, cc_grid g) {
+    constexpr int U = 8;
+    if (dev->compactor.status != CC_OK) return;
+    const u32 lane = threadIdx.x & 31u;
+    for (int s = 0; s < CC_MAX_REGIONS; s++) {
+        if (!dev->region_used[s]) continue;
+        const cc_region_dev& r = dev->regions[s];
+        const u32 k = r.hdr->k;
+        if (k == 0) continue;
+        u8* base = out + r.hdr->W_start;
+        const u64 rec_stride = (u64)r.page_bytes + CC_RECORD_HEADER_BYTES;
+        const u32 spp = r.spp;
+        const u64 n_items = (u64)k * spp;
+        for (u64 item = g.warp(); item < n_items; item += g.nwarps()) {
+            u32 i, c;
+            if (r.spp_shift >= 0) { i = (u32)(item >> r.spp_shift); c = (u32)(item & (spp - 1)); }
+            else { i = (u32)(item / spp); c = (u32)(item - (u64)i * spp); }
+            const u32 p = r.D[i];
+            const cc_rec rec = T.recs[r.latest[p] - 1];
+            const u64 so = (u64)c * CC_SEG_BYTES;
+            if (so >= rec.len) continue;
+            const u64 rem = rec.len - so;
+            const u32 nv = (u32)(rem < CC_SEG_BYTES ? rem : CC_SEG_BYTES) >> 4;
+            const uint4* src = reinterpret_cast<const uint4*>(in + rec.off + CC_RECORD_HEADER_BYTES + so);
+            u8* orec = base + (u64)i * rec_stride;
+            uint4* dst = reinterpret_cast<uint4*>(orec + CC_RECORD_HEADER_BYTES + so);
+            uint4 v[U];
+#pragma unroll
+            for (int u = 0; u < U; u++) {
+                const u32 j = lane + 32 * u;
+                if (j < nv) v[u] = ld_v4(src + j);
+            }
+#pragma unroll
+            for (int u = 0; u < U; u++) {
+                const u32 j = lane + 32 * u;
+                if (j < nv) st_stream(dst + j, v[u]);
+            }
+            if (c == 0 && lane == 0) st_u32x4(orec, r.region_id, p, rec.len, rec.crc);
+        }
+        if (g.block == 0 && threadIdx.x == 0) {             // the region's commit record
+            u8* cm = base + r.hdr->need - CC_COMMIT_RECORD_BYTES;
+            const u64 epoch = dev->compactor.region_epoch[s];
+            u32 pay[4] = {(u32)epoch, (u32)(epoch >> 32), r.region_id, k};
+            const u32 crc = crc_serial(&dev->crc, reinterpret_cast<const u8*>(pay), 16);
+            st_u32x4(cm + 16, pay[0], pay[1], pay[2], pay[3]);
+            st_u32x4(cm, CC_COMMIT_ID, CC_COMMIT_ID, 16u, crc);
+        }
+    }
+}
+
+// latest[] back to zero (the rank phase already cleared the bitmaps); result.
+__device__ __forceinline__ void cc_compactor_cleanup_phase(cc_dev* dev, const cc_apply_tabs& T, cc_grid g, cc_result* out,
+                                                           u32 kind) {
+    cc_apply_state* A = &dev->apply;
+    if (A->status == CC_OK) {
+        const u32 n = A->n_commit_recs;
+        for (u32 i = g.block * blockDim.x + threadIdx.x; i < n; i += g.nblocks * blockDim.x) {
+            const cc_rec rec = T.recs[i];
+            dev->regions[rec.slot].latest[rec.page_idx] = 0;
+        }
+    }
+    if (g.block == 0 && threadIdx.x == 0 && out) {
+        const cc_compactor_state* C = &dev->compactor;
+        out->n_dirty = C->n_out;
+        out->bytes = C->bytes_out;
+        out->log_offset_after = A->consumed;
+        out->epoch = C->n_regions_out;
+        out->status = C->status;
+        out->flags = kind;
+        out->t_start_ns = A->t_start_ns;
+        out->t_end_ns = globaltimer_ns();
+        __threadfence_system();
+        st_release_sys_u64(&out->seq_done, 1ull);
+    }
+}

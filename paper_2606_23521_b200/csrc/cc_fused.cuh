@@ -133,25 +133,8 @@ __device__ __forceinline__ void cc_fused_phase(const cc_region_dev& r, cc_dev* d
         cc_fused_lookback(r.flb_status, run, t, lane, true, &excl);
         if (lane == 0) st_release_gpu_u64(&r.flb_status[t], lb_pack(run, CC_LB_INC, excl + cnt));
         if ((mask >> lane) & 1u) r.D[excl + __popc(mask & ((1u << lane) - 1u))] = (u32)(p0 + lane);
-        if (last && lane == 0) {            // every earlier tile has published its count: k is final
-            const u32 k = excl + cnt;
-            h->k = k;
-            h->epoch = epoch;
-            u64 need = (u64)k * rec_stride + CC_COMMIT_RECORD_BYTES;
-            if ((mask >> (np - 1)) & 1u) need -= (u64)P - page_len_dev(r, r.n_pages - 1);
-            int32_t st = CC_OK;
-            u32 k_eff = 0;
-            if (mode == CC_MODE_CHECKPOINT && k != 0) {
-                if (log->buf == nullptr || W0 + need > log->capacity) st = CC_ERR_LOG_FULL;
-                else k_eff = k;
-            }
-            h->k_eff = k_eff;
-            h->status = st;
-            h->W_start = W0;
-            h->need = k_eff ? need : 0;
-            h->gather_done = 0;
-            h->inline_done = inline_ok ? 1u : 0u;
-        }
+        if (last && lane == 0)              // every earlier tile has published its count: k is final
+            cc_plan_checkpoint(r, log, mode, epoch, excl + cnt, ((mask >> (np - 1)) & 1u) != 0, inline_ok);
         if (!inline_ok) continue;
         // ---- a3 + a5: this warp gathers its own dirty pages (one read -> log payload, shadow, CRC) ----
         u32 m = mask, i = excl;

@@ -15,6 +15,7 @@
 #include "cc_mark.cuh"
 #include "cc_fused.cuh"
 #include "cc_apply.cuh"
+#include "cc_compactor.cuh"
 
 struct cc_ring_dev {            // all pointers are pinned, device-mapped host memory
     cc_task* slots;             // capacity x 64 B
@@ -54,6 +55,41 @@ __device__ __forceinline__ void cc_task_mutate(const cc_region_dev& r, const cc_
 }
 
 #define CC_WORKER_MAX_THREADS 512
+
+// The recovery-side tasks are cold: kept out of line so that their registers do not weigh on the
+// checkpoint tasks of the dispatch loop.
+__device__ __noinline__ void cc_worker_restore_task(cc_dev* dev, const cc_apply_tabs& tabs, cc_crc_smem* cs,
+                                                    const cc_task& task, cc_grid g, u32& gen) {
+    const u8* log = reinterpret_cast<const u8*>(task.arg0);
+    if (g.block == 0) cc_apply_parse_phase(dev, tabs, log, task.arg1);
+    cc_grid_barrier(dev, g.nblocks, gen);
+    cc_apply_validate_phase(dev, tabs, cs, log, g, false);
+    cc_grid_barrier(dev, g.nblocks, gen);
+    cc_apply_latest_phase(dev, tabs, g);
+    cc_grid_barrier(dev, g.nblocks, gen);
+    cc_apply_scatter_phase(dev, tabs, log, g);
+    cc_grid_barrier(dev, g.nblocks, gen);
+    cc_apply_cleanup_phase(dev, tabs, g, nullptr, task.kind);
+}
+
+__device__ __noinline__ void cc_worker_compact_task(cc_dev* dev, const cc_apply_tabs& tabs, cc_crc_smem* cs,
+                                                    const cc_task& task, cc_grid g, u32& gen) {
+    const u8* in = reinterpret_cast<const u8*>(task.arg0);
+    u8* outl = reinterpret_cast<u8*>(task.arg2);
+    if (g.block == 0) cc_apply_parse_phase(dev, tabs, in, task.arg1);
+    cc_grid_barrier(dev, g.nblocks, gen);
+    cc_apply_validate_phase(dev, tabs, cs, in, g, false);
+    cc_grid_barrier(dev, g.nblocks, gen);
+    cc_compactor_mark_phase(dev, tabs, g);
+    cc_grid_barrier(dev, g.nblocks, gen);
+    cc_compactor_rank_phase(dev);
+    cc_grid_barrier(dev, g.nblocks, gen);
+    if (g.block == 0 && threadIdx.x == 0) cc_compactor_plan_phase(dev, task.arg3);
+    cc_grid_barrier(dev, g.nblocks, gen);
+    cc_compactor_copy_phase(dev, tabs, in, outl, g);
+    cc_grid_barrier(dev, g.nblocks, gen);
+    cc_compactor_cleanup_phase(dev, tabs, g, nullptr, task.kind);
+}
 
 __global__ void __launch_bounds__(CC_WORKER_MAX_THREADS, 1)
 cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
@@ -131,7 +167,7 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
         int32_t status = CC_OK;
         int slot = -1;
         const bool is_ckpt = task.kind == CC_TASK_DELTA_CKPT || task.kind == CC_TASK_MARKED_CKPT ||
-                             task.kind == CC_TASK_VERSION_CKPT;
+                             task.kind == CC_TASK_VERSION_CKPT || task.kind == CC_TASK_SNAPSHOT;
         if (is_ckpt || task.kind == CC_TASK_TEST_MUTATE) {
             slot = cc_find_slot(dev, task.region_id);
             if (slot < 0) status = CC_ERR_NOT_REGISTERED;
@@ -190,19 +226,19 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
                 cc_mark_finish_phase(r, nullptr, ver, com, g);
                 break;
             }
-            case CC_TASK_RESTORE: {
-                const u8* log = reinterpret_cast<const u8*>(task.arg0);
-                if (g.block == 0) cc_apply_parse_phase(dev, tabs, log, task.arg1);
+            case CC_TASK_SNAPSHOT: {
+                const cc_region_dev& r = dev->regions[slot];
+                cc_snapshot_plan_phase(r, &dev->log, task.epoch, g);
                 cc_grid_barrier(dev, g.nblocks, gen);
-                cc_apply_validate_phase(dev, tabs, cs, log, g, false);
-                cc_grid_barrier(dev, g.nblocks, gen);
-                cc_apply_latest_phase(dev, tabs, g);
-                cc_grid_barrier(dev, g.nblocks, gen);
-                cc_apply_scatter_phase(dev, tabs, log, g);
-                cc_grid_barrier(dev, g.nblocks, gen);
-                cc_apply_cleanup_phase(dev, tabs, g, nullptr, task.kind);
+                cc_gather_phase(r, dev, cs, g, nullptr, task.kind, false);
                 break;
             }
+            case CC_TASK_COMPACT_LOG:
+                cc_worker_compact_task(dev, tabs, cs, task, g, gen);
+                break;
+            case CC_TASK_RESTORE:
+                cc_worker_restore_task(dev, tabs, cs, task, g, gen);
+                break;
             case CC_TASK_TEST_MUTATE:
                 cc_task_mutate(dev->regions[slot], task, g);
                 break;
@@ -218,6 +254,10 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
             if (status == CC_OK && is_ckpt) {
                 const cc_ws_hdr* h = dev->regions[slot].hdr;
                 n_dirty = h->k; bytes = h->need; status = h->status;
+            } else if (status == CC_OK && task.kind == CC_TASK_COMPACT_LOG) {
+                const cc_compactor_state* C = &dev->compactor;
+                n_dirty = C->n_out; bytes = C->bytes_out; off_after = dev->apply.consumed;
+                ep = C->n_regions_out; status = C->status;
             } else if (status == CC_OK && task.kind == CC_TASK_RESTORE) {
                 const cc_apply_state* A = &dev->apply;
                 n_dirty = A->n_commit_recs; bytes = A->consumed; off_after = A->consumed;

@@ -15,6 +15,7 @@
 #include "cc_mark.cuh"
 #include "cc_fused.cuh"
 #include "cc_apply.cuh"
+#include "cc_compactor.cuh"
 #include "cc_worker.cuh"
 
 static_assert(sizeof(cc_result) == 64, "cc_result must be 64 bytes");
@@ -46,6 +47,23 @@ __global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_gather_kernel(cc_dev*
 __global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_fused_kernel(cc_dev* dev, int slot, u64 epoch) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cc_fused_phase(dev->regions[slot], dev, reinterpret_cast<cc_crc_smem*>(smem_raw), CC_MODE_CHECKPOINT, epoch, true);
+}
+
+__global__ void __launch_bounds__(256) cc_snapshot_plan_kernel(const cc_dev* dev, int slot, u64 epoch) {
+    cc_snapshot_plan_phase(dev->regions[slot], &dev->log, epoch, cc_hw_grid());
+}
+
+// log compactor (cc_compactor.cuh)
+__global__ void __launch_bounds__(CC_APPLY_THREADS) cc_compactor_mark_kernel(cc_dev* dev, cc_apply_tabs tabs) {
+    cc_compactor_mark_phase(dev, tabs, cc_hw_grid());
+}
+__global__ void __launch_bounds__(CC_COMPACT_THREADS) cc_compactor_rank_kernel(cc_dev* dev) { cc_compactor_rank_phase(dev); }
+__global__ void cc_compactor_plan_kernel(cc_dev* dev, u64 out_capacity) { cc_compactor_plan_phase(dev, out_capacity); }
+__global__ void __launch_bounds__(CC_APPLY_THREADS) cc_compactor_copy_kernel(cc_dev* dev, cc_apply_tabs tabs, const u8* in, u8* out) {
+    cc_compactor_copy_phase(dev, tabs, in, out, cc_hw_grid());
+}
+__global__ void __launch_bounds__(CC_APPLY_THREADS) cc_compactor_cleanup_kernel(cc_dev* dev, cc_apply_tabs tabs, cc_result* out) {
+    cc_compactor_cleanup_phase(dev, tabs, cc_hw_grid(), out, CC_TASK_COMPACT_LOG);
 }
 
 // allocator-aware discovery (cc_mark.cuh)
@@ -491,6 +509,44 @@ extern "C" int32_t cc_checkpoint_delta_fused(cc_ctx* ctx, uint32_t region_id, ui
     if (ctx->ev_after_compact) cudaEventRecord(ctx->ev_after_compact, st);
     CC_CUDA(ctx, cudaGetLastError());
     return launch_gather(ctx, slot, st, out);
+}
+
+extern "C" int32_t cc_snapshot_region(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out) {
+    if (!ctx) return CC_ERR_INVALID;
+    int slot = find_slot(ctx, region_id);
+    if (slot < 0) return CC_ERR_NOT_REGISTERED;
+    const cc_region_dev& r = ctx->regions[slot].dev;
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    cc_snapshot_plan_kernel<<<small_grid(ctx, r.n_pages, 256), 256, 0, st>>>(ctx->d_dev, slot, epoch);
+    ctx->launches += 1;
+    if (ctx->ev_after_scan) cudaEventRecord(ctx->ev_after_scan, st);
+    if (ctx->ev_after_compact) cudaEventRecord(ctx->ev_after_compact, st);
+    CC_CUDA(ctx, cudaGetLastError());
+    return launch_gather(ctx, slot, st, out);
+}
+
+extern "C" int32_t cc_compact_log(cc_ctx* ctx, const void* in_log, uint64_t in_bytes, void* out_log, uint64_t out_capacity,
+                                  void* stream, cc_result* out) {
+    if (!ctx || !in_log || !out_log || ((uintptr_t)in_log & 15) || ((uintptr_t)out_log & 15)) return CC_ERR_INVALID;
+    if (!ctx->apply_attached) return CC_ERR_INVALID;
+    const uintptr_t a0 = (uintptr_t)in_log, a1 = a0 + in_bytes, b0 = (uintptr_t)out_log, b1 = b0 + out_capacity;
+    if (a0 < b1 && b0 < a1) return CC_ERR_INVALID;       // the two logs must not overlap
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    const u8* lg = (const u8*)in_log;
+    const unsigned gv = (unsigned)(ctx->sm_count * ctx->validate_bps);
+    const unsigned gs = (unsigned)(ctx->sm_count * 8);
+    cc_apply_parse_kernel<<<1, CC_PARSE_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, lg, in_bytes);
+    cc_apply_validate_kernel<<<gv, CC_APPLY_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, ctx->tabs, lg);
+    cc_compactor_mark_kernel<<<(unsigned)ctx->sm_count, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs);
+    cc_compactor_rank_kernel<<<(unsigned)ctx->sm_count, CC_COMPACT_THREADS, 0, st>>>(ctx->d_dev);
+    cc_compactor_plan_kernel<<<1, 1, 0, st>>>(ctx->d_dev, out_capacity);
+    cc_compactor_copy_kernel<<<gs, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, lg, (u8*)out_log);
+    cc_compactor_cleanup_kernel<<<(unsigned)ctx->sm_count, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, out);
+    ctx->launches += 7;
+    CC_CUDA(ctx, cudaGetLastError());
+    return CC_OK;
 }
 
 extern "C" int32_t cc_scan_only(cc_ctx* ctx, uint32_t region_id, void* stream, cc_result* out) {
