@@ -626,3 +626,43 @@ int32_t orc_compact_log(const uint8_t *log, uint64_t n, const orc_region *region
     if (status != ORC_OK) *n_out = 0;
     return status;
 }
+
+/* ------------------- multi-region checkpoint at one boundary --- */
+
+/* PAPER.md:L259 "At each NCCL or kernel boundary, a four-stage GPU-side pipeline executes" over the
+ * registered mutable regions (L217, L257).  Reading (#37): one boundary = one call; the
+ * regions that have a shadow are delta-checkpointed one after the other in ascending region_id order,
+ * every one exactly as orc_checkpoint does it, all with the same epoch number, each with its own
+ * commit record (reading #8: one region per epoch record), the log offset running through.  A region
+ * whose records do not fit is skipped whole (its own all-or-nothing rule, shadow untouched); the
+ * regions after it are still tried.  Regions without a shadow (allocator-aware, immutable) take no
+ * part.  k_out[i] / st_out[i] are per region in the order of `regions`.
+ * Returns ORC_OK or the status of the first (lowest id) region that failed. */
+int32_t orc_checkpoint_all(const orc_region *regions, uint32_t n_regions, uint64_t epoch,
+                           uint8_t *log, uint64_t C, uint64_t *W,
+                           uint64_t *k_out, int32_t *st_out, uint64_t *k_total, uint64_t *bytes_total) {
+    int32_t first_bad = ORC_OK;
+    uint32_t prev_id = 0;
+    *k_total = 0;
+    *bytes_total = 0;
+    for (uint32_t i = 0; i < n_regions; i++) { k_out[i] = 0; st_out[i] = ORC_OK; }
+    for (;;) {
+        uint32_t best = n_regions;
+        for (uint32_t i = 0; i < n_regions; i++)
+            if (regions[i].region_id > prev_id && (best == n_regions || regions[i].region_id < regions[best].region_id))
+                best = i;
+        if (best == n_regions) break;
+        prev_id = regions[best].region_id;
+        const orc_region *r = &regions[best];
+        if (!r->shadow) continue;
+        uint64_t k = 0, nb = 0;
+        int32_t st = orc_checkpoint(r->base, r->shadow, r->bytes, r->page_bytes, r->region_id, epoch, log, C, W,
+                                    NULL, &k, &nb);
+        k_out[best] = k;
+        st_out[best] = st;
+        *k_total += k;
+        *bytes_total += nb;
+        if (st != ORC_OK && first_bad == ORC_OK) first_bad = st;
+    }
+    return first_bad;
+}

@@ -65,6 +65,9 @@ def _load():
         lib.orc_compact_log.restype = ctypes.c_int32
         lib.orc_compact_log.argtypes = [u8p, ctypes.c_uint64, ctypes.POINTER(_CRegion), ctypes.c_uint32,
                                         u8p, ctypes.c_uint64, u64p, u64p, u64p]
+        lib.orc_checkpoint_all.restype = ctypes.c_int32
+        lib.orc_checkpoint_all.argtypes = [ctypes.POINTER(_CRegion), ctypes.c_uint32, ctypes.c_uint64, u8p, ctypes.c_uint64,
+                                           u64p, u8p, u8p, u64p, u64p]
         lib.orc_apply.restype = ctypes.c_int32
         lib.orc_apply.argtypes = [u8p, ctypes.c_uint64, ctypes.POINTER(_CRegion), ctypes.c_uint32, u64p, u64p]
         lib.orc_write_epoch.restype = ctypes.c_int32
@@ -226,6 +229,31 @@ def compact_log(log, nbytes: int, regions, out):
     st = _load().orc_compact_log(_ptr(lg), nbytes, arr, len(regions), _ptr(o), o.size, ctypes.byref(nb),
                                  ctypes.byref(consumed), ctypes.byref(n_out))
     return int(st), int(nb.value), int(consumed.value), int(n_out.value)
+
+
+def checkpoint_all(regions, epoch: int, log, W: int):
+    """One boundary: every region that has a shadow is delta-checkpointed in ascending region_id order (base and
+    shadow are numpy arrays; shadows and the log are modified in place).
+    Returns (status, k per region in the order given, status per region, k_total, bytes_total, W_after)."""
+    lg = _u8(log)
+    arr = (_CRegion * max(len(regions), 1))()
+    keep = []
+    for i, r in enumerate(regions):
+        b = _u8(r.base)
+        keep.append(b)
+        sh = 0
+        if r.shadow is not None:
+            s_ = _u8(r.shadow)
+            assert s_.size == b.size and s_.flags["WRITEABLE"]
+            keep.append(s_)
+            sh = _ptr(s_)
+        arr[i] = _CRegion(r.region_id, r.page_bytes, b.size, _ptr(b), sh)
+    ks = np.zeros(max(len(regions), 1), dtype=np.uint64)
+    sts = np.zeros(max(len(regions), 1), dtype=np.int32)
+    w, kt, bt = ctypes.c_uint64(W), ctypes.c_uint64(0), ctypes.c_uint64(0)
+    st = _load().orc_checkpoint_all(arr, len(regions), epoch, _ptr(lg), lg.size, ctypes.byref(w), _ptr(ks), _ptr(sts),
+                                    ctypes.byref(kt), ctypes.byref(bt))
+    return int(st), ks[: len(regions)].tolist(), sts[: len(regions)].tolist(), int(kt.value), int(bt.value), int(w.value)
 
 
 def write_epoch(log, W: int, region_id: int, epoch: int, region_bytes: int, page_bytes: int, pages, payloads):
