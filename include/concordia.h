@@ -123,6 +123,7 @@ typedef struct {
 #define CC_TASK_VERSION_CKPT 6u    /* region_id, epoch; arg0 = version[] (device), arg1 = committed[] (device) */
 #define CC_TASK_SNAPSHOT 7u        /* region_id, epoch: base snapshot (cc_snapshot_region) */
 #define CC_TASK_COMPACT_LOG 8u     /* arg0 = input log, arg1 = its bytes, arg2 = output log, arg3 = output capacity */
+#define CC_TASK_CKPT_ALL 9u        /* epoch: every region that has a shadow (cc_checkpoint_all) */
 #define CC_TASK_EXIT 255u
 #define CC_TASKF_FUSED 1u          /* cc_task.flags, CC_TASK_DELTA_CKPT only: run the fused single pass (cc_checkpoint_delta_fused) */
 typedef struct {
@@ -213,6 +214,18 @@ int32_t cc_checkpoint_marked(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, ui
  * nothing moves. */
 int32_t cc_checkpoint_versions(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, const uint64_t* version,
                                uint64_t* committed, void* stream, cc_result* out);
+
+/* One boundary, all regions ("At each NCCL or kernel boundary, a four-stage GPU-side
+ * pipeline executes"; L217, L257): every registered region that has a shadow is delta-checkpointed with
+ * the same epoch number.  The log receives the regions' epochs in ascending region_id order, each with
+ * its own commit record -- the same bytes as calling cc_checkpoint_delta region by region in that order --
+ * in four kernel launches whatever the number of regions.  A region whose records do not fit is skipped
+ * whole (shadow untouched); the regions after it are still tried.  The committed offset is published once,
+ * after every region's commit record is visible.  Result: n_dirty / bytes summed over the regions,
+ * log_offset_after = final write offset, status = CC_OK or the status of the lowest-id region that
+ * failed; per-region dirty lists through cc_dirty_list.  Regions registered with CC_REG_NO_SHADOW take
+ * no part.  ASYNCHRONOUS on `stream`. */
+int32_t cc_checkpoint_all(cc_ctx* ctx, uint64_t epoch, void* stream, cc_result* out);
 
 /* Base snapshot ("The initial base snapshot captured all 8,192 pages of the full region";
  * L257: immutable regions "are included in the base snapshot but do not keep GPU shadows"): append EVERY

@@ -83,14 +83,13 @@ __device__ __forceinline__ u64 lb_pack(u32 run, u64 flag, u32 val) { return ((u6
 // The plan of the record writer, written once k is final (one thread): record count, byte need,
 // all-or-nothing log-full decision (reading #10), start offset.  last_dirty: the region's (possibly
 // short) last page is among the k pages.  inline_done: the records are already in place (fused pass).
-__device__ __forceinline__ void cc_plan_checkpoint(const cc_region_dev& r, const cc_log_dev* log, u32 mode, u64 epoch, u32 k,
-                                                   bool last_dirty, bool inline_done) {
+__device__ __forceinline__ void cc_plan_checkpoint_at(const cc_region_dev& r, const cc_log_dev* log, u64 W, u32 mode, u64 epoch,
+                                                      u32 k, bool last_dirty, bool inline_done) {
     cc_ws_hdr* h = r.hdr;
     h->k = k;
     h->epoch = epoch;
     u64 need = (u64)k * (CC_RECORD_HEADER_BYTES + (u64)r.page_bytes) + CC_COMMIT_RECORD_BYTES;
     if (last_dirty) need -= (u64)r.page_bytes - page_len_dev(r, r.n_pages - 1);
-    const u64 W = log->W;
     int32_t st = CC_OK;
     u32 k_eff = 0;
     if (mode == CC_MODE_CHECKPOINT && k != 0) {
@@ -103,6 +102,10 @@ __device__ __forceinline__ void cc_plan_checkpoint(const cc_region_dev& r, const
     h->need = k_eff ? need : 0;
     h->gather_done = 0;
     h->inline_done = inline_done ? 1u : 0u;
+}
+__device__ __forceinline__ void cc_plan_checkpoint(const cc_region_dev& r, const cc_log_dev* log, u32 mode, u64 epoch, u32 k,
+                                                   bool last_dirty, bool inline_done) {
+    cc_plan_checkpoint_at(r, log, log->W, mode, epoch, k, last_dirty, inline_done);
 }
 
 // Only the first CC_COMPACT_THREADS threads of a block work (the worker's blocks may be wider);
@@ -227,8 +230,12 @@ __device__ __forceinline__ void st_u32x4(u8* p, u32 a, u32 b, u32 c, u32 d) {
     st_stream(reinterpret_cast<uint4*>(p), v);
 }
 
+// batch = true (cc_batch.cuh): this region is one of several checkpointed at the same boundary; its last block
+// appends the region's commit record but leaves the log offset, the publication and the result to the batch.
+__device__ __forceinline__ void cc_batch_region_done(cc_dev* dev, cc_result* out, u32 kind);
+
 __device__ __forceinline__ void cc_gather_phase(const cc_region_dev& r, cc_dev* dev, cc_crc_smem* cs, cc_grid g,
-                                                cc_result* out, u32 kind, bool init_tables) {
+                                                cc_result* out, u32 kind, bool init_tables, bool batch = false) {
     constexpr int U = 8;
     cc_ws_hdr* h = r.hdr;
     cc_log_dev* log = &dev->log;
@@ -316,13 +323,17 @@ __device__ __forceinline__ void cc_gather_phase(const cc_region_dev& r, cc_dev* 
             st_u32x4(c, CC_COMMIT_ID, CC_COMMIT_ID, 16u, crc);
             W_after = W0 + h->need;
             __threadfence_system();
-            if (log->committed_off) st_release_sys_u64(log->committed_off, W_after);
-            log->W = W_after;
+            if (!batch) {
+                if (log->committed_off) st_release_sys_u64(log->committed_off, W_after);
+                log->W = W_after;
+            }
         }
         h->gather_done = 0;
         h->fticket = 0;
         h->frun = h->frun + 1;
-        if (out) {
+        if (batch) {
+            cc_batch_region_done(dev, out, kind);
+        } else if (out) {
             out->n_dirty = h->k;
             out->bytes = h->need;
             out->log_offset_after = W_after;

@@ -105,6 +105,19 @@ struct cc_compactor_state {
     u32 n_regions_out;
 };
 
+// Multi-region boundary checkpoint state (cc_batch.cuh).
+struct cc_batch_state {
+    u64 W_final;
+    u64 k_total;
+    u64 bytes_total;
+    u64 t_start_ns;
+    u64 epoch;
+    int32_t status;         // CC_OK or the status of the first (lowest id) region that failed
+    u32 n_active;           // regions taking part (those with a shadow)
+    u32 done;               // regions whose commit record is in place
+    u32 pad;
+};
+
 struct cc_crc_tables {
     u32 t0[256];            // byte table of the reflected polynomial
     u32 s512[4][256];       // multiply by x^(8*512) mod G, one table per register byte
@@ -126,6 +139,7 @@ struct cc_dev {
     u64 max_records;
     cc_apply_state apply;
     cc_compactor_state compactor;
+    cc_batch_state batch;
     // grid barrier + worker doorbell
     u32 bar_count;
     u32 bar_gen;

@@ -16,6 +16,7 @@
 #include "cc_fused.cuh"
 #include "cc_apply.cuh"
 #include "cc_compactor.cuh"
+#include "cc_batch.cuh"
 
 struct cc_ring_dev {            // all pointers are pinned, device-mapped host memory
     cc_task* slots;             // capacity x 64 B
@@ -226,6 +227,15 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
                 cc_mark_finish_phase(r, nullptr, ver, com, g);
                 break;
             }
+            case CC_TASK_CKPT_ALL:
+                cc_batch_scan_phase(dev, g);
+                cc_grid_barrier(dev, g.nblocks, gen);
+                cc_batch_rank_phase(dev, task.epoch);
+                cc_grid_barrier(dev, g.nblocks, gen);
+                if (g.block == 0 && threadIdx.x == 0) cc_batch_plan_phase(dev, task.epoch);
+                cc_grid_barrier(dev, g.nblocks, gen);
+                cc_batch_gather_phase(dev, cs, g, nullptr, task.kind);
+                break;
             case CC_TASK_SNAPSHOT: {
                 const cc_region_dev& r = dev->regions[slot];
                 cc_snapshot_plan_phase(r, &dev->log, task.epoch, g);
@@ -254,6 +264,9 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
             if (status == CC_OK && is_ckpt) {
                 const cc_ws_hdr* h = dev->regions[slot].hdr;
                 n_dirty = h->k; bytes = h->need; status = h->status;
+            } else if (status == CC_OK && task.kind == CC_TASK_CKPT_ALL) {
+                const cc_batch_state* B = &dev->batch;
+                n_dirty = B->k_total; bytes = B->bytes_total; off_after = B->W_final; status = B->status;
             } else if (status == CC_OK && task.kind == CC_TASK_COMPACT_LOG) {
                 const cc_compactor_state* C = &dev->compactor;
                 n_dirty = C->n_out; bytes = C->bytes_out; off_after = dev->apply.consumed;

@@ -16,6 +16,7 @@
 #include "cc_fused.cuh"
 #include "cc_apply.cuh"
 #include "cc_compactor.cuh"
+#include "cc_batch.cuh"
 #include "cc_worker.cuh"
 
 static_assert(sizeof(cc_result) == 64, "cc_result must be 64 bytes");
@@ -64,6 +65,17 @@ __global__ void __launch_bounds__(CC_APPLY_THREADS) cc_compactor_copy_kernel(cc_
 }
 __global__ void __launch_bounds__(CC_APPLY_THREADS) cc_compactor_cleanup_kernel(cc_dev* dev, cc_apply_tabs tabs, cc_result* out) {
     cc_compactor_cleanup_phase(dev, tabs, cc_hw_grid(), out, CC_TASK_COMPACT_LOG);
+}
+
+// one boundary, all regions (cc_batch.cuh)
+__global__ void __launch_bounds__(CC_SCAN_THREADS) cc_batch_scan_kernel(cc_dev* dev) { cc_batch_scan_phase(dev, cc_hw_grid()); }
+__global__ void __launch_bounds__(CC_COMPACT_THREADS) cc_batch_rank_kernel(cc_dev* dev, u64 epoch) { cc_batch_rank_phase(dev, epoch); }
+__global__ void cc_batch_plan_kernel(cc_dev* dev, u64 epoch) { cc_batch_plan_phase(dev, epoch); }
+__global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_batch_gather_kernel(cc_dev* dev, cc_result* out) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cc_crc_smem* cs = reinterpret_cast<cc_crc_smem*>(smem_raw);
+    cc_crc_smem_init(cs, &dev->crc);
+    cc_batch_gather_phase(dev, cs, cc_hw_grid(), out, CC_TASK_CKPT_ALL);
 }
 
 // allocator-aware discovery (cc_mark.cuh)
@@ -221,6 +233,7 @@ extern "C" int32_t cc_init(cc_ctx** out, int32_t device, const cc_config* cfg) {
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->worker_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->worker_done, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_batch_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->fused_bps, cc_fused_kernel, CC_GATHER_THREADS, sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_apply_validate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
@@ -509,6 +522,21 @@ extern "C" int32_t cc_checkpoint_delta_fused(cc_ctx* ctx, uint32_t region_id, ui
     if (ctx->ev_after_compact) cudaEventRecord(ctx->ev_after_compact, st);
     CC_CUDA(ctx, cudaGetLastError());
     return launch_gather(ctx, slot, st, out);
+}
+
+extern "C" int32_t cc_checkpoint_all(cc_ctx* ctx, uint64_t epoch, void* stream, cc_result* out) {
+    if (!ctx) return CC_ERR_INVALID;
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    cc_batch_scan_kernel<<<(unsigned)(ctx->sm_count * ctx->scan_bps), CC_SCAN_THREADS, 0, st>>>(ctx->d_dev);
+    if (ctx->ev_after_scan) cudaEventRecord(ctx->ev_after_scan, st);
+    cc_batch_rank_kernel<<<(unsigned)ctx->sm_count, CC_COMPACT_THREADS, 0, st>>>(ctx->d_dev, epoch);
+    cc_batch_plan_kernel<<<1, 1, 0, st>>>(ctx->d_dev, epoch);
+    if (ctx->ev_after_compact) cudaEventRecord(ctx->ev_after_compact, st);
+    cc_batch_gather_kernel<<<(unsigned)(ctx->sm_count * ctx->gather_bps), CC_GATHER_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, out);
+    ctx->launches += 4;
+    CC_CUDA(ctx, cudaGetLastError());
+    return CC_OK;
 }
 
 extern "C" int32_t cc_snapshot_region(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out) {
