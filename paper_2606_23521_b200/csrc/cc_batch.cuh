@@ -3,68 +3,151 @@
 // Every registered region that has a shadow is delta-checkpointed with the same epoch number, in
 // ascending region_id order in the log, in FOUR launches whatever the number of regions:
 //   scan-all    cc_scan_phase over every region (the grid strides over one region after the other)
-//   rank-all    the ordered compaction of every region's bitmap (k per region)
-//   plan        one thread: ascending region_id, running log offset; a region that does not fit is
-//               skipped whole (its own all-or-nothing rule), the ones after it are still tried
-//   gather-all  cc_gather_phase over every region; a region's last block appends its commit record;
-//               the last region to finish publishes the final offset ONCE (a published offset means
-//               "everything before it is committed", so per-region publishes could not be reordered)
-//               and fills the aggregated result.
+//   rank-all    the ordered compaction of every region's bitmap (k per region); a small region is ranked
+//               by ONE block (round-robin over the blocks), a large one by the whole grid
+//   plan        one block, one thread per region slot: rank the regions by id, sizes in parallel, one thread
+//               chains the log offset over the (<= 64) sizes in shared memory, plans written in parallel.
+//               A region that does not fit is skipped whole (its own all-or-nothing rule), the ones after
+//               it are still tried
+//   gather-all  cc_gather_work over every region with no synchronisation in between; ONE completion for
+//               the whole boundary: the last block appends every region's commit record, fences, publishes
+//               the final offset once (a published offset means "everything before it is committed") and
+//               fills the aggregated result.
 // Same bytes as calling cc_checkpoint_delta region by region in ascending id order.
 #pragma once
 #include "cc_common.cuh"
 #include "cc_ckpt.cuh"
 
+#define CC_BATCH_SMALL_TILES 4u     // regions with at most this many compaction tiles are ranked by a single block
+
 __device__ __forceinline__ bool cc_batch_takes_part(const cc_dev* dev, int s) {
     return dev->region_used[s] && dev->regions[s].shadow != nullptr;
 }
 
-__device__ __forceinline__ void cc_batch_scan_phase(cc_dev* dev, cc_grid g) {
+// The regions' work items form ONE index space (region after region); warp w takes the global items
+// w, w + nwarps, ...  A per-block table in shared memory (item count per region slot, built by one thread per
+// slot) tells a warp which of its items fall into which region, so that it never touches a region it has no
+// item in -- with many small regions the cost is the sum of the work, not a chain of per-region latencies.
+struct cc_batch_tab {
+    u64 n_items[CC_MAX_REGIONS];
+    u64 cum[CC_MAX_REGIONS + 1];
+};
+
+// call with all threads of the block; n_items[] filled by threads < CC_MAX_REGIONS beforehand
+__device__ __forceinline__ void cc_batch_tab_finish(cc_batch_tab* T) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        u64 c = 0;
+        for (int s = 0; s < CC_MAX_REGIONS; s++) { T->cum[s] = c; c += T->n_items[s]; }
+        T->cum[CC_MAX_REGIONS] = c;
+    }
+    __syncthreads();
+}
+
+// first local item of region slot s for this warp (>= n_items[s] if none)
+__device__ __forceinline__ u64 cc_batch_first(const cc_batch_tab* T, int s, u64 warp, u64 nwarps) {
+    const u64 m = T->cum[s] % nwarps;
+    return (warp + nwarps - m) % nwarps;
+}
+
+__device__ __forceinline__ void cc_batch_scan_phase(cc_dev* dev, cc_batch_tab* T, cc_grid g) {
     if (g.block == 0 && threadIdx.x == 0) {
         dev->batch.t_start_ns = globaltimer_ns();
         dev->batch.done = 0;
     }
-    for (int s = 0; s < CC_MAX_REGIONS; s++)
-        if (cc_batch_takes_part(dev, s)) cc_scan_phase<8>(dev->regions[s], g);
+    if (threadIdx.x < CC_MAX_REGIONS) {
+        const int s = (int)threadIdx.x;
+        u64 n = 0;
+        if (cc_batch_takes_part(dev, s)) {
+            const cc_region_dev& r = dev->regions[s];
+            n = r.n_pages * (u64)r.spp;
+            if (g.block == 0) {                             // open the region's compaction run (as cc_scan_phase does)
+                r.hdr->t_start_ns = dev->batch.t_start_ns;
+                r.hdr->ticket = 0;
+                r.hdr->run_id = r.hdr->run_id + 1;
+            }
+        }
+        T->n_items[s] = n;
+    }
+    cc_batch_tab_finish(T);
+    const u64 w = g.warp(), nw = g.nwarps();
+    for (int s = 0; s < CC_MAX_REGIONS; s++) {
+        if (T->n_items[s] == 0) continue;
+        const u64 first = cc_batch_first(T, s, w, nw);
+        if (first < T->n_items[s]) cc_scan_items<8>(dev->regions[s], first, nw);
+    }
 }
 
-__device__ __forceinline__ void cc_batch_rank_phase(cc_dev* dev, u64 epoch) {
-    for (int s = 0; s < CC_MAX_REGIONS; s++)
-        if (cc_batch_takes_part(dev, s)) cc_compact_phase(dev->regions[s], &dev->log, CC_MODE_SCAN_ONLY, epoch, nullptr);
+__device__ __forceinline__ void cc_batch_rank_phase(cc_dev* dev, u64 epoch, cc_grid g) {
+    u32 ordinal = 0;
+    for (int s = 0; s < CC_MAX_REGIONS; s++) {
+        if (!cc_batch_takes_part(dev, s)) continue;
+        const cc_region_dev& r = dev->regions[s];
+        const u64 nt = (r.n_words + CC_COMPACT_TILE_WORDS - 1) / CC_COMPACT_TILE_WORDS;
+        const bool mine = nt > CC_BATCH_SMALL_TILES || (ordinal % g.nblocks) == g.block;
+        ordinal++;
+        if (mine) cc_compact_phase(r, &dev->log, CC_MODE_SCAN_ONLY, epoch, nullptr);
+    }
 }
 
-// One thread.
+// One block of at least CC_MAX_REGIONS threads.
 __device__ __forceinline__ void cc_batch_plan_phase(cc_dev* dev, u64 epoch) {
+    __shared__ u32 s_id[CC_MAX_REGIONS], s_order[CC_MAX_REGIONS], s_n;
+    __shared__ u64 s_need[CC_MAX_REGIONS], s_W[CC_MAX_REGIONS];
     cc_batch_state* B = &dev->batch;
     const cc_log_dev* log = &dev->log;
-    u64 W = log->W, k_total = 0;
-    const u64 W_begin = W;
-    int32_t first_bad = CC_OK;
-    u32 n_active = 0, prev = 0;
-    for (;;) {
-        int best = -1;
-        for (int s = 0; s < CC_MAX_REGIONS; s++)
-            if (cc_batch_takes_part(dev, s) && dev->regions[s].region_id > prev &&
-                (best < 0 || dev->regions[s].region_id < dev->regions[best].region_id))
-                best = s;
-        if (best < 0) break;
-        const cc_region_dev& r = dev->regions[best];
-        prev = r.region_id;
-        n_active++;
-        const u32 k = r.hdr->k;
-        const bool last_dirty = k != 0 && r.D[k - 1] == (u32)(r.n_pages - 1);
-        cc_plan_checkpoint_at(r, log, W, CC_MODE_CHECKPOINT, epoch, k, last_dirty, false);
-        W += r.hdr->need;
-        k_total += k;
-        if (r.hdr->status != CC_OK && first_bad == CC_OK) first_bad = r.hdr->status;
+    const u32 t = threadIdx.x;
+    const bool part = t < CC_MAX_REGIONS && cc_batch_takes_part(dev, (int)t);
+    if (t < CC_MAX_REGIONS) s_id[t] = part ? dev->regions[t].region_id : 0xFFFFFFFFu;
+    if (t == 0) s_n = 0;
+    __syncthreads();
+    u32 k = 0;
+    bool last_dirty = false;
+    if (part) {
+        const cc_region_dev& r = dev->regions[t];
+        u32 rank = 0;
+        for (u32 q = 0; q < CC_MAX_REGIONS; q++) rank += (s_id[q] < s_id[t]) ? 1u : 0u;     // ids are distinct
+        s_order[rank] = t;
+        atomicAdd(&s_n, 1u);
+        k = r.hdr->k;
+        last_dirty = k != 0 && r.D[k - 1] == (u32)(r.n_pages - 1);
+        u64 need = 0;
+        if (k) {
+            need = (u64)k * (CC_RECORD_HEADER_BYTES + (u64)r.page_bytes) + CC_COMMIT_RECORD_BYTES;
+            if (last_dirty) need -= (u64)r.page_bytes - page_len_dev(r, r.n_pages - 1);
+        }
+        s_need[t] = need;
     }
-    B->W_final = W;
-    B->k_total = k_total;
-    B->bytes_total = W - W_begin;
-    B->epoch = epoch;
-    B->status = first_bad;
-    B->n_active = n_active;
-    __threadfence();
+    __syncthreads();
+    if (t == 0) {                       // the only sequential part: <= 64 additions in shared memory
+        u64 W = log->W;
+        const u64 W_begin = W;
+        for (u32 i = 0; i < s_n; i++) {
+            const u32 q = s_order[i];
+            s_W[q] = W;
+            if (s_need[q] != 0 && log->buf != nullptr && W + s_need[q] <= log->capacity) W += s_need[q];
+        }
+        B->W_final = W;
+        B->bytes_total = W - W_begin;
+        B->epoch = epoch;
+        B->n_active = s_n;
+        B->k_total = 0;
+        B->status = CC_OK;
+    }
+    __syncthreads();
+    if (part) {
+        const cc_region_dev& r = dev->regions[t];
+        cc_plan_checkpoint_at(r, log, s_W[t], CC_MODE_CHECKPOINT, epoch, k, last_dirty, false);
+        atomicAdd(reinterpret_cast<unsigned long long*>(&B->k_total), (unsigned long long)k);
+    }
+    __syncthreads();
+    if (t == 0) {                       // status of the lowest-id region that failed
+        for (u32 i = 0; i < s_n; i++) {
+            const int32_t st = dev->regions[s_order[i]].hdr->status;
+            if (st != CC_OK) { B->status = st; break; }
+        }
+        __threadfence();
+    }
 }
 
 __device__ __forceinline__ void cc_batch_write_result(cc_dev* dev, cc_result* out, u32 kind) {
@@ -82,26 +165,49 @@ __device__ __forceinline__ void cc_batch_write_result(cc_dev* dev, cc_result* ou
     st_release_sys_u64(&out->seq_done, 1ull);
 }
 
-// Called by the last block of a region's gather (one thread), after the region's commit record and a
-// system-scope fence.  The last region to arrive publishes for the whole boundary.
-__device__ __forceinline__ void cc_batch_region_done(cc_dev* dev, cc_result* out, u32 kind) {
+// cs must already hold the CRC tables.
+__device__ __forceinline__ void cc_batch_gather_phase(cc_dev* dev, cc_crc_smem* cs, cc_batch_tab* T, cc_grid g, cc_result* out,
+                                                      u32 kind) {
     cc_batch_state* B = &dev->batch;
-    __threadfence();
-    if (atomicAdd(&B->done, 1u) != B->n_active - 1) return;
+    if (threadIdx.x < CC_MAX_REGIONS) {
+        const int s = (int)threadIdx.x;
+        u64 n = 0;
+        if (cc_batch_takes_part(dev, s)) n = (u64)dev->regions[s].hdr->k_eff * dev->regions[s].spp;
+        T->n_items[s] = n;
+    }
+    cc_batch_tab_finish(T);
+    {
+        const u64 w = g.warp(), nw = g.nwarps();
+        for (int s = 0; s < CC_MAX_REGIONS; s++) {
+            if (T->n_items[s] == 0) continue;
+            const u64 first = cc_batch_first(T, s, w, nw);
+            if (first < T->n_items[s]) cc_gather_items(dev->regions[s], dev, cs, first, nw);
+        }
+    }
+    // ---- one completion for the whole boundary ----
+    __shared__ u32 s_last;
     __threadfence_system();
-    cc_log_dev* log = &dev->log;
-    if (B->bytes_total != 0) {
-        if (log->committed_off) st_release_sys_u64(log->committed_off, B->W_final);
-        log->W = B->W_final;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence_system();
+        s_last = (atomicAdd(&B->done, 1u) == g.nblocks - 1) ? 1u : 0u;
     }
-    cc_batch_write_result(dev, out, kind);
-}
-
-__device__ __forceinline__ void cc_batch_gather_phase(cc_dev* dev, cc_crc_smem* cs, cc_grid g, cc_result* out, u32 kind) {
-    if (dev->batch.n_active == 0) {
-        if (g.block == 0 && threadIdx.x == 0) cc_batch_write_result(dev, out, kind);
-        return;
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence_system();
+    if (threadIdx.x < CC_MAX_REGIONS && cc_batch_takes_part(dev, (int)threadIdx.x))
+        cc_gather_commit_record(dev->regions[threadIdx.x], dev);
+    __threadfence_system();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence_system();
+        cc_log_dev* log = &dev->log;
+        if (B->bytes_total != 0) {
+            if (log->committed_off) st_release_sys_u64(log->committed_off, B->W_final);
+            log->W = B->W_final;
+        }
+        B->done = 0;
+        cc_batch_write_result(dev, out, kind);
+        __threadfence();
     }
-    for (int s = 0; s < CC_MAX_REGIONS; s++)
-        if (cc_batch_takes_part(dev, s)) cc_gather_phase(dev->regions[s], dev, cs, g, out, kind, false, true);
 }

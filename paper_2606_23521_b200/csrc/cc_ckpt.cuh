@@ -11,14 +11,10 @@
 // independent 16-byte streaming loads (cur, shadow), XOR/ORs them, the warp votes, and lane 0
 // sets the page's bit in the bitmap only if the segment differs.  The bitmap is all-zero on
 // entry (the compaction clears what it consumes).
+// Items first, first + step, ... of the region (the caller decides which warp takes which items).
 template <int U>
-__device__ __forceinline__ void cc_scan_phase(const cc_region_dev& r, cc_grid g) {
+__device__ __forceinline__ void cc_scan_items(const cc_region_dev& r, u64 first, u64 step) {
     const u32 lane = threadIdx.x & 31u;
-    if (g.block == 0 && threadIdx.x == 0) {
-        r.hdr->t_start_ns = globaltimer_ns();
-        r.hdr->ticket = 0;
-        r.hdr->run_id = r.hdr->run_id + 1;
-    }
     constexpr u32 SEGV = 32u * U;            // vectors per item
     constexpr u32 SEGB = SEGV * 16u;         // bytes per item
     const u32 P = r.page_bytes;
@@ -27,8 +23,7 @@ __device__ __forceinline__ void cc_scan_phase(const cc_region_dev& r, cc_grid g)
     const bool pow2 = (spp & (spp - 1)) == 0;
     const u32 sh = 31 - __clz(spp);
     const bool uniform = (r.bytes % P == 0) && (P % SEGB == 0);
-    const u64 stride = g.nwarps();
-    for (u64 item = g.warp(); item < n_items; item += stride) {
+    for (u64 item = first; item < n_items; item += step) {
         u64 p;
         u32 s;
         if (pow2) { p = item >> sh; s = (u32)(item & (spp - 1)); }
@@ -64,6 +59,16 @@ __device__ __forceinline__ void cc_scan_phase(const cc_region_dev& r, cc_grid g)
         if (__any_sync(0xFFFFFFFFu, acc != 0) && lane == 0)
             atomicOr(&r.bitmap[p >> 5], 1u << (p & 31));
     }
+}
+
+template <int U>
+__device__ __forceinline__ void cc_scan_phase(const cc_region_dev& r, cc_grid g) {
+    if (g.block == 0 && threadIdx.x == 0) {
+        r.hdr->t_start_ns = globaltimer_ns();
+        r.hdr->ticket = 0;
+        r.hdr->run_id = r.hdr->run_id + 1;
+    }
+    cc_scan_items<U>(r, g.warp(), g.nwarps());
 }
 
 // ------------------------------------------------------------------ a2: compaction --
@@ -230,12 +235,9 @@ __device__ __forceinline__ void st_u32x4(u8* p, u32 a, u32 b, u32 c, u32 d) {
     st_stream(reinterpret_cast<uint4*>(p), v);
 }
 
-// batch = true (cc_batch.cuh): this region is one of several checkpointed at the same boundary; its last block
-// appends the region's commit record but leaves the log offset, the publication and the result to the batch.
-__device__ __forceinline__ void cc_batch_region_done(cc_dev* dev, cc_result* out, u32 kind);
-
-__device__ __forceinline__ void cc_gather_phase(const cc_region_dev& r, cc_dev* dev, cc_crc_smem* cs, cc_grid g,
-                                                cc_result* out, u32 kind, bool init_tables, bool batch = false) {
+// The record writer proper (no synchronisation with other blocks): items first, first + step, ... of the
+// region's k_eff * spp (record, segment) items.  cs must hold the CRC tables.
+__device__ __forceinline__ void cc_gather_items(const cc_region_dev& r, cc_dev* dev, cc_crc_smem* cs, u64 first, u64 step) {
     constexpr int U = 8;
     cc_ws_hdr* h = r.hdr;
     cc_log_dev* log = &dev->log;
@@ -243,15 +245,11 @@ __device__ __forceinline__ void cc_gather_phase(const cc_region_dev& r, cc_dev* 
     const u32 lane = threadIdx.x & 31u;
     const u32 P = r.page_bytes;
     const u64 W0 = h->W_start;
-    // warps take items round-robin, so a block has work iff its first warp index is < n_items
-    // (after a fused pass that already wrote the records -- cc_fused.cuh -- only the commit below is left)
-    if (k_eff != 0 && !h->inline_done && (u64)g.block * (blockDim.x >> 5) < (u64)k_eff * r.spp) {
-        if (init_tables) cc_crc_smem_init(cs, &dev->crc);
+    {
         const u32 spp = r.spp;
         const u64 n_items = (u64)k_eff * spp;
         const u64 rec_stride = (u64)P + CC_RECORD_HEADER_BYTES;
-        const u64 stride = g.nwarps();
-        for (u64 item = g.warp(); item < n_items; item += stride) {
+        for (u64 item = first; item < n_items; item += step) {
             u32 i, c;
             if (r.spp_shift >= 0) { i = (u32)(item >> r.spp_shift); c = (u32)(item & (spp - 1)); }
             else { i = (u32)(item / spp); c = (u32)(item - (u64)i * spp); }
@@ -302,6 +300,47 @@ __device__ __forceinline__ void cc_gather_phase(const cc_region_dev& r, cc_dev* 
             }
         }
     }
+}
+
+__device__ __forceinline__ void cc_gather_work(const cc_region_dev& r, cc_dev* dev, cc_crc_smem* cs, cc_grid g, bool init_tables) {
+    const cc_ws_hdr* h = r.hdr;
+    const u32 k_eff = h->k_eff;
+    // warps take items round-robin, so a block has work iff its first warp index is < n_items
+    // (after a fused pass that already wrote the records -- cc_fused.cuh -- only the commit is left)
+    if (k_eff != 0 && !h->inline_done && (u64)g.block * (blockDim.x >> 5) < (u64)k_eff * r.spp) {
+        if (init_tables) cc_crc_smem_init(cs, &dev->crc);
+        cc_gather_items(r, dev, cs, g.warp(), g.nwarps());
+    }
+}
+
+// One thread: the region's commit record ("write commit marker"); returns the offset after it
+// (W_start if nothing was appended).  Also re-arms the per-region counters for the next call.
+__device__ __forceinline__ u64 cc_gather_commit_record(const cc_region_dev& r, cc_dev* dev) {
+    cc_ws_hdr* h = r.hdr;
+    cc_log_dev* log = &dev->log;
+    const u32 k_eff = h->k_eff;
+    const u64 W0 = h->W_start;
+    u64 W_after = W0;
+    if (k_eff != 0) {
+        u8* c = log->buf + W0 + h->need - CC_COMMIT_RECORD_BYTES;
+        const u64 epoch = h->epoch;
+        u32 pay[4] = {(u32)epoch, (u32)(epoch >> 32), r.region_id, k_eff};
+        const u32 crc = crc_serial(&dev->crc, reinterpret_cast<const u8*>(pay), 16);
+        st_u32x4(c + 16, pay[0], pay[1], pay[2], pay[3]);
+        st_u32x4(c, CC_COMMIT_ID, CC_COMMIT_ID, 16u, crc);
+        W_after = W0 + h->need;
+    }
+    h->gather_done = 0;
+    h->fticket = 0;
+    h->frun = h->frun + 1;
+    return W_after;
+}
+
+__device__ __forceinline__ void cc_gather_phase(const cc_region_dev& r, cc_dev* dev, cc_crc_smem* cs, cc_grid g,
+                                                cc_result* out, u32 kind, bool init_tables) {
+    cc_ws_hdr* h = r.hdr;
+    cc_log_dev* log = &dev->log;
+    cc_gather_work(r, dev, cs, g, init_tables);
     // ---- completion: last block commits ----
     __shared__ u32 s_last;
     __threadfence_system();
@@ -313,27 +352,14 @@ __device__ __forceinline__ void cc_gather_phase(const cc_region_dev& r, cc_dev* 
     __syncthreads();
     if (s_last && threadIdx.x == 0) {
         __threadfence_system();
-        u64 W_after = W0;
-        if (k_eff != 0) {
-            u8* c = log->buf + W0 + h->need - CC_COMMIT_RECORD_BYTES;
-            const u64 epoch = h->epoch;
-            u32 pay[4] = {(u32)epoch, (u32)(epoch >> 32), r.region_id, k_eff};
-            const u32 crc = crc_serial(&dev->crc, reinterpret_cast<const u8*>(pay), 16);
-            st_u32x4(c + 16, pay[0], pay[1], pay[2], pay[3]);
-            st_u32x4(c, CC_COMMIT_ID, CC_COMMIT_ID, 16u, crc);
-            W_after = W0 + h->need;
+        const bool appended = h->k_eff != 0;
+        const u64 W_after = cc_gather_commit_record(r, dev);
+        if (appended) {
             __threadfence_system();
-            if (!batch) {
-                if (log->committed_off) st_release_sys_u64(log->committed_off, W_after);
-                log->W = W_after;
-            }
+            if (log->committed_off) st_release_sys_u64(log->committed_off, W_after);
+            log->W = W_after;
         }
-        h->gather_done = 0;
-        h->fticket = 0;
-        h->frun = h->frun + 1;
-        if (batch) {
-            cc_batch_region_done(dev, out, kind);
-        } else if (out) {
+        if (out) {
             out->n_dirty = h->k;
             out->bytes = h->need;
             out->log_offset_after = W_after;

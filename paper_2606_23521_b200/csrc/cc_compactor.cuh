@@ -42,41 +42,57 @@ __device__ __forceinline__ void cc_compactor_rank_phase(cc_dev* dev) {
         if (dev->region_used[s]) cc_compact_phase(dev->regions[s], &dev->log, CC_MODE_SCAN_ONLY, 0, nullptr);
 }
 
-// One thread.  hdr->W_start of every region := its offset in the output; hdr->need := its bytes.
+// One block of at least CC_MAX_REGIONS threads (one per region slot).  hdr->W_start of every region := its
+// offset in the output; hdr->need := its bytes.  Regions are ranked by id in parallel; the only sequential
+// part is the running offset over <= 64 sizes held in shared memory.
 __device__ __forceinline__ void cc_compactor_plan_phase(cc_dev* dev, u64 out_capacity) {
+    __shared__ u32 s_id[CC_MAX_REGIONS], s_order[CC_MAX_REGIONS], s_k[CC_MAX_REGIONS], s_n;
+    __shared__ u64 s_need[CC_MAX_REGIONS], s_off[CC_MAX_REGIONS];
     cc_compactor_state* C = &dev->compactor;
-    u64 o = 0, n_out = 0;
-    u32 n_reg = 0;
-    if (cc_compactor_ok(dev)) {
-        u32 prev = 0;
-        for (;;) {
-            int best = -1;
-            for (int s = 0; s < CC_MAX_REGIONS; s++)
-                if (dev->region_used[s] && dev->regions[s].region_id > prev &&
-                    (best < 0 || dev->regions[s].region_id < dev->regions[best].region_id))
-                    best = s;
-            if (best < 0) break;
-            const cc_region_dev& r = dev->regions[best];
-            prev = r.region_id;
-            const u32 k = r.hdr->k;
-            u64 need = 0;
-            if (k) {
-                need = (u64)k * ((u64)r.page_bytes + CC_RECORD_HEADER_BYTES) + CC_COMMIT_RECORD_BYTES;
-                if (r.D[k - 1] == (u32)(r.n_pages - 1)) need -= (u64)r.page_bytes - page_len_dev(r, r.n_pages - 1);
-                n_reg++;
-            }
-            r.hdr->W_start = o;
-            r.hdr->need = need;
-            o += need;
-            n_out += k;
+    const u32 t = threadIdx.x;
+    const bool ok = cc_compactor_ok(dev);
+    const bool part = ok && t < CC_MAX_REGIONS && dev->region_used[t];
+    if (t < CC_MAX_REGIONS) s_id[t] = part ? dev->regions[t].region_id : 0xFFFFFFFFu;
+    if (t == 0) s_n = 0;
+    __syncthreads();
+    if (part) {
+        const cc_region_dev& r = dev->regions[t];
+        u32 rank = 0;
+        for (u32 q = 0; q < CC_MAX_REGIONS; q++) rank += (s_id[q] < s_id[t]) ? 1u : 0u;
+        s_order[rank] = t;
+        atomicAdd(&s_n, 1u);
+        const u32 k = r.hdr->k;
+        u64 need = 0;
+        if (k) {
+            need = (u64)k * ((u64)r.page_bytes + CC_RECORD_HEADER_BYTES) + CC_COMMIT_RECORD_BYTES;
+            if (r.D[k - 1] == (u32)(r.n_pages - 1)) need -= (u64)r.page_bytes - page_len_dev(r, r.n_pages - 1);
         }
+        s_k[t] = k;
+        s_need[t] = need;
     }
-    int32_t st = dev->apply.status;
-    if (st == CC_OK && o > out_capacity) st = CC_ERR_LOG_FULL;
-    C->status = st;
-    C->bytes_out = st == CC_OK ? o : 0;
-    C->n_out = st == CC_OK ? n_out : 0;
-    C->n_regions_out = st == CC_OK ? n_reg : 0;
+    __syncthreads();
+    if (t == 0) {
+        u64 o = 0, n_out = 0;
+        u32 n_reg = 0;
+        for (u32 i = 0; i < s_n; i++) {
+            const u32 q = s_order[i];
+            s_off[q] = o;
+            o += s_need[q];
+            n_out += s_k[q];
+            n_reg += s_k[q] ? 1u : 0u;
+        }
+        int32_t st = dev->apply.status;
+        if (st == CC_OK && o > out_capacity) st = CC_ERR_LOG_FULL;
+        C->status = st;
+        C->bytes_out = st == CC_OK ? o : 0;
+        C->n_out = st == CC_OK ? n_out : 0;
+        C->n_regions_out = st == CC_OK ? n_reg : 0;
+    }
+    __syncthreads();
+    if (part) {
+        dev->regions[t].hdr->W_start = s_off[t];
+        dev->regions[t].hdr->need = s_need[t];
+    }
     __threadfence();
 }
 

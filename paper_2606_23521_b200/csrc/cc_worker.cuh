@@ -85,7 +85,7 @@ __device__ __noinline__ void cc_worker_compact_task(cc_dev* dev, const cc_apply_
     cc_grid_barrier(dev, g.nblocks, gen);
     cc_compactor_rank_phase(dev);
     cc_grid_barrier(dev, g.nblocks, gen);
-    if (g.block == 0 && threadIdx.x == 0) cc_compactor_plan_phase(dev, task.arg3);
+    if (g.block == 0) cc_compactor_plan_phase(dev, task.arg3);
     cc_grid_barrier(dev, g.nblocks, gen);
     cc_compactor_copy_phase(dev, tabs, in, outl, g);
     cc_grid_barrier(dev, g.nblocks, gen);
@@ -97,6 +97,7 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cc_crc_smem* cs = reinterpret_cast<cc_crc_smem*>(smem_raw);
     __shared__ __align__(16) cc_task s_task;
+    __shared__ cc_batch_tab s_btab;
     const cc_grid g = cc_hw_grid();
     u32 gen = ld_acquire_gpu_u32(&dev->bar_gen);
     u64 head = 0;       // ring sequence number of the next task (meaningful in the leader thread only)
@@ -228,13 +229,13 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
                 break;
             }
             case CC_TASK_CKPT_ALL:
-                cc_batch_scan_phase(dev, g);
+                cc_batch_scan_phase(dev, &s_btab, g);
                 cc_grid_barrier(dev, g.nblocks, gen);
-                cc_batch_rank_phase(dev, task.epoch);
+                cc_batch_rank_phase(dev, task.epoch, g);
                 cc_grid_barrier(dev, g.nblocks, gen);
-                if (g.block == 0 && threadIdx.x == 0) cc_batch_plan_phase(dev, task.epoch);
+                if (g.block == 0) cc_batch_plan_phase(dev, task.epoch);
                 cc_grid_barrier(dev, g.nblocks, gen);
-                cc_batch_gather_phase(dev, cs, g, nullptr, task.kind);
+                cc_batch_gather_phase(dev, cs, &s_btab, g, nullptr, task.kind);
                 break;
             case CC_TASK_SNAPSHOT: {
                 const cc_region_dev& r = dev->regions[slot];

@@ -59,7 +59,7 @@ __global__ void __launch_bounds__(CC_APPLY_THREADS) cc_compactor_mark_kernel(cc_
     cc_compactor_mark_phase(dev, tabs, cc_hw_grid());
 }
 __global__ void __launch_bounds__(CC_COMPACT_THREADS) cc_compactor_rank_kernel(cc_dev* dev) { cc_compactor_rank_phase(dev); }
-__global__ void cc_compactor_plan_kernel(cc_dev* dev, u64 out_capacity) { cc_compactor_plan_phase(dev, out_capacity); }
+__global__ void __launch_bounds__(CC_MAX_REGIONS) cc_compactor_plan_kernel(cc_dev* dev, u64 out_capacity) { cc_compactor_plan_phase(dev, out_capacity); }
 __global__ void __launch_bounds__(CC_APPLY_THREADS) cc_compactor_copy_kernel(cc_dev* dev, cc_apply_tabs tabs, const u8* in, u8* out) {
     cc_compactor_copy_phase(dev, tabs, in, out, cc_hw_grid());
 }
@@ -68,14 +68,20 @@ __global__ void __launch_bounds__(CC_APPLY_THREADS) cc_compactor_cleanup_kernel(
 }
 
 // one boundary, all regions (cc_batch.cuh)
-__global__ void __launch_bounds__(CC_SCAN_THREADS) cc_batch_scan_kernel(cc_dev* dev) { cc_batch_scan_phase(dev, cc_hw_grid()); }
-__global__ void __launch_bounds__(CC_COMPACT_THREADS) cc_batch_rank_kernel(cc_dev* dev, u64 epoch) { cc_batch_rank_phase(dev, epoch); }
-__global__ void cc_batch_plan_kernel(cc_dev* dev, u64 epoch) { cc_batch_plan_phase(dev, epoch); }
+__global__ void __launch_bounds__(CC_SCAN_THREADS) cc_batch_scan_kernel(cc_dev* dev) {
+    __shared__ cc_batch_tab tab;
+    cc_batch_scan_phase(dev, &tab, cc_hw_grid());
+}
+__global__ void __launch_bounds__(CC_COMPACT_THREADS) cc_batch_rank_kernel(cc_dev* dev, u64 epoch) {
+    cc_batch_rank_phase(dev, epoch, cc_hw_grid());
+}
+__global__ void __launch_bounds__(CC_MAX_REGIONS) cc_batch_plan_kernel(cc_dev* dev, u64 epoch) { cc_batch_plan_phase(dev, epoch); }
 __global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_batch_gather_kernel(cc_dev* dev, cc_result* out) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cc_crc_smem* cs = reinterpret_cast<cc_crc_smem*>(smem_raw);
+    __shared__ cc_batch_tab tab;
     cc_crc_smem_init(cs, &dev->crc);
-    cc_batch_gather_phase(dev, cs, cc_hw_grid(), out, CC_TASK_CKPT_ALL);
+    cc_batch_gather_phase(dev, cs, &tab, cc_hw_grid(), out, CC_TASK_CKPT_ALL);
 }
 
 // allocator-aware discovery (cc_mark.cuh)
@@ -531,7 +537,7 @@ extern "C" int32_t cc_checkpoint_all(cc_ctx* ctx, uint64_t epoch, void* stream, 
     cc_batch_scan_kernel<<<(unsigned)(ctx->sm_count * ctx->scan_bps), CC_SCAN_THREADS, 0, st>>>(ctx->d_dev);
     if (ctx->ev_after_scan) cudaEventRecord(ctx->ev_after_scan, st);
     cc_batch_rank_kernel<<<(unsigned)ctx->sm_count, CC_COMPACT_THREADS, 0, st>>>(ctx->d_dev, epoch);
-    cc_batch_plan_kernel<<<1, 1, 0, st>>>(ctx->d_dev, epoch);
+    cc_batch_plan_kernel<<<1, CC_MAX_REGIONS, 0, st>>>(ctx->d_dev, epoch);
     if (ctx->ev_after_compact) cudaEventRecord(ctx->ev_after_compact, st);
     cc_batch_gather_kernel<<<(unsigned)(ctx->sm_count * ctx->gather_bps), CC_GATHER_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, out);
     ctx->launches += 4;
@@ -569,7 +575,7 @@ extern "C" int32_t cc_compact_log(cc_ctx* ctx, const void* in_log, uint64_t in_b
     cc_apply_validate_kernel<<<gv, CC_APPLY_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, ctx->tabs, lg);
     cc_compactor_mark_kernel<<<(unsigned)ctx->sm_count, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs);
     cc_compactor_rank_kernel<<<(unsigned)ctx->sm_count, CC_COMPACT_THREADS, 0, st>>>(ctx->d_dev);
-    cc_compactor_plan_kernel<<<1, 1, 0, st>>>(ctx->d_dev, out_capacity);
+    cc_compactor_plan_kernel<<<1, CC_MAX_REGIONS, 0, st>>>(ctx->d_dev, out_capacity);
     cc_compactor_copy_kernel<<<gs, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, lg, (u8*)out_log);
     cc_compactor_cleanup_kernel<<<(unsigned)ctx->sm_count, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, out);
     ctx->launches += 7;
