@@ -270,6 +270,14 @@ int32_t cc_dirty_list(cc_ctx* ctx, uint32_t region_id, const uint32_t** d_list, 
 uint64_t cc_apply_scratch_bytes(uint64_t max_records);
 int32_t cc_apply_attach(cc_ctx* ctx, void* scratch, uint64_t scratch_bytes);
 
+/* Optional device staging buffer for HOST-resident logs (16-byte aligned device memory; NULL / 0 detaches).
+ * The applier and the compactor read a log twice (validate, then scatter / copy).  When the log passed to
+ * cc_apply_log / cc_compact_log is pinned host memory of at most `bytes` bytes, it is first copied into this
+ * buffer by the copy engine on the call's stream (one pass over the host link at DMA speed) and the kernels
+ * read the device copy; results are identical.  Logs that do not fit, device-resident logs and the worker's
+ * RESTORE / COMPACT_LOG tasks are unaffected.  Only while the worker is stopped. */
+int32_t cc_apply_stage_attach(cc_ctx* ctx, void* device_buf, uint64_t bytes);
+
 /* Recovery applier: parse log[0, nbytes) (device or pinned host,
  * 16-byte aligned), validate structure and CRC32C of every record, and for every committed epoch
  * before the first failed check, in log order, write each page record's payload into its

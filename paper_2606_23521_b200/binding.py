@@ -48,7 +48,7 @@ EXPORTS = [
     "cc_init", "cc_shutdown", "cc_last_cuda_error", "cc_kernel_launches", "cc_workspace_bytes",
     "cc_register_region", "cc_unregister_region", "cc_log_attach", "cc_log_reset", "cc_log_reset_async",
     "cc_checkpoint_delta", "cc_checkpoint_delta_fused", "cc_checkpoint_marked", "cc_checkpoint_versions",
-    "cc_checkpoint_all", "cc_snapshot_region", "cc_compact_log", "cc_scan_only", "cc_trace_events", "cc_dirty_list", "cc_apply_scratch_bytes", "cc_apply_attach", "cc_apply_log",
+    "cc_checkpoint_all", "cc_snapshot_region", "cc_compact_log", "cc_scan_only", "cc_trace_events", "cc_dirty_list", "cc_apply_scratch_bytes", "cc_apply_attach", "cc_apply_stage_attach", "cc_apply_log",
     "cc_worker_start", "cc_worker_stop", "cc_worker_alive", "cc_peek_queue", "cc_submit", "cc_poll", "cc_wait",
 ]
 
@@ -122,6 +122,7 @@ def load_library():
         "cc_dirty_list": (i32, [vp, u32, P(vp), P(vp)]),
         "cc_apply_scratch_bytes": (u64, [u64]),
         "cc_apply_attach": (i32, [vp, vp, u64]),
+        "cc_apply_stage_attach": (i32, [vp, vp, u64]),
         "cc_apply_log": (i32, [vp, vp, u64, vp, vp]),
         "cc_worker_start": (i32, [vp]),
         "cc_worker_stop": (i32, [vp]),
@@ -184,6 +185,7 @@ class Context:
         self._log = None
         self._committed = None
         self._scratch = None
+        self._stage = None
 
     # -- helpers
     def _check(self, call, rc):
@@ -316,6 +318,17 @@ class Context:
         off = (-s.data_ptr()) % 256
         self._check("cc_apply_attach", self.lib.cc_apply_attach(self.h, s.data_ptr() + off, nb))
         self._scratch = s
+
+    def apply_stage_attach(self, nbytes: int):
+        """Allocate and attach a device staging buffer for host-resident logs (0 detaches)."""
+        if nbytes == 0:
+            self._check("cc_apply_stage_attach", self.lib.cc_apply_stage_attach(self.h, None, 0))
+            self._stage = None
+            return
+        s = torch.empty(nbytes + 16, dtype=torch.uint8, device=torch.device("cuda", self.device))
+        off = (-s.data_ptr()) % 16
+        self._check("cc_apply_stage_attach", self.lib.cc_apply_stage_attach(self.h, s.data_ptr() + off, nbytes))
+        self._stage = s
 
     def apply_log(self, log: torch.Tensor, nbytes: int, result: Result = None, stream=None):
         assert log.dtype == torch.uint8 and log.is_contiguous() and (log.is_cuda or log.is_pinned())

@@ -139,6 +139,8 @@ struct cc_ctx {
     bool log_attached;
     cc_apply_tabs tabs;
     bool apply_attached;
+    void* stage;                // optional device staging buffer for host-resident logs (cc_apply_stage_attach)
+    uint64_t stage_bytes;
     int last_cuda;
     uint64_t launches;
     int scan_bps, gather_bps, validate_bps, fused_bps;     // blocks per SM from the occupancy API
@@ -162,6 +164,8 @@ struct cc_ctx {
             return CC_ERR_CUDA;                                \
         }                                                      \
     } while (0)
+
+static const u8* stage_log(cc_ctx* ctx, const void* log, uint64_t nbytes, cudaStream_t st);
 
 static inline uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
 
@@ -568,7 +572,7 @@ extern "C" int32_t cc_compact_log(cc_ctx* ctx, const void* in_log, uint64_t in_b
     if (a0 < b1 && b0 < a1) return CC_ERR_INVALID;       // the two logs must not overlap
     CC_CUDA(ctx, cudaSetDevice(ctx->device));
     cudaStream_t st = (cudaStream_t)stream;
-    const u8* lg = (const u8*)in_log;
+    const u8* lg = stage_log(ctx, in_log, in_bytes, st);
     const unsigned gv = (unsigned)(ctx->sm_count * ctx->validate_bps);
     const unsigned gs = (unsigned)(ctx->sm_count * 8);
     cc_apply_parse_kernel<<<1, CC_PARSE_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, lg, in_bytes);
@@ -638,12 +642,31 @@ extern "C" int32_t cc_apply_attach(cc_ctx* ctx, void* scratch, uint64_t scratch_
     return CC_OK;
 }
 
+extern "C" int32_t cc_apply_stage_attach(cc_ctx* ctx, void* device_buf, uint64_t bytes) {
+    if (!ctx || ((uintptr_t)device_buf & 15)) return CC_ERR_INVALID;
+    if (ctx->worker_running) return CC_ERR_WORKER;
+    ctx->stage = bytes ? device_buf : nullptr;
+    ctx->stage_bytes = device_buf ? bytes : 0;
+    return CC_OK;
+}
+
+// A host-resident log is read twice by the kernels (validate, then scatter / copy): with a staging buffer
+// attached it crosses the host link once, by the copy engine, and the kernels read the device copy.
+static const u8* stage_log(cc_ctx* ctx, const void* log, uint64_t nbytes, cudaStream_t st) {
+    if (!ctx->stage || nbytes == 0 || nbytes > ctx->stage_bytes) return (const u8*)log;
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, log) != cudaSuccess) { cudaGetLastError(); return (const u8*)log; }
+    if (at.type != cudaMemoryTypeHost) return (const u8*)log;
+    if (cudaMemcpyAsync(ctx->stage, log, nbytes, cudaMemcpyHostToDevice, st) != cudaSuccess) { cudaGetLastError(); return (const u8*)log; }
+    return (const u8*)ctx->stage;
+}
+
 extern "C" int32_t cc_apply_log(cc_ctx* ctx, const void* log, uint64_t nbytes, void* stream, cc_result* out) {
     if (!ctx || !log || ((uintptr_t)log & 15)) return CC_ERR_INVALID;
     if (!ctx->apply_attached) return CC_ERR_INVALID;
     CC_CUDA(ctx, cudaSetDevice(ctx->device));
     cudaStream_t st = (cudaStream_t)stream;
-    const u8* lg = (const u8*)log;
+    const u8* lg = stage_log(ctx, log, nbytes, st);
     const unsigned gv = (unsigned)(ctx->sm_count * ctx->validate_bps);
     const unsigned gs = (unsigned)(ctx->sm_count * 8);
     cc_apply_parse_kernel<<<1, CC_PARSE_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, lg, nbytes);

@@ -104,12 +104,15 @@ def main():
     def scramble():
         for rid, (v, P, n_pages) in views.items():
             v.view(-1, P)[:, :64] = 0                     # every page differs from the logged bytes again
-    for name, lg in (("apply_from_pinned_host_log", log_pin), ("apply_from_device_log", log_dev)):
+    for name, lg in (("apply_from_pinned_host_log", log_pin), ("apply_from_pinned_host_log_staged", log_pin),
+                     ("apply_from_device_log", log_dev)):
+        ctx.apply_stage_attach(W if name.endswith("staged") else 0)      # staged: one DMA pass over the host link
         med, best = timed(lambda: ctx.apply_log(lg, W, res), a.reps, scramble)
         rr = res.read()
         assert rr.status == 0 and rr.bytes == W, rr.as_dict()
         out[name] = {"ms": round(med, 4), "best_ms": round(best, 4), "records": int(rr.n_dirty),
                      "records_per_s": round(rr.n_dirty / (med * 1e-3)), "log_GBps": round(W / (med * 1e-3) / 1e9, 2)}
+    ctx.apply_stage_attach(0)
     out["config"]["page_records"] = int(rr.n_dirty)
     # ---- compact ----
     out_log = torch.zeros(W, dtype=torch.uint8, device=dev)

@@ -136,13 +136,15 @@ def test_config5a_scaled_mixed_pages_duplicates(pinned=False):
     exp = oracle.apply_log(olog, W, regs_o)
     assert exp[0] == 0 and exp[1] == sum(e.pages.numel() for e in eps)
 
-    for pinned in (False, True):
+    for pinned, staged in ((False, False), (True, False), (True, True), (False, True)):
         work = arena.clone()
         ctx = cc.Context()
         shadows = {}
         for rid, (o, sz, P) in views.items():
             shadows[rid] = ctx.register_region(rid, work[o:o + sz], P)
         ctx.apply_attach(exp[1] + 64)
+        if staged:
+            ctx.apply_stage_attach(W)          # host logs cross the link once (copy engine); device logs are unaffected
         lt = torch.from_numpy(olog)
         lt = lt.pin_memory() if pinned else lt.cuda()
         r = _gpu_apply(ctx, lt, W)
