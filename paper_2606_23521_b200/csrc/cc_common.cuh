@@ -181,6 +181,16 @@ __device__ __forceinline__ u64 ld_acquire_gpu_u64(const u64* p) {
 __device__ __forceinline__ void st_release_gpu_u64(u64* p, u64 v) {
     asm volatile("st.release.gpu.global.u64 [%0], %1;" :: "l"(p), "l"(v) : "memory");
 }
+// Relaxed gpu-scope accesses: for words whose VALUE is the whole message (look-back status words), so that
+// publishing them does not have to wait for the thread's earlier (possibly host-link) stores.
+__device__ __forceinline__ u64 ld_relaxed_gpu_u64(const u64* p) {
+    u64 v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_relaxed_gpu_u64(u64* p, u64 v) {
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" :: "l"(p), "l"(v) : "memory");
+}
 __device__ __forceinline__ u32 ld_acquire_gpu_u32(const u32* p) {
     u32 v;
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");

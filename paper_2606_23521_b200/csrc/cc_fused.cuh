@@ -22,7 +22,10 @@
 #include "cc_crc.cuh"
 #include "cc_ckpt.cuh"
 
-// Warp-wide decoupled look-back: sum of the dirty counts of tiles [0, t).  blocking = false gives up
+// Warp-wide decoupled look-back: sum of the dirty counts of tiles [0, t).  The status words are read and
+// written with RELAXED gpu-scope accesses: the count a word carries is the whole message (nothing else a tile
+// wrote is read by another tile inside this kernel), and a release here would make the publishing warp wait
+// for its earlier record stores -- over the host link with a pinned log -- and stall every tile behind it.  blocking = false gives up
 // (returns false) as soon as a predecessor that has not published yet is met before an inclusive one.
 __device__ __forceinline__ bool cc_fused_lookback(const u64* status, u32 run, u32 t, u32 lane, bool blocking, u32* excl_out) {
     u32 excl = 0;
@@ -30,7 +33,7 @@ __device__ __forceinline__ bool cc_fused_lookback(const u64* status, u32 run, u3
     for (;;) {
         const int j = base - (int)lane;
         u64 s = lb_pack(run, CC_LB_INC, 0);                 // virtual tile -1: inclusive sum 0
-        if (j >= 0) s = ld_acquire_gpu_u64(&status[j]);
+        if (j >= 0) s = ld_relaxed_gpu_u64(&status[j]);
         const u32 flag = (u32)(s >> 32) & 3u;
         const bool valid = ((u32)(s >> 34) == run) && flag != 0;
         const u32 inv = __ballot_sync(0xFFFFFFFFu, !valid);
@@ -126,12 +129,12 @@ __device__ __forceinline__ void cc_fused_phase(const cc_region_dev& r, cc_dev* d
         if (cnt == 0 && !last) {
             // nothing to place: publish, upgrading to an inclusive sum only if that costs no waiting
             const bool got = cc_fused_lookback(r.flb_status, run, t, lane, false, &excl);
-            if (lane == 0) st_release_gpu_u64(&r.flb_status[t], got ? lb_pack(run, CC_LB_INC, excl) : lb_pack(run, CC_LB_AGG, 0));
+            if (lane == 0) st_relaxed_gpu_u64(&r.flb_status[t], got ? lb_pack(run, CC_LB_INC, excl) : lb_pack(run, CC_LB_AGG, 0));
             continue;
         }
-        if (t != 0 && lane == 0) st_release_gpu_u64(&r.flb_status[t], lb_pack(run, CC_LB_AGG, cnt));
+        if (t != 0 && lane == 0) st_relaxed_gpu_u64(&r.flb_status[t], lb_pack(run, CC_LB_AGG, cnt));
         cc_fused_lookback(r.flb_status, run, t, lane, true, &excl);
-        if (lane == 0) st_release_gpu_u64(&r.flb_status[t], lb_pack(run, CC_LB_INC, excl + cnt));
+        if (lane == 0) st_relaxed_gpu_u64(&r.flb_status[t], lb_pack(run, CC_LB_INC, excl + cnt));
         if ((mask >> lane) & 1u) r.D[excl + __popc(mask & ((1u << lane) - 1u))] = (u32)(p0 + lane);
         if (last && lane == 0)              // every earlier tile has published its count: k is final
             cc_plan_checkpoint(r, log, mode, epoch, excl + cnt, ((mask >> (np - 1)) & 1u) != 0, inline_ok);
