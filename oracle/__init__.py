@@ -6,5 +6,5 @@ See oracle/concordia_oracle.c for what it follows in the paper and how it is pin
 """
 from .oracle import (  # noqa: F401
     ORC_OK, ORC_ERR_INVALID, ORC_ERR_LOG_FULL, ORC_ERR_CORRUPT,
-    Region, crc32c, crc32c_bitwise, scan, scan_mt, checkpoint, checkpoint_marked, checkpoint_versions, apply_log, write_epoch, snapshot, compact_log, checkpoint_all, build,
+    Region, crc32c, crc32c_bitwise, scan, scan_mt, checkpoint, checkpoint_rle, checkpoint_marked, checkpoint_versions, apply_log, write_epoch, snapshot, compact_log, checkpoint_all, build,
 )

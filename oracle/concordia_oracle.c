@@ -200,6 +200,20 @@ int32_t orc_checkpoint(const uint8_t *cur, uint8_t *shadow, uint64_t N, uint64_t
 
 /* ----------------------------------------------------------------- apply --- */
 
+/* A page record may carry a RUN of consecutive pages ("contiguous dirty ranges use
+ * run-length encoding"; reading #38): {region_id, first page, len, crc32c} + len payload
+ * bytes, where the payload is the pages first, first+1, ... back to back.  (page_idx, len) is
+ * well-formed iff it denotes a whole number (>= 1) of pages inside the region: len > 0, the range
+ * [page_idx*P, page_idx*P + len) lies in the region and ends on a page boundary or at the region's
+ * end.  A single-page record is the run of length one, so every log of the first format is valid. */
+static int rec_len_ok(uint64_t N, uint64_t P, uint64_t pidx, uint64_t len) {
+    uint64_t n_pages = (N + P - 1) / P;
+    if (pidx >= n_pages || len == 0) return 0;
+    uint64_t start = pidx * P;
+    if (len > N - start) return 0;
+    return (len % P == 0) || (start + len == N);
+}
+
 typedef struct {
     uint32_t region_id;
     uint32_t page_bytes;
@@ -265,9 +279,8 @@ int32_t orc_apply(const uint8_t *log, uint64_t n, const orc_region *regions, uin
             int ok = (r != NULL);
             if (ok) {
                 uint64_t n_pages = (r->bytes + r->page_bytes - 1) / r->page_bytes;
-                ok = ((uint64_t)pidx < n_pages) &&
-                     ((uint64_t)len == page_len(r->bytes, r->page_bytes, pidx)) &&
-                     (orc_crc32c(payload, len) == crc);
+                (void)n_pages;
+                ok = rec_len_ok(r->bytes, r->page_bytes, pidx, len) && (orc_crc32c(payload, len) == crc);
             }
             if (!ok) { status = ORC_ERR_CORRUPT; break; }
             if (pend_n == pend_cap) {
@@ -513,8 +526,10 @@ int32_t orc_snapshot(const uint8_t *cur, uint8_t *shadow, uint64_t N, uint64_t P
  * #33-#36): the input is walked and validated exactly as orc_apply walks it (same torn / corrupt
  * rules); within its committed prefix the LAST record of every page survives (what a replay would
  * leave in that page); the output holds, for every region that has a surviving record, in ascending
- * region_id order, ONE committed epoch: the surviving page records in ascending page order (header
- * copied: region_id, page_idx, len, crc32c; payload copied) and a commit record carrying the epoch
+ * region_id order, ONE committed epoch: one single-page record per surviving page in ascending page
+ * order (region_id, page_idx, len, crc32c of the page's bytes; for a page that came from a
+ * single-page record this is that record byte for byte, for a page out of a run record it is cut
+ * out of the run) and a commit record carrying the epoch
  * number of the last input epoch that touched the region and k = number of surviving pages.
  * A failed check makes the call ORC_ERR_CORRUPT and writes nothing (compaction must not launder a
  * damaged log); a torn tail is dropped (it holds no committed data); ORC_ERR_LOG_FULL writes nothing.
@@ -553,7 +568,9 @@ int32_t orc_compact_log(const uint8_t *log, uint64_t n, const orc_region *region
             for (uint64_t i = 0; i < pend_n; i++) {
                 const uint8_t *ph = log + pend[i];
                 uint32_t ri = (uint32_t)(find_region(regions, n_regions, get_u32(ph + 0)) - regions);
-                last[ri][get_u32(ph + 4)] = pend[i] + 1;                /* later records overwrite earlier ones */
+                uint64_t P = regions[ri].page_bytes, first = get_u32(ph + 4), rlen = get_u32(ph + 8);
+                for (uint64_t q = 0; q * P < rlen; q++)                 /* every page of the run; later records overwrite */
+                    last[ri][first + q] = (pend[i] + ORC_HDR + q * P) + 1;     /* offset of the page's payload, + 1 */
                 last_epoch[ri] = (uint64_t)get_u32(payload + 0) | ((uint64_t)get_u32(payload + 4) << 32);
             }
             off += ORC_COMMIT_BYTES;
@@ -564,8 +581,8 @@ int32_t orc_compact_log(const uint8_t *log, uint64_t n, const orc_region *region
             int ok = (r != NULL);
             if (ok) {
                 uint64_t n_pages = (r->bytes + r->page_bytes - 1) / r->page_bytes;
-                ok = ((uint64_t)pidx < n_pages) && ((uint64_t)len == page_len(r->bytes, r->page_bytes, pidx)) &&
-                     (orc_crc32c(payload, len) == crc);
+                (void)n_pages;
+                ok = rec_len_ok(r->bytes, r->page_bytes, pidx, len) && (orc_crc32c(payload, len) == crc);
             }
             if (!ok) { status = ORC_ERR_CORRUPT; break; }
             if (pend_n == pend_cap) {
@@ -599,9 +616,13 @@ int32_t orc_compact_log(const uint8_t *log, uint64_t n, const orc_region *region
                 uint64_t np = (regions[best].bytes + regions[best].page_bytes - 1) / regions[best].page_bytes, k = 0;
                 for (uint64_t p = 0; p < np; p++) {
                     if (!last[best][p]) continue;
-                    const uint8_t *ph = log + (last[best][p] - 1);
-                    uint32_t plen = get_u32(ph + 8);
-                    memcpy(out + o, ph, ORC_HDR + plen);
+                    const uint8_t *pp = log + (last[best][p] - 1);      /* the page's payload inside its record */
+                    uint64_t plen = page_len(regions[best].bytes, regions[best].page_bytes, p);
+                    put_u32(out + o + 0, regions[best].region_id);
+                    put_u32(out + o + 4, (uint32_t)p);
+                    put_u32(out + o + 8, (uint32_t)plen);
+                    put_u32(out + o + 12, orc_crc32c(pp, plen));
+                    memcpy(out + o + ORC_HDR, pp, plen);
                     o += ORC_HDR + plen;
                     k++;
                 }
@@ -665,4 +686,71 @@ int32_t orc_checkpoint_all(const orc_region *regions, uint32_t n_regions, uint64
         if (st != ORC_OK && first_bad == ORC_OK) first_bad = st;
     }
     return first_bad;
+}
+
+/* --------------------------- run-length records --- */
+
+/* Delta checkpoint with run records ("contiguous dirty ranges use run-length encoding", L221).
+ * Same steps as orc_checkpoint except step 6: the ascending dirty pages are grouped into RUNS of
+ * consecutive pages; a run never crosses a page index that is a multiple of run_pages (so a run has at
+ * most run_pages pages and its byte length fits the u32 len field; run_pages >= 1, run_pages * P <
+ * 2^32).  Each run is ONE record {region_id, first page, len = bytes of the whole run,
+ * crc32c(all payload bytes of the run)} + the run's pages back to back.  The commit record's count
+ * is the number of RECORDS (runs).  run_pages = 1 gives exactly orc_checkpoint's bytes.
+ *   *k_out = dirty pages, *runs_out = records written (also on LOG_FULL: what would be written). */
+int32_t orc_checkpoint_rle(const uint8_t *cur, uint8_t *shadow, uint64_t N, uint64_t P,
+                           uint32_t region_id, uint64_t epoch, uint64_t run_pages,
+                           uint8_t *log, uint64_t C, uint64_t *W,
+                           uint32_t *D_out, uint64_t *k_out, uint64_t *runs_out, uint64_t *bytes_out) {
+    if (P == 0 || N == 0 || region_id == 0 || region_id == ORC_COMMIT_ID) return ORC_ERR_INVALID;
+    if (run_pages == 0 || run_pages * P > 0xFFFFFFFFull) return ORC_ERR_INVALID;
+    uint64_t n_pages = (N + P - 1) / P;
+    if (n_pages > 0xFFFFFFFEull) return ORC_ERR_INVALID;
+    uint8_t *dirty = (uint8_t *)malloc(n_pages);
+    if (!dirty) return ORC_ERR_INVALID;
+    uint64_t k = orc_scan(cur, shadow, N, P, dirty);
+    *k_out = k;
+    *bytes_out = 0;
+    /* a page starts a run iff it is dirty and (it is page 0, or the page before it is clean, or its
+     * index is a multiple of run_pages) */
+    uint64_t runs = 0, need = ORC_COMMIT_BYTES, j = 0;
+    for (uint64_t p = 0; p < n_pages; p++) {
+        if (!dirty[p]) continue;
+        if (D_out) D_out[j++] = (uint32_t)p;
+        if (p == 0 || !dirty[p - 1] || p % run_pages == 0) { runs++; need += ORC_HDR; }
+        need += page_len(N, P, p);
+    }
+    *runs_out = runs;
+    if (k == 0) { free(dirty); return ORC_OK; }
+    if (*W + need > C) { free(dirty); return ORC_ERR_LOG_FULL; }
+    uint64_t off = *W;
+    for (uint64_t p = 0; p < n_pages; ) {
+        if (!dirty[p]) { p++; continue; }
+        uint64_t q = p + 1;                                  /* the run is [p, q) */
+        while (q < n_pages && dirty[q] && q % run_pages != 0) q++;
+        uint64_t len = (q == n_pages ? N : q * P) - p * P;
+        put_u32(log + off + 0, region_id);
+        put_u32(log + off + 4, (uint32_t)p);
+        put_u32(log + off + 8, (uint32_t)len);
+        put_u32(log + off + 12, orc_crc32c(cur + p * P, len));
+        memcpy(log + off + ORC_HDR, cur + p * P, len);
+        off += ORC_HDR + len;
+        p = q;
+    }
+    uint8_t cp[16];
+    put_u64(cp + 0, epoch);
+    put_u32(cp + 8, region_id);
+    put_u32(cp + 12, (uint32_t)runs);
+    put_u32(log + off + 0, ORC_COMMIT_ID);
+    put_u32(log + off + 4, ORC_COMMIT_ID);
+    put_u32(log + off + 8, 16u);
+    put_u32(log + off + 12, orc_crc32c(cp, 16));
+    memcpy(log + off + ORC_HDR, cp, 16);
+    off += ORC_COMMIT_BYTES;
+    for (uint64_t p = 0; p < n_pages; p++)
+        if (dirty[p]) memcpy(shadow + p * P, cur + p * P, page_len(N, P, p));
+    *bytes_out = off - *W;
+    *W = off;
+    free(dirty);
+    return ORC_OK;
 }

@@ -68,6 +68,9 @@ def _load():
         lib.orc_checkpoint_all.restype = ctypes.c_int32
         lib.orc_checkpoint_all.argtypes = [ctypes.POINTER(_CRegion), ctypes.c_uint32, ctypes.c_uint64, u8p, ctypes.c_uint64,
                                            u64p, u8p, u8p, u64p, u64p]
+        lib.orc_checkpoint_rle.restype = ctypes.c_int32
+        lib.orc_checkpoint_rle.argtypes = [u8p, u8p, ctypes.c_uint64, ctypes.c_uint64, ctypes.c_uint32, ctypes.c_uint64,
+                                           ctypes.c_uint64, u8p, ctypes.c_uint64, u64p, u32p, u64p, u64p, u64p]
         lib.orc_apply.restype = ctypes.c_int32
         lib.orc_apply.argtypes = [u8p, ctypes.c_uint64, ctypes.POINTER(_CRegion), ctypes.c_uint32, u64p, u64p]
         lib.orc_write_epoch.restype = ctypes.c_int32
@@ -137,6 +140,19 @@ def checkpoint(cur, shadow, page_bytes: int, region_id: int, epoch: int, log, W:
     st = _load().orc_checkpoint(_ptr(c), _ptr(s), c.size, page_bytes, region_id, epoch,
                                 _ptr(lg), lg.size, ctypes.byref(w), _ptr(D), ctypes.byref(k), ctypes.byref(nb))
     return int(st), D[: k.value].copy(), int(nb.value), int(w.value)
+
+
+def checkpoint_rle(cur, shadow, page_bytes: int, region_id: int, epoch: int, run_pages: int, log, W: int):
+    """Delta checkpoint with run records (one record per run of consecutive dirty pages; runs never cross a
+    multiple of run_pages).  Returns (status, D, n_runs, bytes_appended, W_after)."""
+    c, s, lg = _u8(cur), _u8(shadow), _u8(log)
+    assert c.size == s.size
+    n_pages = (c.size + page_bytes - 1) // page_bytes
+    D = np.zeros(max(n_pages, 1), dtype=np.uint32)
+    w, k, runs, nb = ctypes.c_uint64(W), ctypes.c_uint64(0), ctypes.c_uint64(0), ctypes.c_uint64(0)
+    st = _load().orc_checkpoint_rle(_ptr(c), _ptr(s), c.size, page_bytes, region_id, epoch, run_pages, _ptr(lg), lg.size,
+                                    ctypes.byref(w), _ptr(D), ctypes.byref(k), ctypes.byref(runs), ctypes.byref(nb))
+    return int(st), D[: k.value].copy(), int(runs.value), int(nb.value), int(w.value)
 
 
 def checkpoint_marked(cur, shadow, page_bytes: int, region_id: int, epoch: int, marked, log, W: int,
