@@ -33,6 +33,24 @@ __device__ __forceinline__ int cc_find_slot(const cc_dev* dev, u32 rid) {
     return -1;
 }
 
+// A page record may carry a run of consecutive pages (PAPER.md:L221 run-length encoding; reading #38):
+// (page_idx, len) is well-formed iff it denotes a whole number (>= 1) of pages inside the region.
+__device__ __forceinline__ bool cc_rec_len_ok(const cc_region_dev& r, u64 page_idx, u64 len) {
+    if (page_idx >= r.n_pages || len == 0) return false;
+    const u64 start = page_idx * (u64)r.page_bytes;
+    if (len > r.bytes - start) return false;
+    return (len % r.page_bytes == 0) || (start + len == r.bytes);
+}
+__device__ __forceinline__ u32 cc_rec_pages(const cc_region_dev& r, u32 len) {
+    return (u32)(((u64)len + r.page_bytes - 1) / r.page_bytes);
+}
+// 0xFFFFFFFF * x^(8*len): the CRC init term of a record of len bytes
+__device__ __forceinline__ u32 cc_crc_init_term(const cc_dev* dev, const cc_region_dev& r, u32 len) {
+    if (len == r.page_bytes) return r.crc_init_full;
+    if ((u64)len == page_len_dev(r, r.n_pages - 1)) return r.crc_init_tail;
+    return gf_mul(0xFFFFFFFFu, gf_xpow_bytes(dev->crc.xp, len));
+}
+
 #define CC_PA_STOP 0u
 #define CC_PA_NEXT 1u
 #define CC_PA_RUN 2u
@@ -83,7 +101,7 @@ __device__ __forceinline__ void cc_apply_parse_phase(cc_dev* dev, const cc_apply
                 const int slot = cc_find_slot(dev, h.x);
                 if (slot < 0) { A->struct_fail = 1; break; }
                 const cc_region_dev& r = dev->regions[slot];
-                if ((u64)h.y >= r.n_pages || (u64)h.z != page_len_dev(r, h.y)) { A->struct_fail = 1; break; }
+                if (!cc_rec_len_ok(r, h.y, h.z)) { A->struct_fail = 1; break; }
                 if (s_pending != 0 && s_pend_rid != h.x) s_mixed = 1;
                 s_pend_rid = h.x;
                 s_slot = (u32)slot;
@@ -104,10 +122,9 @@ __device__ __forceinline__ void cc_apply_parse_phase(cc_dev* dev, const cc_apply
             bool ok = (off_t + CC_RECORD_HEADER_BYTES <= n);
             if (ok) {
                 h = ld_v4(reinterpret_cast<const uint4*>(log + off_t));
-                ok = ((u64)h.z <= n - off_t - CC_RECORD_HEADER_BYTES) && (h.x == r.region_id) &&
-                     ((u64)h.y < r.n_pages) && ((u64)h.z == page_len_dev(r, h.y));
+                ok = ((u64)h.z <= n - off_t - CC_RECORD_HEADER_BYTES) && (h.x == r.region_id) && cc_rec_len_ok(r, h.y, h.z);
             }
-            // a short (tail) page is valid but breaks the stride: it may only END a run
+            // a short (tail) page or a multi-page run record is valid but breaks the stride: it may only END a run
             const bool full = ok && ((u64)h.z == P);
             if (!ok) atomicMin(&s_first_fail, tid);
             else if (!full) atomicMin(&s_first_fail, tid + 1);
@@ -190,8 +207,7 @@ __device__ __forceinline__ void cc_apply_validate_phase(cc_dev* dev, const cc_ap
                 u32 acc = 0;
                 const bool finish = crc_record_combine(&T.rec_state[ri], nseg, c, contrib, &acc);
                 if (finish) {
-                    const cc_region_dev& rg = dev->regions[rec.slot];
-                    const u32 it = rec.len == rg.page_bytes ? rg.crc_init_full : rg.crc_init_tail;
+                    const u32 it = cc_crc_init_term(dev, dev->regions[rec.slot], rec.len);
                     if (crc_finalize(acc, it) != rec.crc) atomicMin(&A->first_bad_rec, ri);
                 }
             }
@@ -229,7 +245,9 @@ __device__ __forceinline__ void cc_apply_latest_phase(cc_dev* dev, const cc_appl
     const u32 n = dev->apply.n_commit_recs;
     for (u32 i = g.block * blockDim.x + threadIdx.x; i < n; i += g.nblocks * blockDim.x) {
         const cc_rec rec = T.recs[i];
-        atomicMax(&dev->regions[rec.slot].latest[rec.page_idx], i + 1);
+        const cc_region_dev& r = dev->regions[rec.slot];
+        const u32 m = cc_rec_pages(r, rec.len);
+        for (u32 q = 0; q < m; q++) atomicMax(&r.latest[rec.page_idx + q], i + 1);
     }
 }
 
@@ -243,25 +261,31 @@ __device__ __forceinline__ void cc_apply_scatter_phase(cc_dev* dev, const cc_app
         const u32 ri = cc_find_rec(T.seg_begin, n, item, lane);
         const cc_rec rec = T.recs[ri];
         const cc_region_dev& r = dev->regions[rec.slot];
-        if (r.latest[rec.page_idx] != ri + 1) continue;              // an earlier duplicate: a later record wins
         const u32 c = item - T.seg_begin[ri];
         const u64 so = (u64)c * CC_SEG_BYTES;
         const u64 rem = rec.len - so;
         const u32 nv = (u32)(rem < CC_SEG_BYTES ? rem : CC_SEG_BYTES) >> 4;
+        // a page takes its bytes from its LATEST record only.  A segment lies inside one page when pages are
+        // whole multiples of 4 KiB (or the record is a single page); otherwise the check is per 16-byte vector.
+        const bool one_page = (r.page_bytes % CC_SEG_BYTES == 0) || rec.len <= r.page_bytes;
+        if (one_page && r.latest[rec.page_idx + (u32)(so / r.page_bytes)] != ri + 1) continue;
         const uint4* src = reinterpret_cast<const uint4*>(log + rec.off + CC_RECORD_HEADER_BYTES + so);
         const u64 dst_off = (u64)rec.page_idx * r.page_bytes + so;
         uint4* d0 = reinterpret_cast<uint4*>(r.base + dst_off);
         uint4* d1 = reinterpret_cast<uint4*>(r.shadow + dst_off);
         uint4 v[U];
+        bool take[U];
 #pragma unroll
         for (int u = 0; u < U; u++) {
             const u32 j = lane + 32 * u;
-            if (j < nv) v[u] = ld_v4(src + j);
+            take[u] = j < nv;
+            if (take[u] && !one_page) take[u] = r.latest[rec.page_idx + (u32)((so + 16ull * j) / r.page_bytes)] == ri + 1;
+            if (take[u]) v[u] = ld_v4(src + j);
         }
 #pragma unroll
         for (int u = 0; u < U; u++) {
             const u32 j = lane + 32 * u;
-            if (j < nv) { st_stream(d0 + j, v[u]); if (r.shadow) st_stream(d1 + j, v[u]); }
+            if (take[u]) { st_stream(d0 + j, v[u]); if (r.shadow) st_stream(d1 + j, v[u]); }
         }
     }
 }
@@ -272,7 +296,9 @@ __device__ __forceinline__ void cc_apply_cleanup_phase(cc_dev* dev, const cc_app
     const u32 n = A->n_commit_recs;
     for (u32 i = g.block * blockDim.x + threadIdx.x; i < n; i += g.nblocks * blockDim.x) {
         const cc_rec rec = T.recs[i];
-        dev->regions[rec.slot].latest[rec.page_idx] = 0;
+        const cc_region_dev& r = dev->regions[rec.slot];
+        const u32 m = cc_rec_pages(r, rec.len);
+        for (u32 q = 0; q < m; q++) r.latest[rec.page_idx + q] = 0;
     }
     if (g.block == 0 && threadIdx.x == 0 && out) {
         out->n_dirty = n;

@@ -8,8 +8,9 @@
 //   rank     the ordered compaction of cc_ckpt.cuh over every region's bitmap -> ascending page list
 //   plan     one thread: regions in ascending region_id order get their output offsets; all-or-nothing
 //            capacity check
-//   copy     warp per 4 KiB segment: surviving record -> output log at its final place; the header
-//            (region, page, len, crc) is copied from the validated input record, no CRC is recomputed;
+//   copy     warp per 4 KiB segment: surviving page -> single-page record at its final place in the output; the
+//            header of a page that came from a single-page record is that validated record's, a page cut out of
+//            a run record gets its own CRC32C;
 //            one commit record per region with the epoch number of the last input epoch that touched it
 //   cleanup  latest[] back to zero; result
 // A failed check (CC_ERR_CORRUPT) or a too small scratch writes nothing: compaction must not launder a
@@ -32,8 +33,12 @@ __device__ __forceinline__ void cc_compactor_mark_phase(cc_dev* dev, const cc_ap
     for (u32 i = g.block * blockDim.x + threadIdx.x; i < n; i += g.nblocks * blockDim.x) {
         const cc_rec rec = T.recs[i];
         const cc_region_dev& r = dev->regions[rec.slot];
-        atomicMax(&r.latest[rec.page_idx], i + 1);
-        atomicOr(&r.bitmap[rec.page_idx >> 5], 1u << (rec.page_idx & 31));
+        const u32 m = cc_rec_pages(r, rec.len);              // a run record covers m consecutive pages
+        for (u32 q = 0; q < m; q++) {
+            const u32 p = rec.page_idx + q;
+            atomicMax(&r.latest[p], i + 1);
+            atomicOr(&r.bitmap[p >> 5], 1u << (p & 31));
+        }
     }
 }
 
@@ -96,7 +101,9 @@ __device__ __forceinline__ void cc_compactor_plan_phase(cc_dev* dev, u64 out_cap
     __threadfence();
 }
 
-__device__ __forceinline__ void cc_compactor_copy_phase(cc_dev* dev, const cc_apply_tabs& T, const u8* in, u8* out, cc_grid g) {
+// cs must hold the CRC tables (a page cut out of a run record needs its own CRC).
+__device__ __forceinline__ void cc_compactor_copy_phase(cc_dev* dev, const cc_apply_tabs& T, cc_crc_smem* cs, const u8* in, u8* out,
+                                                        cc_grid g) {
     constexpr int U = 8;
     if (dev->compactor.status != CC_OK) return;
     const u32 lane = threadIdx.x & 31u;
@@ -115,25 +122,40 @@ __device__ __forceinline__ void cc_compactor_copy_phase(cc_dev* dev, const cc_ap
             else { i = (u32)(item / spp); c = (u32)(item - (u64)i * spp); }
             const u32 p = r.D[i];
             const cc_rec rec = T.recs[r.latest[p] - 1];
+            const u64 plen = page_len_dev(r, p);
             const u64 so = (u64)c * CC_SEG_BYTES;
-            if (so >= rec.len) continue;
-            const u64 rem = rec.len - so;
-            const u32 nv = (u32)(rem < CC_SEG_BYTES ? rem : CC_SEG_BYTES) >> 4;
-            const uint4* src = reinterpret_cast<const uint4*>(in + rec.off + CC_RECORD_HEADER_BYTES + so);
+            if (so >= plen) continue;
+            const u64 rem = plen - so;
+            const u32 seg_len = (u32)(rem < CC_SEG_BYTES ? rem : CC_SEG_BYTES);
+            const u32 nv = seg_len >> 4;
+            // the page's bytes inside its (possibly multi-page) record
+            const uint4* src = reinterpret_cast<const uint4*>(in + rec.off + CC_RECORD_HEADER_BYTES +
+                                                              (u64)(p - rec.page_idx) * r.page_bytes + so);
             u8* orec = base + (u64)i * rec_stride;
             uint4* dst = reinterpret_cast<uint4*>(orec + CC_RECORD_HEADER_BYTES + so);
             uint4 v[U];
 #pragma unroll
             for (int u = 0; u < U; u++) {
                 const u32 j = lane + 32 * u;
-                if (j < nv) v[u] = ld_v4(src + j);
+                v[u] = (j < nv) ? ld_v4(src + j) : make_uint4(0, 0, 0, 0);
             }
 #pragma unroll
             for (int u = 0; u < U; u++) {
                 const u32 j = lane + 32 * u;
                 if (j < nv) st_stream(dst + j, v[u]);
             }
-            if (c == 0 && lane == 0) st_u32x4(orec, r.region_id, p, rec.len, rec.crc);
+            if ((u64)rec.len == plen) {                     // single-page record: its validated header is the page's
+                if (c == 0 && lane == 0) st_u32x4(orec, r.region_id, p, rec.len, rec.crc);
+            } else {                                        // cut out of a run: the page gets its own CRC
+                const u32 nseg = (u32)((plen + CC_SEG_BYTES - 1) / CC_SEG_BYTES);
+                const u32 contrib = crc_segment_warp<U>(cs, &dev->crc, v, nv, rem - seg_len, lane);
+                if (lane == 0) {
+                    u32 acc = 0;
+                    if (crc_record_combine(&r.rec_state[i], nseg, c, contrib, &acc))
+                        st_u32x4(orec, r.region_id, p, (u32)plen,
+                                 crc_finalize(acc, plen == r.page_bytes ? r.crc_init_full : r.crc_init_tail));
+                }
+            }
         }
         if (g.block == 0 && threadIdx.x == 0) {             // the region's commit record
             u8* cm = base + r.hdr->need - CC_COMMIT_RECORD_BYTES;
@@ -154,7 +176,9 @@ __device__ __forceinline__ void cc_compactor_cleanup_phase(cc_dev* dev, const cc
         const u32 n = A->n_commit_recs;
         for (u32 i = g.block * blockDim.x + threadIdx.x; i < n; i += g.nblocks * blockDim.x) {
             const cc_rec rec = T.recs[i];
-            dev->regions[rec.slot].latest[rec.page_idx] = 0;
+            const cc_region_dev& r = dev->regions[rec.slot];
+            const u32 m = cc_rec_pages(r, rec.len);
+            for (u32 q = 0; q < m; q++) r.latest[rec.page_idx + q] = 0;
         }
     }
     if (g.block == 0 && threadIdx.x == 0 && out) {

@@ -87,7 +87,7 @@ __device__ __noinline__ void cc_worker_compact_task(cc_dev* dev, const cc_apply_
     cc_grid_barrier(dev, g.nblocks, gen);
     if (g.block == 0) cc_compactor_plan_phase(dev, task.arg3);
     cc_grid_barrier(dev, g.nblocks, gen);
-    cc_compactor_copy_phase(dev, tabs, in, outl, g);
+    cc_compactor_copy_phase(dev, tabs, cs, in, outl, g);
     cc_grid_barrier(dev, g.nblocks, gen);
     cc_compactor_cleanup_phase(dev, tabs, g, nullptr, task.kind);
 }

@@ -61,7 +61,10 @@ __global__ void __launch_bounds__(CC_APPLY_THREADS) cc_compactor_mark_kernel(cc_
 __global__ void __launch_bounds__(CC_COMPACT_THREADS) cc_compactor_rank_kernel(cc_dev* dev) { cc_compactor_rank_phase(dev); }
 __global__ void __launch_bounds__(CC_MAX_REGIONS) cc_compactor_plan_kernel(cc_dev* dev, u64 out_capacity) { cc_compactor_plan_phase(dev, out_capacity); }
 __global__ void __launch_bounds__(CC_APPLY_THREADS) cc_compactor_copy_kernel(cc_dev* dev, cc_apply_tabs tabs, const u8* in, u8* out) {
-    cc_compactor_copy_phase(dev, tabs, in, out, cc_hw_grid());
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cc_crc_smem* cs = reinterpret_cast<cc_crc_smem*>(smem_raw);
+    cc_crc_smem_init(cs, &dev->crc);
+    cc_compactor_copy_phase(dev, tabs, cs, in, out, cc_hw_grid());
 }
 __global__ void __launch_bounds__(CC_APPLY_THREADS) cc_compactor_cleanup_kernel(cc_dev* dev, cc_apply_tabs tabs, cc_result* out) {
     cc_compactor_cleanup_phase(dev, tabs, cc_hw_grid(), out, CC_TASK_COMPACT_LOG);
@@ -243,6 +246,7 @@ extern "C" int32_t cc_init(cc_ctx** out, int32_t device, const cc_config* cfg) {
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->worker_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->worker_done, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_compactor_copy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_batch_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->fused_bps, cc_fused_kernel, CC_GATHER_THREADS, sizeof(cc_crc_smem));
@@ -574,13 +578,12 @@ extern "C" int32_t cc_compact_log(cc_ctx* ctx, const void* in_log, uint64_t in_b
     cudaStream_t st = (cudaStream_t)stream;
     const u8* lg = stage_log(ctx, in_log, in_bytes, st);
     const unsigned gv = (unsigned)(ctx->sm_count * ctx->validate_bps);
-    const unsigned gs = (unsigned)(ctx->sm_count * 8);
     cc_apply_parse_kernel<<<1, CC_PARSE_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, lg, in_bytes);
     cc_apply_validate_kernel<<<gv, CC_APPLY_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, ctx->tabs, lg);
     cc_compactor_mark_kernel<<<(unsigned)ctx->sm_count, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs);
     cc_compactor_rank_kernel<<<(unsigned)ctx->sm_count, CC_COMPACT_THREADS, 0, st>>>(ctx->d_dev);
     cc_compactor_plan_kernel<<<1, CC_MAX_REGIONS, 0, st>>>(ctx->d_dev, out_capacity);
-    cc_compactor_copy_kernel<<<gs, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, lg, (u8*)out_log);
+    cc_compactor_copy_kernel<<<gv, CC_APPLY_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, ctx->tabs, lg, (u8*)out_log);
     cc_compactor_cleanup_kernel<<<(unsigned)ctx->sm_count, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, out);
     ctx->launches += 7;
     CC_CUDA(ctx, cudaGetLastError());
