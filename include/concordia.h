@@ -33,6 +33,7 @@
  * On-log record format (the paper lists the fields, PAPER.md:L85,
  * L219, not their widths).  All integers little-endian, no padding:
  *   page record   : { u32 region_id; u32 page_idx; u32 len; u32 crc32c(payload) } + len payload bytes
+ *                   (len = one page, or a run of consecutive pages starting at page_idx: cc_checkpoint_delta_rle)
  *   commit record : { 0xFFFFFFFF; 0xFFFFFFFF; 16; crc32c(payload) } + { u64 epoch; u32 region_id; u32 k }
  *   CRC32C        : Castagnoli, reflected 0x82F63B78, init 0xFFFFFFFF, xorout 0xFFFFFFFF.
  * One checkpoint of one region appends its k dirty pages in ascending page order followed by
@@ -125,6 +126,7 @@ typedef struct {
 #define CC_TASK_COMPACT_LOG 8u     /* arg0 = input log, arg1 = its bytes, arg2 = output log, arg3 = output capacity */
 #define CC_TASK_CKPT_ALL 9u        /* epoch: every region that has a shadow (cc_checkpoint_all) */
 #define CC_TASK_EXIT 255u
+#define CC_TASKF_RLE 2u            /* cc_task.flags, CC_TASK_DELTA_CKPT only: run records, arg0 = run_pages (cc_checkpoint_delta_rle) */
 #define CC_TASKF_FUSED 1u          /* cc_task.flags, CC_TASK_DELTA_CKPT only: run the fused single pass (cc_checkpoint_delta_fused) */
 typedef struct {
     uint32_t kind;
@@ -192,6 +194,17 @@ int32_t cc_checkpoint_delta(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, voi
  * the scan; otherwise the records are written by the gather kernel afterwards as in
  * cc_checkpoint_delta.  A short commit kernel follows in both cases. */
 int32_t cc_checkpoint_delta_fused(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out);
+
+/* Delta checkpoint with RUN-LENGTH records ("Sparse page maps use index-value records;
+ * contiguous dirty ranges use run-length encoding"): as cc_checkpoint_delta, but consecutive dirty pages
+ * form ONE record { region_id, first page, len = bytes of the whole run, crc32c(all payload bytes of the
+ * run) } + the run's pages back to back.  A run never crosses a page index that is a multiple of
+ * run_pages (>= 1, run_pages * page_bytes < 2^32), so it has at most run_pages pages; run_pages = 1 gives
+ * cc_checkpoint_delta's bytes.  The commit record counts RECORDS; out->n_dirty still counts pages.
+ * cc_apply_log and cc_compact_log read both kinds of record (a single-page record is the run of length
+ * one). */
+int32_t cc_checkpoint_delta_rle(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, uint32_t run_pages, void* stream,
+                                cc_result* out);
 
 /* Allocator-aware delta checkpoint ("reads allocator dirty metadata", L266
  * "discovery is proportional to the dirty block bitmap"): the dirty set comes from the runtime's

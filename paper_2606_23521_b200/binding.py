@@ -43,11 +43,12 @@ CC_TASK_COMPACT_LOG = 8
 CC_TASK_CKPT_ALL = 9
 CC_TASK_EXIT = 255
 CC_TASKF_FUSED = 1
+CC_TASKF_RLE = 2
 
 EXPORTS = [
     "cc_init", "cc_shutdown", "cc_last_cuda_error", "cc_kernel_launches", "cc_workspace_bytes",
     "cc_register_region", "cc_unregister_region", "cc_log_attach", "cc_log_reset", "cc_log_reset_async",
-    "cc_checkpoint_delta", "cc_checkpoint_delta_fused", "cc_checkpoint_marked", "cc_checkpoint_versions",
+    "cc_checkpoint_delta", "cc_checkpoint_delta_fused", "cc_checkpoint_delta_rle", "cc_checkpoint_marked", "cc_checkpoint_versions",
     "cc_checkpoint_all", "cc_snapshot_region", "cc_compact_log", "cc_scan_only", "cc_trace_events", "cc_dirty_list", "cc_apply_scratch_bytes", "cc_apply_attach", "cc_apply_stage_attach", "cc_apply_log",
     "cc_worker_start", "cc_worker_stop", "cc_worker_alive", "cc_peek_queue", "cc_submit", "cc_poll", "cc_wait",
 ]
@@ -112,6 +113,7 @@ def load_library():
         "cc_log_reset_async": (i32, [vp, vp]),
         "cc_checkpoint_delta": (i32, [vp, u32, u64, vp, vp]),
         "cc_checkpoint_delta_fused": (i32, [vp, u32, u64, vp, vp]),
+        "cc_checkpoint_delta_rle": (i32, [vp, u32, u64, u32, vp, vp]),
         "cc_checkpoint_marked": (i32, [vp, u32, u64, vp, u32, vp, vp]),
         "cc_checkpoint_versions": (i32, [vp, u32, u64, vp, vp, vp, vp]),
         "cc_checkpoint_all": (i32, [vp, u64, vp, vp]),
@@ -254,6 +256,10 @@ class Context:
     def checkpoint_delta_fused(self, region_id: int, epoch: int, result: Result = None, stream=None):
         self._check("cc_checkpoint_delta_fused", self.lib.cc_checkpoint_delta_fused(
             self.h, region_id, epoch, _stream_ptr(stream), ctypes.c_void_p(result.ptr) if result else None))
+
+    def checkpoint_delta_rle(self, region_id: int, epoch: int, run_pages: int, result: Result = None, stream=None):
+        self._check("cc_checkpoint_delta_rle", self.lib.cc_checkpoint_delta_rle(
+            self.h, region_id, epoch, run_pages, _stream_ptr(stream), ctypes.c_void_p(result.ptr) if result else None))
 
     def checkpoint_marked(self, region_id: int, epoch: int, dirty_bitmap: torch.Tensor, flags: int = 0,
                           result: Result = None, stream=None):

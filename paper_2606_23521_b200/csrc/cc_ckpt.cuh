@@ -102,6 +102,7 @@ __device__ __forceinline__ void cc_plan_checkpoint_at(const cc_region_dev& r, co
         else k_eff = k;
     }
     h->k_eff = k_eff;
+    h->commit_k = k_eff;
     h->status = st;
     h->W_start = W;
     h->need = k_eff ? need : 0;
@@ -115,7 +116,7 @@ __device__ __forceinline__ void cc_plan_checkpoint(const cc_region_dev& r, const
 
 // Only the first CC_COMPACT_THREADS threads of a block work (the worker's blocks may be wider);
 // every thread takes part in the barriers.
-__device__ __forceinline__ void cc_compact_phase(const cc_region_dev& r, cc_log_dev* log, u32 mode, u64 epoch,
+__device__ __forceinline__ void cc_compact_phase(const cc_region_dev& r, const cc_log_dev* log, u32 mode, u64 epoch,
                                                  cc_result* out) {
     __shared__ u32 s_ticket, s_excl, s_last_dirty;
     __shared__ u32 s_warp[CC_COMPACT_THREADS / 32];
@@ -324,7 +325,7 @@ __device__ __forceinline__ u64 cc_gather_commit_record(const cc_region_dev& r, c
     if (k_eff != 0) {
         u8* c = log->buf + W0 + h->need - CC_COMMIT_RECORD_BYTES;
         const u64 epoch = h->epoch;
-        u32 pay[4] = {(u32)epoch, (u32)(epoch >> 32), r.region_id, k_eff};
+        u32 pay[4] = {(u32)epoch, (u32)(epoch >> 32), r.region_id, h->commit_k};
         const u32 crc = crc_serial(&dev->crc, reinterpret_cast<const u8*>(pay), 16);
         st_u32x4(c + 16, pay[0], pay[1], pay[2], pay[3]);
         st_u32x4(c, CC_COMMIT_ID, CC_COMMIT_ID, 16u, crc);
@@ -336,12 +337,12 @@ __device__ __forceinline__ u64 cc_gather_commit_record(const cc_region_dev& r, c
     return W_after;
 }
 
-__device__ __forceinline__ void cc_gather_phase(const cc_region_dev& r, cc_dev* dev, cc_crc_smem* cs, cc_grid g,
-                                                cc_result* out, u32 kind, bool init_tables) {
+// Completion of a region's record writer: every block fences its stores at system scope and counts itself
+// done; the last block appends the commit record, fences, publishes the committed offset with a system-scope
+// release store (L263) and fills the result.
+__device__ __forceinline__ void cc_gather_complete(const cc_region_dev& r, cc_dev* dev, cc_grid g, cc_result* out, u32 kind) {
     cc_ws_hdr* h = r.hdr;
     cc_log_dev* log = &dev->log;
-    cc_gather_work(r, dev, cs, g, init_tables);
-    // ---- completion: last block commits ----
     __shared__ u32 s_last;
     __threadfence_system();
     __syncthreads();
@@ -373,4 +374,10 @@ __device__ __forceinline__ void cc_gather_phase(const cc_region_dev& r, cc_dev* 
         }
         __threadfence();
     }
+}
+
+__device__ __forceinline__ void cc_gather_phase(const cc_region_dev& r, cc_dev* dev, cc_crc_smem* cs, cc_grid g,
+                                                cc_result* out, u32 kind, bool init_tables) {
+    cc_gather_work(r, dev, cs, g, init_tables);
+    cc_gather_complete(r, dev, g, out, kind);
 }

@@ -11,6 +11,7 @@ typedef uint64_t u64;
 
 #define CC_SEG_BYTES 4096u        // one warp item: 32 lanes x 8 x 16 B
 #define CC_SEG_VECS 256u          // 16-byte vectors per segment
+#define CC_SEG_POW_MAX 256u       // table of x^(8*4096*m) up to m = 256 (1 MiB of message after a segment)
 #define CC_COMPACT_THREADS 256
 #define CC_COMPACT_WORDS_PER_THREAD 4
 #define CC_COMPACT_TILE_WORDS (CC_COMPACT_THREADS * CC_COMPACT_WORDS_PER_THREAD)   // 1024 words = 32768 pages
@@ -32,6 +33,8 @@ struct cc_ws_hdr {
     u64 t_start_ns;
     u64 epoch;
     u32 inline_done;    // fused pass already wrote the records, headers and shadow: the gather only commits
+    u32 commit_k;       // record count that goes into the commit record (= k_eff, or the number of runs)
+    u32 n_runs;         // run-length records: runs of the last plan
     u32 pad0;
 };
 
@@ -51,6 +54,13 @@ struct cc_region_dev {
     u64* rec_state;     // n_pages u64: per-record {done-mask or count : 32 | CRC accumulator : 32}, zero between calls
     u64* lb_status;     // compaction look-back status, one per tile
     u64* flb_status;    // fused pass look-back status, one per page tile
+    // run-length records (cc_rle.cuh)
+    u32* S;             // bitmap over dirty RANKS: rank i starts a run; same padded size as `bitmap`, zero between calls
+    u32* Rfirst;        // n_pages + 1 u32: first rank of run j (and k as a sentinel after the last run)
+    u32* Rn;            // n_pages u32: run index of rank i
+    u64* run_state;     // n_pages u64: per-run {finished pages : 32 | CRC accumulator : 32}, zero between calls
+    cc_ws_hdr* hdr2;    // control block of the ranking pass over S
+    u64* lb2;           // its look-back status words
     u32 ftile_pages;    // pages per fused warp tile (~64 KiB of region, 1..32 pages)
     u32 n_ftiles;
     u32* latest;        // n_pages u32: applier last-wins table, all zero between calls
@@ -122,10 +132,10 @@ struct cc_crc_tables {
     u32 t0[256];            // byte table of the reflected polynomial
     u32 s512[4][256];       // multiply by x^(8*512) mod G, one table per register byte
     u32 lane_mul[32];       // x^(8*16*(31-lane))
-    u32 seg_mul[65];        // x^(8*4096*m), m = 0..64
+    u32 seg_mul[CC_SEG_POW_MAX + 1];   // x^(8*4096*m), m = 0..CC_SEG_POW_MAX
     u32 xp[48];             // x^(8*2^j), j = 0..47
     u32 lane_nib[8 * 16 * 32];  // (v << 4n) * lane_mul[l] at [(n*16 + v)*32 + l]
-    u32 seg_pow[65 * 32];   // seg_mul[m] * x^i at [m*32 + i]
+    u32 seg_pow[(CC_SEG_POW_MAX + 1) * 32];   // seg_mul[m] * x^i at [m*32 + i]
 };
 
 struct cc_dev {

@@ -54,13 +54,13 @@ static inline void cc_crc_build_tables(cc_crc_tables* t) {
     for (int b = 0; b < 4; b++)
         for (u32 v = 0; v < 256; v++) t->s512[b][v] = gf_mul(v << (8 * b), s512);
     for (u32 l = 0; l < 32; l++) t->lane_mul[l] = gf_xpow_bytes(t->xp, 16ull * (31 - l));
-    for (u32 m = 0; m <= 64; m++) t->seg_mul[m] = gf_xpow_bytes(t->xp, 4096ull * m);
+    for (u32 m = 0; m <= CC_SEG_POW_MAX; m++) t->seg_mul[m] = gf_xpow_bytes(t->xp, 4096ull * m);
     // lane_nib[(n*16 + v)*32 + l] = (v << 4n) * lane_mul[l]: multiply by the lane constant in 8 lookups
     for (u32 n = 0; n < 8; n++)
         for (u32 v = 0; v < 16; v++)
             for (u32 l = 0; l < 32; l++) t->lane_nib[(n * 16 + v) * 32 + l] = gf_mul(v << (4 * n), t->lane_mul[l]);
     // seg_pow[m*32 + i] = seg_mul[m] * x^i: multiply by the segment constant with one term per lane
-    for (u32 m = 0; m <= 64; m++) {
+    for (u32 m = 0; m <= CC_SEG_POW_MAX; m++) {
         u32 b = t->seg_mul[m];
         for (u32 i = 0; i < 32; i++) { t->seg_pow[m * 32 + i] = b; b = gf_mulx(b); }
     }
@@ -155,7 +155,7 @@ __device__ __forceinline__ u32 crc_segment_warp(const cc_crc_smem* s, const cc_c
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) acc ^= __shfl_xor_sync(0xFFFFFFFFu, acc, o);
     if (after != 0) {
-        if ((after & 4095u) == 0 && (after >> 12) <= 64) {
+        if ((after & 4095u) == 0 && (after >> 12) <= CC_SEG_POW_MAX) {
             // acc * seg_mul[m]: lane i contributes bit (31-i) of acc times seg_mul[m]*x^i
             u32 term = ((acc >> (31 - lane)) & 1u) ? g->seg_pow[(u32)(after >> 12) * 32 + lane] : 0u;
 #pragma unroll

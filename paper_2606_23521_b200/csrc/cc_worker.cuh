@@ -14,6 +14,7 @@
 #include "cc_ckpt.cuh"
 #include "cc_mark.cuh"
 #include "cc_fused.cuh"
+#include "cc_rle.cuh"
 #include "cc_apply.cuh"
 #include "cc_compactor.cuh"
 #include "cc_batch.cuh"
@@ -184,6 +185,20 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
             switch (task.kind) {
             case CC_TASK_DELTA_CKPT: {
                 const cc_region_dev& r = dev->regions[slot];
+                if ((task.flags & CC_TASKF_RLE) && task.arg0 != 0 && task.arg0 * r.page_bytes <= 0xFFFFFFFFull) {
+                    cc_scan_phase<8>(r, g);
+                    cc_grid_barrier(dev, g.nblocks, gen);
+                    cc_compact_phase(r, &dev->log, CC_MODE_SCAN_ONLY, task.epoch, nullptr);
+                    cc_grid_barrier(dev, g.nblocks, gen);
+                    cc_rle_starts_phase(r, (u32)task.arg0, g);
+                    cc_grid_barrier(dev, g.nblocks, gen);
+                    cc_rle_rank_phase(r, &dev->log);
+                    cc_grid_barrier(dev, g.nblocks, gen);
+                    cc_rle_plan_phase(r, &dev->log, task.epoch, g);
+                    cc_grid_barrier(dev, g.nblocks, gen);
+                    cc_rle_gather_phase(r, dev, cs, g, nullptr, task.kind, false);
+                    break;
+                }
                 if (task.flags & CC_TASKF_FUSED) {
                     cc_fused_phase(r, dev, cs, CC_MODE_CHECKPOINT, task.epoch, false);
                 } else {

@@ -14,6 +14,7 @@
 #include "cc_ckpt.cuh"
 #include "cc_mark.cuh"
 #include "cc_fused.cuh"
+#include "cc_rle.cuh"
 #include "cc_apply.cuh"
 #include "cc_compactor.cuh"
 #include "cc_batch.cuh"
@@ -68,6 +69,22 @@ __global__ void __launch_bounds__(CC_APPLY_THREADS) cc_compactor_copy_kernel(cc_
 }
 __global__ void __launch_bounds__(CC_APPLY_THREADS) cc_compactor_cleanup_kernel(cc_dev* dev, cc_apply_tabs tabs, cc_result* out) {
     cc_compactor_cleanup_phase(dev, tabs, cc_hw_grid(), out, CC_TASK_COMPACT_LOG);
+}
+
+// run-length records (cc_rle.cuh)
+__global__ void __launch_bounds__(256) cc_rle_starts_kernel(const cc_dev* dev, int slot, u32 run_pages) {
+    cc_rle_starts_phase(dev->regions[slot], run_pages, cc_hw_grid());
+}
+__global__ void __launch_bounds__(CC_COMPACT_THREADS) cc_rle_rank_kernel(const cc_dev* dev, int slot) {
+    cc_rle_rank_phase(dev->regions[slot], &dev->log);
+}
+__global__ void __launch_bounds__(256) cc_rle_plan_kernel(const cc_dev* dev, int slot, u64 epoch) {
+    cc_rle_plan_phase(dev->regions[slot], &dev->log, epoch, cc_hw_grid());
+}
+__global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_rle_gather_kernel(cc_dev* dev, int slot, cc_result* out) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cc_rle_gather_phase(dev->regions[slot], dev, reinterpret_cast<cc_crc_smem*>(smem_raw), cc_hw_grid(), out,
+                        CC_TASK_DELTA_CKPT, true);
 }
 
 // one boundary, all regions (cc_batch.cuh)
@@ -179,7 +196,7 @@ static int find_slot(cc_ctx* ctx, uint32_t id) {
 }
 
 struct cc_ws_layout {
-    uint64_t hdr, bitmap, D, rec_state, latest, lb, flb, total;
+    uint64_t hdr, bitmap, D, rec_state, latest, lb, flb, S, Rfirst, Rn, run_state, hdr2, lb2, total;
     uint64_t n_pages, n_words, n_tiles, ftile_pages, n_ftiles;
 };
 
@@ -203,6 +220,13 @@ static bool ws_layout(uint64_t bytes, uint32_t P, cc_ws_layout* L) {
     L->ftile_pages = tp;
     L->n_ftiles = (n_pages + tp - 1) / tp;
     L->flb = o; o += align_up(L->n_ftiles * 8, 256);
+    // run-length records (cc_rle.cuh)
+    L->S = o; o += align_up(L->n_tiles * CC_COMPACT_TILE_WORDS * 4, 256);
+    L->Rfirst = o; o += align_up((n_pages + 1) * 4, 256);
+    L->Rn = o; o += align_up(n_pages * 4, 256);
+    L->run_state = o; o += align_up(n_pages * 8, 256);
+    L->hdr2 = o; o += 256;
+    L->lb2 = o; o += align_up(L->n_tiles * 8, 256);
     L->total = o;
     return true;
 }
@@ -246,6 +270,7 @@ extern "C" int32_t cc_init(cc_ctx** out, int32_t device, const cc_config* cfg) {
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->worker_stream, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->worker_done, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_rle_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_compactor_copy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_batch_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
@@ -343,6 +368,12 @@ extern "C" int32_t cc_register_region(cc_ctx* ctx, const cc_region_desc* d) {
     r.latest = (u32*)(ws + L.latest);
     r.lb_status = (u64*)(ws + L.lb);
     r.flb_status = (u64*)(ws + L.flb);
+    r.S = (u32*)(ws + L.S);
+    r.Rfirst = (u32*)(ws + L.Rfirst);
+    r.Rn = (u32*)(ws + L.Rn);
+    r.run_state = (u64*)(ws + L.run_state);
+    r.hdr2 = (cc_ws_hdr*)(ws + L.hdr2);
+    r.lb2 = (u64*)(ws + L.lb2);
     r.ftile_pages = (u32)L.ftile_pages;
     r.n_ftiles = (u32)L.n_ftiles;
     {
@@ -536,6 +567,32 @@ extern "C" int32_t cc_checkpoint_delta_fused(cc_ctx* ctx, uint32_t region_id, ui
     if (ctx->ev_after_compact) cudaEventRecord(ctx->ev_after_compact, st);
     CC_CUDA(ctx, cudaGetLastError());
     return launch_gather(ctx, slot, st, out);
+}
+
+extern "C" int32_t cc_checkpoint_delta_rle(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, uint32_t run_pages, void* stream,
+                                           cc_result* out) {
+    if (!ctx || run_pages == 0) return CC_ERR_INVALID;
+    int slot = find_slot(ctx, region_id);
+    if (slot < 0) return CC_ERR_NOT_REGISTERED;
+    const cc_region_dev& r = ctx->regions[slot].dev;
+    if (!r.shadow || (uint64_t)run_pages * r.page_bytes > 0xFFFFFFFFull) return CC_ERR_INVALID;
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaEvent_t ec = ctx->ev_after_compact;
+    ctx->ev_after_compact = nullptr;                    // the trace event goes after the whole ranking
+    int32_t rc = launch_scan_compact(ctx, slot, CC_MODE_SCAN_ONLY, epoch, st, nullptr);
+    ctx->ev_after_compact = ec;
+    if (rc != CC_OK) return rc;
+    const uint64_t n_tiles = (r.n_words + CC_COMPACT_TILE_WORDS - 1) / CC_COMPACT_TILE_WORDS;
+    const unsigned g2 = (unsigned)(n_tiles < (uint64_t)ctx->sm_count * 4 ? n_tiles : (uint64_t)ctx->sm_count * 4);
+    cc_rle_starts_kernel<<<small_grid(ctx, r.n_words, 8), 256, 0, st>>>(ctx->d_dev, slot, run_pages);
+    cc_rle_rank_kernel<<<g2, CC_COMPACT_THREADS, 0, st>>>(ctx->d_dev, slot);
+    cc_rle_plan_kernel<<<small_grid(ctx, r.n_pages, 256), 256, 0, st>>>(ctx->d_dev, slot, epoch);
+    if (ec) cudaEventRecord(ec, st);
+    cc_rle_gather_kernel<<<(unsigned)(ctx->sm_count * ctx->gather_bps), CC_GATHER_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, slot, out);
+    ctx->launches += 4;
+    CC_CUDA(ctx, cudaGetLastError());
+    return CC_OK;
 }
 
 extern "C" int32_t cc_checkpoint_all(cc_ctx* ctx, uint64_t epoch, void* stream, cc_result* out) {

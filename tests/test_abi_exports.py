@@ -39,7 +39,7 @@ def test_pure_host_entry_points():
     assert lib.cc_workspace_bytes(4096 + 8, 4096) == 0       # size not a multiple of 16
     w = lib.cc_workspace_bytes(8 << 30, 65536)
     assert 0 < w < (8 << 20)
-    assert lib.cc_workspace_bytes(64 << 30, 4096) < (400 << 20)
+    assert lib.cc_workspace_bytes(64 << 30, 4096) < (640 << 20)      # ~32 B per page: < 1 % of the region
     assert lib.cc_apply_scratch_bytes(0) == 0
     assert lib.cc_apply_scratch_bytes(10100) < (1 << 20)
 
