@@ -315,6 +315,10 @@ int32_t cc_peek_queue(cc_ctx* ctx, uint64_t* head, uint64_t* tail);
  * no CUDA call.  Non-blocking: CC_ERR_RING_FULL when `capacity` tasks are outstanding.
  * *seq_out (may be NULL) = the sequence number to poll / wait on. */
 int32_t cc_submit(cc_ctx* ctx, const cc_task* task, uint64_t* seq_out);
+/* Measurement hook: mean host cost of one cc_submit in ns over n CC_TASK_NOP submissions, timed inside the library
+ * so that no language binding is in the way (Table 7).  Waits for free slots outside the timed
+ * sections and for the last task before returning.  Needs a running worker. */
+int32_t cc_measure_submit_cost(cc_ctx* ctx, uint32_t n, double* ns_per_submit);
 /* CC_OK and *out filled when task `seq` has completed; CC_PENDING otherwise.  A completion slot
  * is reused `capacity` submissions later: poll before then. */
 int32_t cc_poll(cc_ctx* ctx, uint64_t seq, cc_result* out);

@@ -811,6 +811,37 @@ extern "C" int32_t cc_submit(cc_ctx* ctx, const cc_task* task, uint64_t* seq_out
     return CC_OK;
 }
 
+// Measurement hook: the host cost of cc_submit itself, without a language binding in the way (PAPER.md:L162,
+// Table 7 "ring submit < 0.1 us").  Submits n CC_TASK_NOP tasks; only the cc_submit calls are inside the timed
+// sections (when the ring is full the wait for a free slot is not).  Returns the mean ns per cc_submit.
+extern "C" int32_t cc_measure_submit_cost(cc_ctx* ctx, uint32_t n, double* ns_per_submit) {
+    if (!ctx || !ns_per_submit || n == 0) return CC_ERR_INVALID;
+    if (!ctx->worker_running) return CC_ERR_WORKER;
+    cc_task t;
+    memset(&t, 0, sizeof(t));
+    t.kind = CC_TASK_NOP;
+    u64 total = 0, seq = 0;
+    uint32_t done = 0;
+    while (done < n) {
+        const u64 room = ctx->cfg.ring_capacity - (ctx->submitted - __atomic_load_n(ctx->ring_words + 8, __ATOMIC_ACQUIRE));
+        uint32_t burst = (uint32_t)(room < (n - done) ? room : (n - done));
+        if (burst == 0) {
+            if (cudaEventQuery(ctx->worker_done) != cudaErrorNotReady) return CC_ERR_WORKER;
+            continue;
+        }
+        const u64 t0 = now_ns();
+        for (uint32_t i = 0; i < burst; i++)
+            if (cc_submit(ctx, &t, &seq) != CC_OK) return CC_ERR_RING_FULL;
+        total += now_ns() - t0;
+        done += burst;
+    }
+    cc_result r;
+    int32_t rc = cc_wait(ctx, seq, 10ull * 1000000000ull, &r);
+    if (rc != CC_OK) return rc;
+    *ns_per_submit = (double)total / (double)n;
+    return CC_OK;
+}
+
 extern "C" int32_t cc_poll(cc_ctx* ctx, uint64_t seq, cc_result* out) {
     if (!ctx) return CC_ERR_INVALID;
     if (seq >= ctx->submitted) return CC_ERR_INVALID;

@@ -83,6 +83,7 @@ def main():
             t2 = time.perf_counter_ns()
             submit_ns.append(t1 - t0)
             nop_rt.append(t2 - t0)
+        native_submit_ns = ctx.measure_submit_cost(200000)
         # (iii) + (iv): mutate -> checkpoint tasks
         rt, dev_ns, ks = [], [], []
         used = 0
@@ -108,7 +109,8 @@ def main():
             "config": {"region_MiB": a.region_mib, "page_bytes": P, "dirty_pages_per_task": n_mut, "tasks": a.tasks,
                        "log": "device" if a.device_log else "pinned host", "bytes_per_task": per,
                        "path": "fused single pass" if a.fused else "scan + compact + gather"},
-            "submit_host_cost_us": {"p50": us(submit_ns, 0.5), "p99": us(submit_ns, 0.99)},
+            "submit_host_cost_us": {"p50": us(submit_ns, 0.5), "p99": us(submit_ns, 0.99), "through": "ctypes"},
+            "submit_host_cost_native_ns": round(native_submit_ns, 1),
             "nop_round_trip_us": {"p50": us(nop_rt, 0.5), "p99": us(nop_rt, 0.99)},
             "checkpoint_task_round_trip_us": {"p50": us(rt, 0.5), "p99": us(rt, 0.99)},
             "checkpoint_task_device_us": {"p50": us(dev_ns, 0.5), "p99": us(dev_ns, 0.99)},
