@@ -340,15 +340,23 @@ __device__ __forceinline__ u64 cc_gather_commit_record(const cc_region_dev& r, c
 // Completion of a region's record writer: every block fences its stores at system scope and counts itself
 // done; the last block appends the commit record, fences, publishes the committed offset with a system-scope
 // release store (L263) and fills the result.
-__device__ __forceinline__ void cc_gather_complete(const cc_region_dev& r, cc_dev* dev, cc_grid g, cc_result* out, u32 kind) {
+// Only the blocks that had items take part (n_items = items of the record writer; at least block 0): with a
+// small dirty set the other blocks leave at once instead of queueing fences and atomics on one counter.
+__device__ __forceinline__ void cc_gather_complete(const cc_region_dev& r, cc_dev* dev, cc_grid g, cc_result* out, u32 kind,
+                                                   u64 n_items) {
     cc_ws_hdr* h = r.hdr;
     cc_log_dev* log = &dev->log;
+    const u64 wpb = blockDim.x >> 5;
+    u64 n_work = (n_items + wpb - 1) / wpb;
+    if (n_work > g.nblocks) n_work = g.nblocks;
+    if (n_work == 0) n_work = 1;
+    if (g.block >= n_work) return;
     __shared__ u32 s_last;
     __threadfence_system();
     __syncthreads();
     if (threadIdx.x == 0) {
         __threadfence_system();
-        s_last = (atomicAdd(&h->gather_done, 1u) == g.nblocks - 1) ? 1u : 0u;
+        s_last = (atomicAdd(&h->gather_done, 1u) == (u32)n_work - 1) ? 1u : 0u;
     }
     __syncthreads();
     if (s_last && threadIdx.x == 0) {
@@ -378,6 +386,7 @@ __device__ __forceinline__ void cc_gather_complete(const cc_region_dev& r, cc_de
 
 __device__ __forceinline__ void cc_gather_phase(const cc_region_dev& r, cc_dev* dev, cc_crc_smem* cs, cc_grid g,
                                                 cc_result* out, u32 kind, bool init_tables) {
+    const u64 n_items = r.hdr->inline_done ? 0ull : (u64)r.hdr->k_eff * r.spp;
     cc_gather_work(r, dev, cs, g, init_tables);
-    cc_gather_complete(r, dev, g, out, kind);
+    cc_gather_complete(r, dev, g, out, kind, n_items);
 }

@@ -128,13 +128,13 @@ struct cc_batch_state {
     u32 pad;
 };
 
-struct cc_crc_tables {
+struct alignas(16) cc_crc_tables {
     u32 t0[256];            // byte table of the reflected polynomial
-    u32 s512[4][256];       // multiply by x^(8*512) mod G, one table per register byte
+    alignas(16) u32 s512[4][256];       // multiply by x^(8*512) mod G, one table per register byte
     u32 lane_mul[32];       // x^(8*16*(31-lane))
     u32 seg_mul[CC_SEG_POW_MAX + 1];   // x^(8*4096*m), m = 0..CC_SEG_POW_MAX
     u32 xp[48];             // x^(8*2^j), j = 0..47
-    u32 lane_nib[8 * 16 * 32];  // (v << 4n) * lane_mul[l] at [(n*16 + v)*32 + l]
+    alignas(16) u32 lane_nib[8 * 16 * 32];  // (v << 4n) * lane_mul[l] at [(n*16 + v)*32 + l]
     u32 seg_pow[(CC_SEG_POW_MAX + 1) * 32];   // seg_mul[m] * x^i at [m*32 + i]
 };
 

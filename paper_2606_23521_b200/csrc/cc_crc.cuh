@@ -71,19 +71,31 @@ static inline void cc_crc_build_tables(cc_crc_tables* t) {
 // offset entry*128 + lane*4.  The CRC register is kept rotated left by 7 as well ("z"), so the low
 // byte of the register already sits at bits 7..14 = the table's byte offset: one LOP3 forms the
 // address, one funnel shift + one LOP3 form the next state -> 3 ALU + 1 LDS per message byte.
-struct cc_crc_smem {
+struct alignas(16) cc_crc_smem {
     u32 t0[256 * 32];
-    u32 lane_nib[8 * 16 * 32];
-    u32 s512[4 * 256];
+    alignas(16) u32 lane_nib[8 * 16 * 32];
+    alignas(16) u32 s512[4 * 256];
 };
 
 __device__ __forceinline__ u32 rotl32(u32 x, int n) { return __funnelshift_l(x, x, n); }
 __device__ __forceinline__ u32 rotr32(u32 x, int n) { return __funnelshift_r(x, x, n); }
 
+// Few, independent, coalesced global loads per thread (one latency, not a chain of them: the fill used to cost
+// ~20 us of every launch): a warp loads 32 byte-table entries with ONE load and spreads them by shuffle; the
+// other two tables are straight 16-byte copies.
 __device__ __forceinline__ void cc_crc_smem_init(cc_crc_smem* s, const cc_crc_tables* g) {
-    for (u32 i = threadIdx.x; i < 256 * 32; i += blockDim.x) s->t0[i] = rotl32(g->t0[i >> 5], 7);
-    for (u32 i = threadIdx.x; i < 8 * 16 * 32; i += blockDim.x) s->lane_nib[i] = g->lane_nib[i];
-    for (u32 i = threadIdx.x; i < 4 * 256; i += blockDim.x) s->s512[i] = (&g->s512[0][0])[i];
+    const u32 lane = threadIdx.x & 31u, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    for (u32 e0 = w * 32u; e0 < 256u; e0 += nw * 32u) {
+        const u32 mine = rotl32(g->t0[e0 + lane], 7);
+#pragma unroll
+        for (u32 e = 0; e < 32u; e++) s->t0[(e0 + e) * 32u + lane] = __shfl_sync(0xFFFFFFFFu, mine, e);
+    }
+    const uint4* nib = reinterpret_cast<const uint4*>(g->lane_nib);
+    uint4* dn = reinterpret_cast<uint4*>(s->lane_nib);
+    for (u32 i = threadIdx.x; i < 8 * 16 * 32 / 4; i += blockDim.x) dn[i] = nib[i];
+    const uint4* s5 = reinterpret_cast<const uint4*>(&g->s512[0][0]);
+    uint4* d5 = reinterpret_cast<uint4*>(s->s512);
+    for (u32 i = threadIdx.x; i < 4 * 256 / 4; i += blockDim.x) d5[i] = s5[i];
     __syncthreads();
 }
 
@@ -172,10 +184,15 @@ __device__ __forceinline__ u32 crc_segment_warp(const cc_crc_smem* s, const cc_c
 // is precomputed per region for its full and its tail page length.
 __device__ __forceinline__ u32 crc_finalize(u32 acc, u32 init_term) { return acc ^ init_term ^ 0xFFFFFFFFu; }
 
-// Serial CRC32C of a few bytes (commit payload), single thread, global table.
-__device__ inline u32 crc_serial(const cc_crc_tables* g, const u8* p, u32 n) {
+// Serial CRC32C of a few bytes (commit payload), single thread: bit by bit in registers -- 128 shift/xor steps
+// for a commit payload, cheaper than 16 dependent lookups in a global table that is cold in this SM's L1.
+__device__ inline u32 crc_serial(const cc_crc_tables*, const u8* p, u32 n) {
     u32 c = 0xFFFFFFFFu;
-    for (u32 i = 0; i < n; i++) c = g->t0[(c ^ p[i]) & 0xFFu] ^ (c >> 8);
+    for (u32 i = 0; i < n; i++) {
+        c ^= p[i];
+#pragma unroll
+        for (int b = 0; b < 8; b++) c = gf_mulx(c);
+    }
     return c ^ 0xFFFFFFFFu;
 }
 

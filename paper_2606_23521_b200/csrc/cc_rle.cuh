@@ -169,5 +169,5 @@ __device__ __forceinline__ void cc_rle_gather_phase(const cc_region_dev& r, cc_d
         if (init_tables) cc_crc_smem_init(cs, &dev->crc);
         cc_rle_gather_items(r, dev, cs, g.warp(), g.nwarps());
     }
-    cc_gather_complete(r, dev, g, out, kind);
+    cc_gather_complete(r, dev, g, out, kind, (u64)k_eff * r.spp);
 }
