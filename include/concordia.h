@@ -165,10 +165,10 @@ int32_t cc_unregister_region(cc_ctx* ctx, uint32_t region_id);
  * offset with a system-scope release store after every commit record.  W := 0.
  * Only while the worker is stopped. */
 int32_t cc_log_attach(cc_ctx* ctx, void* log_buf, uint64_t capacity, uint64_t* committed_off);
-/* W := 0 (synchronous; only while the worker is stopped -- use CC_TASK_LOG_RESET otherwise). */
+/* W := 0 and *committed_off := 0 (synchronous; only while the worker is stopped -- use CC_TASK_LOG_RESET otherwise). */
 int32_t cc_log_reset(cc_ctx* ctx);
 
-/* W := 0, ASYNCHRONOUS on `stream` (ordered after the checkpoints already queued there): what a log
+/* W := 0 and *committed_off := 0, ASYNCHRONOUS on `stream` (ordered after the checkpoints already queued there): what a log
  * drainer calls once it has consumed the committed prefix.  Only while the worker is stopped. */
 int32_t cc_log_reset_async(cc_ctx* ctx, void* stream);
 

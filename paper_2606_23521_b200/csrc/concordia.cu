@@ -157,6 +157,7 @@ struct cc_ctx {
     cudaStream_t internal;
     cc_host_region regions[CC_MAX_REGIONS];
     bool log_attached;
+    uint64_t* committed_off;    // the caller's published-offset word (may be null)
     cc_apply_tabs tabs;
     bool apply_attached;
     void* stage;                // optional device staging buffer for host-resident logs (cc_apply_stage_attach)
@@ -421,6 +422,7 @@ extern "C" int32_t cc_log_attach(cc_ctx* ctx, void* log_buf, uint64_t capacity, 
     CC_CUDA(ctx, cudaMemcpyAsync(&ctx->d_dev->log, &l, sizeof(l), cudaMemcpyHostToDevice, 0));
     CC_CUDA(ctx, cudaStreamSynchronize(0));
     ctx->log_attached = true;
+    ctx->committed_off = committed_off;
     return CC_OK;
 }
 
@@ -430,6 +432,7 @@ extern "C" int32_t cc_log_reset(cc_ctx* ctx) {
     CC_CUDA(ctx, cudaSetDevice(ctx->device));
     const u64 zero = 0;
     CC_CUDA(ctx, cudaMemcpyAsync(&ctx->d_dev->log.W, &zero, sizeof(zero), cudaMemcpyHostToDevice, 0));
+    if (ctx->committed_off) CC_CUDA(ctx, cudaMemsetAsync(ctx->committed_off, 0, sizeof(u64), 0));     // publish the rewind too
     CC_CUDA(ctx, cudaStreamSynchronize(0));
     return CC_OK;
 }
@@ -439,6 +442,7 @@ extern "C" int32_t cc_log_reset_async(cc_ctx* ctx, void* stream) {
     if (ctx->worker_running) return CC_ERR_WORKER;
     CC_CUDA(ctx, cudaSetDevice(ctx->device));
     CC_CUDA(ctx, cudaMemsetAsync(&ctx->d_dev->log.W, 0, sizeof(u64), (cudaStream_t)stream));
+    if (ctx->committed_off) CC_CUDA(ctx, cudaMemsetAsync(ctx->committed_off, 0, sizeof(u64), (cudaStream_t)stream));
     return CC_OK;
 }
 

@@ -107,9 +107,9 @@ def main():
         cur = synth.raw_region(64 << 20, 1001, dev)
         pages, offs, masks = synth.sparse_xor_flips(cur, 4096, 0.01, 1001)
         synth.toggle_flips(cur, offs, masks)                        # back to the registered state; re-armed per iteration
-        for cold in (True, False):
+        for cold, fused in ((True, False), (False, False), (False, True)):
             _time_config("C1 raw 64 MiB / 4 KiB / 1 % dirty", cur, 4096, lambda it: synth.toggle_flips(cur, offs, masks),
-                         len(pages), a.reps, cold, peak)
+                         len(pages), a.reps, cold, peak, fused=fused)
         del cur
     # ---- C2 ----
     if on("c2"):
@@ -122,9 +122,9 @@ def main():
     if on("c3"):
         cur = synth.lora_region(32, 1003, dev)
         k3 = 52
-        for cold in (True, False):
+        for cold, fused in ((True, False), (False, False), (False, True)):
             _time_config("C3 LoRA 64 MiB / 64 KiB / 5 % dirty", cur, 65536, lambda it: synth.lora_update(cur, 65536, 0.05, 4000 + it),
-                         k3, a.reps, cold, peak)
+                         k3, a.reps, cold, peak, fused=fused)
         del cur
     torch.cuda.empty_cache()
     # ---- C4 ----
