@@ -62,7 +62,7 @@ __device__ __forceinline__ void cc_batch_scan_phase(cc_dev* dev, cc_batch_tab* T
             const cc_region_dev& r = dev->regions[s];
             n = r.n_pages * (u64)r.spp;
             if (g.block == 0) {                             // open the region's compaction run (as cc_scan_phase does)
-                r.hdr->t_start_ns = dev->batch.t_start_ns;
+                r.hdr->t_start_ns = globaltimer_ns();
                 r.hdr->ticket = 0;
                 r.hdr->run_id = r.hdr->run_id + 1;
             }

@@ -178,6 +178,9 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
                      (task.kind == CC_TASK_DELTA_CKPT || (task.kind == CC_TASK_MARKED_CKPT && (task.arg1 & CC_MARK_VERIFY))))
                 status = CC_ERR_INVALID;
             if (task.kind == CC_TASK_MARKED_CKPT && (task.arg0 == 0 || (task.arg0 & 3))) status = CC_ERR_INVALID;
+            if (slot >= 0 && task.kind == CC_TASK_DELTA_CKPT && (task.flags & CC_TASKF_RLE) &&
+                (task.arg0 == 0 || task.arg0 * dev->regions[slot].page_bytes > 0xFFFFFFFFull))
+                status = CC_ERR_INVALID;
             if (task.kind == CC_TASK_VERSION_CKPT && (task.arg0 == 0 || task.arg1 == 0 || ((task.arg0 | task.arg1) & 7)))
                 status = CC_ERR_INVALID;
         }
@@ -185,7 +188,7 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
             switch (task.kind) {
             case CC_TASK_DELTA_CKPT: {
                 const cc_region_dev& r = dev->regions[slot];
-                if ((task.flags & CC_TASKF_RLE) && task.arg0 != 0 && task.arg0 * r.page_bytes <= 0xFFFFFFFFull) {
+                if (task.flags & CC_TASKF_RLE) {
                     cc_scan_phase<8>(r, g);
                     cc_grid_barrier(dev, g.nblocks, gen);
                     cc_compact_phase(r, &dev->log, CC_MODE_SCAN_ONLY, task.epoch, nullptr);
