@@ -55,110 +55,167 @@ __device__ __forceinline__ u32 cc_crc_init_term(const cc_dev* dev, const cc_regi
 #define CC_PA_NEXT 1u
 #define CC_PA_RUN 2u
 
+struct cc_parse_smem {
+    // the region table, copied once: the walk is a chain of dependent decisions, and every global load in it is
+    // a round trip to L2 (a few hundred ns) -- with the table in shared memory an epoch costs one load round
+    u64 r_bytes[CC_MAX_REGIONS], r_pages[CC_MAX_REGIONS];
+    u32 r_id[CC_MAX_REGIONS], r_P[CC_MAX_REGIONS], r_spp[CC_MAX_REGIONS];       // r_id = 0: slot unused
+    u64 off;                // offset of the next unread record
+    u32 action, slot, first_fail, first_short, nrecs, nepochs, pending, pend_rid, mixed, segs;
+    u32 width;              // speculation width of the next step: about the size of the previous epoch (reads far beyond
+                            // the epoch's end are wasted and only lengthen the step's slowest load)
+    u32 pre;                // the record at `off` has already been examined (action / slot are set)
+    u32 cand;               // thread whose speculative header sits right after the accepted run (or 0xFFFFFFFF)
+};
+
+__device__ __forceinline__ int cc_parse_find_slot(const cc_parse_smem* S, u32 rid) {
+    for (int q = 0; q < CC_MAX_REGIONS; q++)
+        if (S->r_id[q] == rid) return rid ? q : -1;
+    return -1;
+}
+__device__ __forceinline__ bool cc_parse_len_ok(const cc_parse_smem* S, u32 slot, u64 page_idx, u64 len) {
+    if (page_idx >= S->r_pages[slot] || len == 0) return false;
+    const u64 start = page_idx * (u64)S->r_P[slot];
+    if (len > S->r_bytes[slot] - start) return false;
+    return (len % S->r_P[slot] == 0) || (start + len == S->r_bytes[slot]);
+}
+
+// Examine the record at S->off (one thread).  A commit record is validated and its epoch pushed (CC_PA_NEXT); a
+// page record opens a speculative run (CC_PA_RUN); anything torn or invalid stops the walk (CC_PA_STOP), exactly
+// where the sequential definition stops.  pre_h / pre_pl: the header / the 16 bytes after it, if already loaded.
+__device__ __forceinline__ u32 cc_parse_examine(cc_dev* dev, const cc_apply_tabs& T, const u8* log, u64 n, cc_parse_smem* S, u32 nthr,
+                                                bool have_h, uint4 pre_h, bool have_pl, uint4 pre_pl) {
+    cc_apply_state* A = &dev->apply;
+    const u64 off = S->off;
+    if (n - off < CC_RECORD_HEADER_BYTES) return CC_PA_STOP;                               // torn
+    const uint4 h = have_h ? pre_h : ld_v4(reinterpret_cast<const uint4*>(log + off));
+    if ((u64)h.z > n - off - CC_RECORD_HEADER_BYTES) return CC_PA_STOP;                    // torn
+    if (h.x == CC_COMMIT_ID) {
+        bool ok = (h.y == CC_COMMIT_ID) && (h.z == 16u);
+        uint4 pl = make_uint4(0, 0, 0, 0);
+        if (ok) {
+            pl = have_pl ? pre_pl : ld_v4(reinterpret_cast<const uint4*>(log + off + 16));
+            u32 pay[4] = {pl.x, pl.y, pl.z, pl.w};
+            ok = crc_serial(&dev->crc, reinterpret_cast<const u8*>(pay), 16) == h.w;
+            ok = ok && (pl.w == S->pending) && !S->mixed && (S->pending == 0 || S->pend_rid == pl.z);
+        }
+        if (!ok) { A->struct_fail = 1; return CC_PA_STOP; }
+        if (S->nepochs >= T.max_records) { A->scratch_overflow = 1; return CC_PA_STOP; }
+        if (S->pending != 0) {                   // for the log compactor: last epoch number per region
+            const int cs = cc_parse_find_slot(S, pl.z);
+            if (cs >= 0) dev->compactor.region_epoch[cs] = (u64)pl.x | ((u64)pl.y << 32);
+        }
+        T.epochs[S->nepochs].off_after = off + CC_COMMIT_RECORD_BYTES;
+        T.epochs[S->nepochs].rec_end = S->nrecs;
+        S->nepochs++;
+        S->width = S->pending + 16u < 32u ? 32u : (S->pending + 16u > nthr ? nthr : S->pending + 16u);
+        S->pending = 0; S->mixed = 0;
+        S->off = off + CC_COMMIT_RECORD_BYTES;
+        return CC_PA_NEXT;
+    }
+    const int slot = cc_parse_find_slot(S, h.x);
+    if (slot < 0) { A->struct_fail = 1; return CC_PA_STOP; }
+    if (!cc_parse_len_ok(S, (u32)slot, h.y, h.z)) { A->struct_fail = 1; return CC_PA_STOP; }
+    if (S->pending != 0 && S->pend_rid != h.x) S->mixed = 1;
+    S->pend_rid = h.x;
+    S->slot = (u32)slot;
+    S->first_fail = nthr;
+    S->first_short = nthr + 1;
+    return CC_PA_RUN;
+}
+
+// One block walks the log.  Steady state is ONE step per epoch: every thread speculatively reads the header at its
+// stride position (and, if that is a commit record, the 32 bytes after it); the leading run of full single-page records is accepted; the thread
+// sitting right behind the run usually holds the epoch's commit record -- it validates it from the bytes it
+// already has and examines the first header of the next epoch (also already loaded), so that the next step can
+// start its speculative reads at once.
 __device__ __forceinline__ void cc_apply_parse_phase(cc_dev* dev, const cc_apply_tabs& T, const u8* log, u64 n) {
-    __shared__ u64 s_off;
-    __shared__ u32 s_action, s_slot, s_first_fail, s_nrecs, s_nepochs, s_pending, s_pend_rid, s_mixed, s_segs;
+    __shared__ cc_parse_smem S;
     cc_apply_state* A = &dev->apply;
     const u32 tid = threadIdx.x, nthr = blockDim.x;
     if (tid == 0) {
-        s_off = 0; s_nrecs = 0; s_nepochs = 0; s_pending = 0; s_pend_rid = 0; s_mixed = 0; s_segs = 0;
+        S.off = 0; S.nrecs = 0; S.nepochs = 0; S.pending = 0; S.pend_rid = 0; S.mixed = 0; S.segs = 0; S.pre = 0;
+        S.action = CC_PA_STOP; S.cand = 0xFFFFFFFFu; S.width = nthr < 128u ? nthr : 128u;
         A->struct_fail = 0; A->scratch_overflow = 0; A->first_bad_rec = 0xFFFFFFFFu; A->validate_done = 0;
         A->n_commit_recs = 0; A->n_commit_epochs = 0; A->consumed = 0; A->status = CC_OK; A->final_done = 0;
         A->t_start_ns = globaltimer_ns();
     }
+    if (tid < CC_MAX_REGIONS) {
+        const bool used = dev->region_used[tid] != 0;
+        const cc_region_dev& rg = dev->regions[tid];
+        S.r_id[tid] = used ? rg.region_id : 0u;
+        S.r_P[tid] = used ? rg.page_bytes : 1u;
+        S.r_spp[tid] = used ? rg.spp : 1u;
+        S.r_bytes[tid] = used ? rg.bytes : 0ull;
+        S.r_pages[tid] = used ? rg.n_pages : 0ull;
+    }
     __syncthreads();
     for (;;) {
         if (tid == 0) {
-            u32 action = CC_PA_STOP;
-            const u64 off = s_off;
-            do {
-                if (n - off < CC_RECORD_HEADER_BYTES) break;                               // torn
-                const uint4 h = ld_v4(reinterpret_cast<const uint4*>(log + off));
-                if ((u64)h.z > n - off - CC_RECORD_HEADER_BYTES) break;                    // torn
-                if (h.x == CC_COMMIT_ID) {
-                    bool ok = (h.y == CC_COMMIT_ID) && (h.z == 16u);
-                    uint4 pl = make_uint4(0, 0, 0, 0);
-                    if (ok) {
-                        pl = ld_v4(reinterpret_cast<const uint4*>(log + off + 16));
-                        u32 pay[4] = {pl.x, pl.y, pl.z, pl.w};
-                        ok = crc_serial(&dev->crc, reinterpret_cast<const u8*>(pay), 16) == h.w;
-                        ok = ok && (pl.w == s_pending) && !s_mixed && (s_pending == 0 || s_pend_rid == pl.z);
-                    }
-                    if (!ok) { A->struct_fail = 1; break; }
-                    if (s_nepochs >= T.max_records) { A->scratch_overflow = 1; break; }
-                    if (s_pending != 0) {                   // for the log compactor: last epoch number per region
-                        const int cs = cc_find_slot(dev, pl.z);
-                        if (cs >= 0) dev->compactor.region_epoch[cs] = (u64)pl.x | ((u64)pl.y << 32);
-                    }
-                    T.epochs[s_nepochs].off_after = off + CC_COMMIT_RECORD_BYTES;
-                    T.epochs[s_nepochs].rec_end = s_nrecs;
-                    s_nepochs++;
-                    s_pending = 0; s_mixed = 0;
-                    s_off = off + CC_COMMIT_RECORD_BYTES;
-                    action = CC_PA_NEXT;
-                    break;
-                }
-                const int slot = cc_find_slot(dev, h.x);
-                if (slot < 0) { A->struct_fail = 1; break; }
-                const cc_region_dev& r = dev->regions[slot];
-                if (!cc_rec_len_ok(r, h.y, h.z)) { A->struct_fail = 1; break; }
-                if (s_pending != 0 && s_pend_rid != h.x) s_mixed = 1;
-                s_pend_rid = h.x;
-                s_slot = (u32)slot;
-                s_first_fail = nthr;
-                action = CC_PA_RUN;
-            } while (0);
-            s_action = action;
+            if (!S.pre) S.action = cc_parse_examine(dev, T, log, n, &S, nthr, false, make_uint4(0, 0, 0, 0), false, make_uint4(0, 0, 0, 0));
+            S.pre = 0;
         }
         __syncthreads();
-        const u32 action = s_action;
+        const u32 action = S.action;
         if (action == CC_PA_STOP) break;
         if (action == CC_PA_RUN) {
-            const cc_region_dev& r = dev->regions[s_slot];
-            const u64 P = r.page_bytes;
+            const u32 slot = S.slot, rid = S.r_id[slot], spp = S.r_spp[slot];
+            const u64 P = S.r_P[slot];
             const u64 stride = P + CC_RECORD_HEADER_BYTES;
-            const u64 off_t = s_off + (u64)tid * stride;
-            uint4 h = make_uint4(0, 0, 0, 0);
-            bool ok = (off_t + CC_RECORD_HEADER_BYTES <= n);
-            if (ok) {
-                h = ld_v4(reinterpret_cast<const uint4*>(log + off_t));
-                ok = ((u64)h.z <= n - off_t - CC_RECORD_HEADER_BYTES) && (h.x == r.region_id) && cc_rec_len_ok(r, h.y, h.z);
-            }
+            const u64 off_t = S.off + (u64)tid * stride;
+            const u32 width = S.width;
+            uint4 h = make_uint4(0, 0, 0, 0), pl = h, nx = h;
+            const bool active = tid < width;
+            const bool in_h = active && off_t + 16 <= n, in_pl = active && off_t + 32 <= n, in_nx = active && off_t + 48 <= n;
+            bool ok = in_h;
+            if (in_h) h = ld_v4(reinterpret_cast<const uint4*>(log + off_t));
+            const bool commit_here = in_pl && h.x == CC_COMMIT_ID;      // (normally one thread per step)
+            if (commit_here) pl = ld_v4(reinterpret_cast<const uint4*>(log + off_t + 16));           // the commit record's payload
+            if (commit_here && in_nx) nx = ld_v4(reinterpret_cast<const uint4*>(log + off_t + 32));  // ... and the header after it
+            if (ok) ok = ((u64)h.z <= n - off_t - CC_RECORD_HEADER_BYTES) && (h.x == rid) && cc_parse_len_ok(&S, slot, h.y, h.z);
             // a short (tail) page or a multi-page run record is valid but breaks the stride: it may only END a run
             const bool full = ok && ((u64)h.z == P);
-            if (!ok) atomicMin(&s_first_fail, tid);
-            else if (!full) atomicMin(&s_first_fail, tid + 1);
+            if (active && !ok) atomicMin(&S.first_fail, tid);
+            else if (active && !full) { atomicMin(&S.first_fail, tid + 1); atomicMin(&S.first_short, tid + 1); }
             __syncthreads();
-            u32 run = s_first_fail < nthr ? s_first_fail : nthr;      // >= 1: thread 0 re-checked record 0
-            const u32 base = s_nrecs;
+            const u32 run = S.first_fail < width ? S.first_fail : width;    // >= 1: record 0 was examined before
+            const u32 base = S.nrecs;
             const bool overflow = (u64)base + run > T.max_records;
             if (!overflow && tid < run) {
                 cc_rec rec;
                 rec.off = off_t; rec.page_idx = h.y; rec.len = h.z; rec.crc = h.w;
-                rec.slot = s_slot; rec.epoch_idx = s_nepochs; rec.pad = 0;
+                rec.slot = slot; rec.epoch_idx = S.nepochs; rec.pad = 0;
                 T.recs[base + tid] = rec;
                 T.rec_state[base + tid] = 0;
-                T.seg_begin[base + tid] = s_segs + tid * r.spp;        // only the run's last record can be short
+                T.seg_begin[base + tid] = S.segs + tid * spp;          // only the run's last record can be short
+            }
+            const u32 first_short = S.first_short;
+            __syncthreads();
+            if (!overflow && tid == run - 1) {                         // the run's last record knows where the run ends
+                S.off = off_t + CC_RECORD_HEADER_BYTES + h.z;
+                S.nrecs = base + run;
+                S.pending += run;
+                S.segs += (run - 1) * spp + (h.z + CC_SEG_BYTES - 1) / CC_SEG_BYTES;
+                // the thread right behind the run sits on the next record iff the run ended on a full page
+                S.cand = (run < width && first_short > run) ? run : 0xFFFFFFFFu;
+                if (run == width) S.width = 2 * width > nthr ? nthr : 2 * width;      // the epoch is longer than expected
+            }
+            if (overflow && tid == 0) { A->scratch_overflow = 1; S.action = CC_PA_STOP; S.cand = 0xFFFFFFFFu; }
+            __syncthreads();
+            if (S.action == CC_PA_STOP) break;
+            if (tid == S.cand && in_h && h.x == CC_COMMIT_ID) {
+                // S.off == off_t here.  Commit from the preloaded bytes, then the next epoch's first header.
+                u32 act = cc_parse_examine(dev, T, log, n, &S, nthr, true, h, commit_here, pl);
+                if (act == CC_PA_NEXT) act = cc_parse_examine(dev, T, log, n, &S, nthr, commit_here && in_nx, nx, false, make_uint4(0, 0, 0, 0));
+                if (act != CC_PA_NEXT) { S.action = act; S.pre = 1; }      // NEXT again (an empty epoch): thread 0 goes on
             }
             __syncthreads();
-            if (tid == 0) {
-                if (overflow) { A->scratch_overflow = 1; s_action = CC_PA_STOP; }
-                else {
-                    const cc_rec& last = T.recs[base + run - 1];
-                    s_off = last.off + CC_RECORD_HEADER_BYTES + last.len;
-                    s_nrecs = base + run;
-                    s_pending += run;
-                    s_segs += (run - 1) * r.spp + (last.len + CC_SEG_BYTES - 1) / CC_SEG_BYTES;
-                }
-            }
-            __syncthreads();
-            if (s_action == CC_PA_STOP) break;
         }
     }
     if (tid == 0) {
-        A->n_recs = s_nrecs;
-        A->n_epochs = s_nepochs;
-        T.seg_begin[s_nrecs] = s_segs;          // table has max_records + 1 entries
+        A->n_recs = S.nrecs;
+        A->n_epochs = S.nepochs;
+        T.seg_begin[S.nrecs] = S.segs;          // table has max_records + 1 entries
         __threadfence();
     }
 }
