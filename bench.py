@@ -350,8 +350,8 @@ def run_ours(args):
         scan_ms = statistics.mean(t_scan)
         achieved = 2 * N / (scan_ms * 1e-3) / 1e9
         # dram__bytes_read.sum + dram__bytes_write.sum of cc_scan_kernel on this workload, one launch, from the
-        # ncu --set full capture summarised in profiles/r01_ncu_full.md (17.179931 GB read + 0.003497 GB written)
-        traffic = 17_183_428_000 if args.workload == "c2" else None
+        # ncu --set full capture summarised in profiles/r01_ncu_full.md (17.179897 GB read + 0.003812 GB written)
+        traffic = 17_183_709_000 if args.workload == "c2" else None
         value = world * K * N / (ms_total * 1e-3) / 1e9
         line = {
             "metric": METRIC, "value": round(value, 2), "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,

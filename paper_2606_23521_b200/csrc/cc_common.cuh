@@ -15,7 +15,7 @@ typedef uint64_t u64;
 #define CC_COMPACT_THREADS 256
 #define CC_COMPACT_WORDS_PER_THREAD 4
 #define CC_COMPACT_TILE_WORDS (CC_COMPACT_THREADS * CC_COMPACT_WORDS_PER_THREAD)   // 1024 words = 32768 pages
-#define CC_FUSED_TILE_BYTES (64u * 1024u)    // fused pass: one WARP scans (and gathers) this much of the region per ticket
+#define CC_FUSED_TILE_BYTES (32u * 1024u)    // fused pass: one WARP scans (and gathers) this much of the region per ticket
 #define CC_FUSED_MAX_TP 32u                  // ... but at most this many pages (the tile's dirty mask is one register)
 
 // Per-region control block in the workspace (device memory).
@@ -61,7 +61,7 @@ struct cc_region_dev {
     u64* run_state;     // n_pages u64: per-run {finished pages : 32 | CRC accumulator : 32}, zero between calls
     cc_ws_hdr* hdr2;    // control block of the ranking pass over S
     u64* lb2;           // its look-back status words
-    u32 ftile_pages;    // pages per fused warp tile (~64 KiB of region, 1..32 pages)
+    u32 ftile_pages;    // pages per fused warp tile (~32 KiB of region, 1..32 pages)
     u32 n_ftiles;
     u32* latest;        // n_pages u32: applier last-wins table, all zero between calls
     cc_ws_hdr* hdr;
