@@ -172,6 +172,20 @@ int32_t cc_log_reset(cc_ctx* ctx);
  * drainer calls once it has consumed the committed prefix.  Only while the worker is stopped. */
 int32_t cc_log_reset_async(cc_ctx* ctx, void* stream);
 
+/* Host mirror of a DEVICE-resident log, filled by the copy engine (records are built in a
+ * staging buffer, then "copied to a CXL-backed or DRAM-backed append-only log; a commit marker publishes the epoch
+ * only after all bytes are visible").  With the log attached in device memory a checkpoint appends at HBM speed;
+ * cc_log_drain then copies the newly committed bytes [drained, upto) to the same offsets of `host_log` (pinned host
+ * memory, 16-byte aligned) with cudaMemcpyAsync on `copy_stream` -- ordered after the work already queued on
+ * `after_stream` -- and, once the bytes have landed, release-stores `upto` into *committed_off_host (may be NULL)
+ * from a host callback on that stream.  The copy engine reaches the full link rate and takes no SM; the drain
+ * of one checkpoint overlaps the scan of the next.  `upto` must be a committed offset the caller has read from a
+ * result (cc_result.log_offset_after), non-decreasing between resets.  cc_log_reset rewinds the drain position too;
+ * the caller makes sure the copy stream has drained before it resets or reuses log space.  host_log = NULL detaches.
+ * CC_ERR_LOG_FULL if upto exceeds the mirror's capacity. */
+int32_t cc_log_mirror_attach(cc_ctx* ctx, void* host_log, uint64_t capacity, uint64_t* committed_off_host);
+int32_t cc_log_drain(cc_ctx* ctx, uint64_t upto, void* after_stream, void* copy_stream);
+
 /* ---- host-launched path -------------------------------------------------------------------- */
 
 /* Delta-checkpoint one region: scan live vs shadow per page, compact the

@@ -47,7 +47,7 @@ CC_TASKF_RLE = 2
 
 EXPORTS = [
     "cc_init", "cc_shutdown", "cc_last_cuda_error", "cc_kernel_launches", "cc_workspace_bytes",
-    "cc_register_region", "cc_unregister_region", "cc_log_attach", "cc_log_reset", "cc_log_reset_async",
+    "cc_register_region", "cc_unregister_region", "cc_log_attach", "cc_log_reset", "cc_log_reset_async", "cc_log_mirror_attach", "cc_log_drain",
     "cc_checkpoint_delta", "cc_checkpoint_delta_fused", "cc_checkpoint_delta_rle", "cc_checkpoint_marked", "cc_checkpoint_versions",
     "cc_checkpoint_all", "cc_snapshot_region", "cc_compact_log", "cc_scan_only", "cc_trace_events", "cc_dirty_list", "cc_apply_scratch_bytes", "cc_apply_attach", "cc_apply_stage_attach", "cc_apply_log",
     "cc_worker_start", "cc_worker_stop", "cc_worker_alive", "cc_peek_queue", "cc_submit", "cc_measure_submit_cost", "cc_poll", "cc_wait",
@@ -111,6 +111,8 @@ def load_library():
         "cc_log_attach": (i32, [vp, vp, u64, vp]),
         "cc_log_reset": (i32, [vp]),
         "cc_log_reset_async": (i32, [vp, vp]),
+        "cc_log_mirror_attach": (i32, [vp, vp, u64, vp]),
+        "cc_log_drain": (i32, [vp, u64, vp, vp]),
         "cc_checkpoint_delta": (i32, [vp, u32, u64, vp, vp]),
         "cc_checkpoint_delta_fused": (i32, [vp, u32, u64, vp, vp]),
         "cc_checkpoint_delta_rle": (i32, [vp, u32, u64, u32, vp, vp]),
@@ -189,6 +191,7 @@ class Context:
         self._committed = None
         self._scratch = None
         self._stage = None
+        self._mirror = None
 
     # -- helpers
     def _check(self, call, rc):
@@ -242,6 +245,20 @@ class Context:
             cptr = ctypes.c_void_p(committed_off.data_ptr())
         self._check("cc_log_attach", self.lib.cc_log_attach(self.h, log.data_ptr(), log.numel(), cptr))
         self._log, self._committed = log, committed_off
+
+    def log_mirror_attach(self, host_log: torch.Tensor, committed_off: torch.Tensor = None):
+        """host_log: pinned uint8 tensor mirroring the (device-resident) attached log; None detaches."""
+        if host_log is None:
+            self._check("cc_log_mirror_attach", self.lib.cc_log_mirror_attach(self.h, None, 0, None))
+            self._mirror = None
+            return
+        assert host_log.dtype == torch.uint8 and host_log.is_contiguous() and host_log.is_pinned()
+        cptr = ctypes.c_void_p(committed_off.data_ptr()) if committed_off is not None else None
+        self._check("cc_log_mirror_attach", self.lib.cc_log_mirror_attach(self.h, host_log.data_ptr(), host_log.numel(), cptr))
+        self._mirror = (host_log, committed_off)
+
+    def log_drain(self, upto: int, copy_stream, after_stream=None):
+        self._check("cc_log_drain", self.lib.cc_log_drain(self.h, upto, _stream_ptr(after_stream), _stream_ptr(copy_stream)))
 
     def log_reset(self):
         self._check("cc_log_reset", self.lib.cc_log_reset(self.h))

@@ -158,6 +158,14 @@ struct cc_ctx {
     cc_host_region regions[CC_MAX_REGIONS];
     bool log_attached;
     uint64_t* committed_off;    // the caller's published-offset word (may be null)
+    void* log_buf;              // the attached log (device or pinned host)
+    uint64_t log_capacity;
+    // host mirror of a device-resident log, filled by the copy engine (cc_log_mirror_attach / cc_log_drain)
+    void* mirror;
+    uint64_t mirror_capacity;
+    uint64_t* mirror_committed;
+    uint64_t drained;
+    cudaEvent_t drain_ev;
     cc_apply_tabs tabs;
     bool apply_attached;
     void* stage;                // optional device staging buffer for host-resident logs (cc_apply_stage_attach)
@@ -315,6 +323,7 @@ extern "C" int32_t cc_shutdown(cc_ctx* ctx) {
         if (ctx->internal) cudaStreamDestroy(ctx->internal);
         if (ctx->worker_stream) cudaStreamDestroy(ctx->worker_stream);
         if (ctx->worker_done) cudaEventDestroy(ctx->worker_done);
+        if (ctx->drain_ev) cudaEventDestroy(ctx->drain_ev);
     }
     delete ctx;
     return rc;
@@ -423,6 +432,9 @@ extern "C" int32_t cc_log_attach(cc_ctx* ctx, void* log_buf, uint64_t capacity, 
     CC_CUDA(ctx, cudaStreamSynchronize(0));
     ctx->log_attached = true;
     ctx->committed_off = committed_off;
+    ctx->log_buf = log_buf;
+    ctx->log_capacity = capacity;
+    ctx->drained = 0;
     return CC_OK;
 }
 
@@ -434,6 +446,52 @@ extern "C" int32_t cc_log_reset(cc_ctx* ctx) {
     CC_CUDA(ctx, cudaMemcpyAsync(&ctx->d_dev->log.W, &zero, sizeof(zero), cudaMemcpyHostToDevice, 0));
     if (ctx->committed_off) CC_CUDA(ctx, cudaMemsetAsync(ctx->committed_off, 0, sizeof(u64), 0));     // publish the rewind too
     CC_CUDA(ctx, cudaStreamSynchronize(0));
+    ctx->drained = 0;
+    if (ctx->mirror_committed) __atomic_store_n(ctx->mirror_committed, 0ull, __ATOMIC_RELEASE);
+    return CC_OK;
+}
+
+// ---- host mirror of a device-resident log, drained by the copy engine ----
+
+struct cc_drain_note { uint64_t* word; uint64_t value; };
+static void CUDART_CB cc_drain_publish(void* p) {
+    cc_drain_note* nt = (cc_drain_note*)p;
+    __atomic_store_n(nt->word, nt->value, __ATOMIC_RELEASE);     // after the bytes: stream order + release
+    free(nt);
+}
+
+extern "C" int32_t cc_log_mirror_attach(cc_ctx* ctx, void* host_log, uint64_t capacity, uint64_t* committed_off_host) {
+    if (!ctx || ((uintptr_t)host_log & 15)) return CC_ERR_INVALID;
+    if (ctx->worker_running) return CC_ERR_WORKER;
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    if (host_log && !ctx->drain_ev) CC_CUDA(ctx, cudaEventCreateWithFlags(&ctx->drain_ev, cudaEventDisableTiming));
+    ctx->mirror = host_log;
+    ctx->mirror_capacity = host_log ? capacity : 0;
+    ctx->mirror_committed = host_log ? committed_off_host : nullptr;
+    ctx->drained = 0;
+    if (ctx->mirror_committed) __atomic_store_n(ctx->mirror_committed, 0ull, __ATOMIC_RELEASE);
+    return CC_OK;
+}
+
+extern "C" int32_t cc_log_drain(cc_ctx* ctx, uint64_t upto, void* after_stream, void* copy_stream) {
+    if (!ctx || !ctx->log_attached || !ctx->mirror) return CC_ERR_INVALID;
+    if (upto < ctx->drained || upto > ctx->log_capacity) return CC_ERR_INVALID;
+    if (upto > ctx->mirror_capacity) return CC_ERR_LOG_FULL;
+    if (upto == ctx->drained) return CC_OK;
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t cs = (cudaStream_t)copy_stream;
+    CC_CUDA(ctx, cudaEventRecord(ctx->drain_ev, (cudaStream_t)after_stream));
+    CC_CUDA(ctx, cudaStreamWaitEvent(cs, ctx->drain_ev, 0));
+    CC_CUDA(ctx, cudaMemcpyAsync((u8*)ctx->mirror + ctx->drained, (const u8*)ctx->log_buf + ctx->drained, upto - ctx->drained,
+                                 cudaMemcpyDefault, cs));
+    if (ctx->mirror_committed) {
+        cc_drain_note* nt = (cc_drain_note*)malloc(sizeof(cc_drain_note));
+        if (!nt) return CC_ERR_INVALID;
+        nt->word = ctx->mirror_committed;
+        nt->value = upto;
+        CC_CUDA(ctx, cudaLaunchHostFunc(cs, cc_drain_publish, nt));
+    }
+    ctx->drained = upto;
     return CC_OK;
 }
 

@@ -219,3 +219,67 @@ def test_argument_errors():
     cur[0] ^= 1
     r = gpu_checkpoint(ctx, 1, 1)
     assert r.status == cc.CC_ERR_LOG_FULL and r.n_dirty == 1
+
+
+def test_log_mirror_drain_by_the_copy_engine():
+    """Device log + host mirror: after every epoch the committed bytes are handed to the copy engine; the mirror and its
+    published offset follow the oracle's log; reset rewinds both; argument errors."""
+    P, n_pages = 4096, 600
+    cur = _region(P * n_pages, 21)
+    ctx = cc.Context()
+    sh = ctx.register_region(1, cur, P)
+    cap = 4 << 20
+    log = torch.zeros(cap, dtype=torch.uint8, device="cuda")
+    mirror = torch.zeros(cap, dtype=torch.uint8, pin_memory=True)
+    pub = torch.zeros(1, dtype=torch.int64, pin_memory=True)
+    ctx.log_attach(log)
+    ctx.log_mirror_attach(mirror, pub)
+    copy_stream = torch.cuda.Stream()
+    host_cur = cur.cpu().numpy().copy()
+    host_sh = host_cur.copy()
+    olog = np.zeros(cap, np.uint8)
+    rng = np.random.default_rng(4)
+    res = cc.Result()
+    W = 0
+    for e in range(6):
+        for p in rng.integers(0, n_pages, 20).tolist():
+            off = p * P + int(rng.integers(0, P))
+            host_cur[off] ^= 0x33
+            cur[off] ^= 0x33
+        res.clear()
+        ctx.checkpoint_delta(1, e, res)
+        torch.cuda.current_stream().synchronize()
+        r = res.read()
+        st, D, nb, W = oracle.checkpoint(host_cur, host_sh, P, 1, e, olog, W)
+        assert (r.status, r.n_dirty, r.log_offset_after) == (st, D.size, W)
+        ctx.log_drain(r.log_offset_after, copy_stream)
+        if e == 2:
+            ctx.log_drain(r.log_offset_after, copy_stream)          # nothing new: a no-op
+    copy_stream.synchronize()
+    assert int(pub.item()) == W and np.array_equal(mirror.numpy()[:W], olog[:W]) and not mirror[W:].any()
+    with pytest.raises(cc.ConcordiaError):
+        ctx.log_drain(W - 16, copy_stream)                           # going backwards
+    with pytest.raises(cc.ConcordiaError):
+        ctx.log_drain(cap + 16, copy_stream)                         # beyond the log
+    ctx.log_reset()
+    assert int(pub.item()) == 0
+    cur[7] ^= 1
+    host_cur[7] ^= 1
+    res.clear()
+    ctx.checkpoint_delta(1, 9, res)
+    torch.cuda.current_stream().synchronize()
+    r = res.read()
+    st, D, nb, W = oracle.checkpoint(host_cur, host_sh, P, 1, 9, olog, 0)
+    ctx.log_drain(r.log_offset_after, copy_stream)
+    copy_stream.synchronize()
+    assert int(pub.item()) == W == 16 + P + 32 and np.array_equal(mirror.numpy()[:W], olog[:W])
+    # a mirror smaller than the committed prefix
+    small = torch.zeros(W - 16, dtype=torch.uint8, pin_memory=True)
+    ctx.log_mirror_attach(small)
+    with pytest.raises(cc.ConcordiaError) as ei:
+        ctx.log_drain(W, copy_stream)
+    assert ei.value.code == cc.CC_ERR_LOG_FULL
+    ctx.log_mirror_attach(None)
+    with pytest.raises(cc.ConcordiaError):
+        ctx.log_drain(W, copy_stream)
+    ctx.shutdown()
