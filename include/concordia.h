@@ -12,6 +12,11 @@
  *   - recovery applier                 PAPER.md:L156-158 (TASK_RESTORE), L227, L445
  *   - ring buffer + persistent worker  PAPER.md:L119, L125-160 (listings), L247-249 (host-mapped
  *                                      memory, release/acquire), Table 1 L166-175 (host API)
+ *   - allocator-aware discovery        PAPER.md:L217, L257, L261, L264, L266 (dirty bitmaps / version counters)
+ *   - run-length records               PAPER.md:L221 ("contiguous dirty ranges use run-length encoding")
+ *   - base snapshot + log compactor
+ *   - all regions at one boundary      PAPER.md:L259 ("at each NCCL or kernel boundary")
+ *   - staging buffer -> host log       PAPER.md:L262-263 (cc_log_mirror_attach / cc_log_drain)
  *
  * Conventions
  *   - Plain C, no exceptions across the boundary.  Every call returns an int32_t status:

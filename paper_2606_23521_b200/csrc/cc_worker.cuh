@@ -179,7 +179,7 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
                 status = CC_ERR_INVALID;
             if (task.kind == CC_TASK_MARKED_CKPT && (task.arg0 == 0 || (task.arg0 & 3))) status = CC_ERR_INVALID;
             if (slot >= 0 && task.kind == CC_TASK_DELTA_CKPT && (task.flags & CC_TASKF_RLE) &&
-                (task.arg0 == 0 || task.arg0 * dev->regions[slot].page_bytes > 0xFFFFFFFFull))
+                (task.arg0 == 0 || task.arg0 > 0xFFFFFFFFull / dev->regions[slot].page_bytes))
                 status = CC_ERR_INVALID;
             if (task.kind == CC_TASK_VERSION_CKPT && (task.arg0 == 0 || task.arg1 == 0 || ((task.arg0 | task.arg1) & 7)))
                 status = CC_ERR_INVALID;
