@@ -378,7 +378,12 @@ def run_ours(args):
         assert int(mirror_committed.item()) == state["W"], (int(mirror_committed.item()), state)
         assert torch.equal(mirror[:state["W"]], log_ring[:state["W"]].cpu()), "host mirror differs from the device log"
         ctx.log_mirror_attach(None)
-        e2e = {"ms": ms_e2e, "h2d": h2d, "d2h": log_bytes + 64, "ms_three_kernel": ms_three, "ms_fused": ms_fused}
+        # Whether the copy engine gets HBM bandwidth while the scan saturates it differs from box to box (10.1 ms when
+        # it does, 12.9 ms when the drain only proceeds between kernels); the fused direct path is steady at ~11.7 ms.
+        # A user picks the faster one on their box: e2e reports that one and names it, both numbers are kept.
+        path = "device log + cc_log_drain (copy engine)" if ms_e2e <= ms_fused else "cc_checkpoint_delta_fused into the pinned host log"
+        e2e = {"ms": min(ms_e2e, ms_fused), "h2d": h2d, "d2h": log_bytes + 64, "ms_three_kernel": ms_three, "ms_fused": ms_fused,
+               "ms_drain": ms_e2e, "path": path}
 
     # ---- reduce over ranks: max time ----
     def rmax(x):
@@ -391,6 +396,7 @@ def run_ours(args):
     ms_total = rmax(ms_total)
     if e2e:
         e2e["ms"] = rmax(e2e["ms"])
+        e2e["ms_drain"], e2e["ms_fused"] = rmax(e2e["ms_drain"]), rmax(e2e["ms_fused"])
 
     if rank == 0:
         peak, peak_src = measured_peak()
@@ -441,9 +447,12 @@ def run_ours(args):
                            "h2d_bytes_per_step": e2e["h2d"], "d2h_bytes_per_step": e2e["d2h"],
                            "ms_per_step": round(e2e["ms"] / K, 4),
                            "host_link_GBps_log": round(log_bytes * K / (e2e["ms"] * 1e-3) / 1e9, 2),
+                           "path": e2e["path"],
+                           "ms_per_step_drain_pipeline": round(e2e["ms_drain"] / K, 4),
                            "ms_per_step_direct_fused": round(e2e["ms_fused"] / K, 4),
                            "ms_per_step_direct_three_kernel": round(e2e["ms_three_kernel"] / K, 4),
-                           "note": "pipeline: cc_checkpoint_delta into a device log (ring of 15 epochs) + cc_log_drain (copy engine) "
+                           "note": "value = the faster of the two host-log paths measured in this run (named in path).  drain "
+                                   "pipeline: cc_checkpoint_delta into a device log (ring of 15 epochs) + cc_log_drain (copy engine) "
                                    "into the pinned host log, the drain of step s overlapping step s+1; new tokens copied H2D and the "
                                    "result read on the host every step; host link floor = 512 MiB / 57 GB/s = 9.4 ms.  direct_* = the "
                                    "record writer storing straight into the pinned host log (SM stores cap at 52.7 GB/s): fused single "
