@@ -482,8 +482,13 @@ extern "C" int32_t cc_log_drain(cc_ctx* ctx, uint64_t upto, void* after_stream, 
     cudaStream_t cs = (cudaStream_t)copy_stream;
     CC_CUDA(ctx, cudaEventRecord(ctx->drain_ev, (cudaStream_t)after_stream));
     CC_CUDA(ctx, cudaStreamWaitEvent(cs, ctx->drain_ev, 0));
-    CC_CUDA(ctx, cudaMemcpyAsync((u8*)ctx->mirror + ctx->drained, (const u8*)ctx->log_buf + ctx->drained, upto - ctx->drained,
-                                 cudaMemcpyDefault, cs));
+    // In pieces: a copy engine serves its queue one command at a time, and another stream's small copy that lands on the
+    // same engine (the application's own H2D / D2H traffic) would otherwise wait behind the whole drain.
+    const uint64_t piece = 16ull << 20;
+    for (uint64_t o = ctx->drained; o < upto; o += piece) {
+        const uint64_t nb = upto - o < piece ? upto - o : piece;
+        CC_CUDA(ctx, cudaMemcpyAsync((u8*)ctx->mirror + o, (const u8*)ctx->log_buf + o, nb, cudaMemcpyDefault, cs));
+    }
     if (ctx->mirror_committed) {
         cc_drain_note* nt = (cc_drain_note*)malloc(sizeof(cc_drain_note));
         if (!nt) return CC_ERR_INVALID;
