@@ -7,7 +7,6 @@ GPU (so that the symbol table can be checked), but creating a Context without th
 without a CUDA device raises.
 """
 import ctypes
-import os
 
 import torch
 

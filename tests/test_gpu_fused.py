@@ -8,7 +8,7 @@ import torch
 import oracle
 import synth
 import paper_2606_23521_b200 as cc
-from gpu_util import check_checkpoint_parity, gpu_checkpoint
+from gpu_util import check_checkpoint_parity
 
 pytestmark = pytest.mark.gpu
 

@@ -1,5 +1,4 @@
 """Pins for the checkpoint oracle (-m "not gpu"): worked examples, brute force, invariants."""
-import itertools
 import os
 import struct
 
