@@ -338,6 +338,10 @@ int32_t cc_submit(cc_ctx* ctx, const cc_task* task, uint64_t* seq_out);
  * so that no language binding is in the way (Table 7).  Waits for free slots outside the timed
  * sections and for the last task before returning.  Needs a running worker. */
 int32_t cc_measure_submit_cost(cc_ctx* ctx, uint32_t n, double* ns_per_submit);
+/* Measurement hook for the comparison with PAPER.md Table 7 (L368-370): mean ns per launch of an empty kernel on
+ * `stream`, with a synchronisation after every launch (*ns_sync) and launched back to back with one synchronisation
+ * at the end (*ns_batched).  Not while a worker occupies every SM. */
+int32_t cc_measure_launch_cost(cc_ctx* ctx, uint32_t n, void* stream, double* ns_sync, double* ns_batched);
 /* CC_OK and *out filled when task `seq` has completed; CC_PENDING otherwise.  A completion slot
  * is reused `capacity` submissions later: poll before then. */
 int32_t cc_poll(cc_ctx* ctx, uint64_t seq, cc_result* out);

@@ -49,7 +49,7 @@ EXPORTS = [
     "cc_register_region", "cc_unregister_region", "cc_log_attach", "cc_log_reset", "cc_log_reset_async", "cc_log_mirror_attach", "cc_log_drain",
     "cc_checkpoint_delta", "cc_checkpoint_delta_fused", "cc_checkpoint_delta_rle", "cc_checkpoint_marked", "cc_checkpoint_versions",
     "cc_checkpoint_all", "cc_snapshot_region", "cc_compact_log", "cc_scan_only", "cc_trace_events", "cc_dirty_list", "cc_apply_scratch_bytes", "cc_apply_attach", "cc_apply_stage_attach", "cc_apply_log",
-    "cc_worker_start", "cc_worker_stop", "cc_worker_alive", "cc_peek_queue", "cc_submit", "cc_measure_submit_cost", "cc_poll", "cc_wait",
+    "cc_worker_start", "cc_worker_stop", "cc_worker_alive", "cc_peek_queue", "cc_submit", "cc_measure_submit_cost", "cc_measure_launch_cost", "cc_poll", "cc_wait",
 ]
 
 
@@ -133,6 +133,7 @@ def load_library():
         "cc_peek_queue": (i32, [vp, P(u64), P(u64)]),
         "cc_submit": (i32, [vp, P(cc_task), P(u64)]),
         "cc_measure_submit_cost": (i32, [vp, u32, P(ctypes.c_double)]),
+        "cc_measure_launch_cost": (i32, [vp, u32, vp, P(ctypes.c_double), P(ctypes.c_double)]),
         "cc_poll": (i32, [vp, u64, P(cc_result)]),
         "cc_wait": (i32, [vp, u64, u64, P(cc_result)]),
     }
@@ -389,6 +390,12 @@ class Context:
         v = ctypes.c_double()
         self._check("cc_measure_submit_cost", self.lib.cc_measure_submit_cost(self.h, n, ctypes.byref(v)))
         return v.value
+
+    def measure_launch_cost(self, n: int = 2000, stream=None):
+        """(ns per empty-kernel launch with a sync each, ns per launch when batched) -- PAPER.md Table 7."""
+        a, b = ctypes.c_double(), ctypes.c_double()
+        self._check("cc_measure_launch_cost", self.lib.cc_measure_launch_cost(self.h, n, _stream_ptr(stream), ctypes.byref(a), ctypes.byref(b)))
+        return a.value, b.value
 
     def poll(self, seq: int):
         r = cc_result()

@@ -878,6 +878,31 @@ extern "C" int32_t cc_submit(cc_ctx* ctx, const cc_task* task, uint64_t* seq_out
     return CC_OK;
 }
 
+__global__ void cc_empty_kernel() {}
+
+// Measurement hook for the comparison of PAPER.md Table 7 (L368-370: cudaLaunchKernel 7.6 us with a sync per launch,
+// 2.5 us batched): mean ns per launch of an empty kernel on `stream`, (a) synchronising after every launch and
+// (b) launching n back to back and synchronising once.  Must not be called while the worker is resident on every SM.
+extern "C" int32_t cc_measure_launch_cost(cc_ctx* ctx, uint32_t n, void* stream, double* ns_sync, double* ns_batched) {
+    if (!ctx || n == 0 || !ns_sync || !ns_batched) return CC_ERR_INVALID;
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    for (int i = 0; i < 16; i++) cc_empty_kernel<<<1, 32, 0, st>>>();
+    CC_CUDA(ctx, cudaStreamSynchronize(st));
+    u64 t0 = now_ns();
+    for (uint32_t i = 0; i < n; i++) {
+        cc_empty_kernel<<<1, 32, 0, st>>>();
+        CC_CUDA(ctx, cudaStreamSynchronize(st));
+    }
+    *ns_sync = (double)(now_ns() - t0) / n;
+    t0 = now_ns();
+    for (uint32_t i = 0; i < n; i++) cc_empty_kernel<<<1, 32, 0, st>>>();
+    CC_CUDA(ctx, cudaStreamSynchronize(st));
+    *ns_batched = (double)(now_ns() - t0) / n;
+    ctx->launches += 2ull * n + 16;
+    return CC_OK;
+}
+
 // Measurement hook: the host cost of cc_submit itself, without a language binding in the way (PAPER.md:L162,
 // Table 7 "ring submit < 0.1 us").  Submits n CC_TASK_NOP tasks; only the cc_submit calls are inside the timed
 // sections (when the ring is full the wait for a free slot is not).  Returns the mean ns per cc_submit.

@@ -66,6 +66,7 @@ def main():
         host_launched.append(time.perf_counter_ns() - t0)
         ctx.log_reset()
     assert res.read().n_dirty == n_mut
+    launch_sync_ns, launch_batched_ns = ctx.measure_launch_cost(2000)
 
     ctx.worker_start()
     out = {}
@@ -124,6 +125,7 @@ def main():
             "checkpoint_task_device_us": {"p50": us(dev_ns, 0.5), "p99": us(dev_ns, 0.99)},
             "fused_checkpoint_task_round_trip_us": {"p50": us(rt_f, 0.5), "p99": us(rt_f, 0.99)},
             "fused_checkpoint_task_device_us": {"p50": us(dev_f, 0.5), "p99": us(dev_f, 0.99)},
+            "empty_kernel_launch_us": {"sync_each": round(launch_sync_ns / 1e3, 2), "batched": round(launch_batched_ns / 1e3, 2)},
             "host_launched_checkpoint_us": {"p50": us(host_launched, 0.5), "p99": us(host_launched, 0.99)},
             "paper_context": "Table 7 (RTX PRO 6000): ring submit < 0.1 us, cudaLaunchKernel 7.6 us sync / 2.5 us batch; "
                              "round trip ~80 us for a trivial op (L307)",
