@@ -162,3 +162,23 @@ def test_worker_lifetime_watchdog():
     assert not ctx.worker_alive()
     ctx.worker_stop()
     ctx.shutdown()
+
+
+def test_measurement_hooks():
+    """cc_measure_submit_cost / cc_measure_launch_cost return sane numbers and leave the ring consistent."""
+    ctx, cur, sh, log, committed = _mk(cap=16)
+    with pytest.raises(cc.ConcordiaError):
+        ctx.measure_submit_cost(10)                     # needs a running worker
+    a, b = ctx.measure_launch_cost(200)
+    assert 0 < b <= a < 1e6                             # batched launches are cheaper than launch + sync
+    ctx.worker_start()
+    try:
+        ns = ctx.measure_submit_cost(5000)              # many more than the ring holds
+        assert 0 < ns < 20000
+        h, t = ctx.peek_queue()
+        assert h == t == 5000
+        s = ctx.submit(cc.CC_TASK_NOP)
+        assert ctx.wait(s, 10.0).status == 0 and s == 5000
+    finally:
+        ctx.worker_stop()
+    ctx.shutdown()
