@@ -328,6 +328,10 @@ int32_t cc_worker_start(cc_ctx* ctx);
 int32_t cc_worker_stop(cc_ctx* ctx);
 /* Table 1 worker_alive(): 1 if the worker runs and its heartbeat advanced within 1 s, else 0. */
 int32_t cc_worker_alive(cc_ctx* ctx);
+/* Footprint of the persistent worker (Table 9): CTAs, threads per CTA, shared memory per CTA, registers
+ * per thread, SMs of the device.  Any output pointer may be NULL. */
+int32_t cc_worker_footprint(cc_ctx* ctx, uint32_t* blocks, uint32_t* threads, uint32_t* smem_bytes, uint32_t* regs,
+                            uint32_t* sm_count);
 /* Table 1 peek_queue(): head = tasks completed, tail = tasks submitted. */
 int32_t cc_peek_queue(cc_ctx* ctx, uint64_t* head, uint64_t* tail);
 /* Copy *task into the next ring slot and publish it with a store-release;

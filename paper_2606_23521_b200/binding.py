@@ -49,7 +49,7 @@ EXPORTS = [
     "cc_register_region", "cc_unregister_region", "cc_log_attach", "cc_log_reset", "cc_log_reset_async", "cc_log_mirror_attach", "cc_log_drain",
     "cc_checkpoint_delta", "cc_checkpoint_delta_fused", "cc_checkpoint_delta_rle", "cc_checkpoint_marked", "cc_checkpoint_versions",
     "cc_checkpoint_all", "cc_snapshot_region", "cc_compact_log", "cc_scan_only", "cc_trace_events", "cc_dirty_list", "cc_apply_scratch_bytes", "cc_apply_attach", "cc_apply_stage_attach", "cc_apply_log",
-    "cc_worker_start", "cc_worker_stop", "cc_worker_alive", "cc_peek_queue", "cc_submit", "cc_measure_submit_cost", "cc_measure_launch_cost", "cc_poll", "cc_wait",
+    "cc_worker_start", "cc_worker_stop", "cc_worker_alive", "cc_worker_footprint", "cc_peek_queue", "cc_submit", "cc_measure_submit_cost", "cc_measure_launch_cost", "cc_poll", "cc_wait",
 ]
 
 
@@ -130,6 +130,7 @@ def load_library():
         "cc_worker_start": (i32, [vp]),
         "cc_worker_stop": (i32, [vp]),
         "cc_worker_alive": (i32, [vp]),
+        "cc_worker_footprint": (i32, [vp, P(u32), P(u32), P(u32), P(u32), P(u32)]),
         "cc_peek_queue": (i32, [vp, P(u64), P(u64)]),
         "cc_submit": (i32, [vp, P(cc_task), P(u64)]),
         "cc_measure_submit_cost": (i32, [vp, u32, P(ctypes.c_double)]),
@@ -371,6 +372,13 @@ class Context:
 
     def worker_alive(self) -> bool:
         return self.lib.cc_worker_alive(self.h) == 1
+
+    def worker_footprint(self) -> dict:
+        v = [ctypes.c_uint32() for _ in range(5)]
+        self._check("cc_worker_footprint", self.lib.cc_worker_footprint(self.h, *[ctypes.byref(x) for x in v]))
+        b, t, sm, rg, sms = [x.value for x in v]
+        return {"blocks": b, "threads_per_block": t, "smem_bytes_per_block": sm, "registers_per_thread": rg, "sm_count": sms,
+                "sm_share_pct": round(100.0 * min(b, sms) / sms, 2)}
 
     def peek_queue(self):
         h, t = ctypes.c_uint64(), ctypes.c_uint64()

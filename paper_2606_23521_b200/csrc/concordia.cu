@@ -975,6 +975,30 @@ extern "C" int32_t cc_worker_alive(cc_ctx* ctx) {
     return 0;
 }
 
+// Footprint of the persistent worker (Table 9: "1 block out of 188 SMs = 0.53 % of GPU resources"):
+// CTAs (of the running worker, else what cc_worker_start would launch), threads per CTA, shared memory per CTA
+// (static + dynamic), registers per thread, SMs of the device.
+extern "C" int32_t cc_worker_footprint(cc_ctx* ctx, uint32_t* blocks, uint32_t* threads, uint32_t* smem_bytes, uint32_t* regs,
+                                       uint32_t* sm_count) {
+    if (!ctx) return CC_ERR_INVALID;
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    cudaFuncAttributes fa;
+    CC_CUDA(ctx, cudaFuncGetAttributes(&fa, cc_worker_kernel));
+    const int th = (int)ctx->cfg.worker_threads;
+    uint32_t b = ctx->worker_blocks_used;
+    if (!ctx->worker_running) {
+        int bps = 0;
+        CC_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, cc_worker_kernel, th, sizeof(cc_crc_smem)));
+        b = ctx->cfg.worker_blocks ? ctx->cfg.worker_blocks : (uint32_t)(bps * ctx->sm_count);
+    }
+    if (blocks) *blocks = b;
+    if (threads) *threads = (uint32_t)th;
+    if (smem_bytes) *smem_bytes = (uint32_t)(fa.sharedSizeBytes + sizeof(cc_crc_smem));
+    if (regs) *regs = (uint32_t)fa.numRegs;
+    if (sm_count) *sm_count = (uint32_t)ctx->sm_count;
+    return CC_OK;
+}
+
 extern "C" int32_t cc_worker_stop(cc_ctx* ctx) {
     if (!ctx) return CC_ERR_INVALID;
     if (!ctx->worker_running) return CC_ERR_WORKER;

@@ -85,6 +85,7 @@ def main():
             submit_ns.append(t1 - t0)
             nop_rt.append(t2 - t0)
         native_submit_ns = ctx.measure_submit_cost(200000)
+        footprint = ctx.worker_footprint()
         # (iii) + (iv): mutate -> checkpoint tasks, as three-phase tasks and as fused single-pass tasks
         def ckpt_tasks(flags):
             rt, dev_ns, ks = [], [], []
@@ -118,6 +119,7 @@ def main():
             "config": {"region_MiB": a.region_mib, "page_bytes": P, "dirty_pages_per_task": n_mut, "tasks": a.tasks,
                        "log": "device" if a.device_log else "pinned host", "bytes_per_task": per,
                        "path": "fused single pass" if a.fused else "scan + compact + gather"},
+            "worker_footprint": footprint,
             "submit_host_cost_us": {"p50": us(submit_ns, 0.5), "p99": us(submit_ns, 0.99), "through": "ctypes"},
             "submit_host_cost_native_ns": round(native_submit_ns, 1),
             "nop_round_trip_us": {"p50": us(nop_rt, 0.5), "p99": us(nop_rt, 0.99)},
