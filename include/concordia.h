@@ -123,8 +123,7 @@ typedef struct {
 #define CC_TASK_DELTA_CKPT 1u      /* region_id, epoch */
 #define CC_TASK_RESTORE 2u         /* arg0 = log pointer, arg1 = nbytes */
 #define CC_TASK_LOG_RESET 3u       /* W := 0 */
-#define CC_TASK_TEST_MUTATE 4u     /* bench/test only: region_id; arg0 = n_mut, arg1 = A (odd), arg2 = h:
-                                      for j < n_mut: page (j*A + h) mod n_pages, byte (h + j) mod len_p, ^= 0x5A */
+/* kind 4 is CC_TASK_TEST_MUTATE, a bench / test hook (end of this header) */
 #define CC_TASK_MARKED_CKPT 5u     /* region_id, epoch; arg0 = dirty bitmap (device), arg1 = CC_MARK_* flags */
 #define CC_TASK_VERSION_CKPT 6u    /* region_id, epoch; arg0 = version[] (device), arg1 = committed[] (device) */
 #define CC_TASK_SNAPSHOT 7u        /* region_id, epoch: base snapshot (cc_snapshot_region) */
@@ -287,11 +286,6 @@ int32_t cc_compact_log(cc_ctx* ctx, const void* in_log, uint64_t in_bytes, void*
  * leaves the shadow alone.  out->n_dirty = k. */
 int32_t cc_scan_only(cc_ctx* ctx, uint32_t region_id, void* stream, cc_result* out);
 
-/* Measurement hook: if non-NULL, the next host-launched cc_checkpoint_delta / cc_scan_only calls
- * record these cudaEvent_t (passed as void*) on the call's stream right after the scan kernel and
- * right after the compaction kernel.  Pass NULLs to switch it off.  No effect on results. */
-int32_t cc_trace_events(cc_ctx* ctx, void* ev_after_scan, void* ev_after_compact);
-
 /* Device pointer to the u32 ascending dirty page list of the region's last scan and to its
  * u32 count (valid after the stream reached the end of that call). */
 int32_t cc_dirty_list(cc_ctx* ctx, uint32_t region_id, const uint32_t** d_list, const uint32_t** d_count);
@@ -338,19 +332,37 @@ int32_t cc_peek_queue(cc_ctx* ctx, uint64_t* head, uint64_t* tail);
  * no CUDA call.  Non-blocking: CC_ERR_RING_FULL when `capacity` tasks are outstanding.
  * *seq_out (may be NULL) = the sequence number to poll / wait on. */
 int32_t cc_submit(cc_ctx* ctx, const cc_task* task, uint64_t* seq_out);
-/* Measurement hook: mean host cost of one cc_submit in ns over n CC_TASK_NOP submissions, timed inside the library
- * so that no language binding is in the way (Table 7).  Waits for free slots outside the timed
- * sections and for the last task before returning.  Needs a running worker. */
-int32_t cc_measure_submit_cost(cc_ctx* ctx, uint32_t n, double* ns_per_submit);
-/* Measurement hook for the comparison with PAPER.md Table 7 (L368-370): mean ns per launch of an empty kernel on
- * `stream`, with a synchronisation after every launch (*ns_sync) and launched back to back with one synchronisation
- * at the end (*ns_batched).  Not while a worker occupies every SM. */
-int32_t cc_measure_launch_cost(cc_ctx* ctx, uint32_t n, void* stream, double* ns_sync, double* ns_batched);
 /* CC_OK and *out filled when task `seq` has completed; CC_PENDING otherwise.  A completion slot
  * is reused `capacity` submissions later: poll before then. */
 int32_t cc_poll(cc_ctx* ctx, uint64_t seq, cc_result* out);
 /* Spin (host) until done or timeout_ns elapsed (CC_ERR_TIMEOUT). */
 int32_t cc_wait(cc_ctx* ctx, uint64_t seq, uint64_t timeout_ns, cc_result* out);
+
+/* ============================ BENCH / TEST HOOKS -- not part of the product API ============================
+ * Measurement and test instrumentation used by bench.py and tests/ only.  They change no result.  Compiled in by
+ * default; build with -DCC_BENCH_HOOKS=0 for a library without them (the worker then answers CC_TASK_TEST_MUTATE
+ * with CC_ERR_INVALID). */
+#ifndef CC_BENCH_HOOKS
+#define CC_BENCH_HOOKS 1
+#endif
+#if CC_BENCH_HOOKS
+/* cc_task.kind 4 -- mutate a region from inside the worker, in closed form so that the oracle side can replay it
+ * (SURVEY.md 8d C5b): region_id; arg0 = n_mut, arg1 = A (odd), arg2 = h:
+ * for j < n_mut: page (j*A + h) mod n_pages, byte (h + j) mod len_p, ^= 0x5A */
+#define CC_TASK_TEST_MUTATE 4u
+/* If non-NULL, the next host-launched checkpoint / cc_scan_only calls record these cudaEvent_t (passed as void*) on
+ * the call's stream right after the discovery (scan) kernel and right after the compaction kernel: per-phase CUDA
+ * event timing for bench.py's roofline line.  Pass NULLs to switch it off. */
+int32_t cc_trace_events(cc_ctx* ctx, void* ev_after_scan, void* ev_after_compact);
+/* Mean host cost of one cc_submit in ns over n CC_TASK_NOP submissions, timed inside the library so that no language
+ * binding is in the way (Table 7).  Waits for free slots outside the timed sections and for the last
+ * task before returning.  Needs a running worker. */
+int32_t cc_measure_submit_cost(cc_ctx* ctx, uint32_t n, double* ns_per_submit);
+/* For the comparison with PAPER.md Table 7 (L368-370): mean ns per launch of an empty kernel on `stream`, with a
+ * synchronisation after every launch (*ns_sync) and launched back to back with one synchronisation at the end
+ * (*ns_batched).  Not while a worker occupies every SM. */
+int32_t cc_measure_launch_cost(cc_ctx* ctx, uint32_t n, void* stream, double* ns_sync, double* ns_batched);
+#endif /* CC_BENCH_HOOKS */
 
 #ifdef __cplusplus
 }

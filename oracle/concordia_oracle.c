@@ -586,8 +586,10 @@ int32_t orc_compact_log(const uint8_t *log, uint64_t n, const orc_region *region
             }
             if (!ok) { status = ORC_ERR_CORRUPT; break; }
             if (pend_n == pend_cap) {
+                uint64_t *grown = (uint64_t *)realloc(pend, 2 * pend_cap * sizeof(uint64_t));
+                if (!grown) { status = ORC_ERR_INVALID; break; }     /* out of host memory: report, do not crash */
+                pend = grown;
                 pend_cap *= 2;
-                pend = (uint64_t *)realloc(pend, pend_cap * sizeof(uint64_t));
             }
             pend[pend_n++] = off;
             off += ORC_HDR + len;

@@ -31,23 +31,5 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
-PROBES = ["link_probe.cu", "scan_probe.cu"]        # standalone measurement programs (profiles/r01_*_probe.md)
-
-
-def build_probes(force: bool = False) -> list:
-    """Compile the standalone measurement programs into paper_2606_23521_b200/bin/ (git-ignored)."""
-    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    out_dir = os.path.join(_HERE, "bin")
-    os.makedirs(out_dir, exist_ok=True)
-    outs = []
-    for src in PROBES:
-        s = os.path.join(CSRC, src)
-        o = os.path.join(out_dir, src[:-3])
-        if force or not os.path.exists(o) or os.path.getmtime(o) < os.path.getmtime(s):
-            subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-o", o, s], check=True)
-        outs.append(o)
-    return outs
-
-
 if __name__ == "__main__":
     print(build(force=True, verbose=True))

@@ -160,10 +160,23 @@ struct cc_dev {
 
 // ------------------------------------------------------------------ PTX helpers --
 
+// Streaming 16-byte load of region / shadow bytes.  COHERENT (no .nc): the same device code runs inside the
+// persistent worker, where base and shadow are rewritten by earlier tasks (gather, restore, the application's
+// kernels) while the kernel stays resident -- PTX allows .nc only for data that is read-only for the kernel's
+// whole lifetime.  L1::no_allocate keeps the stream out of L1 either way.  -DCC_LD_NC=1 builds the
+// non-coherent variant for an A/B measurement (profiles/r02_ld_nc.md: no bandwidth difference).
+#ifndef CC_LD_NC
+#define CC_LD_NC 0
+#endif
 __device__ __forceinline__ uint4 ld_stream(const uint4* p) {
     uint4 r;
+#if CC_LD_NC
     asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
                  : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+#else
+    asm volatile("ld.global.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+#endif
     return r;
 }
 // Plain (coherent) 16-byte load: log buffers may live in host memory and may have been

@@ -47,6 +47,7 @@ __device__ __forceinline__ void cc_grid_barrier(cc_dev* dev, u32 nblocks, u32& g
     __syncthreads();
 }
 
+#if CC_BENCH_HOOKS
 __device__ __forceinline__ void cc_task_mutate(const cc_region_dev& r, const cc_task& t, cc_grid g) {
     const u64 n_mut = t.arg0, A = t.arg1, h = t.arg2;
     for (u64 j = (u64)g.block * blockDim.x + threadIdx.x; j < n_mut; j += (u64)g.nblocks * blockDim.x) {
@@ -55,6 +56,9 @@ __device__ __forceinline__ void cc_task_mutate(const cc_region_dev& r, const cc_
         r.base[page * r.page_bytes + off] ^= 0x5A;
     }
 }
+#else
+#define CC_TASK_TEST_MUTATE 4u      // recognised only to be refused
+#endif
 
 #define CC_WORKER_MAX_THREADS 512
 
@@ -184,6 +188,15 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
             if (task.kind == CC_TASK_VERSION_CKPT && (task.arg0 == 0 || task.arg1 == 0 || ((task.arg0 | task.arg1) & 7)))
                 status = CC_ERR_INVALID;
         }
+        // recovery-side tasks: the applier tables must be attached (cc_apply_attach before cc_worker_start) and the
+        // log pointers non-null and 16-byte aligned -- same checks as the host-launched cc_apply_log / cc_compact_log
+        if (task.kind == CC_TASK_RESTORE || task.kind == CC_TASK_COMPACT_LOG) {
+            if (tabs.max_records == 0 || task.arg0 == 0 || (task.arg0 & 15)) status = CC_ERR_INVALID;
+            if (task.kind == CC_TASK_COMPACT_LOG) {
+                if (task.arg2 == 0 || (task.arg2 & 15)) status = CC_ERR_INVALID;
+                else if (task.arg0 < task.arg2 + task.arg3 && task.arg2 < task.arg0 + task.arg1) status = CC_ERR_INVALID;   // overlap
+            }
+        }
         if (status == CC_OK) {
             switch (task.kind) {
             case CC_TASK_DELTA_CKPT: {
@@ -269,7 +282,11 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
                 cc_worker_restore_task(dev, tabs, cs, task, g, gen);
                 break;
             case CC_TASK_TEST_MUTATE:
+#if CC_BENCH_HOOKS
                 cc_task_mutate(dev->regions[slot], task, g);
+#else
+                status = CC_ERR_INVALID;
+#endif
                 break;
             default:
                 break;

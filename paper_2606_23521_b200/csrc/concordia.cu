@@ -178,6 +178,7 @@ struct cc_ctx {
     cc_result* ring_results;
     u64* ring_words;            // [0] tail, [8] completed, [16] heartbeat (one cache line apart)
     u64 submitted;
+    std::atomic<uint32_t> in_submit;   // single-producer guard of cc_submit
     bool worker_running;
     cudaStream_t worker_stream;
     cudaEvent_t worker_done;
@@ -195,6 +196,13 @@ struct cc_ctx {
     } while (0)
 
 static const u8* stage_log(cc_ctx* ctx, const void* log, uint64_t nbytes, cudaStream_t st);
+
+// The host-launched data-path calls share the per-region control blocks, the log write offset and the applier
+// tables with the resident worker: while it runs they are refused (submit the matching task instead).
+#define CC_NO_WORKER(ctx)                                      \
+    do {                                                       \
+        if ((ctx)->worker_running) return CC_ERR_WORKER;       \
+    } while (0)
 
 static inline uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
 
@@ -245,9 +253,8 @@ static bool ws_layout(uint64_t bytes, uint32_t P, cc_ws_layout* L) {
 extern "C" int32_t cc_init(cc_ctx** out, int32_t device, const cc_config* cfg) {
     if (!out) return CC_ERR_INVALID;
     *out = nullptr;
-    cc_ctx* ctx = new (std::nothrow) cc_ctx();
+    cc_ctx* ctx = new (std::nothrow) cc_ctx();       // value-initialised: every field zero
     if (!ctx) return CC_ERR_INVALID;
-    memset(ctx, 0, sizeof(*ctx));
     ctx->device = device;
     if (cfg) ctx->cfg = *cfg;
     if (ctx->cfg.ring_capacity == 0) ctx->cfg.ring_capacity = 256;
@@ -315,6 +322,7 @@ extern "C" int32_t cc_shutdown(cc_ctx* ctx) {
     cudaSetDevice(ctx->device);
     int32_t rc = CC_OK;
     if (ctx->worker_running) rc = cc_worker_stop(ctx);
+    if (rc == CC_ERR_TIMEOUT) return rc;    // the kernel may still be resident and reads *ctx's ring: leak rather than free under it
     if (rc == CC_OK) {   // never free under a resident kernel
         if (ctx->d_dev) cudaFree(ctx->d_dev);
         if (ctx->ring_slots) cudaFreeHost(ctx->ring_slots);
@@ -494,7 +502,8 @@ extern "C" int32_t cc_log_drain(cc_ctx* ctx, uint64_t upto, void* after_stream, 
         if (!nt) return CC_ERR_INVALID;
         nt->word = ctx->mirror_committed;
         nt->value = upto;
-        CC_CUDA(ctx, cudaLaunchHostFunc(cs, cc_drain_publish, nt));
+        const cudaError_t e = cudaLaunchHostFunc(cs, cc_drain_publish, nt);
+        if (e != cudaSuccess) { free(nt); ctx->last_cuda = (int)e; return CC_ERR_CUDA; }
     }
     ctx->drained = upto;
     return CC_OK;
@@ -506,6 +515,17 @@ extern "C" int32_t cc_log_reset_async(cc_ctx* ctx, void* stream) {
     CC_CUDA(ctx, cudaSetDevice(ctx->device));
     CC_CUDA(ctx, cudaMemsetAsync(&ctx->d_dev->log.W, 0, sizeof(u64), (cudaStream_t)stream));
     if (ctx->committed_off) CC_CUDA(ctx, cudaMemsetAsync(ctx->committed_off, 0, sizeof(u64), (cudaStream_t)stream));
+    // the mirror's drain position and published offset rewind with the log: drains issued after this call (in host
+    // order) copy from offset 0 again; the mirror's word is zeroed in stream order, like committed_off
+    ctx->drained = 0;
+    if (ctx->mirror_committed) {
+        cc_drain_note* nt = (cc_drain_note*)malloc(sizeof(cc_drain_note));
+        if (!nt) return CC_ERR_INVALID;
+        nt->word = ctx->mirror_committed;
+        nt->value = 0;
+        const cudaError_t e = cudaLaunchHostFunc((cudaStream_t)stream, cc_drain_publish, nt);
+        if (e != cudaSuccess) { free(nt); ctx->last_cuda = (int)e; return CC_ERR_CUDA; }
+    }
     return CC_OK;
 }
 
@@ -553,6 +573,7 @@ static unsigned small_grid(cc_ctx* ctx, uint64_t items, uint64_t per_block) {
 extern "C" int32_t cc_checkpoint_marked(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, uint32_t* dirty_bitmap,
                                         uint32_t flags, void* stream, cc_result* out) {
     if (!ctx || !dirty_bitmap || ((uintptr_t)dirty_bitmap & 3) || (flags & ~(CC_MARK_VERIFY | CC_MARK_CONSUME))) return CC_ERR_INVALID;
+    CC_NO_WORKER(ctx);
     int slot = find_slot(ctx, region_id);
     if (slot < 0) return CC_ERR_NOT_REGISTERED;
     const cc_region_dev& r = ctx->regions[slot].dev;
@@ -587,6 +608,7 @@ extern "C" int32_t cc_checkpoint_marked(cc_ctx* ctx, uint32_t region_id, uint64_
 extern "C" int32_t cc_checkpoint_versions(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, const uint64_t* version,
                                           uint64_t* committed, void* stream, cc_result* out) {
     if (!ctx || !version || !committed || ((uintptr_t)version & 7) || ((uintptr_t)committed & 7)) return CC_ERR_INVALID;
+    CC_NO_WORKER(ctx);
     int slot = find_slot(ctx, region_id);
     if (slot < 0) return CC_ERR_NOT_REGISTERED;
     const cc_region_dev& r = ctx->regions[slot].dev;
@@ -607,6 +629,7 @@ extern "C" int32_t cc_checkpoint_versions(cc_ctx* ctx, uint32_t region_id, uint6
 
 extern "C" int32_t cc_checkpoint_delta(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out) {
     if (!ctx) return CC_ERR_INVALID;
+    CC_NO_WORKER(ctx);
     int slot = find_slot(ctx, region_id);
     if (slot < 0) return CC_ERR_NOT_REGISTERED;
     if (!ctx->regions[slot].dev.shadow) return CC_ERR_INVALID;
@@ -619,6 +642,7 @@ extern "C" int32_t cc_checkpoint_delta(cc_ctx* ctx, uint32_t region_id, uint64_t
 
 extern "C" int32_t cc_checkpoint_delta_fused(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out) {
     if (!ctx) return CC_ERR_INVALID;
+    CC_NO_WORKER(ctx);
     int slot = find_slot(ctx, region_id);
     if (slot < 0) return CC_ERR_NOT_REGISTERED;
     const cc_region_dev& r = ctx->regions[slot].dev;
@@ -639,6 +663,7 @@ extern "C" int32_t cc_checkpoint_delta_fused(cc_ctx* ctx, uint32_t region_id, ui
 extern "C" int32_t cc_checkpoint_delta_rle(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, uint32_t run_pages, void* stream,
                                            cc_result* out) {
     if (!ctx || run_pages == 0) return CC_ERR_INVALID;
+    CC_NO_WORKER(ctx);
     int slot = find_slot(ctx, region_id);
     if (slot < 0) return CC_ERR_NOT_REGISTERED;
     const cc_region_dev& r = ctx->regions[slot].dev;
@@ -664,6 +689,7 @@ extern "C" int32_t cc_checkpoint_delta_rle(cc_ctx* ctx, uint32_t region_id, uint
 
 extern "C" int32_t cc_checkpoint_all(cc_ctx* ctx, uint64_t epoch, void* stream, cc_result* out) {
     if (!ctx) return CC_ERR_INVALID;
+    CC_NO_WORKER(ctx);
     CC_CUDA(ctx, cudaSetDevice(ctx->device));
     cudaStream_t st = (cudaStream_t)stream;
     cc_batch_scan_kernel<<<(unsigned)(ctx->sm_count * ctx->scan_bps), CC_SCAN_THREADS, 0, st>>>(ctx->d_dev);
@@ -679,6 +705,7 @@ extern "C" int32_t cc_checkpoint_all(cc_ctx* ctx, uint64_t epoch, void* stream, 
 
 extern "C" int32_t cc_snapshot_region(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out) {
     if (!ctx) return CC_ERR_INVALID;
+    CC_NO_WORKER(ctx);
     int slot = find_slot(ctx, region_id);
     if (slot < 0) return CC_ERR_NOT_REGISTERED;
     const cc_region_dev& r = ctx->regions[slot].dev;
@@ -695,6 +722,7 @@ extern "C" int32_t cc_snapshot_region(cc_ctx* ctx, uint32_t region_id, uint64_t 
 extern "C" int32_t cc_compact_log(cc_ctx* ctx, const void* in_log, uint64_t in_bytes, void* out_log, uint64_t out_capacity,
                                   void* stream, cc_result* out) {
     if (!ctx || !in_log || !out_log || ((uintptr_t)in_log & 15) || ((uintptr_t)out_log & 15)) return CC_ERR_INVALID;
+    CC_NO_WORKER(ctx);
     if (!ctx->apply_attached) return CC_ERR_INVALID;
     const uintptr_t a0 = (uintptr_t)in_log, a1 = a0 + in_bytes, b0 = (uintptr_t)out_log, b1 = b0 + out_capacity;
     if (a0 < b1 && b0 < a1) return CC_ERR_INVALID;       // the two logs must not overlap
@@ -716,6 +744,7 @@ extern "C" int32_t cc_compact_log(cc_ctx* ctx, const void* in_log, uint64_t in_b
 
 extern "C" int32_t cc_scan_only(cc_ctx* ctx, uint32_t region_id, void* stream, cc_result* out) {
     if (!ctx) return CC_ERR_INVALID;
+    CC_NO_WORKER(ctx);
     int slot = find_slot(ctx, region_id);
     if (slot < 0) return CC_ERR_NOT_REGISTERED;
     if (!ctx->regions[slot].dev.shadow) return CC_ERR_INVALID;
@@ -723,12 +752,14 @@ extern "C" int32_t cc_scan_only(cc_ctx* ctx, uint32_t region_id, void* stream, c
     return launch_scan_compact(ctx, slot, CC_MODE_SCAN_ONLY, 0, (cudaStream_t)stream, out);
 }
 
+#if CC_BENCH_HOOKS
 extern "C" int32_t cc_trace_events(cc_ctx* ctx, void* ev_after_scan, void* ev_after_compact) {
     if (!ctx) return CC_ERR_INVALID;
     ctx->ev_after_scan = (cudaEvent_t)ev_after_scan;
     ctx->ev_after_compact = (cudaEvent_t)ev_after_compact;
     return CC_OK;
 }
+#endif
 
 extern "C" int32_t cc_dirty_list(cc_ctx* ctx, uint32_t region_id, const uint32_t** d_list, const uint32_t** d_count) {
     if (!ctx) return CC_ERR_INVALID;
@@ -790,6 +821,7 @@ static const u8* stage_log(cc_ctx* ctx, const void* log, uint64_t nbytes, cudaSt
 
 extern "C" int32_t cc_apply_log(cc_ctx* ctx, const void* log, uint64_t nbytes, void* stream, cc_result* out) {
     if (!ctx || !log || ((uintptr_t)log & 15)) return CC_ERR_INVALID;
+    CC_NO_WORKER(ctx);
     if (!ctx->apply_attached) return CC_ERR_INVALID;
     CC_CUDA(ctx, cudaSetDevice(ctx->device));
     cudaStream_t st = (cudaStream_t)stream;
@@ -862,12 +894,28 @@ extern "C" int32_t cc_worker_start(cc_ctx* ctx) {
     return CC_OK;
 }
 
+// Has the worker kernel left by itself (max_lifetime_ns expiry, a fault)?  Then nothing will ever complete again:
+// mark it stopped so that cc_submit / cc_wait report CC_ERR_WORKER (or CC_ERR_CUDA) instead of spinning.
+static int32_t worker_gone(cc_ctx* ctx) {
+    if (!ctx->worker_running) return CC_ERR_WORKER;
+    const cudaError_t q = cudaEventQuery(ctx->worker_done);
+    if (q == cudaErrorNotReady) return CC_OK;
+    ctx->worker_running = false;
+    if (q != cudaSuccess) { ctx->last_cuda = (int)q; return CC_ERR_CUDA; }
+    return CC_ERR_WORKER;
+}
+
 extern "C" int32_t cc_submit(cc_ctx* ctx, const cc_task* task, uint64_t* seq_out) {
     if (!ctx || !task) return CC_ERR_INVALID;
     if (!ctx->worker_running) return CC_ERR_WORKER;
+    if (ctx->in_submit.exchange(1u, std::memory_order_acquire)) return CC_ERR_INVALID;   // a second producer is inside
     const u64 seq = ctx->submitted;
     const u64 done = __atomic_load_n(ctx->ring_words + 8, __ATOMIC_ACQUIRE);
-    if (seq - done >= ctx->cfg.ring_capacity) return CC_ERR_RING_FULL;
+    if (seq - done >= ctx->cfg.ring_capacity) {
+        const int32_t g = worker_gone(ctx);          // full because the worker died?
+        ctx->in_submit.store(0u, std::memory_order_release);
+        return g != CC_OK ? g : CC_ERR_RING_FULL;
+    }
     cc_task* slot = &ctx->ring_slots[seq & (ctx->cfg.ring_capacity - 1)];
     cc_task t = *task;
     t.seq = seq;
@@ -875,9 +923,11 @@ extern "C" int32_t cc_submit(cc_ctx* ctx, const cc_task* task, uint64_t* seq_out
     __atomic_store_n(ctx->ring_words + 0, seq + 1, __ATOMIC_RELEASE);    // commit(slot): store-release
     ctx->submitted = seq + 1;
     if (seq_out) *seq_out = seq;
+    ctx->in_submit.store(0u, std::memory_order_release);
     return CC_OK;
 }
 
+#if CC_BENCH_HOOKS
 __global__ void cc_empty_kernel() {}
 
 // Measurement hook for the comparison of PAPER.md Table 7 (L368-370: cudaLaunchKernel 7.6 us with a sync per launch,
@@ -934,6 +984,8 @@ extern "C" int32_t cc_measure_submit_cost(cc_ctx* ctx, uint32_t n, double* ns_pe
     return CC_OK;
 }
 
+#endif  // CC_BENCH_HOOKS
+
 extern "C" int32_t cc_poll(cc_ctx* ctx, uint64_t seq, cc_result* out) {
     if (!ctx) return CC_ERR_INVALID;
     if (seq >= ctx->submitted) return CC_ERR_INVALID;
@@ -946,10 +998,17 @@ extern "C" int32_t cc_poll(cc_ctx* ctx, uint64_t seq, cc_result* out) {
 
 extern "C" int32_t cc_wait(cc_ctx* ctx, uint64_t seq, uint64_t timeout_ns, cc_result* out) {
     const u64 t0 = now_ns();
+    u64 next_check = t0 + 2000000ull;       // look at the worker kernel itself every 2 ms
     for (;;) {
         int32_t rc = cc_poll(ctx, seq, out);
         if (rc != CC_PENDING) return rc;
-        if (now_ns() - t0 > timeout_ns) return CC_ERR_TIMEOUT;
+        const u64 now = now_ns();
+        if (now - t0 > timeout_ns) return CC_ERR_TIMEOUT;
+        if (now >= next_check) {
+            const int32_t g = worker_gone(ctx);
+            if (g != CC_OK) return cc_poll(ctx, seq, out) == CC_OK ? CC_OK : g;     // it may have finished this task last
+            next_check = now + 2000000ull;
+        }
 #if defined(__x86_64__)
         __builtin_ia32_pause();
 #endif
@@ -1002,6 +1061,7 @@ extern "C" int32_t cc_worker_footprint(cc_ctx* ctx, uint32_t* blocks, uint32_t* 
 extern "C" int32_t cc_worker_stop(cc_ctx* ctx) {
     if (!ctx) return CC_ERR_INVALID;
     if (!ctx->worker_running) return CC_ERR_WORKER;
+    ctx->in_submit.store(0u, std::memory_order_release);
     cudaSetDevice(ctx->device);
     cc_task t;
     memset(&t, 0, sizeof(t));

@@ -182,3 +182,83 @@ def test_measurement_hooks():
     finally:
         ctx.worker_stop()
     ctx.shutdown()
+
+
+def test_recovery_tasks_without_apply_scratch_are_refused():
+    """RESTORE / COMPACT_LOG on a worker started without cc_apply_attach used to store through a
+    null table pointer; they must answer CC_ERR_INVALID, as must null / misaligned log pointers."""
+    cur = synth.raw_region(4096 * 64, 7, "cuda")
+    ctx = cc.Context(ring_capacity=8, max_lifetime_ns=int(30e9))
+    ctx.register_region(1, cur, 4096)
+    log = torch.zeros(1 << 16, dtype=torch.uint8, device="cuda")
+    out = torch.zeros(1 << 16, dtype=torch.uint8, device="cuda")
+    ctx.log_attach(log)
+    ctx.worker_start()                                      # no apply_attach
+    try:
+        for kind, args in ((cc.CC_TASK_RESTORE, dict(arg0=log.data_ptr(), arg1=64)),
+                           (cc.CC_TASK_COMPACT_LOG, dict(arg0=log.data_ptr(), arg1=64, arg2=out.data_ptr(), arg3=out.numel()))):
+            r = ctx.wait(ctx.submit(kind, **args), 10.0)
+            assert r.status == cc.CC_ERR_INVALID, (kind, r.as_dict())
+        assert ctx.worker_alive()                           # the resident kernel survived
+        r = ctx.wait(ctx.submit(cc.CC_TASK_NOP), 5.0)
+        assert r.status == 0
+    finally:
+        ctx.worker_stop()
+    ctx.apply_attach(256)
+    ctx.worker_start()
+    try:
+        for args in (dict(arg0=0, arg1=64), dict(arg0=log.data_ptr() + 8, arg1=64)):
+            r = ctx.wait(ctx.submit(cc.CC_TASK_RESTORE, **args), 10.0)
+            assert r.status == cc.CC_ERR_INVALID, r.as_dict()
+        r = ctx.wait(ctx.submit(cc.CC_TASK_COMPACT_LOG, arg0=log.data_ptr(), arg1=4096, arg2=log.data_ptr() + 1024, arg3=4096), 10.0)
+        assert r.status == cc.CC_ERR_INVALID                # overlapping input / output
+        r = ctx.wait(ctx.submit(cc.CC_TASK_RESTORE, arg0=log.data_ptr(), arg1=0), 10.0)
+        assert (r.status, r.n_dirty, r.bytes) == (0, 0, 0)  # an empty log is a valid log
+    finally:
+        ctx.worker_stop()
+    ctx.shutdown()
+
+
+def test_host_launched_calls_are_refused_while_the_worker_runs():
+    """the host-launched data path shares control blocks with the resident worker."""
+    ctx, cur, sh, log, committed = _mk()
+    res = cc.Result()
+    marks = torch.zeros(16, dtype=torch.int32, device="cuda")
+    ctx.worker_start()
+    try:
+        calls = [lambda: ctx.checkpoint_delta(1, 1, res), lambda: ctx.checkpoint_delta_fused(1, 1, res),
+                 lambda: ctx.checkpoint_delta_rle(1, 1, 4, res), lambda: ctx.checkpoint_marked(1, 1, marks, 0, res),
+                 lambda: ctx.checkpoint_all(1, res), lambda: ctx.snapshot_region(1, 1, res), lambda: ctx.scan_only(1, res),
+                 lambda: ctx.apply_log(log, 0, res)]
+        for c in calls:
+            with pytest.raises(cc.ConcordiaError) as e:
+                c()
+            assert e.value.code == cc.CC_ERR_WORKER
+    finally:
+        ctx.worker_stop()
+    ctx.checkpoint_delta(1, 1, res)
+    torch.cuda.synchronize()
+    assert res.read().status == 0
+    ctx.shutdown()
+
+
+def test_wait_and_submit_notice_a_worker_that_left_by_itself():
+    """after max_lifetime_ns the kernel exits; cc_wait must not spin to its timeout and cc_submit must
+    stop accepting tasks."""
+    cur = synth.raw_region(4096 * 64, 8, "cuda")
+    ctx = cc.Context(ring_capacity=4, max_lifetime_ns=int(0.3e9))
+    ctx.register_region(1, cur, 4096)
+    ctx.worker_start()
+    time.sleep(0.6)                                         # the worker's lifetime is over
+    t0 = time.time()
+    got = None
+    try:
+        for _ in range(8):                                  # at most `capacity` submissions go through, then WORKER
+            s = ctx.submit(cc.CC_TASK_NOP)
+            ctx.wait(s, 20.0)
+    except cc.ConcordiaError as e:
+        got = e.code
+    assert got == cc.CC_ERR_WORKER, got
+    assert time.time() - t0 < 5.0                           # not the 20 s timeout
+    assert not ctx.worker_alive()
+    ctx.shutdown()
