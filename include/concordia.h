@@ -190,6 +190,21 @@ int32_t cc_log_reset_async(cc_ctx* ctx, void* stream);
 int32_t cc_log_mirror_attach(cc_ctx* ctx, void* host_log, uint64_t capacity, uint64_t* committed_off_host);
 int32_t cc_log_drain(cc_ctx* ctx, uint64_t upto, void* after_stream, void* copy_stream);
 
+/* Library-side drainer for the same mirror: cc_log_drain_start launches a host thread that follows the committed
+ * offset every checkpoint publishes (host-launched calls and worker tasks alike -- no per-step call, no result to
+ * read first) and hands each newly committed byte range to the copy engine on an internal stream; once a range
+ * has landed in host_log, *committed_off_host is release-stored.  A log reset (cc_log_reset, cc_log_reset_async,
+ * CC_TASK_LOG_RESET) starts a new generation: the thread starts again at offset 0 and zeroes *committed_off_host.
+ * As with cc_log_drain, the caller resets or reuses log space only after the mirror has caught up
+ * (cc_log_drain_wait, or poll *committed_off_host).  cc_log_drain_wait blocks until the first `upto` bytes of the
+ * current generation have landed (CC_ERR_TIMEOUT after timeout_ns; the thread's error if it stopped:
+ * CC_ERR_LOG_FULL = mirror too small, CC_ERR_CUDA).  cc_log_drain_stop drains what is committed, joins the thread
+ * and returns its status.  cc_log_drain, cc_log_attach and cc_log_mirror_attach are refused (CC_ERR_INVALID)
+ * while the thread runs; cc_shutdown stops it.  Needs an attached log and mirror. */
+int32_t cc_log_drain_start(cc_ctx* ctx);
+int32_t cc_log_drain_wait(cc_ctx* ctx, uint64_t upto, uint64_t timeout_ns);
+int32_t cc_log_drain_stop(cc_ctx* ctx);
+
 /* ---- host-launched path -------------------------------------------------------------------- */
 
 /* Delta-checkpoint one region: scan live vs shadow per page, compact the

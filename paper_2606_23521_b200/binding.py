@@ -46,7 +46,7 @@ CC_TASKF_RLE = 2
 
 EXPORTS = [
     "cc_init", "cc_shutdown", "cc_last_cuda_error", "cc_kernel_launches", "cc_workspace_bytes",
-    "cc_register_region", "cc_unregister_region", "cc_log_attach", "cc_log_reset", "cc_log_reset_async", "cc_log_mirror_attach", "cc_log_drain",
+    "cc_register_region", "cc_unregister_region", "cc_log_attach", "cc_log_reset", "cc_log_reset_async", "cc_log_mirror_attach", "cc_log_drain", "cc_log_drain_start", "cc_log_drain_wait", "cc_log_drain_stop",
     "cc_checkpoint_delta", "cc_checkpoint_delta_fused", "cc_checkpoint_delta_rle", "cc_checkpoint_marked", "cc_checkpoint_versions",
     "cc_checkpoint_all", "cc_snapshot_region", "cc_compact_log", "cc_scan_only", "cc_trace_events", "cc_dirty_list", "cc_apply_scratch_bytes", "cc_apply_attach", "cc_apply_stage_attach", "cc_apply_log",
     "cc_worker_start", "cc_worker_stop", "cc_worker_alive", "cc_worker_footprint", "cc_peek_queue", "cc_submit", "cc_measure_submit_cost", "cc_measure_launch_cost", "cc_poll", "cc_wait",
@@ -112,6 +112,9 @@ def load_library():
         "cc_log_reset_async": (i32, [vp, vp]),
         "cc_log_mirror_attach": (i32, [vp, vp, u64, vp]),
         "cc_log_drain": (i32, [vp, u64, vp, vp]),
+        "cc_log_drain_start": (i32, [vp]),
+        "cc_log_drain_wait": (i32, [vp, u64, u64]),
+        "cc_log_drain_stop": (i32, [vp]),
         "cc_checkpoint_delta": (i32, [vp, u32, u64, vp, vp]),
         "cc_checkpoint_delta_fused": (i32, [vp, u32, u64, vp, vp]),
         "cc_checkpoint_delta_rle": (i32, [vp, u32, u64, u32, vp, vp]),
@@ -260,6 +263,16 @@ class Context:
 
     def log_drain(self, upto: int, copy_stream, after_stream=None):
         self._check("cc_log_drain", self.lib.cc_log_drain(self.h, upto, _stream_ptr(after_stream), _stream_ptr(copy_stream)))
+
+    def log_drain_start(self):
+        """Start the library's drainer thread (device log -> attached host mirror, copy engine, no per-step call)."""
+        self._check("cc_log_drain_start", self.lib.cc_log_drain_start(self.h))
+
+    def log_drain_wait(self, upto: int, timeout_s: float = 30.0):
+        self._check("cc_log_drain_wait", self.lib.cc_log_drain_wait(self.h, upto, int(timeout_s * 1e9)))
+
+    def log_drain_stop(self):
+        self._check("cc_log_drain_stop", self.lib.cc_log_drain_stop(self.h))
 
     def log_reset(self):
         self._check("cc_log_reset", self.lib.cc_log_reset(self.h))

@@ -202,10 +202,7 @@ __device__ __forceinline__ void cc_batch_gather_phase(cc_dev* dev, cc_crc_smem* 
     if (threadIdx.x == 0) {
         __threadfence_system();
         cc_log_dev* log = &dev->log;
-        if (B->bytes_total != 0) {
-            if (log->committed_off) st_release_sys_u64(log->committed_off, B->W_final);
-            log->W = B->W_final;
-        }
+        if (B->bytes_total != 0) cc_log_publish(log, B->W_final);
         B->done = 0;
         cc_batch_write_result(dev, out, kind);
         __threadfence();

@@ -365,8 +365,7 @@ __device__ __forceinline__ void cc_gather_complete(const cc_region_dev& r, cc_de
         const u64 W_after = cc_gather_commit_record(r, dev);
         if (appended) {
             __threadfence_system();
-            if (log->committed_off) st_release_sys_u64(log->committed_off, W_after);
-            log->W = W_after;
+            cc_log_publish(log, W_after);
         }
         if (out) {
             out->n_dirty = h->k;

@@ -74,7 +74,10 @@ struct cc_log_dev {
     u64 capacity;
     u64 W;                  // running write offset (device-resident so that async calls chain)
     u64* committed_off;     // host-visible published offset (may be null)
+    u64 gen;                // number of resets so far: the log's generation
+    u64* pub;               // library-owned pinned word (gen << 48 | committed offset) that the drainer thread follows
 };
+#define CC_PUB_SHIFT 48
 
 // Applier tables (in the attached scratch).
 struct cc_rec {             // 32 bytes
@@ -240,6 +243,22 @@ __device__ __forceinline__ u32 ld_relaxed_sys_u32(const u32* p) {
     u32 v;
     asm volatile("ld.relaxed.sys.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
+}
+
+// One thread, after the commit record's bytes have been fenced at system scope ("a commit marker publishes
+// the epoch only after all bytes are visible"): advance the write offset and publish the committed offset -- to the
+// caller's word and to the library's own (generation-tagged) word.
+__device__ __forceinline__ void cc_log_publish(cc_log_dev* log, u64 W_after) {
+    if (log->committed_off) st_release_sys_u64(log->committed_off, W_after);
+    if (log->pub) st_release_sys_u64(log->pub, (log->gen << CC_PUB_SHIFT) | W_after);
+    log->W = W_after;
+}
+// W := 0: a new generation of the log (cc_log_reset*, CC_TASK_LOG_RESET).
+__device__ __forceinline__ void cc_log_rewind(cc_log_dev* log) {
+    log->gen = log->gen + 1;
+    log->W = 0;
+    if (log->committed_off) st_release_sys_u64(log->committed_off, 0ull);
+    if (log->pub) st_release_sys_u64(log->pub, log->gen << CC_PUB_SHIFT);
 }
 
 __device__ __forceinline__ u64 page_len_dev(const cc_region_dev& r, u64 p) {

@@ -139,10 +139,7 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
                 }
                 if (t.kind == CC_TASK_NOP || t.kind == CC_TASK_LOG_RESET) {
                     const u64 ts = globaltimer_ns();
-                    if (t.kind == CC_TASK_LOG_RESET) {
-                        dev->log.W = 0;
-                        if (dev->log.committed_off) st_release_sys_u64(dev->log.committed_off, 0ull);
-                    }
+                    if (t.kind == CC_TASK_LOG_RESET) cc_log_rewind(&dev->log);
                     cc_result* out = &ring.results[t.seq & (ring.capacity - 1)];
                     out->n_dirty = 0; out->bytes = 0; out->log_offset_after = dev->log.W; out->epoch = t.epoch;
                     out->status = CC_OK; out->flags = t.kind; out->t_start_ns = ts; out->t_end_ns = globaltimer_ns();

@@ -8,6 +8,9 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <mutex>
+#include <thread>
+#include <time.h>
 
 #include "cc_common.cuh"
 #include "cc_crc.cuh"
@@ -166,6 +169,13 @@ struct cc_ctx {
     uint64_t* mirror_committed;
     uint64_t drained;
     cudaEvent_t drain_ev;
+    // library-side drainer (cc_log_drain_start / _stop): a host thread that follows the published offset
+    std::thread* drainer;
+    std::atomic<uint32_t> drainer_stop;
+    std::atomic<uint64_t> drainer_gen;      // generation the thread is draining
+    std::atomic<uint64_t> drainer_landed;   // bytes of that generation whose copies have completed
+    std::atomic<int32_t> drainer_status;
+    cudaStream_t drainer_stream;
     cc_apply_tabs tabs;
     bool apply_attached;
     void* stage;                // optional device staging buffer for host-resident logs (cc_apply_stage_attach)
@@ -321,6 +331,7 @@ extern "C" int32_t cc_shutdown(cc_ctx* ctx) {
     if (!ctx) return CC_ERR_INVALID;
     cudaSetDevice(ctx->device);
     int32_t rc = CC_OK;
+    if (ctx->drainer) cc_log_drain_stop(ctx);
     if (ctx->worker_running) rc = cc_worker_stop(ctx);
     if (rc == CC_ERR_TIMEOUT) return rc;    // the kernel may still be resident and reads *ctx's ring: leak rather than free under it
     if (rc == CC_OK) {   // never free under a resident kernel
@@ -332,6 +343,7 @@ extern "C" int32_t cc_shutdown(cc_ctx* ctx) {
         if (ctx->worker_stream) cudaStreamDestroy(ctx->worker_stream);
         if (ctx->worker_done) cudaEventDestroy(ctx->worker_done);
         if (ctx->drain_ev) cudaEventDestroy(ctx->drain_ev);
+        if (ctx->drainer_stream) cudaStreamDestroy(ctx->drainer_stream);
     }
     delete ctx;
     return rc;
@@ -436,6 +448,10 @@ extern "C" int32_t cc_log_attach(cc_ctx* ctx, void* log_buf, uint64_t capacity, 
     l.capacity = capacity;
     l.W = 0;
     l.committed_off = committed_off;
+    l.gen = 0;
+    l.pub = (u64*)(ctx->ring_words + 24);
+    if (ctx->drainer) return CC_ERR_INVALID;             // stop the drainer before re-attaching
+    __atomic_store_n(ctx->ring_words + 24, 0ull, __ATOMIC_RELEASE);
     CC_CUDA(ctx, cudaMemcpyAsync(&ctx->d_dev->log, &l, sizeof(l), cudaMemcpyHostToDevice, 0));
     CC_CUDA(ctx, cudaStreamSynchronize(0));
     ctx->log_attached = true;
@@ -446,16 +462,20 @@ extern "C" int32_t cc_log_attach(cc_ctx* ctx, void* log_buf, uint64_t capacity, 
     return CC_OK;
 }
 
+__global__ void cc_log_reset_kernel(cc_dev* dev) { cc_log_rewind(&dev->log); }
+
 extern "C" int32_t cc_log_reset(cc_ctx* ctx) {
     if (!ctx || !ctx->log_attached) return CC_ERR_INVALID;
     if (ctx->worker_running) return CC_ERR_WORKER;
     CC_CUDA(ctx, cudaSetDevice(ctx->device));
-    const u64 zero = 0;
-    CC_CUDA(ctx, cudaMemcpyAsync(&ctx->d_dev->log.W, &zero, sizeof(zero), cudaMemcpyHostToDevice, 0));
-    if (ctx->committed_off) CC_CUDA(ctx, cudaMemsetAsync(ctx->committed_off, 0, sizeof(u64), 0));     // publish the rewind too
+    cc_log_reset_kernel<<<1, 1, 0, 0>>>(ctx->d_dev);     // W := 0, next generation, publish the rewind too
+    ctx->launches += 1;
+    CC_CUDA(ctx, cudaGetLastError());
     CC_CUDA(ctx, cudaStreamSynchronize(0));
-    ctx->drained = 0;
-    if (ctx->mirror_committed) __atomic_store_n(ctx->mirror_committed, 0ull, __ATOMIC_RELEASE);
+    if (!ctx->drainer) {                                 // (a running drainer thread follows the generation itself)
+        ctx->drained = 0;
+        if (ctx->mirror_committed) __atomic_store_n(ctx->mirror_committed, 0ull, __ATOMIC_RELEASE);
+    }
     return CC_OK;
 }
 
@@ -469,7 +489,7 @@ static void CUDART_CB cc_drain_publish(void* p) {
 }
 
 extern "C" int32_t cc_log_mirror_attach(cc_ctx* ctx, void* host_log, uint64_t capacity, uint64_t* committed_off_host) {
-    if (!ctx || ((uintptr_t)host_log & 15)) return CC_ERR_INVALID;
+    if (!ctx || ((uintptr_t)host_log & 15) || ctx->drainer) return CC_ERR_INVALID;
     if (ctx->worker_running) return CC_ERR_WORKER;
     CC_CUDA(ctx, cudaSetDevice(ctx->device));
     if (host_log && !ctx->drain_ev) CC_CUDA(ctx, cudaEventCreateWithFlags(&ctx->drain_ev, cudaEventDisableTiming));
@@ -482,7 +502,7 @@ extern "C" int32_t cc_log_mirror_attach(cc_ctx* ctx, void* host_log, uint64_t ca
 }
 
 extern "C" int32_t cc_log_drain(cc_ctx* ctx, uint64_t upto, void* after_stream, void* copy_stream) {
-    if (!ctx || !ctx->log_attached || !ctx->mirror) return CC_ERR_INVALID;
+    if (!ctx || !ctx->log_attached || !ctx->mirror || ctx->drainer) return CC_ERR_INVALID;
     if (upto < ctx->drained || upto > ctx->log_capacity) return CC_ERR_INVALID;
     if (upto > ctx->mirror_capacity) return CC_ERR_LOG_FULL;
     if (upto == ctx->drained) return CC_OK;
@@ -513,10 +533,12 @@ extern "C" int32_t cc_log_reset_async(cc_ctx* ctx, void* stream) {
     if (!ctx || !ctx->log_attached) return CC_ERR_INVALID;
     if (ctx->worker_running) return CC_ERR_WORKER;
     CC_CUDA(ctx, cudaSetDevice(ctx->device));
-    CC_CUDA(ctx, cudaMemsetAsync(&ctx->d_dev->log.W, 0, sizeof(u64), (cudaStream_t)stream));
-    if (ctx->committed_off) CC_CUDA(ctx, cudaMemsetAsync(ctx->committed_off, 0, sizeof(u64), (cudaStream_t)stream));
+    cc_log_reset_kernel<<<1, 1, 0, (cudaStream_t)stream>>>(ctx->d_dev);
+    ctx->launches += 1;
+    CC_CUDA(ctx, cudaGetLastError());
     // the mirror's drain position and published offset rewind with the log: drains issued after this call (in host
     // order) copy from offset 0 again; the mirror's word is zeroed in stream order, like committed_off
+    if (ctx->drainer) return CC_OK;                      // the drainer thread follows the generation by itself
     ctx->drained = 0;
     if (ctx->mirror_committed) {
         cc_drain_note* nt = (cc_drain_note*)malloc(sizeof(cc_drain_note));
@@ -527,6 +549,113 @@ extern "C" int32_t cc_log_reset_async(cc_ctx* ctx, void* stream) {
         if (e != cudaSuccess) { free(nt); ctx->last_cuda = (int)e; return CC_ERR_CUDA; }
     }
     return CC_OK;
+}
+
+// ---- library-side drainer: staging buffer -> host log without a per-step call ----
+// A host thread follows the library's published word (generation << 48 | committed offset, release-stored by the
+// commit of every checkpoint, host-launched or worker) and hands every newly committed byte range of the
+// device-resident log to the copy engine; after a range has landed it publishes the mirror's offset.  A log reset
+// starts a new generation: the thread starts again at offset 0 of the mirror.
+
+struct cc_landed_note { cc_ctx* ctx; uint64_t gen, upto; };
+static void CUDART_CB cc_drain_landed(void* p) {
+    cc_landed_note* nt = (cc_landed_note*)p;
+    cc_ctx* c = nt->ctx;
+    if (c->drainer_gen.load(std::memory_order_acquire) == nt->gen) {
+        if (c->mirror_committed) __atomic_store_n(c->mirror_committed, nt->upto, __ATOMIC_RELEASE);
+        c->drainer_landed.store(nt->upto, std::memory_order_release);
+    }
+    free(nt);
+}
+
+static void cc_drainer_main(cc_ctx* ctx) {
+    if (cudaSetDevice(ctx->device) != cudaSuccess) { ctx->drainer_status.store(CC_ERR_CUDA); return; }
+    cudaStream_t cs = ctx->drainer_stream;
+    uint64_t gen = ctx->drainer_gen.load(), drained = ctx->drainer_landed.load();
+    const uint64_t piece = 16ull << 20;
+    uint32_t idle = 0;
+    for (;;) {
+        const bool stopping = ctx->drainer_stop.load(std::memory_order_acquire) != 0;
+        const uint64_t pub = __atomic_load_n(ctx->ring_words + 24, __ATOMIC_ACQUIRE);
+        const uint64_t g = pub >> CC_PUB_SHIFT, c = pub & ((1ull << CC_PUB_SHIFT) - 1);
+        if (g != gen) {                                  // the log was reset: a new generation starts at offset 0
+            cudaStreamSynchronize(cs);                   // copies of the old generation finish first
+            gen = g;
+            drained = 0;
+            ctx->drainer_landed.store(0, std::memory_order_release);
+            ctx->drainer_gen.store(g, std::memory_order_release);
+            if (ctx->mirror_committed) __atomic_store_n(ctx->mirror_committed, 0ull, __ATOMIC_RELEASE);
+        }
+        if (c > drained) {
+            idle = 0;
+            if (c > ctx->mirror_capacity) { ctx->drainer_status.store(CC_ERR_LOG_FULL); return; }
+            cudaError_t e = cudaSuccess;
+            for (uint64_t o = drained; o < c && e == cudaSuccess; o += piece) {
+                const uint64_t nb = c - o < piece ? c - o : piece;
+                e = cudaMemcpyAsync((u8*)ctx->mirror + o, (const u8*)ctx->log_buf + o, nb, cudaMemcpyDefault, cs);
+            }
+            cc_landed_note* nt = (cc_landed_note*)malloc(sizeof(cc_landed_note));
+            if (e == cudaSuccess && nt) {
+                nt->ctx = ctx; nt->gen = gen; nt->upto = c;
+                e = cudaLaunchHostFunc(cs, cc_drain_landed, nt);
+                if (e != cudaSuccess) free(nt);
+            } else if (nt) free(nt);
+            if (e != cudaSuccess || !nt) { ctx->last_cuda = (int)e; ctx->drainer_status.store(CC_ERR_CUDA); return; }
+            drained = c;
+            continue;
+        }
+        if (stopping) break;
+        if (++idle < 2000) {
+#if defined(__x86_64__)
+            __builtin_ia32_pause();
+#endif
+        } else {
+            struct timespec ts = {0, 20000};             // 20 us naps once nothing has been committed for a while
+            nanosleep(&ts, nullptr);
+        }
+    }
+    cudaStreamSynchronize(cs);
+}
+
+extern "C" int32_t cc_log_drain_start(cc_ctx* ctx) {
+    if (!ctx || !ctx->log_attached || !ctx->mirror) return CC_ERR_INVALID;
+    if (ctx->drainer) return CC_ERR_EXISTS;
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    if (!ctx->drainer_stream) CC_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->drainer_stream, cudaStreamNonBlocking));
+    const uint64_t pub = __atomic_load_n(ctx->ring_words + 24, __ATOMIC_ACQUIRE);
+    ctx->drainer_gen.store(pub >> CC_PUB_SHIFT);
+    ctx->drainer_landed.store(ctx->drained);             // what cc_log_drain has already carried over
+    ctx->drainer_stop.store(0);
+    ctx->drainer_status.store(CC_OK);
+    ctx->drainer = new (std::nothrow) std::thread(cc_drainer_main, ctx);
+    return ctx->drainer ? CC_OK : CC_ERR_INVALID;
+}
+
+extern "C" int32_t cc_log_drain_wait(cc_ctx* ctx, uint64_t upto, uint64_t timeout_ns) {
+    if (!ctx || !ctx->drainer) return CC_ERR_INVALID;
+    const auto t0 = std::chrono::steady_clock::now();
+    for (;;) {
+        // "landed" counts bytes of the generation the thread is on: it must be the log's current one
+        const uint64_t g = __atomic_load_n(ctx->ring_words + 24, __ATOMIC_ACQUIRE) >> CC_PUB_SHIFT;
+        if (ctx->drainer_gen.load(std::memory_order_acquire) == g && ctx->drainer_landed.load(std::memory_order_acquire) >= upto) return CC_OK;
+        const int32_t st = ctx->drainer_status.load();
+        if (st != CC_OK) return st;
+        if ((uint64_t)std::chrono::duration_cast<std::chrono::nanoseconds>(std::chrono::steady_clock::now() - t0).count() > timeout_ns)
+            return CC_ERR_TIMEOUT;
+#if defined(__x86_64__)
+        __builtin_ia32_pause();
+#endif
+    }
+}
+
+extern "C" int32_t cc_log_drain_stop(cc_ctx* ctx) {
+    if (!ctx || !ctx->drainer) return CC_ERR_INVALID;
+    ctx->drainer_stop.store(1, std::memory_order_release);
+    ctx->drainer->join();
+    delete ctx->drainer;
+    ctx->drainer = nullptr;
+    ctx->drained = ctx->drainer_landed.load();
+    return ctx->drainer_status.load();
 }
 
 // ------------------------------------------------------------- host-launched path --

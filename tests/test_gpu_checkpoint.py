@@ -283,3 +283,69 @@ def test_log_mirror_drain_by_the_copy_engine():
     with pytest.raises(cc.ConcordiaError):
         ctx.log_drain(W, copy_stream)
     ctx.shutdown()
+
+
+def test_library_side_drainer_thread_follows_commits_and_resets():
+    """cc_log_drain_start: a host thread follows the published committed offset; the host mirror equals the oracle's
+    log after every generation, with no per-step drain call -- host-launched checkpoints, then the same through the
+    ring / persistent worker, with log resets in between."""
+    P, n_pages = 4096, 600
+    cur = _region(P * n_pages, 22)
+    ctx = cc.Context(ring_capacity=16, max_lifetime_ns=int(60e9))
+    ctx.register_region(1, cur, P)
+    cap = 4 << 20
+    log = torch.zeros(cap, dtype=torch.uint8, device="cuda")
+    mirror = torch.zeros(cap, dtype=torch.uint8, pin_memory=True)
+    pub = torch.zeros(1, dtype=torch.int64, pin_memory=True)
+    ctx.log_attach(log)
+    ctx.log_mirror_attach(mirror, pub)
+    with pytest.raises(cc.ConcordiaError):
+        ctx.log_drain_stop()                                        # not running
+    ctx.log_drain_start()
+    with pytest.raises(cc.ConcordiaError):
+        ctx.log_drain_start()                                       # already running
+    with pytest.raises(cc.ConcordiaError):
+        ctx.log_drain(16, torch.cuda.Stream())                      # manual drains are refused meanwhile
+    host_cur = cur.cpu().numpy().copy()
+    host_sh = host_cur.copy()
+    rng = np.random.default_rng(5)
+    res = cc.Result()
+
+    def mutate():
+        for p in rng.integers(0, n_pages, 20).tolist():
+            off = p * P + int(rng.integers(0, P))
+            host_cur[off] ^= 0x33
+            cur[off] ^= 0x33
+        torch.cuda.synchronize()
+
+    for generation in range(2):                                     # host-launched, with a reset in between
+        olog = np.zeros(cap, np.uint8)
+        W = 0
+        for e in range(4):
+            mutate()
+            ctx.checkpoint_delta(1, 10 * generation + e, res)
+            st, D, nb, W = oracle.checkpoint(host_cur, host_sh, P, 1, 10 * generation + e, olog, W)
+        ctx.log_drain_wait(W, 20.0)
+        assert int(pub.item()) == W and np.array_equal(mirror.numpy()[:W], olog[:W])
+        (ctx.log_reset if generation == 0 else ctx.log_reset_async)()
+    torch.cuda.synchronize()
+    # the worker publishes through the same word
+    ctx.worker_start()
+    try:
+        ctx.wait(ctx.submit(cc.CC_TASK_LOG_RESET), 10.0)
+        olog = np.zeros(cap, np.uint8)
+        W = 0
+        for e in range(3):
+            A, h = 77, 1000 + e
+            ctx.wait(ctx.submit(cc.CC_TASK_TEST_MUTATE, region_id=1, arg0=9, arg1=A, arg2=h), 10.0)
+            for j in range(9):
+                host_cur[((j * A + h) % n_pages) * P + (h + j) % P] ^= 0x5A
+            r = ctx.wait(ctx.submit(cc.CC_TASK_DELTA_CKPT, region_id=1, epoch=50 + e), 10.0)
+            st, D, nb, W = oracle.checkpoint(host_cur, host_sh, P, 1, 50 + e, olog, W)
+            assert (r.status, r.n_dirty, r.log_offset_after) == (st, D.size, W)
+        ctx.log_drain_wait(W, 20.0)
+        assert int(pub.item()) == W and np.array_equal(mirror.numpy()[:W], olog[:W])
+    finally:
+        ctx.worker_stop()
+    ctx.log_drain_stop()
+    ctx.shutdown()

@@ -239,3 +239,44 @@ def test_c5b_full_10000_ring_tasks():
     torch.cuda.synchronize()
     assert torch.equal(sh, cur)
     ctx.shutdown()
+
+
+@pytest.mark.parametrize("P", [4096, 16384, 65536])
+def test_c4_full_32gib_all_dirty_every_record_against_the_oracle(P):
+    """Config 4, 100 % dirty leg AT THE MEASURED SIZE: 32 GiB (the largest slice whose device log fits beside region
+    and shadow, SURVEY.md 8d fallback ii), every page dirty, at 4 / 16 / 64 KiB pages.  EVERY record of the 32 GiB
+    device log -- header, CRC32C, payload -- and the commit record are compared with oracle.checkpoint run on every
+    1 GiB chunk of the region (oracle/chunked.py); shadow == region afterwards."""
+    import bench
+    _need(100, 60)
+    N = 32 << 30
+    cur = synth.bf16_normal_region(N, 1004, "cuda")
+    ctx = cc.Context()
+    shadow = ctx.register_region(1, cur, P)
+    n_pages = N // P
+    log = torch.empty(n_pages * (16 + P) + 32, dtype=torch.uint8, device="cuda")
+    ctx.log_attach(log)
+    offs, masks = bench.all_dirty_flips(torch, synth, N, P, 1004 + P, "cuda")
+    synth.toggle_flips(cur, offs, masks)
+    r = gpu_checkpoint(ctx, 1, 6)
+    assert (r.status, r.n_dirty, r.bytes) == (0, n_pages, log.numel())
+    k, nb, D = bench.verify_all_dirty(torch, cc, ctx, 1, cur, log, offs, masks, P, 6, N)
+    assert (k, nb) == (n_pages, log.numel())
+    assert _equal_chunked(shadow, cur)
+    r = gpu_checkpoint(ctx, 1, 7)
+    assert r.n_dirty == 0 and r.bytes == 0
+    ctx.shutdown()
+
+
+def test_c4_full_64gib_arena_as_8_regions_through_one_pinned_log():
+    """SURVEY.md 8d capacity fallback (i): the 64 GiB arena registered as 8 x 8 GiB regions, every page dirty, each
+    checkpointed into ONE pinned 8.1 GiB host log that the harness verifies against the oracle (every record,
+    chunk-wise) and rewinds between regions."""
+    import bench
+
+    class A:
+        steps = 4
+    _need(140, 40)
+    out = bench.c4_full_arena(A, bench.Env(), cc, 65536, verify=True)
+    assert out["parity"].startswith("arena: all 8 x 131072 records"), out
+    assert out["host_link_GBps_log"] > 20.0, out
