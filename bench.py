@@ -413,8 +413,14 @@ def run_c2(args, env):
     pools_host = [p.cpu().pin_memory() for p in pools]
     stage = torch.empty_like(pools[0])
 
+    wstate = {"n": 0}
+
     def decode_write(values):
         rows.index_copy_(0, row_idx, values)         # the application's KV append (torch, not part of the library)
+        wstate["n"] += 1
+
+    def next_pool():
+        return wstate["n"] & 1                       # consecutive writes alternate the two value pools: every step dirties k_exp blocks
 
     ctx = cc.Context(env.local)
     shadow = ctx.register_region(1, cur, P)          # shadow := cur
@@ -430,7 +436,7 @@ def run_c2(args, env):
         import oracle
         ctx.log_attach(log_dev, committed)
         host_old = cur.cpu().numpy()                                         # == shadow
-        decode_write(pools[0])
+        decode_write(pools[next_pool()])
         ctx.checkpoint_delta(1, 4242, warm_res)
         torch.cuda.synchronize()
         r = warm_res.read()
@@ -446,7 +452,7 @@ def run_c2(args, env):
         ctx.log_reset()
 
     def step_dev(s, res, evs=None):
-        decode_write(pools[s & 1])
+        decode_write(pools[next_pool()])
         if evs:
             evs[0].record(stream)
             ctx.trace_events(evs[1], evs[2])
@@ -496,7 +502,7 @@ def run_c2(args, env):
         marks = torch.empty_like(bm_src)
         mk_evs = [[env.ev() for _ in range(2)] for _ in range(K)]
         for s in range(Wm + K):
-            decode_write(pools[s & 1])
+            decode_write(pools[next_pool()])
             marks.copy_(bm_src)                          # the allocator's bitmap for this step
             if s >= Wm:
                 mk_evs[s - Wm][0].record(stream)
@@ -531,7 +537,7 @@ def run_c2(args, env):
         state = {"epochs": 0, "W": 0}
 
         def step_drain(s, res):
-            stage.copy_(pools_host[s & 1], non_blocking=True)      # H2D: this step's new tokens
+            stage.copy_(pools_host[next_pool()], non_blocking=True)      # H2D: this step's new tokens
             decode_write(stage)
             ctx.checkpoint_delta(1, s, res)                        # device log
             stream.synchronize()                                   # this stream only: the copy engine keeps draining
@@ -566,9 +572,9 @@ def run_c2(args, env):
         ctx.log_attach(log_host, committed)
 
         def step_direct(s, res, fused):
-            stage.copy_(pools_host[s & 1], non_blocking=True)
+            stage.copy_(pools_host[next_pool()], non_blocking=True)
             decode_write(stage)
-            (ctx.checkpoint_delta_fused if fused else ctx.checkpoint_delta)(1, s, res)
+            (ctx.checkpoint_delta_fused if fused else ctx.checkpoint_ex)(1, s, res, **({} if fused else {"path": cc.CC_PATH_PHASES}))
             torch.cuda.synchronize()
             r = res.read()
             assert r.status == 0 and r.n_dirty == k_exp
@@ -594,7 +600,7 @@ def run_c2(args, env):
     # ================= arm 3: the same checkpoint through the ring / persistent worker =================
     ring = None
     if not args.no_extras and rank == 0:
-        ring = ring_on_region(cc, env, cur, shadow, P, k_exp, log_bytes, lambda s: decode_write(pools[s & 1]))
+        ring = ring_on_region(cc, env, cur, shadow, P, k_exp, log_bytes, lambda s: decode_write(pools[next_pool()]))
 
     ms_total = env.rmax(ms_total)
     if e2e:
@@ -1063,7 +1069,9 @@ def run_c4_full(args, env):
     ms = env.rmax(head["ms_total"])
     e2e = None
     if not args.no_e2e and env.rank == 0:
-        del cur
+        import gc
+        del cur, offs, masks
+        gc.collect()
         torch.cuda.empty_cache()
         e2e = c4_full_arena(args, env, cc, 65536, verify=not args.no_parity)
         if parity and e2e.get("parity"):
@@ -1267,7 +1275,9 @@ def run_c5b(args, env):
     out = {}
     launches_total = 0
     for mode, flags in (("three_phase", 0), ("fused", cc.CC_TASKF_FUSED)):
-        ctx = cc.Context(env.local, ring_capacity=256, max_lifetime_ns=int(300e9))
+        # latency configuration: every co-resident worker CTA (the default footprint, CC_WORKER_BLOCKS_DEFAULT = 16 CTAs,
+        # trades task time for SMs left to the application: see --workload overlap)
+        ctx = cc.Context(env.local, ring_capacity=256, worker_blocks=cc.CC_WORKER_BLOCKS_ALL, max_lifetime_ns=int(300e9))
         sh = ctx.register_region(1, cur, P)
         log = torch.zeros(1 << 30, dtype=torch.uint8, pin_memory=True)
         ctx.log_attach(log)
@@ -1415,7 +1425,7 @@ def run_overlap(args, env):
 
     base = copy_gbps()
     rows = []
-    for B in (1, 2, 4, 8, 16, 32, 64, 148):
+    for B in (1, 2, 4, 8, 16, 32, 64):
         ctx = cc.Context(env.local, ring_capacity=256, worker_blocks=B, max_lifetime_ns=int(120e9))
         ctx.register_region(1, cur, P)
         log = torch.empty(64 * per, dtype=torch.uint8, device=dev)
@@ -1423,6 +1433,7 @@ def run_overlap(args, env):
         stream.synchronize()
         ctx.worker_start()
         row = {"worker_blocks": B, "sm_share_pct": round(100.0 * B / 148, 2)}
+        print("overlap: worker_blocks", B, file=sys.stderr, flush=True)
         try:
             row["copy_alone_GBps"] = round(copy_gbps(), 1)
 

@@ -81,11 +81,15 @@ extern "C" {
 #define CC_MARK_VERIFY 1u          /* compare the marked pages with the shadow and log only those that differ */
 #define CC_MARK_CONSUME 2u         /* clear the caller's bitmap once the checkpoint went through (not on LOG_FULL) */
 
+#define CC_WORKER_BLOCKS_DEFAULT 16u /* ~11 % of B200's 148 SMs; the trade-off is tabulated in DESIGN.md section 9 */
+#define CC_WORKER_BLOCKS_ALL 0xFFFFFFFFu
+
 typedef struct cc_ctx cc_ctx;
 
 typedef struct {
     uint32_t ring_capacity;    /* slots, power of two, 0 = 256 (256 x 64 B) */
-    uint32_t worker_blocks;    /* persistent worker CTAs, 0 = as many as are co-resident with worker_threads */
+    uint32_t worker_blocks;    /* persistent worker CTAs: 0 = CC_WORKER_BLOCKS_DEFAULT, CC_WORKER_BLOCKS_ALL = as many as are
+                                  co-resident with worker_threads (maximum checkpoint bandwidth, every SM taken) */
     uint32_t worker_threads;   /* threads per worker CTA ("tpb" of Table 1), multiple of 32, 0 = 512 */
     uint32_t backoff_ns;       /* idle poll back-off of the worker (set_yield_every analogue, L172), 0 = 500 */
     uint64_t max_lifetime_ns;  /* worker exits by itself after this long (safety net), 0 = 600 s */
@@ -207,6 +211,41 @@ int32_t cc_log_drain_stop(cc_ctx* ctx);
 
 /* ---- host-launched path -------------------------------------------------------------------- */
 
+/* One checkpoint of one region -- the general entry point; the named calls below are this call with fixed options.
+ *   discovery   where the dirty set comes from: CC_DISC_SCAN compare live vs shadow; CC_DISC_MARKS the
+ *               runtime's dirty-page bitmap (L257; mark_flags = CC_MARK_VERIFY / CC_MARK_CONSUME); CC_DISC_VERSIONS
+ *               per-page version counters (L257, L264); CC_DISC_ALL every page (base snapshot, L394)
+ *   run_pages   0 / 1: one record per dirty page; >= 2: run-length records (L221), a run never crossing a page index
+ *               that is a multiple of run_pages (run_pages * page_bytes < 2^32)
+ *   path        CC_PATH_SINGLE_PASS: ONE kernel launch -- warp tiles of pages are discovered, ranked by decoupled
+ *               look-back and written (records, CRC32C, shadow) by the same warp, the last warp of the grid commits
+ *               and publishes; needs run_pages <= 32 and at most 2^25 pages (CC_ERR_INVALID otherwise).  When the
+ *               worst case (every page dirty) does not fit behind the log's write offset, the same launch runs the
+ *               classic phases behind grid barriers instead (all-or-nothing needs the count first).
+ *               CC_PATH_PHASES: the classic phases as separate launches (discovery, ordered compaction,
+ *               [run ranking,] gather + commit), each sized for its own work.
+ *               CC_PATH_AUTO: single pass when the attached log is pinned host memory (the host-link transfer then
+ *               overlaps the scan); phases otherwise (with a device log they are faster at every size measured).
+ * Every path writes the same bytes.  Result, asynchrony, CC_ERR_LOG_FULL rule: as cc_checkpoint_delta below. */
+#define CC_DISC_SCAN 0u
+#define CC_DISC_MARKS 1u
+#define CC_DISC_VERSIONS 3u
+#define CC_DISC_ALL 4u
+#define CC_PATH_AUTO 0u
+#define CC_PATH_SINGLE_PASS 1u
+#define CC_PATH_PHASES 2u
+typedef struct {
+    uint32_t discovery;        /* CC_DISC_* */
+    uint32_t path;             /* CC_PATH_* */
+    uint32_t run_pages;
+    uint32_t mark_flags;       /* CC_DISC_MARKS: CC_MARK_* */
+    uint32_t* dirty_bitmap;    /* CC_DISC_MARKS: device, ceil(n_pages/32) u32 words */
+    const uint64_t* version;   /* CC_DISC_VERSIONS: device, n_pages u64 */
+    uint64_t* committed;       /* CC_DISC_VERSIONS: device, n_pages u64, advanced by the call */
+} cc_ckpt_opts;
+int32_t cc_checkpoint_ex(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, const cc_ckpt_opts* opts /* NULL = all zero */,
+                         void* stream, cc_result* out);
+
 /* Delta-checkpoint one region: scan live vs shadow per page, compact the
  * dirty page indices in ascending order, append k page records + one commit record at the log
  * write offset, refresh the shadow of the dirty pages, publish the committed offset.
@@ -219,13 +258,8 @@ int32_t cc_log_drain_stop(cc_ctx* ctx);
  * (cc_dirty_list). */
 int32_t cc_checkpoint_delta(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out);
 
-/* Same contract, same log bytes, same result as cc_checkpoint_delta, computed by the fused single pass
- * (DESIGN.md "Fused pass"): one kernel scans the region in page tiles, ranks the dirty pages by
- * decoupled look-back and -- when the worst case (every page dirty) fits behind the current log write
- * offset, so that all-or-nothing can be decided up front -- writes each tile's records, CRCs and shadow
- * right away, overlapping the record writer (and, for a pinned host log, the host-link transfer) with
- * the scan; otherwise the records are written by the gather kernel afterwards as in
- * cc_checkpoint_delta.  A short commit kernel follows in both cases. */
+/* Same contract, same log bytes, same result as cc_checkpoint_delta, always by the single pass
+ * (cc_checkpoint_ex with CC_PATH_SINGLE_PASS; cc_checkpoint_delta itself is CC_PATH_AUTO). */
 int32_t cc_checkpoint_delta_fused(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out);
 
 /* Delta checkpoint with RUN-LENGTH records ("Sparse page maps use index-value records;
@@ -233,7 +267,8 @@ int32_t cc_checkpoint_delta_fused(cc_ctx* ctx, uint32_t region_id, uint64_t epoc
  * form ONE record { region_id, first page, len = bytes of the whole run, crc32c(all payload bytes of the
  * run) } + the run's pages back to back.  A run never crosses a page index that is a multiple of
  * run_pages (>= 1, run_pages * page_bytes < 2^32), so it has at most run_pages pages; run_pages = 1 gives
- * cc_checkpoint_delta's bytes.  The commit record counts RECORDS; out->n_dirty still counts pages.
+ * cc_checkpoint_delta's bytes.  run_pages <= 32 follows CC_PATH_AUTO (single pass where that applies: runs are cut
+ * inside a warp tile, whose dirty mask is one register); larger run_pages take the phases.  The commit record counts RECORDS; out->n_dirty still counts pages.
  * cc_apply_log and cc_compact_log read both kinds of record (a single-page record is the run of length
  * one). */
 int32_t cc_checkpoint_delta_rle(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, uint32_t run_pages, void* stream,

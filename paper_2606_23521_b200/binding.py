@@ -44,10 +44,15 @@ CC_TASK_EXIT = 255
 CC_TASKF_FUSED = 1
 CC_TASKF_RLE = 2
 
+CC_WORKER_BLOCKS_DEFAULT = 16
+CC_WORKER_BLOCKS_ALL = 0xFFFFFFFF
+CC_DISC_SCAN, CC_DISC_MARKS, CC_DISC_VERSIONS, CC_DISC_ALL = 0, 1, 3, 4
+CC_PATH_AUTO, CC_PATH_SINGLE_PASS, CC_PATH_PHASES = 0, 1, 2
+
 EXPORTS = [
     "cc_init", "cc_shutdown", "cc_last_cuda_error", "cc_kernel_launches", "cc_workspace_bytes",
     "cc_register_region", "cc_unregister_region", "cc_log_attach", "cc_log_reset", "cc_log_reset_async", "cc_log_mirror_attach", "cc_log_drain", "cc_log_drain_start", "cc_log_drain_wait", "cc_log_drain_stop",
-    "cc_checkpoint_delta", "cc_checkpoint_delta_fused", "cc_checkpoint_delta_rle", "cc_checkpoint_marked", "cc_checkpoint_versions",
+    "cc_checkpoint_ex", "cc_checkpoint_delta", "cc_checkpoint_delta_fused", "cc_checkpoint_delta_rle", "cc_checkpoint_marked", "cc_checkpoint_versions",
     "cc_checkpoint_all", "cc_snapshot_region", "cc_compact_log", "cc_scan_only", "cc_trace_events", "cc_dirty_list", "cc_apply_scratch_bytes", "cc_apply_attach", "cc_apply_stage_attach", "cc_apply_log",
     "cc_worker_start", "cc_worker_stop", "cc_worker_alive", "cc_worker_footprint", "cc_peek_queue", "cc_submit", "cc_measure_submit_cost", "cc_measure_launch_cost", "cc_poll", "cc_wait",
 ]
@@ -63,6 +68,12 @@ class cc_region_desc(ctypes.Structure):
     _fields_ = [("region_id", ctypes.c_uint32), ("page_bytes", ctypes.c_uint32), ("bytes", ctypes.c_uint64),
                 ("base", ctypes.c_void_p), ("shadow", ctypes.c_void_p), ("workspace", ctypes.c_void_p),
                 ("workspace_bytes", ctypes.c_uint64), ("flags", ctypes.c_uint32), ("reserved", ctypes.c_uint32)]
+
+
+class cc_ckpt_opts(ctypes.Structure):
+    _fields_ = [("discovery", ctypes.c_uint32), ("path", ctypes.c_uint32), ("run_pages", ctypes.c_uint32),
+                ("mark_flags", ctypes.c_uint32), ("dirty_bitmap", ctypes.c_void_p), ("version", ctypes.c_void_p),
+                ("committed", ctypes.c_void_p)]
 
 
 class cc_result(ctypes.Structure):
@@ -115,6 +126,7 @@ def load_library():
         "cc_log_drain_start": (i32, [vp]),
         "cc_log_drain_wait": (i32, [vp, u64, u64]),
         "cc_log_drain_stop": (i32, [vp]),
+        "cc_checkpoint_ex": (i32, [vp, u32, u64, P(cc_ckpt_opts), vp, vp]),
         "cc_checkpoint_delta": (i32, [vp, u32, u64, vp, vp]),
         "cc_checkpoint_delta_fused": (i32, [vp, u32, u64, vp, vp]),
         "cc_checkpoint_delta_rle": (i32, [vp, u32, u64, u32, vp, vp]),
@@ -284,6 +296,17 @@ class Context:
     def checkpoint_delta(self, region_id: int, epoch: int, result: Result = None, stream=None):
         self._check("cc_checkpoint_delta", self.lib.cc_checkpoint_delta(
             self.h, region_id, epoch, _stream_ptr(stream), ctypes.c_void_p(result.ptr) if result else None))
+
+    def checkpoint_ex(self, region_id: int, epoch: int, result: Result = None, stream=None, discovery: int = CC_DISC_SCAN,
+                      path: int = CC_PATH_AUTO, run_pages: int = 0, dirty_bitmap: torch.Tensor = None, mark_flags: int = 0,
+                      version: torch.Tensor = None, committed: torch.Tensor = None):
+        """The general checkpoint call (cc_checkpoint_ex): discovery x record kind x path."""
+        o = cc_ckpt_opts(discovery, path, run_pages, mark_flags,
+                         dirty_bitmap.data_ptr() if dirty_bitmap is not None else None,
+                         version.data_ptr() if version is not None else None,
+                         committed.data_ptr() if committed is not None else None)
+        self._check("cc_checkpoint_ex", self.lib.cc_checkpoint_ex(
+            self.h, region_id, epoch, ctypes.byref(o), _stream_ptr(stream), ctypes.c_void_p(result.ptr) if result else None))
 
     def checkpoint_delta_fused(self, region_id: int, epoch: int, result: Result = None, stream=None):
         self._check("cc_checkpoint_delta_fused", self.lib.cc_checkpoint_delta_fused(

@@ -6,7 +6,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libconcordia.so")
 SOURCES = ["concordia.cu"]
-HEADERS = ["cc_common.cuh", "cc_crc.cuh", "cc_ckpt.cuh", "cc_mark.cuh", "cc_fused.cuh", "cc_rle.cuh", "cc_apply.cuh", "cc_compactor.cuh", "cc_batch.cuh", "cc_worker.cuh"]
+HEADERS = ["cc_common.cuh", "cc_crc.cuh", "cc_ckpt.cuh", "cc_mark.cuh", "cc_fused.cuh", "cc_pass.cuh", "cc_tasks.cuh", "cc_rle.cuh", "cc_apply.cuh",
+           "cc_apply_parse.cuh", "cc_compactor.cuh", "cc_batch.cuh", "cc_worker.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
 
@@ -24,7 +25,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or _stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         tmp = LIB + ".tmp.%d" % os.getpid()
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + \
+        extra = os.environ.get("CC_NVCC_FLAGS", "").split()         # e.g. -DCC_LD_NC=1 for an A/B build
+        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + \
               [os.path.join(CSRC, s) for s in SOURCES]
         subprocess.run(cmd, check=True)
         os.replace(tmp, LIB)

@@ -2,12 +2,13 @@
 // "Recovery ignores any suffix without a commit marker", L227 "replays ... committed AOF suffix").
 //
 // The sequential definition (walk record by record; hold page records pending until their commit
-// validates; apply epochs in log order) is reproduced exactly by five data-parallel phases:
-//   parse    one block walks the headers.  Inside an epoch all full-page records of a region
-//            have the same stride 16+P, so the block reads blockDim headers speculatively per
-//            step and accepts the leading run that is structurally valid; commit records, short
-//            tail pages and region changes are handled one at a time.  The walk stops at the
-//            first torn or structurally invalid record, exactly where the definition stops.
+// validates; apply epochs in log order) is reproduced exactly by data-parallel phases:
+//   parse    cc_apply_parse.cuh: candidate commit records by signature search over the whole log, then every
+//            epoch walked by its own block, chained by look-back (sequential record numbers); a one-block serial
+//            walk (below) is the fallback when the speculation does not hold (false candidates, list overflow).
+//            Inside an epoch all full-page records of a region have the same stride 16+P, so a walk reads
+//            blockDim headers speculatively per step and accepts the leading run that is structurally valid.
+//            The walk stops at the first torn or structurally invalid record, exactly where the definition stops.
 //   validate every 4 KiB payload segment is CRC'd by a warp; a record whose CRC differs lowers
 //            first_bad_rec (atomicMin).  The last block then resolves the committed prefix:
 //            the epochs whose records all precede the first failed check.
@@ -21,9 +22,11 @@
 
 struct cc_apply_tabs {      // carved out of the attached scratch
     cc_rec* recs;
-    cc_epoch_ent* epochs;
+    cc_epoch_ent* epochs;   // max_records + 1
     u64* rec_state;         // per-record {done-mask or count | CRC accumulator} (crc_record_combine)
     u32* seg_begin;         // per-record first segment number (+ one trailing total)
+    u32* cand;              // max_records + 1: candidate commit records, log offset / 16, ascending
+    u64* span_status;       // max_records + 2: look-back words of the epoch walk
     u64 max_records;
 };
 
@@ -101,12 +104,18 @@ __device__ __forceinline__ u32 cc_parse_examine(cc_dev* dev, const cc_apply_tabs
         }
         if (!ok) { A->struct_fail = 1; return CC_PA_STOP; }
         if (S->nepochs >= T.max_records) { A->scratch_overflow = 1; return CC_PA_STOP; }
-        if (S->pending != 0) {                   // for the log compactor: last epoch number per region
-            const int cs = cc_parse_find_slot(S, pl.z);
-            if (cs >= 0) dev->compactor.region_epoch[cs] = (u64)pl.x | ((u64)pl.y << 32);
+        {
+            const int cs = S->pending != 0 ? cc_parse_find_slot(S, pl.z) : -1;
+            if (cs >= 0) dev->compactor.region_last[cs] = S->nepochs + 1;       // for the log compactor: last epoch per region
+            cc_epoch_ent e;
+            e.off_after = off + CC_COMMIT_RECORD_BYTES;
+            e.epoch_no = (u64)pl.x | ((u64)pl.y << 32);
+            e.rec_end = S->nrecs;
+            e.slot = cs >= 0 ? (u32)cs : 0xFFFFFFFFu;
+            e.pending = S->pending;
+            e.pad = 0;
+            T.epochs[S->nepochs] = e;
         }
-        T.epochs[S->nepochs].off_after = off + CC_COMMIT_RECORD_BYTES;
-        T.epochs[S->nepochs].rec_end = S->nrecs;
         S->nepochs++;
         S->width = S->pending + 16u < 32u ? 32u : (S->pending + 16u > nthr ? nthr : S->pending + 16u);
         S->pending = 0; S->mixed = 0;
@@ -129,16 +138,30 @@ __device__ __forceinline__ u32 cc_parse_examine(cc_dev* dev, const cc_apply_tabs
 // sitting right behind the run usually holds the epoch's commit record -- it validates it from the bytes it
 // already has and examines the first header of the next epoch (also already loaded), so that the next step can
 // start its speculative reads at once.
-__device__ __forceinline__ void cc_apply_parse_phase(cc_dev* dev, const cc_apply_tabs& T, const u8* log, u64 n) {
+// One thread, before any parse phase: the applier's state for a new log.
+__device__ __forceinline__ void cc_apply_reset_state(cc_dev* dev) {
+    cc_apply_state* A = &dev->apply;
+    A->n_recs = 0; A->n_epochs = 0;
+    A->struct_fail = 0; A->scratch_overflow = 0; A->first_bad_rec = 0xFFFFFFFFu; A->validate_done = 0;
+    A->n_commit_recs = 0; A->n_commit_epochs = 0; A->consumed = 0; A->status = CC_OK; A->final_done = 0;
+    A->t_start_ns = globaltimer_ns();
+    for (int s = 0; s < CC_MAX_REGIONS; s++) dev->compactor.region_last[s] = 0;
+}
+
+// The serial walk: ONE block.  It is the fallback of the parallel parse (cc_apply_parse.cuh) and runs only when
+// that raised need_serial (force = false), or as the parser proper (force = true).
+__device__ __forceinline__ void cc_apply_parse_phase(cc_dev* dev, const cc_apply_tabs& T, const u8* log, u64 n, bool force) {
     __shared__ cc_parse_smem S;
     cc_apply_state* A = &dev->apply;
     const u32 tid = threadIdx.x, nthr = blockDim.x;
+    if (!force && !dev->parse.need_serial) return;
+    __syncthreads();                             // (every thread has read need_serial before it is touched)
     if (tid == 0) {
         S.off = 0; S.nrecs = 0; S.nepochs = 0; S.pending = 0; S.pend_rid = 0; S.mixed = 0; S.segs = 0; S.pre = 0;
         S.action = CC_PA_STOP; S.cand = 0xFFFFFFFFu; S.width = nthr < 128u ? nthr : 128u;
-        A->struct_fail = 0; A->scratch_overflow = 0; A->first_bad_rec = 0xFFFFFFFFu; A->validate_done = 0;
-        A->n_commit_recs = 0; A->n_commit_epochs = 0; A->consumed = 0; A->status = CC_OK; A->final_done = 0;
-        A->t_start_ns = globaltimer_ns();
+        const u64 t0 = A->t_start_ns;
+        cc_apply_reset_state(dev);
+        if (!force) A->t_start_ns = t0;
     }
     if (tid < CC_MAX_REGIONS) {
         const bool used = dev->region_used[tid] != 0;
@@ -220,6 +243,8 @@ __device__ __forceinline__ void cc_apply_parse_phase(cc_dev* dev, const cc_apply
     }
 }
 
+#include "cc_apply_parse.cuh"
+
 // warp-cooperative search: largest rec with seg_begin[rec] <= item, rec in [0, n)
 __device__ __forceinline__ u32 cc_find_rec(const u32* seg_begin, u32 n, u32 item, u32 lane) {
     u32 lo = 0, hi = n;
@@ -234,38 +259,50 @@ __device__ __forceinline__ u32 cc_find_rec(const u32* seg_begin, u32 n, u32 item
     return lo;
 }
 
+#define CC_APPLY_CHUNK 4u       // consecutive 4 KiB segments one warp takes per search of the record table
+
 __device__ __forceinline__ void cc_apply_validate_phase(cc_dev* dev, const cc_apply_tabs& T, cc_crc_smem* cs,
                                                         const u8* log, cc_grid g, bool init_tables) {
     constexpr int U = 8;
     cc_apply_state* A = &dev->apply;
     const u32 n_recs = A->n_recs;
     const u32 lane = threadIdx.x & 31u;
+    if (g.block == 0 && threadIdx.x == 0) dev->parse.wticket = 0;      // (the walk is over) for the next parse
     if (n_recs != 0 && !A->scratch_overflow) {
         if (init_tables) cc_crc_smem_init(cs, &dev->crc);
         const u32 n_items = T.seg_begin[n_recs];
-        for (u32 item = g.warp(); item < n_items; item += g.nwarps()) {
-            const u32 ri = cc_find_rec(T.seg_begin, n_recs, item, lane);
-            const cc_rec rec = T.recs[ri];
-            const u32 c = item - T.seg_begin[ri];
-            const u64 so = (u64)c * CC_SEG_BYTES;
-            const u64 rem = rec.len - so;
-            const u32 seg_len = (u32)(rem < CC_SEG_BYTES ? rem : CC_SEG_BYTES);
-            const u32 nv = seg_len >> 4;
-            const u32 nseg = (rec.len + CC_SEG_BYTES - 1) / CC_SEG_BYTES;
-            const uint4* src = reinterpret_cast<const uint4*>(log + rec.off + CC_RECORD_HEADER_BYTES + so);
-            uint4 v[U];
+        const u32 n_chunks = (n_items + CC_APPLY_CHUNK - 1) / CC_APPLY_CHUNK;
+        // from the END of the log to its head: the candidate search has just streamed the log front to back, so
+        // its tail is what the L2 still holds
+        for (u32 ch = g.warp(); ch < n_chunks; ch += g.nwarps()) {
+            const u32 item0 = (n_chunks - 1 - ch) * CC_APPLY_CHUNK;
+            const u32 item1 = item0 + CC_APPLY_CHUNK < n_items ? item0 + CC_APPLY_CHUNK : n_items;
+            u32 ri = cc_find_rec(T.seg_begin, n_recs, item0, lane);
+            cc_rec rec = T.recs[ri];
+            u32 sb = T.seg_begin[ri], next = T.seg_begin[ri + 1];
+            for (u32 item = item0; item < item1; item++) {
+                while (item >= next) { ri++; rec = T.recs[ri]; sb = next; next = T.seg_begin[ri + 1]; }
+                const u32 c = item - sb;
+                const u64 so = (u64)c * CC_SEG_BYTES;
+                const u64 rem = rec.len - so;
+                const u32 seg_len = (u32)(rem < CC_SEG_BYTES ? rem : CC_SEG_BYTES);
+                const u32 nv = seg_len >> 4;
+                const u32 nseg = (rec.len + CC_SEG_BYTES - 1) / CC_SEG_BYTES;
+                const uint4* src = reinterpret_cast<const uint4*>(log + rec.off + CC_RECORD_HEADER_BYTES + so);
+                uint4 v[U];
 #pragma unroll
-            for (int u = 0; u < U; u++) {
-                const u32 j = lane + 32 * u;
-                v[u] = (j < nv) ? ld_v4(src + j) : make_uint4(0, 0, 0, 0);
-            }
-            const u32 contrib = crc_segment_warp<U>(cs, &dev->crc, v, nv, rem - seg_len, lane);
-            if (lane == 0) {
-                u32 acc = 0;
-                const bool finish = crc_record_combine(&T.rec_state[ri], nseg, c, contrib, &acc);
-                if (finish) {
-                    const u32 it = cc_crc_init_term(dev, dev->regions[rec.slot], rec.len);
-                    if (crc_finalize(acc, it) != rec.crc) atomicMin(&A->first_bad_rec, ri);
+                for (int u = 0; u < U; u++) {
+                    const u32 j = lane + 32 * u;
+                    v[u] = (j < nv) ? ld_v4(src + j) : make_uint4(0, 0, 0, 0);
+                }
+                const u32 contrib = crc_segment_warp<U>(cs, &dev->crc, v, nv, rem - seg_len, lane);
+                if (lane == 0) {
+                    u32 acc = 0;
+                    const bool finish = crc_record_combine(&T.rec_state[ri], nseg, c, contrib, &acc);
+                    if (finish) {
+                        const u32 it = cc_crc_init_term(dev, dev->regions[rec.slot], rec.len);
+                        if (crc_finalize(acc, it) != rec.crc) atomicMin(&A->first_bad_rec, ri);
+                    }
                 }
             }
         }
@@ -294,6 +331,8 @@ __device__ __forceinline__ void cc_apply_validate_phase(cc_dev* dev, const cc_ap
         A->consumed = E ? T.epochs[E - 1].off_after : 0;
         A->status = st;
         A->validate_done = 0;
+        dev->parse.cand_overflow = 0;             // re-arm the parallel parse for the next log
+        dev->parse.need_serial = 0;
         __threadfence();
     }
 }
@@ -314,35 +353,42 @@ __device__ __forceinline__ void cc_apply_scatter_phase(cc_dev* dev, const cc_app
     if (n == 0) return;
     const u32 lane = threadIdx.x & 31u;
     const u32 n_items = T.seg_begin[n];
-    for (u32 item = g.warp(); item < n_items; item += g.nwarps()) {
-        const u32 ri = cc_find_rec(T.seg_begin, n, item, lane);
-        const cc_rec rec = T.recs[ri];
-        const cc_region_dev& r = dev->regions[rec.slot];
-        const u32 c = item - T.seg_begin[ri];
-        const u64 so = (u64)c * CC_SEG_BYTES;
-        const u64 rem = rec.len - so;
-        const u32 nv = (u32)(rem < CC_SEG_BYTES ? rem : CC_SEG_BYTES) >> 4;
-        // a page takes its bytes from its LATEST record only.  A segment lies inside one page when pages are
-        // whole multiples of 4 KiB (or the record is a single page); otherwise the check is per 16-byte vector.
-        const bool one_page = (r.page_bytes % CC_SEG_BYTES == 0) || rec.len <= r.page_bytes;
-        if (one_page && r.latest[rec.page_idx + (u32)(so / r.page_bytes)] != ri + 1) continue;
-        const uint4* src = reinterpret_cast<const uint4*>(log + rec.off + CC_RECORD_HEADER_BYTES + so);
-        const u64 dst_off = (u64)rec.page_idx * r.page_bytes + so;
-        uint4* d0 = reinterpret_cast<uint4*>(r.base + dst_off);
-        uint4* d1 = reinterpret_cast<uint4*>(r.shadow + dst_off);
-        uint4 v[U];
-        bool take[U];
+    const u32 n_chunks = (n_items + CC_APPLY_CHUNK - 1) / CC_APPLY_CHUNK;
+    for (u32 ch = g.warp(); ch < n_chunks; ch += g.nwarps()) {
+        const u32 item0 = ch * CC_APPLY_CHUNK;
+        const u32 item1 = item0 + CC_APPLY_CHUNK < n_items ? item0 + CC_APPLY_CHUNK : n_items;
+        u32 ri = cc_find_rec(T.seg_begin, n, item0, lane);
+        cc_rec rec = T.recs[ri];
+        u32 sb = T.seg_begin[ri], next = T.seg_begin[ri + 1];
+        for (u32 item = item0; item < item1; item++) {
+            while (item >= next) { ri++; rec = T.recs[ri]; sb = next; next = T.seg_begin[ri + 1]; }
+            const cc_region_dev& r = dev->regions[rec.slot];
+            const u32 c = item - sb;
+            const u64 so = (u64)c * CC_SEG_BYTES;
+            const u64 rem = rec.len - so;
+            const u32 nv = (u32)(rem < CC_SEG_BYTES ? rem : CC_SEG_BYTES) >> 4;
+            // a page takes its bytes from its LATEST record only.  A segment lies inside one page when pages are
+            // whole multiples of 4 KiB (or the record is a single page); otherwise the check is per 16-byte vector.
+            const bool one_page = (r.page_bytes % CC_SEG_BYTES == 0) || rec.len <= r.page_bytes;
+            if (one_page && r.latest[rec.page_idx + (u32)(so / r.page_bytes)] != ri + 1) continue;
+            const uint4* src = reinterpret_cast<const uint4*>(log + rec.off + CC_RECORD_HEADER_BYTES + so);
+            const u64 dst_off = (u64)rec.page_idx * r.page_bytes + so;
+            uint4* d0 = reinterpret_cast<uint4*>(r.base + dst_off);
+            uint4* d1 = reinterpret_cast<uint4*>(r.shadow + dst_off);
+            uint4 v[U];
+            bool take[U];
 #pragma unroll
-        for (int u = 0; u < U; u++) {
-            const u32 j = lane + 32 * u;
-            take[u] = j < nv;
-            if (take[u] && !one_page) take[u] = r.latest[rec.page_idx + (u32)((so + 16ull * j) / r.page_bytes)] == ri + 1;
-            if (take[u]) v[u] = ld_v4(src + j);
-        }
+            for (int u = 0; u < U; u++) {
+                const u32 j = lane + 32 * u;
+                take[u] = j < nv;
+                if (take[u] && !one_page) take[u] = r.latest[rec.page_idx + (u32)((so + 16ull * j) / r.page_bytes)] == ri + 1;
+                if (take[u]) v[u] = ld_v4(src + j);
+            }
 #pragma unroll
-        for (int u = 0; u < U; u++) {
-            const u32 j = lane + 32 * u;
-            if (take[u]) { st_stream(d0 + j, v[u]); if (r.shadow) st_stream(d1 + j, v[u]); }
+            for (int u = 0; u < U; u++) {
+                const u32 j = lane + 32 * u;
+                if (take[u]) { st_stream(d0 + j, v[u]); if (r.shadow) st_stream(d1 + j, v[u]); }
+            }
         }
     }
 }

@@ -1,0 +1,336 @@
+// cc_apply_parse.cuh -- a6, parallel parse of the log.
+//
+// The sequential definition walks record by record; every epoch ends in a 32-byte commit record.  Here the epochs
+// are parsed CONCURRENTLY, with exactly the sequential result:
+//   candidates  every 16-byte-aligned position of the log is tested for a commit record's signature
+//               {0xFFFFFFFF, 0xFFFFFFFF, 16, crc32c(next 16 bytes)}; the positions that pass are listed in ascending
+//               order (contiguous ranges per block by ticket, per-warp ordered lists, look-back over the tickets).
+//               Every real commit record is on the list; a payload that happens to contain the image of a commit
+//               record puts a FALSE candidate on it.
+//   walk        span j = [end of candidate j-1, candidate j) is walked by one block from its start, as the sequential
+//               parser would (speculative strided header reads inside a run of equal-sized records).  A span whose walk
+//               lands exactly on its candidate is one committed epoch.  Spans are chained in order by a decoupled
+//               look-back that carries (records, segments) of all earlier spans -- the record numbers are therefore
+//               the sequential ones.  The first span of the chain that does NOT end on its candidate is where the
+//               sequential parser stops (torn or structurally invalid: its partial records are kept, pending, exactly
+//               as the definition holds them) -- unless the walk ran PAST its candidate (a false candidate inside a
+//               payload): then, and when the candidate list overflows, `need_serial` is raised and the one-block serial
+//               parser of cc_apply.cuh redoes the parse.  Correctness never depends on the speculation.
+#pragma once
+#include "cc_common.cuh"
+#include "cc_crc.cuh"
+#include "cc_ckpt.cuh"
+
+#define CC_CAND_THREADS 256
+#define CC_CAND_WARP_CAP 256u            // candidates one warp can hold for its part of a range
+#define CC_WALK_THREADS 128
+
+// span look-back word: bits 0-30 records, bits 31-61 segments, bits 62-63 flag
+#define CC_SP_AGG 1ull
+#define CC_SP_INC 2ull
+#define CC_SP_STOP 3ull
+__device__ __forceinline__ u64 sp_pack(u64 flag, u32 recs, u32 segs) { return (flag << 62) | ((u64)segs << 31) | recs; }
+__device__ __forceinline__ u32 sp_recs(u64 w) { return (u32)(w & 0x7FFFFFFFull); }
+__device__ __forceinline__ u32 sp_segs(u64 w) { return (u32)((w >> 31) & 0x7FFFFFFFull); }
+__device__ __forceinline__ u32 sp_flag(u64 w) { return (u32)(w >> 62); }
+
+// ---------------------------------------------------------------------------- candidates --
+// grid-wide; scratch: T.cand[0 .. max_records], T.span_status[0 .. max_records + 1]
+__device__ __forceinline__ void cc_parse_cand_phase(cc_dev* dev, cc_parse_ctl* C, u32* cand, u64* span_status, u64 max_records,
+                                                    const u8* log, u64 n, bool first_block) {
+    __shared__ u32 s_list[CC_CAND_THREADS / 32][CC_CAND_WARP_CAP];
+    __shared__ u32 s_cnt[CC_CAND_THREADS / 32];
+    __shared__ u32 s_ticket, s_base, s_over;
+    const u32 tid = threadIdx.x, lane = tid & 31u, wid = tid >> 5;
+    constexpr u32 NW = CC_CAND_THREADS / 32;
+    const u64 units = n >> 4;                                    // 16-byte units of the log
+    // ranges of whole 4 KiB steps per warp, at most CC_CAND_TICKETS of them, at least 128 KiB each (fine ranges spread
+    // a few-hundred-MB log evenly over the SMs: 1 MiB ranges left half of them with twice the work of the rest)
+    u64 range_units = (units + CC_CAND_TICKETS - 1) / CC_CAND_TICKETS;
+    if (range_units < (1u << 13)) range_units = 1u << 13;
+    range_units = (range_units + 2047) / 2048 * 2048;            // a multiple of NW warps x 256 units
+    const u32 n_ranges = (u32)((units + range_units - 1) / range_units);
+    const u64 warp_units = range_units / NW;
+    const u32 run = C->run & 0x3FFFFFFFu;
+    if (n_ranges == 0) {                                         // a log shorter than 16 bytes: nothing to find
+        if (first_block && tid == 0) { cc_apply_reset_state(dev); C->n_cand = 0; span_status[0] = 0; }
+        return;
+    }
+    for (;;) {
+        if (tid == 0) { s_ticket = atomicAdd(&C->ticket, 1u); s_over = 0; }
+        if (lane == 0) s_cnt[wid] = 0;
+        __syncthreads();
+        const u32 t = s_ticket;
+        if (t >= n_ranges) break;
+        // warp `wid` owns the contiguous part [u0, u1) of the range and keeps its hits in ascending order
+        const u64 u0 = (u64)t * range_units + (u64)wid * warp_units;
+        u64 u1 = u0 + warp_units;
+        if (u1 > units) u1 = units;
+        u32 cnt = 0;
+        for (u64 ub = u0; ub < u1; ub += 256) {
+            uint4 v[8];
+#pragma unroll
+            for (int q = 0; q < 8; q++) {
+                const u64 u = ub + 32u * q + lane;
+                v[q] = (u < u1) ? ld_v4(reinterpret_cast<const uint4*>(log) + u) : make_uint4(0, 0, 0, 0);
+            }
+#pragma unroll
+            for (int q = 0; q < 8; q++) {
+                const u64 u = ub + 32u * q + lane;
+                bool hit = (v[q].x == CC_COMMIT_ID) && (v[q].y == CC_COMMIT_ID) && (v[q].z == 16u) && (u + 2 <= units) && (u < u1);
+                if (hit) {                                       // rare: check the commit payload's CRC
+                    const uint4 pl = ld_v4(reinterpret_cast<const uint4*>(log) + u + 1);
+                    u32 pay[4] = {pl.x, pl.y, pl.z, pl.w};
+                    hit = crc_serial(&dev->crc, reinterpret_cast<const u8*>(pay), 16) == v[q].w;
+                }
+                const u32 b = __ballot_sync(0xFFFFFFFFu, hit);
+                if (hit) {
+                    const u32 pos = cnt + __popc(b & ((1u << lane) - 1u));
+                    if (pos < CC_CAND_WARP_CAP) s_list[wid][pos] = (u32)u;
+                }
+                cnt += __popc(b);
+            }
+        }
+        if (lane == 0) { s_cnt[wid] = cnt; if (cnt > CC_CAND_WARP_CAP) s_over = 1; }
+        __syncthreads();
+        u32 before = 0, total = 0;
+        for (u32 w = 0; w < NW; w++) { const u32 c = s_cnt[w]; if (w < wid) before += c; total += c; }
+        if (tid == 0) {
+            u32 excl = 0;
+            if (t == 0) {
+                cc_apply_reset_state(dev);                       // (read by the walk phase, which starts after this one)
+                span_status[0] = 0;
+                st_release_gpu_u64(&C->cand_status[0], lb_pack(run, CC_LB_INC, total));
+            } else {
+                st_release_gpu_u64(&C->cand_status[t], lb_pack(run, CC_LB_AGG, total));
+                int j = (int)t - 1;
+                while (j >= 0) {
+                    const u64 s = ld_acquire_gpu_u64(&C->cand_status[j]);
+                    if ((u32)(s >> 34) != run || ((s >> 32) & 3ull) == 0) { __nanosleep(20); continue; }
+                    excl += (u32)s;
+                    if (((s >> 32) & 3ull) == CC_LB_INC) break;
+                    j--;
+                }
+                st_release_gpu_u64(&C->cand_status[t], lb_pack(run, CC_LB_INC, excl + total));
+            }
+            s_base = excl;
+            if (s_over) C->cand_overflow = 1;
+            if (t == n_ranges - 1) C->n_cand = excl + total;     // every earlier range has published
+        }
+        __syncthreads();
+        const u32 base = s_base + before;
+        const u32 mine = cnt < CC_CAND_WARP_CAP ? cnt : CC_CAND_WARP_CAP;
+        for (u32 i = lane; i < mine; i += 32) {
+            const u64 idx = (u64)base + i;
+            if (idx <= max_records) { cand[idx] = s_list[wid][i]; span_status[idx + 1] = 0; }
+            else C->cand_overflow = 1;
+        }
+        __syncthreads();
+    }
+}
+
+// ---------------------------------------------------------------------------------- walk --
+struct cc_walk_smem {
+    u64 r_bytes[CC_MAX_REGIONS], r_pages[CC_MAX_REGIONS];
+    u32 r_id[CC_MAX_REGIONS], r_P[CC_MAX_REGIONS], r_spp[CC_MAX_REGIONS];
+    u64 off;                 // next unread record
+    u32 nrec, nseg;          // records / segments of this span so far
+    u32 pend_rid, mixed, slot, have_slot;
+    u32 first_fail, first_short, width;
+    u32 outcome;             // CC_WO_*
+    u32 ticket;
+    u32 base_recs, base_segs, dead;
+    uint4 cpl;               // payload of the commit record the walk landed on
+};
+#define CC_WO_RUN 0u         // still walking
+#define CC_WO_COMMIT 1u      // landed exactly on the span's candidate: a committed epoch
+#define CC_WO_TORN 2u        // ran out of bytes: the sequential parser stops here, status OK
+#define CC_WO_CORRUPT 3u     // a structural check failed: the sequential parser stops here, CC_ERR_CORRUPT
+#define CC_WO_IRREGULAR 4u   // ran past the candidate (a false one): the serial parser takes over
+
+__device__ __forceinline__ int cc_walk_find_slot(const cc_walk_smem* S, u32 rid) {
+    for (int q = 0; q < CC_MAX_REGIONS; q++)
+        if (S->r_id[q] == rid) return rid ? q : -1;
+    return -1;
+}
+__device__ __forceinline__ bool cc_walk_len_ok(const cc_walk_smem* S, u32 slot, u64 page_idx, u64 len) {
+    if (page_idx >= S->r_pages[slot] || len == 0) return false;
+    const u64 start = page_idx * (u64)S->r_P[slot];
+    if (len > S->r_bytes[slot] - start) return false;
+    return (len % S->r_P[slot] == 0) || (start + len == S->r_bytes[slot]);
+}
+
+// One pass over span [start, target): WRITE = false only counts, WRITE = true also fills the record tables at
+// (base_recs, base_segs).  Block-wide; the result is in S (outcome, nrec, nseg, off, pend_rid, mixed, cpl).
+template <bool WRITE>
+__device__ __forceinline__ void cc_walk_span(const cc_apply_tabs& T, const u8* log, u64 n, cc_walk_smem* S, u64 start, u64 target,
+                                             bool has_target, u32 epoch_idx, u32 base_recs, u32 base_segs) {
+    const u32 tid = threadIdx.x, nthr = blockDim.x;
+    if (tid == 0) {
+        S->off = start; S->nrec = 0; S->nseg = 0; S->pend_rid = 0; S->mixed = 0; S->have_slot = 0; S->outcome = CC_WO_RUN;
+        S->width = has_target ? nthr : 32;      // a span with a target is bounded by it: speculate over the whole block at once
+    }
+    __syncthreads();
+    for (;;) {
+        // ---- one thread examines the record at S->off ----
+        if (tid == 0) {
+            const u64 off = S->off;
+            u32 oc = CC_WO_RUN;
+            if (has_target && off > target) oc = CC_WO_IRREGULAR;
+            else if (n - off < CC_RECORD_HEADER_BYTES) oc = CC_WO_TORN;
+            else {
+                const uint4 h = ld_v4(reinterpret_cast<const uint4*>(log + off));
+                if ((u64)h.z > n - off - CC_RECORD_HEADER_BYTES) oc = CC_WO_TORN;
+                else if (h.x == CC_COMMIT_ID) {
+                    // a commit header.  Its signature and CRC hold iff the position is a candidate; the only
+                    // candidate the walk can meet first is its own target
+                    if (has_target && off == target) {
+                        const uint4 pl = ld_v4(reinterpret_cast<const uint4*>(log + off + 16));
+                        const bool ok = (pl.w == S->nrec) && !S->mixed && (S->nrec == 0 || S->pend_rid == pl.z);
+                        S->cpl = pl;
+                        oc = ok ? CC_WO_COMMIT : CC_WO_CORRUPT;
+                    } else oc = CC_WO_CORRUPT;
+                } else {
+                    const int slot = cc_walk_find_slot(S, h.x);
+                    if (slot < 0 || !cc_walk_len_ok(S, (u32)slot, h.y, h.z)) oc = CC_WO_CORRUPT;
+                    else {
+                        if (S->nrec != 0 && S->pend_rid != h.x) S->mixed = 1;
+                        S->pend_rid = h.x;
+                        S->slot = (u32)slot;
+                        S->have_slot = 1;
+                        S->first_fail = nthr;
+                        S->first_short = nthr + 1;
+                    }
+                }
+            }
+            S->outcome = oc;
+        }
+        __syncthreads();
+        if (S->outcome != CC_WO_RUN) break;
+        // ---- speculative run: thread t reads the header at off + t * (16 + P) ----
+        const u32 slot = S->slot, rid = S->r_id[slot], spp = S->r_spp[slot];
+        const u64 P = S->r_P[slot];
+        const u64 stride = P + CC_RECORD_HEADER_BYTES;
+        const u64 off_t = S->off + (u64)tid * stride;
+        const u32 width = S->width;
+        const bool active = tid < width;
+        // positions at or beyond the target are never part of the run (the target itself is the commit record)
+        const bool in_h = active && off_t + 16 <= n && (!has_target || off_t < target);
+        uint4 h = make_uint4(0, 0, 0, 0);
+        if (in_h) h = ld_v4(reinterpret_cast<const uint4*>(log + off_t));
+        bool ok = in_h;
+        if (ok) ok = ((u64)h.z <= n - off_t - CC_RECORD_HEADER_BYTES) && (h.x == rid) && cc_walk_len_ok(S, slot, h.y, h.z);
+        const bool full = ok && ((u64)h.z == P);
+        if (active && !ok) atomicMin(&S->first_fail, tid);
+        else if (active && !full) { atomicMin(&S->first_fail, tid + 1); atomicMin(&S->first_short, tid + 1); }
+        __syncthreads();
+        const u32 run = S->first_fail < width ? S->first_fail : width;      // >= 1: record 0 was examined above
+        if (WRITE && tid < run) {
+            const u64 ri = (u64)base_recs + S->nrec + tid;
+            if (ri < T.max_records) {
+                cc_rec rec;
+                rec.off = off_t; rec.page_idx = h.y; rec.len = h.z; rec.crc = h.w;
+                rec.slot = slot; rec.epoch_idx = epoch_idx; rec.pad = 0;
+                T.recs[ri] = rec;
+                T.rec_state[ri] = 0;
+                T.seg_begin[ri] = base_segs + S->nseg + tid * spp;         // only the run's last record can be short
+            }
+        }
+        __syncthreads();
+        if (tid == run - 1) {
+            S->off = off_t + CC_RECORD_HEADER_BYTES + h.z;
+            S->nrec += run;
+            S->nseg += (run - 1) * spp + (h.z + CC_SEG_BYTES - 1) / CC_SEG_BYTES;
+            if (run == width) S->width = 2 * width > nthr ? nthr : 2 * width;
+        }
+        __syncthreads();
+    }
+}
+
+// grid-wide, blocks of CC_WALK_THREADS.  Needs: C->n_cand, T.cand, T.span_status (zeroed for 0..n_cand), A reset.
+__device__ __forceinline__ void cc_parse_walk_phase(cc_dev* dev, cc_parse_ctl* C, const cc_apply_tabs& T, const u8* log, u64 n, bool first_block) {
+    __shared__ cc_walk_smem S;
+    cc_apply_state* A = &dev->apply;
+    const u32 tid = threadIdx.x;
+    if (first_block && tid == 0) { C->ticket = 0; C->run = C->run + 1; }      // (the candidate search is over) for the next parse
+    if (C->cand_overflow) {                                       // the list is incomplete: the serial parser does it all
+        if (first_block && tid == 0) C->need_serial = 1;
+        return;
+    }
+    if (tid < CC_MAX_REGIONS) {
+        const bool used = dev->region_used[tid] != 0;
+        const cc_region_dev& rg = dev->regions[tid];
+        S.r_id[tid] = used ? rg.region_id : 0u;
+        S.r_P[tid] = used ? rg.page_bytes : 1u;
+        S.r_spp[tid] = used ? rg.spp : 1u;
+        S.r_bytes[tid] = used ? rg.bytes : 0ull;
+        S.r_pages[tid] = used ? rg.n_pages : 0ull;
+    }
+    const u32 m = C->n_cand;
+    const u32 n_spans = m + 1;                                    // the last span has no candidate: the tail of the log
+    for (;;) {
+        __syncthreads();
+        if (tid == 0) S.ticket = atomicAdd(&C->wticket, 1u);
+        __syncthreads();
+        const u32 j = S.ticket;
+        if (j >= n_spans) break;
+        const u64 start = j ? ((u64)T.cand[j - 1] << 4) + CC_COMMIT_RECORD_BYTES : 0ull;
+        const bool has_target = j < m;
+        const u64 target = has_target ? ((u64)T.cand[j] << 4) : 0ull;
+        cc_walk_span<false>(T, log, n, &S, start, target, has_target, j, 0, 0);
+        const u32 oc = S.outcome, nrec = S.nrec, nseg = S.nseg;
+        // ---- chain: records / segments of all earlier spans; dead if an earlier span stopped the parse ----
+        if (tid == 0) {
+            u32 br = 0, bs = 0, dead = 0;
+            if (j != 0) {
+                st_release_gpu_u64(&T.span_status[j], sp_pack(oc == CC_WO_COMMIT ? CC_SP_AGG : CC_SP_STOP, nrec, nseg));
+                int q = (int)j - 1;
+                while (q >= 0) {
+                    const u64 s = ld_acquire_gpu_u64(&T.span_status[q]);
+                    const u32 f = sp_flag(s);
+                    if (f == 0) { __nanosleep(20); continue; }
+                    if (f == CC_SP_STOP) { dead = 1; break; }
+                    br += sp_recs(s); bs += sp_segs(s);
+                    if (f == CC_SP_INC) break;
+                    q--;
+                }
+            }
+            S.base_recs = br; S.base_segs = bs; S.dead = dead;
+        }
+        __syncthreads();
+        if (S.dead) {                                             // something before this span ended the parse
+            if (tid == 0) st_release_gpu_u64(&T.span_status[j], sp_pack(CC_SP_STOP, 0, 0));
+            continue;
+        }
+        const u32 br = S.base_recs, bs = S.base_segs;
+        const bool overflow = (u64)br + nrec > T.max_records || (oc == CC_WO_COMMIT && (u64)j >= T.max_records);
+        if (!overflow && oc != CC_WO_IRREGULAR && nrec != 0)
+            cc_walk_span<true>(T, log, n, &S, start, target, has_target, j, br, bs);
+        if (tid == 0) {
+            if (oc == CC_WO_COMMIT && !overflow) {
+                cc_epoch_ent e;
+                e.off_after = target + CC_COMMIT_RECORD_BYTES;
+                e.epoch_no = (u64)S.cpl.x | ((u64)S.cpl.y << 32);
+                e.rec_end = br + nrec;
+                e.slot = S.have_slot ? S.slot : 0xFFFFFFFFu;
+                e.pending = nrec;
+                e.pad = 0;
+                T.epochs[j] = e;
+                if (nrec != 0) atomicMax(&dev->compactor.region_last[S.slot], j + 1);
+                __threadfence();
+                st_release_gpu_u64(&T.span_status[j], sp_pack(CC_SP_INC, br + nrec, bs + nseg));
+            } else {
+                // this span ends the parse: totals, and why
+                if (oc == CC_WO_IRREGULAR) C->need_serial = 1;
+                if (overflow) A->scratch_overflow = 1;
+                if (oc == CC_WO_CORRUPT) A->struct_fail = 1;
+                const u32 kept = (overflow || oc == CC_WO_IRREGULAR) ? 0u : nrec;
+                A->n_recs = br + kept;
+                A->n_epochs = j;
+                T.seg_begin[br + kept] = bs + (kept ? nseg : 0u);      // table has max_records + 1 entries
+                __threadfence();
+                st_release_gpu_u64(&T.span_status[j], sp_pack(CC_SP_STOP, 0, 0));
+            }
+        }
+    }
+}

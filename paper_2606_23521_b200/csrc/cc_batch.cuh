@@ -60,7 +60,7 @@ __device__ __forceinline__ void cc_batch_scan_phase(cc_dev* dev, cc_batch_tab* T
         u64 n = 0;
         if (cc_batch_takes_part(dev, s)) {
             const cc_region_dev& r = dev->regions[s];
-            n = r.n_pages * (u64)r.spp;
+            n = cc_scan_item_count<8>(r, g.nwarps());
             if (g.block == 0) {                             // open the region's compaction run (as cc_scan_phase does)
                 r.hdr->t_start_ns = globaltimer_ns();
                 r.hdr->ticket = 0;

@@ -7,57 +7,80 @@
 
 // ------------------------------------------------------------------------- a1: scan --
 // dirty[p] = any byte of cur page p differs from shadow page p.
-// Work item = one 4 KiB segment of one page, handled by one warp: each lane issues 8 + 8
-// independent 16-byte streaming loads (cur, shadow), XOR/ORs them, the warp votes, and lane 0
-// sets the page's bit in the bitmap only if the segment differs.  The bitmap is all-zero on
-// entry (the compaction clears what it consumes).
+// One warp compares 4 KiB segments: each lane issues 8 + 8 independent 16-byte streaming loads (cur, shadow),
+// XOR/ORs them, the warp votes.  A work item is a whole page when there are pages enough to keep every warp busy
+// (else a single segment): the warp walks the page's segments in order and STOPS at the first one that differs
+// (per-page early-out: the rest of a dirty page is not read -- the gather reads it anyway), then lane 0 sets the
+// page's bit in the bitmap.  The bitmap is all-zero on entry (the compaction clears what it consumes).
 // Items first, first + step, ... of the region (the caller decides which warp takes which items).
+// segments per work item for a grid of `nwarps` warps: the whole page if that still leaves >= 4 items per warp, else
+// halved until it does (1 when the page's segment count is not a power of two)
+template <int U>
+__device__ __forceinline__ u32 cc_scan_group(const cc_region_dev& r, u64 nwarps) {
+    const u32 spp = (r.page_bytes + 512u * U - 1) / (512u * U);
+    if (spp & (spp - 1)) return 1;
+    u32 G = spp;
+    while (G > 1 && r.n_pages * (u64)(spp / G) < 4 * nwarps) G >>= 1;
+    return G;
+}
+template <int U>
+__device__ __forceinline__ u64 cc_scan_item_count(const cc_region_dev& r, u64 nwarps) {
+    const u32 spp = (r.page_bytes + 512u * U - 1) / (512u * U);
+    return r.n_pages * (u64)(spp / cc_scan_group<U>(r, nwarps));
+}
+
 template <int U>
 __device__ __forceinline__ void cc_scan_items(const cc_region_dev& r, u64 first, u64 step) {
     const u32 lane = threadIdx.x & 31u;
-    constexpr u32 SEGV = 32u * U;            // vectors per item
-    constexpr u32 SEGB = SEGV * 16u;         // bytes per item
+    constexpr u32 SEGV = 32u * U;            // vectors per segment
+    constexpr u32 SEGB = SEGV * 16u;         // bytes per segment
     const u32 P = r.page_bytes;
     const u32 spp = (P + SEGB - 1) / SEGB;
-    const u64 n_items = r.n_pages * (u64)spp;
     const bool pow2 = (spp & (spp - 1)) == 0;
-    const u32 sh = 31 - __clz(spp);
     const bool uniform = (r.bytes % P == 0) && (P % SEGB == 0);
+    const u32 G = cc_scan_group<U>(r, step);
+    const u32 cpp = spp / G;                 // items per page (G divides spp: both powers of two, or G == 1)
+    const u32 csh = 31 - __clz(cpp);
+    const u64 n_items = r.n_pages * (u64)cpp;
     for (u64 item = first; item < n_items; item += step) {
         u64 p;
-        u32 s;
-        if (pow2) { p = item >> sh; s = (u32)(item & (spp - 1)); }
-        else { p = item / spp; s = (u32)(item - p * spp); }
-        const u64 start = p * (u64)P + (u64)s * SEGB;
-        const uint4* a = reinterpret_cast<const uint4*>(r.base + start);
-        const uint4* b = reinterpret_cast<const uint4*>(r.shadow + start);
-        u32 acc = 0;
-        if (uniform) {
-            uint4 va[U], vb[U];
+        u32 ch;
+        if (pow2) { p = item >> csh; ch = (u32)(item & (cpp - 1)); }
+        else { p = item / cpp; ch = (u32)(item - p * cpp); }
+        bool dirty = false;
+        for (u32 c = 0; c < G && !dirty; c++) {
+            const u32 s = ch * G + c;
+            const u64 start = p * (u64)P + (u64)s * SEGB;
+            const uint4* a = reinterpret_cast<const uint4*>(r.base + start);
+            const uint4* b = reinterpret_cast<const uint4*>(r.shadow + start);
+            u32 acc = 0;
+            if (uniform) {
+                uint4 va[U], vb[U];
 #pragma unroll
-            for (int u = 0; u < U; u++) va[u] = ld_stream(a + lane + 32 * u);
+                for (int u = 0; u < U; u++) va[u] = ld_stream(a + lane + 32 * u);
 #pragma unroll
-            for (int u = 0; u < U; u++) vb[u] = ld_stream(b + lane + 32 * u);
+                for (int u = 0; u < U; u++) vb[u] = ld_stream(b + lane + 32 * u);
 #pragma unroll
-            for (int u = 0; u < U; u++)
-                acc |= (va[u].x ^ vb[u].x) | (va[u].y ^ vb[u].y) | (va[u].z ^ vb[u].z) | (va[u].w ^ vb[u].w);
-        } else {
-            const u64 plen = page_len_dev(r, p);
-            const u64 so = (u64)s * SEGB;
-            if (so >= plen) continue;
-            const u64 rem = plen - so;
-            const u32 nv = (u32)((rem < SEGB ? rem : SEGB) >> 4);
+                for (int u = 0; u < U; u++)
+                    acc |= (va[u].x ^ vb[u].x) | (va[u].y ^ vb[u].y) | (va[u].z ^ vb[u].z) | (va[u].w ^ vb[u].w);
+            } else {
+                const u64 plen = page_len_dev(r, p);
+                const u64 so = (u64)s * SEGB;
+                if (so >= plen) break;
+                const u64 rem = plen - so;
+                const u32 nv = (u32)((rem < SEGB ? rem : SEGB) >> 4);
 #pragma unroll
-            for (int u = 0; u < U; u++) {
-                const u32 j = lane + 32 * u;
-                if (j < nv) {
-                    uint4 x = ld_stream(a + j), y = ld_stream(b + j);
-                    acc |= (x.x ^ y.x) | (x.y ^ y.y) | (x.z ^ y.z) | (x.w ^ y.w);
+                for (int u = 0; u < U; u++) {
+                    const u32 j = lane + 32 * u;
+                    if (j < nv) {
+                        uint4 x = ld_stream(a + j), y = ld_stream(b + j);
+                        acc |= (x.x ^ y.x) | (x.y ^ y.y) | (x.z ^ y.z) | (x.w ^ y.w);
+                    }
                 }
             }
+            dirty = __any_sync(0xFFFFFFFFu, acc != 0);
         }
-        if (__any_sync(0xFFFFFFFFu, acc != 0) && lane == 0)
-            atomicOr(&r.bitmap[p >> 5], 1u << (p & 31));
+        if (dirty && lane == 0) atomicOr(&r.bitmap[p >> 5], 1u << (p & 31));
     }
 }
 
@@ -310,7 +333,9 @@ __device__ __forceinline__ void cc_gather_work(const cc_region_dev& r, cc_dev* d
     // (after a fused pass that already wrote the records -- cc_fused.cuh -- only the commit is left)
     if (k_eff != 0 && !h->inline_done && (u64)g.block * (blockDim.x >> 5) < (u64)k_eff * r.spp) {
         if (init_tables) cc_crc_smem_init(cs, &dev->crc);
+        if (g.block == 0 && threadIdx.x == 0) CC_TRACE(dev, 5);
         cc_gather_items(r, dev, cs, g.warp(), g.nwarps());
+        if (g.block == 0 && threadIdx.x == 0) CC_TRACE(dev, 9);
     }
 }
 
@@ -360,13 +385,11 @@ __device__ __forceinline__ void cc_gather_complete(const cc_region_dev& r, cc_de
     }
     __syncthreads();
     if (s_last && threadIdx.x == 0) {
-        __threadfence_system();
+        CC_TRACE(dev, 6);
+        __threadfence_system();                 // (acquire side of the counter: every block's record bytes are behind us)
         const bool appended = h->k_eff != 0;
         const u64 W_after = cc_gather_commit_record(r, dev);
-        if (appended) {
-            __threadfence_system();
-            cc_log_publish(log, W_after);
-        }
+        CC_TRACE(dev, 7);
         if (out) {
             out->n_dirty = h->k;
             out->bytes = h->need;
@@ -376,9 +399,13 @@ __device__ __forceinline__ void cc_gather_complete(const cc_region_dev& r, cc_de
             out->flags = kind;
             out->t_start_ns = h->t_start_ns;
             out->t_end_ns = globaltimer_ns();
-            __threadfence_system();
-            st_release_sys_u64(&out->seq_done, 1ull);
         }
+        // ONE fence behind the commit record and the result fields, then the publishing words (L263: "a commit marker
+        // publishes the epoch only after all bytes are visible")
+        __threadfence_system();
+        if (appended) cc_log_publish_fenced(log, W_after);
+        if (out) st_relaxed_sys_u64(&out->seq_done, 1ull);
+        CC_TRACE(dev, 8);
         __threadfence();
     }
 }

@@ -89,9 +89,12 @@ struct cc_rec {             // 32 bytes
     u32 epoch_idx;
     u32 pad;
 };
-struct cc_epoch_ent {       // 16 bytes
-    u64 off_after;
+struct cc_epoch_ent {       // 32 bytes
+    u64 off_after;          // log offset right after the epoch's commit record
+    u64 epoch_no;           // the epoch number its commit record carries
     u32 rec_end;            // records [.., rec_end) belong to epochs <= this one
+    u32 slot;               // region slot of its records (0xFFFFFFFF: an empty epoch)
+    u32 pending;            // its record count
     u32 pad;
 };
 struct cc_apply_state {
@@ -111,7 +114,7 @@ struct cc_apply_state {
 
 // Log compactor state (cc_compactor.cuh).
 struct cc_compactor_state {
-    u64 region_epoch[CC_MAX_REGIONS];   // epoch number of the last input epoch that touched the region
+    u32 region_last[CC_MAX_REGIONS];    // 1 + index of the last input epoch that touched the region (0: none)
     u64 bytes_out;
     u64 n_out;
     int32_t status;
@@ -129,6 +132,18 @@ struct cc_batch_state {
     u32 n_active;           // regions taking part (those with a shadow)
     u32 done;               // regions whose commit record is in place
     u32 pad;
+};
+
+#define CC_CAND_TICKETS 4096u            // look-back slots of the applier's candidate search (ranges of >= 1 MiB)
+struct cc_parse_ctl {                    // control block of the parallel parse (cc_apply_parse.cuh)
+    u32 ticket;                          // candidate search: range ticket (reset by the walk phase)
+    u32 run;                             // tag of the candidate look-back words (bumped by the walk phase)
+    u32 n_cand;                          // candidates found
+    u32 cand_overflow;                   // reset by the validation's resolver
+    u32 need_serial;                     // the serial parser must redo the parse (reset by the validation's resolver)
+    u32 wticket;                         // walk: span ticket (reset by the validation phase)
+    u32 pad[2];
+    u64 cand_status[CC_CAND_TICKETS];    // look-back over the range tickets (lb_pack)
 };
 
 struct alignas(16) cc_crc_tables {
@@ -151,6 +166,7 @@ struct cc_dev {
     cc_epoch_ent* epochs;
     u64 max_records;
     cc_apply_state apply;
+    cc_parse_ctl parse;
     cc_compactor_state compactor;
     cc_batch_state batch;
     // grid barrier + worker doorbell
@@ -159,7 +175,17 @@ struct cc_dev {
     u64 doorbell;
     alignas(16) cc_task cur_task;
     u32 worker_exit;
+    u64 trace[32];          // -DCC_TRACE_ON=1 probe builds only: %globaltimer stamps of the phases
 };
+
+#ifndef CC_TRACE_ON
+#define CC_TRACE_ON 0
+#endif
+#if CC_TRACE_ON
+#define CC_TRACE(dev, i) do { (dev)->trace[i] = globaltimer_ns(); } while (0)
+#else
+#define CC_TRACE(dev, i) do { } while (0)
+#endif
 
 // ------------------------------------------------------------------ PTX helpers --
 
@@ -193,6 +219,23 @@ __device__ __forceinline__ uint4 ld_v4(const uint4* p) {
 __device__ __forceinline__ void st_stream(uint4* p, const uint4& v) {
     asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};"
                  :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+// Programmatic dependent launch (sm_90+): a kernel launched with the programmatic-stream-serialization attribute may
+// start while its predecessor in the stream is still running; it must execute cc_pdl_wait() before it touches anything
+// the predecessor writes (no-op when launched normally).  cc_pdl_trigger() in the predecessor lets the dependent grid
+// be scheduled as soon as SM resources free up.  -DCC_PDL=0 builds without it (A/B).
+#ifndef CC_PDL
+#define CC_PDL 1
+#endif
+__device__ __forceinline__ void cc_pdl_wait() {
+#if CC_PDL
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+#endif
+}
+__device__ __forceinline__ void cc_pdl_trigger() {
+#if CC_PDL
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+#endif
 }
 __device__ __forceinline__ u64 globaltimer_ns() {
     u64 t;
@@ -251,6 +294,14 @@ __device__ __forceinline__ u32 ld_relaxed_sys_u32(const u32* p) {
 __device__ __forceinline__ void cc_log_publish(cc_log_dev* log, u64 W_after) {
     if (log->committed_off) st_release_sys_u64(log->committed_off, W_after);
     if (log->pub) st_release_sys_u64(log->pub, (log->gen << CC_PUB_SHIFT) | W_after);
+    log->W = W_after;
+}
+// The same after the CALLER has issued __threadfence_system() behind the commit record (and whatever else must be visible
+// first): plain system-scope stores -- every release store would be another full fence, ~2 us each with host-memory
+// stores in flight.
+__device__ __forceinline__ void cc_log_publish_fenced(cc_log_dev* log, u64 W_after) {
+    if (log->committed_off) st_relaxed_sys_u64(log->committed_off, W_after);
+    if (log->pub) st_relaxed_sys_u64(log->pub, (log->gen << CC_PUB_SHIFT) | W_after);
     log->W = W_after;
 }
 // W := 0: a new generation of the log (cc_log_reset*, CC_TASK_LOG_RESET).

@@ -159,7 +159,8 @@ __device__ __forceinline__ void cc_compactor_copy_phase(cc_dev* dev, const cc_ap
         }
         if (g.block == 0 && threadIdx.x == 0) {             // the region's commit record
             u8* cm = base + r.hdr->need - CC_COMMIT_RECORD_BYTES;
-            const u64 epoch = dev->compactor.region_epoch[s];
+            const u32 le = dev->compactor.region_last[s];        // last input epoch that touched the region
+            const u64 epoch = le ? T.epochs[le - 1].epoch_no : 0ull;
             u32 pay[4] = {(u32)epoch, (u32)(epoch >> 32), r.region_id, k};
             const u32 crc = crc_serial(&dev->crc, reinterpret_cast<const u8*>(pay), 16);
             st_u32x4(cm + 16, pay[0], pay[1], pay[2], pay[3]);

@@ -18,6 +18,8 @@
 #include "cc_apply.cuh"
 #include "cc_compactor.cuh"
 #include "cc_batch.cuh"
+#include "cc_pass.cuh"
+#include "cc_tasks.cuh"
 
 struct cc_ring_dev {            // all pointers are pinned, device-mapped host memory
     cc_task* slots;             // capacity x 64 B
@@ -29,23 +31,6 @@ struct cc_ring_dev {            // all pointers are pinned, device-mapped host m
     u32 backoff_ns;
     u64 max_lifetime_ns;
 };
-
-__device__ __forceinline__ void cc_grid_barrier(cc_dev* dev, u32 nblocks, u32& gen) {
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        __threadfence();
-        if (atomicAdd(&dev->bar_count, 1u) == nblocks - 1) {
-            atomicExch(&dev->bar_count, 0u);
-            __threadfence();
-            atomicAdd(&dev->bar_gen, 1u);
-        } else {
-            while (ld_acquire_gpu_u32(&dev->bar_gen) == gen) __nanosleep(40);
-        }
-        __threadfence();
-    }
-    gen++;
-    __syncthreads();
-}
 
 #if CC_BENCH_HOOKS
 __device__ __forceinline__ void cc_task_mutate(const cc_region_dev& r, const cc_task& t, cc_grid g) {
@@ -61,14 +46,27 @@ __device__ __forceinline__ void cc_task_mutate(const cc_region_dev& r, const cc_
 #endif
 
 #define CC_WORKER_MAX_THREADS 512
+// Register budget of the resident kernel: 2 blocks of 512 threads per SM = 64 registers per thread, so that a worker
+// block leaves half of an SM's register file (and 32 of its 64 warp slots) to the application's kernels -- or to a
+// second worker block.  (-DCC_WORKER_MIN_BLOCKS=1 builds the 128-register variant for an A/B measurement.)
+#ifndef CC_WORKER_MIN_BLOCKS
+#define CC_WORKER_MIN_BLOCKS 2
+#endif
+
+// The applier's parse inside the worker: the one-block serial walk.  (The parallel parse of the host-launched path
+// sizes its blocks for the candidate search and the epoch walks; the worker's blocks are wider and its logs -- one
+// restore per recovery -- do not justify a second instantiation in the resident kernel.)
+__device__ __forceinline__ void cc_worker_parse(cc_dev* dev, const cc_apply_tabs& tabs, const u8* log, u64 n, cc_grid g, u32& gen) {
+    if (g.block == 0) cc_apply_parse_phase(dev, tabs, log, n, true);
+    cc_grid_barrier(dev, g.nblocks, gen);
+}
 
 // The recovery-side tasks are cold: kept out of line so that their registers do not weigh on the
 // checkpoint tasks of the dispatch loop.
 __device__ __noinline__ void cc_worker_restore_task(cc_dev* dev, const cc_apply_tabs& tabs, cc_crc_smem* cs,
                                                     const cc_task& task, cc_grid g, u32& gen) {
     const u8* log = reinterpret_cast<const u8*>(task.arg0);
-    if (g.block == 0) cc_apply_parse_phase(dev, tabs, log, task.arg1);
-    cc_grid_barrier(dev, g.nblocks, gen);
+    cc_worker_parse(dev, tabs, log, task.arg1, g, gen);
     cc_apply_validate_phase(dev, tabs, cs, log, g, false);
     cc_grid_barrier(dev, g.nblocks, gen);
     cc_apply_latest_phase(dev, tabs, g);
@@ -82,8 +80,7 @@ __device__ __noinline__ void cc_worker_compact_task(cc_dev* dev, const cc_apply_
                                                     const cc_task& task, cc_grid g, u32& gen) {
     const u8* in = reinterpret_cast<const u8*>(task.arg0);
     u8* outl = reinterpret_cast<u8*>(task.arg2);
-    if (g.block == 0) cc_apply_parse_phase(dev, tabs, in, task.arg1);
-    cc_grid_barrier(dev, g.nblocks, gen);
+    cc_worker_parse(dev, tabs, in, task.arg1, g, gen);
     cc_apply_validate_phase(dev, tabs, cs, in, g, false);
     cc_grid_barrier(dev, g.nblocks, gen);
     cc_compactor_mark_phase(dev, tabs, g);
@@ -97,12 +94,62 @@ __device__ __noinline__ void cc_worker_compact_task(cc_dev* dev, const cc_apply_
     cc_compactor_cleanup_phase(dev, tabs, g, nullptr, task.kind);
 }
 
-__global__ void __launch_bounds__(CC_WORKER_MAX_THREADS, 1)
+// One checkpoint of one region: the single pass (CC_TASKF_FUSED, when the worst case fits behind the write offset) or
+// the classic phases -- the same device code as the host-launched calls.  Out of line, like the recovery-side
+// tasks below: the dispatch loop stays small and every task body gets the register file to itself.
+__device__ __noinline__ void cc_worker_ckpt_task(cc_dev* dev, const cc_region_dev& r, cc_crc_smem* cs, u32* s_crc_ready,
+                                                 cc_pass_smem* s_pass, const cc_task& task, u64 t_start, cc_grid g, u32& gen) {
+    cc_pass_args a;
+    a.epoch = task.epoch; a.kind = task.kind; a.run_pages = 0; a.marks = nullptr; a.consume = 0;
+    a.version = nullptr; a.committed = nullptr; a.disc = CC_DISC_SCAN;
+    if (task.kind == CC_TASK_DELTA_CKPT) {
+        if (task.flags & CC_TASKF_RLE) a.run_pages = (u32)task.arg0;
+    } else if (task.kind == CC_TASK_MARKED_CKPT) {
+        a.disc = (task.arg1 & CC_MARK_VERIFY) ? CC_DISC_MARKS_VERIFY : CC_DISC_MARKS;
+        a.marks = reinterpret_cast<u32*>(task.arg0);
+        a.consume = (task.arg1 & CC_MARK_CONSUME) ? 1u : 0u;
+    } else if (task.kind == CC_TASK_VERSION_CKPT) {
+        a.disc = CC_DISC_VERSIONS;
+        a.version = reinterpret_cast<const u64*>(task.arg0);
+        a.committed = reinterpret_cast<u64*>(task.arg1);
+    } else a.disc = CC_DISC_ALL;
+    const u64 W0 = dev->log.W;
+    const bool single = (task.flags & CC_TASKF_FUSED) && cc_pass_supported(r.n_pages, a.run_pages) &&
+                        dev->log.buf != nullptr && W0 + cc_pass_worst_bytes(r) <= dev->log.capacity;
+    if (single) {
+        if (g.block == 0 && threadIdx.x == 0) r.hdr->t_start_ns = t_start;
+        const u32 TP = cc_pass_tile_pages(r, a.run_pages, g.nwarps());
+        if (cc_pass_tiles(r, dev, cs, s_crc_ready, s_pass, a, TP, W0, g)) __threadfence_system();
+        cc_grid_barrier(dev, g.nblocks, gen);
+        if (g.block == 0 && threadIdx.x < 32) {
+            __threadfence_system();
+            cc_pass_commit(r, dev, nullptr, task.kind, threadIdx.x);
+        }
+    } else {
+        cc_classic_checkpoint(dev, r, cs, a, g, gen, nullptr, false);
+    }
+}
+
+__device__ __noinline__ void cc_worker_ckpt_all_task(cc_dev* dev, cc_crc_smem* cs, cc_batch_tab* btab, const cc_task& task,
+                                                     cc_grid g, u32& gen) {
+    cc_batch_scan_phase(dev, btab, g);
+    cc_grid_barrier(dev, g.nblocks, gen);
+    cc_batch_rank_phase(dev, task.epoch, g);
+    cc_grid_barrier(dev, g.nblocks, gen);
+    if (g.block == 0) cc_batch_plan_phase(dev, task.epoch);
+    cc_grid_barrier(dev, g.nblocks, gen);
+    cc_batch_gather_phase(dev, cs, btab, g, nullptr, task.kind);
+}
+
+__global__ void __launch_bounds__(CC_WORKER_MAX_THREADS, CC_WORKER_MIN_BLOCKS)
 cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cc_crc_smem* cs = reinterpret_cast<cc_crc_smem*>(smem_raw);
     __shared__ __align__(16) cc_task s_task;
     __shared__ cc_batch_tab s_btab;
+    __shared__ cc_pass_smem s_pass;
+    __shared__ u32 s_crc_ready;             // the CRC tables are filled once, at kernel start: always "ready"
+    if (threadIdx.x == 0) s_crc_ready = 2u;
     const cc_grid g = cc_hw_grid();
     u32 gen = ld_acquire_gpu_u32(&dev->bar_gen);
     u64 head = 0;       // ring sequence number of the next task (meaningful in the leader thread only)
@@ -196,82 +243,15 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
         }
         if (status == CC_OK) {
             switch (task.kind) {
-            case CC_TASK_DELTA_CKPT: {
-                const cc_region_dev& r = dev->regions[slot];
-                if (task.flags & CC_TASKF_RLE) {
-                    cc_scan_phase<8>(r, g);
-                    cc_grid_barrier(dev, g.nblocks, gen);
-                    cc_compact_phase(r, &dev->log, CC_MODE_SCAN_ONLY, task.epoch, nullptr);
-                    cc_grid_barrier(dev, g.nblocks, gen);
-                    cc_rle_starts_phase(r, (u32)task.arg0, g);
-                    cc_grid_barrier(dev, g.nblocks, gen);
-                    cc_rle_rank_phase(r, &dev->log);
-                    cc_grid_barrier(dev, g.nblocks, gen);
-                    cc_rle_plan_phase(r, &dev->log, task.epoch, g);
-                    cc_grid_barrier(dev, g.nblocks, gen);
-                    cc_rle_gather_phase(r, dev, cs, g, nullptr, task.kind, false);
-                    break;
-                }
-                if (task.flags & CC_TASKF_FUSED) {
-                    cc_fused_phase(r, dev, cs, CC_MODE_CHECKPOINT, task.epoch, false);
-                } else {
-                    cc_scan_phase<8>(r, g);
-                    cc_grid_barrier(dev, g.nblocks, gen);
-                    cc_compact_phase(r, &dev->log, CC_MODE_CHECKPOINT, task.epoch, nullptr);
-                }
-                cc_grid_barrier(dev, g.nblocks, gen);
-                cc_gather_phase(r, dev, cs, g, nullptr, task.kind, false);
+            case CC_TASK_DELTA_CKPT:
+            case CC_TASK_MARKED_CKPT:
+            case CC_TASK_VERSION_CKPT:
+            case CC_TASK_SNAPSHOT:
+                cc_worker_ckpt_task(dev, dev->regions[slot], cs, &s_crc_ready, &s_pass, task, t_start, g, gen);
                 break;
-            }
-            case CC_TASK_MARKED_CKPT: {
-                const cc_region_dev& r = dev->regions[slot];
-                u32* marks = reinterpret_cast<u32*>(task.arg0);
-                cc_mark_load_phase(r, marks, g);
-                cc_grid_barrier(dev, g.nblocks, gen);
-                if (task.arg1 & CC_MARK_VERIFY) {
-                    cc_compact_phase(r, &dev->log, CC_MODE_SCAN_ONLY, task.epoch, nullptr);
-                    cc_grid_barrier(dev, g.nblocks, gen);
-                    cc_mark_verify_phase(r, g);
-                    cc_grid_barrier(dev, g.nblocks, gen);
-                }
-                cc_compact_phase(r, &dev->log, CC_MODE_CHECKPOINT, task.epoch, nullptr);
-                cc_grid_barrier(dev, g.nblocks, gen);
-                cc_gather_phase(r, dev, cs, g, nullptr, task.kind, false);
-                if (task.arg1 & CC_MARK_CONSUME) {
-                    cc_grid_barrier(dev, g.nblocks, gen);
-                    cc_mark_finish_phase(r, marks, nullptr, nullptr, g);
-                }
-                break;
-            }
-            case CC_TASK_VERSION_CKPT: {
-                const cc_region_dev& r = dev->regions[slot];
-                const u64* ver = reinterpret_cast<const u64*>(task.arg0);
-                u64* com = reinterpret_cast<u64*>(task.arg1);
-                cc_mark_versions_phase(r, ver, com, g);
-                cc_grid_barrier(dev, g.nblocks, gen);
-                cc_compact_phase(r, &dev->log, CC_MODE_CHECKPOINT, task.epoch, nullptr);
-                cc_grid_barrier(dev, g.nblocks, gen);
-                cc_gather_phase(r, dev, cs, g, nullptr, task.kind, false);
-                cc_grid_barrier(dev, g.nblocks, gen);
-                cc_mark_finish_phase(r, nullptr, ver, com, g);
-                break;
-            }
             case CC_TASK_CKPT_ALL:
-                cc_batch_scan_phase(dev, &s_btab, g);
-                cc_grid_barrier(dev, g.nblocks, gen);
-                cc_batch_rank_phase(dev, task.epoch, g);
-                cc_grid_barrier(dev, g.nblocks, gen);
-                if (g.block == 0) cc_batch_plan_phase(dev, task.epoch);
-                cc_grid_barrier(dev, g.nblocks, gen);
-                cc_batch_gather_phase(dev, cs, &s_btab, g, nullptr, task.kind);
+                cc_worker_ckpt_all_task(dev, cs, &s_btab, task, g, gen);
                 break;
-            case CC_TASK_SNAPSHOT: {
-                const cc_region_dev& r = dev->regions[slot];
-                cc_snapshot_plan_phase(r, &dev->log, task.epoch, g);
-                cc_grid_barrier(dev, g.nblocks, gen);
-                cc_gather_phase(r, dev, cs, g, nullptr, task.kind, false);
-                break;
-            }
             case CC_TASK_COMPACT_LOG:
                 cc_worker_compact_task(dev, tabs, cs, task, g, gen);
                 break;

@@ -17,6 +17,8 @@
 #include "cc_ckpt.cuh"
 #include "cc_mark.cuh"
 #include "cc_fused.cuh"
+#include "cc_pass.cuh"
+#include "cc_tasks.cuh"
 #include "cc_rle.cuh"
 #include "cc_apply.cuh"
 #include "cc_compactor.cuh"
@@ -29,29 +31,77 @@ static_assert(sizeof(cc_rec) == 32, "cc_rec must be 32 bytes");
 
 // ------------------------------------------------------------------------ kernels --
 
+#ifndef CC_PASS_LAZY_CRC
+#define CC_PASS_LAZY_CRC 0          // 1: A/B of the lazily filled CRC tables
+#endif
+
 #define CC_SCAN_THREADS 256
 #define CC_GATHER_THREADS 256
 #define CC_APPLY_THREADS 256
 #define CC_PARSE_THREADS 1024
 
-__global__ void __launch_bounds__(CC_SCAN_THREADS) cc_scan_kernel(const cc_dev* dev, int slot) {
+__global__ void __launch_bounds__(CC_SCAN_THREADS) cc_scan_kernel(cc_dev* dev, int slot) {
+    cc_pdl_trigger();                       // the compaction (and behind it the gather) may queue up behind this grid
+    if (blockIdx.x == 0 && threadIdx.x == 0) CC_TRACE(dev, 0);
     cc_scan_phase<8>(dev->regions[slot], cc_hw_grid());
+    if (blockIdx.x == 0 && threadIdx.x == 0) CC_TRACE(dev, 1);
 }
 
 __global__ void __launch_bounds__(CC_COMPACT_THREADS) cc_compact_kernel(cc_dev* dev, int slot, u32 mode, u64 epoch,
                                                                         cc_result* out) {
+    cc_pdl_trigger();
+    cc_pdl_wait();                          // the bitmap is complete
+    if (blockIdx.x == 0 && threadIdx.x == 0) CC_TRACE(dev, 2);
     cc_compact_phase(dev->regions[slot], &dev->log, mode, epoch, out);
+    if (blockIdx.x == 0 && threadIdx.x == 0) CC_TRACE(dev, 3);
 }
 
 __global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_gather_kernel(cc_dev* dev, int slot, cc_result* out) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    cc_gather_phase(dev->regions[slot], dev, reinterpret_cast<cc_crc_smem*>(smem_raw), cc_hw_grid(), out,
-                    CC_TASK_DELTA_CKPT, true);
+    if (blockIdx.x == 0 && threadIdx.x == 0) CC_TRACE(dev, 4);
+    // the CRC tables do not depend on the plan: filled while the compaction is still running (programmatic dependent
+    // launch), then wait for the plan
+    cc_crc_smem* cs = reinterpret_cast<cc_crc_smem*>(smem_raw);
+    cc_crc_smem_init(cs, &dev->crc);
+    cc_pdl_wait();
+    cc_gather_phase(dev->regions[slot], dev, cs, cc_hw_grid(), out, CC_TASK_DELTA_CKPT, false);
 }
 
-__global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_fused_kernel(cc_dev* dev, int slot, u64 epoch) {
+// The whole checkpoint of one region in ONE launch (cc_pass.cuh).  Cooperative: when the worst case does not fit
+// behind the write offset the classic phases run instead, separated by grid barriers.
+__global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_pass_kernel(cc_dev* dev, int slot, cc_pass_args a, cc_result* out) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    cc_fused_phase(dev->regions[slot], dev, reinterpret_cast<cc_crc_smem*>(smem_raw), CC_MODE_CHECKPOINT, epoch, true);
+    cc_crc_smem* cs = reinterpret_cast<cc_crc_smem*>(smem_raw);
+    __shared__ u32 s_crc_state, s_warps_left;
+    __shared__ cc_pass_smem s_pass;
+    const cc_region_dev& r = dev->regions[slot];
+    const cc_grid g = cc_hw_grid();
+    if (threadIdx.x == 0) { s_crc_state = 0; s_warps_left = blockDim.x >> 5; }
+    if (g.block == 0 && threadIdx.x == 0) { r.hdr->t_start_ns = globaltimer_ns(); CC_TRACE(dev, 10); }
+    __syncthreads();
+    const u64 W0 = dev->log.W;
+    const bool inline_ok = dev->log.buf != nullptr && W0 + cc_pass_worst_bytes(r) <= dev->log.capacity;
+    if (inline_ok) {
+        const u32 lane = threadIdx.x & 31u;
+#if !CC_PASS_LAZY_CRC
+        // the CRC tables, by the whole block at once (~2 us).  (Filled lazily by the first warp that needs them, that warp
+        // alone takes ~30 us over it -- on the critical path of every call that has a dirty page.)
+        cc_crc_smem_init(cs, &dev->crc);
+        if (threadIdx.x == 0) s_crc_state = 2u;
+        __syncthreads();
+#endif
+        const u32 TP = cc_pass_tile_pages(r, a.run_pages, g.nwarps());
+        const bool wrote = cc_pass_tiles(r, dev, cs, &s_crc_state, &s_pass, a, TP, W0, g);
+        if (g.block == 0 && threadIdx.x == 0) CC_TRACE(dev, 11);
+        if (cc_pass_leave(r.hdr, &s_warps_left, wrote, g.nblocks, lane)) {
+            if (lane == 0) CC_TRACE(dev, 12);
+            cc_pass_commit(r, dev, out, a.kind, lane);
+            if (lane == 0) CC_TRACE(dev, 13);
+        }
+        return;
+    }
+    u32 gen = ld_acquire_gpu_u32(&dev->bar_gen);
+    cc_classic_checkpoint(dev, r, cs, a, g, gen, out, true);
 }
 
 __global__ void __launch_bounds__(256) cc_snapshot_plan_kernel(const cc_dev* dev, int slot, u64 epoch) {
@@ -123,8 +173,16 @@ __global__ void __launch_bounds__(256) cc_mark_finish_kernel(const cc_dev* dev, 
     cc_mark_finish_phase(dev->regions[slot], marks_to_clear, version, committed, cc_hw_grid());
 }
 
+// parse: candidate commit records (whole log, grid-wide) -> epoch walks (one block per epoch, chained by look-back)
+// -> the one-block serial walk, which returns at once unless the parallel parse asked for it
+__global__ void __launch_bounds__(CC_CAND_THREADS) cc_apply_cand_kernel(cc_dev* dev, cc_apply_tabs tabs, const u8* log, u64 n) {
+    cc_parse_cand_phase(dev, &dev->parse, tabs.cand, tabs.span_status, tabs.max_records, log, n, blockIdx.x == 0);
+}
+__global__ void __launch_bounds__(CC_WALK_THREADS) cc_apply_walk_kernel(cc_dev* dev, cc_apply_tabs tabs, const u8* log, u64 n) {
+    cc_parse_walk_phase(dev, &dev->parse, tabs, log, n, blockIdx.x == 0);
+}
 __global__ void __launch_bounds__(CC_PARSE_THREADS) cc_apply_parse_kernel(cc_dev* dev, cc_apply_tabs tabs, const u8* log, u64 n) {
-    cc_apply_parse_phase(dev, tabs, log, n);
+    cc_apply_parse_phase(dev, tabs, log, n, false);
 }
 
 __global__ void __launch_bounds__(CC_APPLY_THREADS) cc_apply_validate_kernel(cc_dev* dev, cc_apply_tabs tabs, const u8* log) {
@@ -160,6 +218,7 @@ struct cc_ctx {
     cudaStream_t internal;
     cc_host_region regions[CC_MAX_REGIONS];
     bool log_attached;
+    bool log_is_host;           // the attached log is pinned host memory (records cross the host link)
     uint64_t* committed_off;    // the caller's published-offset word (may be null)
     void* log_buf;              // the attached log (device or pinned host)
     uint64_t log_capacity;
@@ -241,19 +300,17 @@ static bool ws_layout(uint64_t bytes, uint32_t P, cc_ws_layout* L) {
     L->rec_state = o; o += align_up(n_pages * 8, 256);
     L->latest = o; o += align_up(n_pages * 4, 256);
     L->lb = o; o += align_up(L->n_tiles * 8, 256);
-    uint64_t tp = CC_FUSED_TILE_BYTES / P;
-    if (tp < 1) tp = 1;
-    if (tp > CC_FUSED_MAX_TP) tp = CC_FUSED_MAX_TP;
-    L->ftile_pages = tp;
-    L->n_ftiles = (n_pages + tp - 1) / tp;
-    L->flb = o; o += align_up(L->n_ftiles * 8, 256);
+    // single pass (cc_pass.cuh): one look-back word per warp tile, at most CC_PASS_MAX_TILES tiles (pages and records)
+    L->n_ftiles = n_pages < CC_PASS_MAX_TILES ? n_pages : CC_PASS_MAX_TILES;
+    L->ftile_pages = 0;
+    L->flb = o; o += align_up((L->n_ftiles + 32) * 8, 256);
     // run-length records (cc_rle.cuh)
     L->S = o; o += align_up(L->n_tiles * CC_COMPACT_TILE_WORDS * 4, 256);
     L->Rfirst = o; o += align_up((n_pages + 1) * 4, 256);
     L->Rn = o; o += align_up(n_pages * 4, 256);
     L->run_state = o; o += align_up(n_pages * 8, 256);
     L->hdr2 = o; o += 256;
-    L->lb2 = o; o += align_up(L->n_tiles * 8, 256);
+    L->lb2 = o; o += align_up(((L->n_ftiles > L->n_tiles ? L->n_ftiles : L->n_tiles) + 32) * 8, 256);
     L->total = o;
     return true;
 }
@@ -299,8 +356,8 @@ extern "C" int32_t cc_init(cc_ctx** out, int32_t device, const cc_config* cfg) {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_rle_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_compactor_copy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_batch_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->fused_bps, cc_fused_kernel, CC_GATHER_THREADS, sizeof(cc_crc_smem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->fused_bps, cc_pass_kernel, CC_GATHER_THREADS, sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_apply_validate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_worker_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->scan_bps, cc_scan_kernel, CC_SCAN_THREADS, 0);
@@ -350,6 +407,11 @@ extern "C" int32_t cc_shutdown(cc_ctx* ctx) {
 }
 
 extern "C" int32_t cc_last_cuda_error(cc_ctx* ctx) { return ctx ? ctx->last_cuda : 0; }
+#if CC_TRACE_ON
+extern "C" int32_t cc_debug_trace(cc_ctx* ctx, uint64_t* out32) {       // probe builds only; not declared in concordia.h
+    return cudaMemcpy(out32, ctx->d_dev->trace, sizeof(ctx->d_dev->trace), cudaMemcpyDeviceToHost) == cudaSuccess ? CC_OK : CC_ERR_CUDA;
+}
+#endif
 extern "C" uint64_t cc_kernel_launches(cc_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
 // -------------------------------------------------------------------------- regions --
@@ -456,6 +518,11 @@ extern "C" int32_t cc_log_attach(cc_ctx* ctx, void* log_buf, uint64_t capacity, 
     CC_CUDA(ctx, cudaStreamSynchronize(0));
     ctx->log_attached = true;
     ctx->committed_off = committed_off;
+    {
+        cudaPointerAttributes at;
+        ctx->log_is_host = cudaPointerGetAttributes(&at, log_buf) == cudaSuccess && at.type == cudaMemoryTypeHost;
+        cudaGetLastError();
+    }
     ctx->log_buf = log_buf;
     ctx->log_capacity = capacity;
     ctx->drained = 0;
@@ -660,14 +727,36 @@ extern "C" int32_t cc_log_drain_stop(cc_ctx* ctx) {
 
 // ------------------------------------------------------------- host-launched path --
 
+// Launch `kernel` so that it may begin while the previous kernel of the stream is still running (programmatic dependent
+// launch); the kernel waits with cc_pdl_wait() before it reads that kernel's results.
+template <typename... KArgs, typename... Args>
+static cudaError_t launch_dependent(void (*kernel)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t st, Args... args) {
+#if CC_PDL
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(block);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+#else
+    kernel<<<grid, block, smem, st>>>(KArgs(args)...);
+    return cudaGetLastError();
+#endif
+}
+
 static int32_t launch_compact(cc_ctx* ctx, int slot, u32 mode, uint64_t epoch, cudaStream_t st, cc_result* out) {
     const cc_region_dev& r = ctx->regions[slot].dev;
     const uint64_t n_tiles = (r.n_words + CC_COMPACT_TILE_WORDS - 1) / CC_COMPACT_TILE_WORDS;
     uint64_t g2 = n_tiles < (uint64_t)ctx->sm_count * 4 ? n_tiles : (uint64_t)ctx->sm_count * 4;
-    cc_compact_kernel<<<(unsigned)g2, CC_COMPACT_THREADS, 0, st>>>(ctx->d_dev, slot, mode, epoch, out);
+    CC_CUDA(ctx, launch_dependent(cc_compact_kernel, (unsigned)g2, CC_COMPACT_THREADS, 0, st, ctx->d_dev, slot, mode, epoch, out));
     if (ctx->ev_after_compact) cudaEventRecord(ctx->ev_after_compact, st);
     ctx->launches += 1;
-    CC_CUDA(ctx, cudaGetLastError());
     return CC_OK;
 }
 
@@ -686,9 +775,8 @@ static int32_t launch_scan_compact(cc_ctx* ctx, int slot, u32 mode, uint64_t epo
 
 static int32_t launch_gather(cc_ctx* ctx, int slot, cudaStream_t st, cc_result* out) {
     const unsigned g3 = (unsigned)(ctx->sm_count * ctx->gather_bps);
-    cc_gather_kernel<<<g3, CC_GATHER_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, slot, out);
+    CC_CUDA(ctx, launch_dependent(cc_gather_kernel, g3, CC_GATHER_THREADS, sizeof(cc_crc_smem), st, ctx->d_dev, slot, out));
     ctx->launches += 1;
-    CC_CUDA(ctx, cudaGetLastError());
     return CC_OK;
 }
 
@@ -699,121 +787,192 @@ static unsigned small_grid(cc_ctx* ctx, uint64_t items, uint64_t per_block) {
     return (unsigned)(g < 1 ? 1 : g);
 }
 
-extern "C" int32_t cc_checkpoint_marked(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, uint32_t* dirty_bitmap,
-                                        uint32_t flags, void* stream, cc_result* out) {
-    if (!ctx || !dirty_bitmap || ((uintptr_t)dirty_bitmap & 3) || (flags & ~(CC_MARK_VERIFY | CC_MARK_CONSUME))) return CC_ERR_INVALID;
-    CC_NO_WORKER(ctx);
-    int slot = find_slot(ctx, region_id);
-    if (slot < 0) return CC_ERR_NOT_REGISTERED;
-    const cc_region_dev& r = ctx->regions[slot].dev;
-    if ((flags & CC_MARK_VERIFY) && !r.shadow) return CC_ERR_INVALID;
-    CC_CUDA(ctx, cudaSetDevice(ctx->device));
-    cudaStream_t st = (cudaStream_t)stream;
-    cc_mark_load_kernel<<<small_grid(ctx, r.n_words, 256), 256, 0, st>>>(ctx->d_dev, slot, dirty_bitmap);
-    ctx->launches += 1;
-    if (flags & CC_MARK_VERIFY) {
-        cudaEvent_t ec = ctx->ev_after_compact;
-        ctx->ev_after_compact = nullptr;                // the trace events bracket discovery as a whole
-        int32_t rc = launch_compact(ctx, slot, CC_MODE_SCAN_ONLY, epoch, st, nullptr);
-        ctx->ev_after_compact = ec;
-        if (rc != CC_OK) return rc;
-        const unsigned gv = (unsigned)(ctx->sm_count * ctx->scan_bps);
-        cc_mark_verify_kernel<<<gv, CC_SCAN_THREADS, 0, st>>>(ctx->d_dev, slot);
-        ctx->launches += 1;
-    }
-    if (ctx->ev_after_scan) cudaEventRecord(ctx->ev_after_scan, st);
-    int32_t rc = launch_compact(ctx, slot, CC_MODE_CHECKPOINT, epoch, st, nullptr);
-    if (rc != CC_OK) return rc;
-    rc = launch_gather(ctx, slot, st, out);
-    if (rc != CC_OK) return rc;
-    if (flags & CC_MARK_CONSUME) {
-        cc_mark_finish_kernel<<<small_grid(ctx, r.n_words, 256), 256, 0, st>>>(ctx->d_dev, slot, dirty_bitmap, nullptr, nullptr);
-        ctx->launches += 1;
-        CC_CUDA(ctx, cudaGetLastError());
-    }
-    return CC_OK;
-}
+// ---- one checkpoint of one region: the general entry point and its path selection ----
+#ifndef CC_PASS_COOP
+#define CC_PASS_COOP 1              // 0: plain launch (A/B of the launch cost only: the kernel NEEDS co-residency)
+#endif
 
-extern "C" int32_t cc_checkpoint_versions(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, const uint64_t* version,
-                                          uint64_t* committed, void* stream, cc_result* out) {
-    if (!ctx || !version || !committed || ((uintptr_t)version & 7) || ((uintptr_t)committed & 7)) return CC_ERR_INVALID;
-    CC_NO_WORKER(ctx);
-    int slot = find_slot(ctx, region_id);
-    if (slot < 0) return CC_ERR_NOT_REGISTERED;
+// Single pass (ONE cooperative launch).
+static int32_t launch_pass(cc_ctx* ctx, int slot, const cc_pass_args& a, cudaStream_t st, cc_result* out) {
     const cc_region_dev& r = ctx->regions[slot].dev;
-    CC_CUDA(ctx, cudaSetDevice(ctx->device));
-    cudaStream_t st = (cudaStream_t)stream;
-    cc_mark_versions_kernel<<<small_grid(ctx, r.n_words, 8), 256, 0, st>>>(ctx->d_dev, slot, version, committed);
-    ctx->launches += 1;
-    if (ctx->ev_after_scan) cudaEventRecord(ctx->ev_after_scan, st);
-    int32_t rc = launch_compact(ctx, slot, CC_MODE_CHECKPOINT, epoch, st, nullptr);
-    if (rc != CC_OK) return rc;
-    rc = launch_gather(ctx, slot, st, out);
-    if (rc != CC_OK) return rc;
-    cc_mark_finish_kernel<<<small_grid(ctx, r.n_pages, 256), 256, 0, st>>>(ctx->d_dev, slot, nullptr, version, committed);
-    ctx->launches += 1;
-    CC_CUDA(ctx, cudaGetLastError());
-    return CC_OK;
-}
-
-extern "C" int32_t cc_checkpoint_delta(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out) {
-    if (!ctx) return CC_ERR_INVALID;
-    CC_NO_WORKER(ctx);
-    int slot = find_slot(ctx, region_id);
-    if (slot < 0) return CC_ERR_NOT_REGISTERED;
-    if (!ctx->regions[slot].dev.shadow) return CC_ERR_INVALID;
-    CC_CUDA(ctx, cudaSetDevice(ctx->device));
-    cudaStream_t st = (cudaStream_t)stream;
-    int32_t rc = launch_scan_compact(ctx, slot, CC_MODE_CHECKPOINT, epoch, st, nullptr);
-    if (rc != CC_OK) return rc;
-    return launch_gather(ctx, slot, st, out);
-}
-
-extern "C" int32_t cc_checkpoint_delta_fused(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out) {
-    if (!ctx) return CC_ERR_INVALID;
-    CC_NO_WORKER(ctx);
-    int slot = find_slot(ctx, region_id);
-    if (slot < 0) return CC_ERR_NOT_REGISTERED;
-    const cc_region_dev& r = ctx->regions[slot].dev;
-    if (!r.shadow) return CC_ERR_INVALID;
-    CC_CUDA(ctx, cudaSetDevice(ctx->device));
-    cudaStream_t st = (cudaStream_t)stream;
-    uint64_t g = (r.n_ftiles + CC_GATHER_THREADS / 32 - 1) / (CC_GATHER_THREADS / 32);
-    const uint64_t cap = (uint64_t)ctx->sm_count * ctx->fused_bps;
+    uint64_t g = (r.n_pages + CC_GATHER_THREADS / 32 - 1) / (CC_GATHER_THREADS / 32);
+    const uint64_t cap = (uint64_t)ctx->sm_count * ctx->fused_bps;       // all blocks co-resident (grid barrier of the fallback)
     if (g > cap) g = cap;
-    cc_fused_kernel<<<(unsigned)g, CC_GATHER_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, slot, epoch);
+    cc_dev* d = ctx->d_dev;
+    cc_pass_args aa = a;
+    void* args[] = {&d, &slot, &aa, &out};
+#if CC_PASS_COOP
+    CC_CUDA(ctx, cudaLaunchCooperativeKernel((const void*)cc_pass_kernel, dim3((unsigned)g), dim3(CC_GATHER_THREADS), args,
+                                             sizeof(cc_crc_smem), st));
+#else
+    (void)args;
+    cc_pass_kernel<<<(unsigned)g, CC_GATHER_THREADS, sizeof(cc_crc_smem), st>>>(d, slot, aa, out);
+    CC_CUDA(ctx, cudaGetLastError());
+#endif
     ctx->launches += 1;
     if (ctx->ev_after_scan) cudaEventRecord(ctx->ev_after_scan, st);
     if (ctx->ev_after_compact) cudaEventRecord(ctx->ev_after_compact, st);
+    return CC_OK;
+}
+
+// Classic phases as separate launches, each sized for its own work (the scanner runs at 47 warps per SM).
+static int32_t launch_phases(cc_ctx* ctx, int slot, const cc_pass_args& a, cudaStream_t st, cc_result* out) {
+    const cc_region_dev& r = ctx->regions[slot].dev;
+    const bool rle = a.run_pages > 1;
+    const u32 final_mode = rle ? CC_MODE_SCAN_ONLY : CC_MODE_CHECKPOINT;
+    cudaEvent_t ec = ctx->ev_after_compact;
+    int32_t rc = CC_OK;
+    if (a.disc == CC_DISC_SCAN) {
+        if (rle) ctx->ev_after_compact = nullptr;             // the trace event goes after the whole ranking
+        rc = launch_scan_compact(ctx, slot, final_mode, a.epoch, st, nullptr);
+        ctx->ev_after_compact = ec;
+    } else if (a.disc == CC_DISC_ALL) {
+        cc_snapshot_plan_kernel<<<small_grid(ctx, r.n_pages, 256), 256, 0, st>>>(ctx->d_dev, slot, a.epoch);
+        ctx->launches += 1;
+        if (ctx->ev_after_scan) cudaEventRecord(ctx->ev_after_scan, st);
+        if (ec && !rle) cudaEventRecord(ec, st);
+    } else {
+        if (a.disc == CC_DISC_VERSIONS)
+            cc_mark_versions_kernel<<<small_grid(ctx, r.n_words, 8), 256, 0, st>>>(ctx->d_dev, slot, a.version, a.committed);
+        else
+            cc_mark_load_kernel<<<small_grid(ctx, r.n_words, 256), 256, 0, st>>>(ctx->d_dev, slot, a.marks);
+        ctx->launches += 1;
+        ctx->ev_after_compact = nullptr;                      // the trace events bracket discovery as a whole
+        if (a.disc == CC_DISC_MARKS_VERIFY) {
+            rc = launch_compact(ctx, slot, CC_MODE_SCAN_ONLY, a.epoch, st, nullptr);
+            if (rc == CC_OK) {
+                cc_mark_verify_kernel<<<(unsigned)(ctx->sm_count * ctx->scan_bps), CC_SCAN_THREADS, 0, st>>>(ctx->d_dev, slot);
+                ctx->launches += 1;
+            }
+        }
+        if (ctx->ev_after_scan) cudaEventRecord(ctx->ev_after_scan, st);
+        if (!rle) ctx->ev_after_compact = ec;
+        if (rc == CC_OK) rc = launch_compact(ctx, slot, final_mode, a.epoch, st, nullptr);
+        ctx->ev_after_compact = ec;
+    }
+    if (rc != CC_OK) return rc;
+    if (rle) {
+        const uint64_t n_tiles = (r.n_words + CC_COMPACT_TILE_WORDS - 1) / CC_COMPACT_TILE_WORDS;
+        const unsigned g2 = (unsigned)(n_tiles < (uint64_t)ctx->sm_count * 4 ? n_tiles : (uint64_t)ctx->sm_count * 4);
+        cc_rle_starts_kernel<<<small_grid(ctx, r.n_words, 8), 256, 0, st>>>(ctx->d_dev, slot, a.run_pages);
+        cc_rle_rank_kernel<<<g2, CC_COMPACT_THREADS, 0, st>>>(ctx->d_dev, slot);
+        cc_rle_plan_kernel<<<small_grid(ctx, r.n_pages, 256), 256, 0, st>>>(ctx->d_dev, slot, a.epoch);
+        if (ec) cudaEventRecord(ec, st);
+        cc_rle_gather_kernel<<<(unsigned)(ctx->sm_count * ctx->gather_bps), CC_GATHER_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, slot, out);
+        ctx->launches += 4;
+        CC_CUDA(ctx, cudaGetLastError());
+    } else {
+        rc = launch_gather(ctx, slot, st, out);
+        if (rc != CC_OK) return rc;
+    }
+    if ((a.disc == CC_DISC_MARKS || a.disc == CC_DISC_MARKS_VERIFY) && a.consume) {
+        cc_mark_finish_kernel<<<small_grid(ctx, r.n_words, 256), 256, 0, st>>>(ctx->d_dev, slot, a.marks, nullptr, nullptr);
+        ctx->launches += 1;
+    } else if (a.disc == CC_DISC_VERSIONS) {
+        cc_mark_finish_kernel<<<small_grid(ctx, r.n_pages, 256), 256, 0, st>>>(ctx->d_dev, slot, nullptr, a.version, a.committed);
+        ctx->launches += 1;
+    }
     CC_CUDA(ctx, cudaGetLastError());
-    return launch_gather(ctx, slot, st, out);
+    return CC_OK;
+}
+
+extern "C" int32_t cc_checkpoint_ex(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, const cc_ckpt_opts* o, void* stream, cc_result* out) {
+    if (!ctx) return CC_ERR_INVALID;
+    CC_NO_WORKER(ctx);
+    cc_ckpt_opts z;
+    memset(&z, 0, sizeof(z));
+    if (o) z = *o;
+    if (z.discovery > CC_DISC_ALL || z.path > CC_PATH_PHASES || (z.mark_flags & ~(CC_MARK_VERIFY | CC_MARK_CONSUME))) return CC_ERR_INVALID;
+    int slot = find_slot(ctx, region_id);
+    if (slot < 0) return CC_ERR_NOT_REGISTERED;
+    const cc_region_dev& r = ctx->regions[slot].dev;
+    cc_pass_args a;
+    memset(&a, 0, sizeof(a));
+    a.epoch = epoch;
+    a.run_pages = z.run_pages;
+    a.kind = CC_TASK_DELTA_CKPT;
+    if (z.run_pages > 1 && (uint64_t)z.run_pages * r.page_bytes > 0xFFFFFFFFull) return CC_ERR_INVALID;
+    switch (z.discovery) {
+    case CC_DISC_SCAN:
+        if (!r.shadow) return CC_ERR_INVALID;
+        a.disc = CC_DISC_SCAN;
+        break;
+    case CC_DISC_MARKS:
+        if (!z.dirty_bitmap || ((uintptr_t)z.dirty_bitmap & 3)) return CC_ERR_INVALID;
+        if ((z.mark_flags & CC_MARK_VERIFY) && !r.shadow) return CC_ERR_INVALID;
+        a.disc = (z.mark_flags & CC_MARK_VERIFY) ? CC_DISC_MARKS_VERIFY : CC_DISC_MARKS;
+        a.marks = z.dirty_bitmap;
+        a.consume = (z.mark_flags & CC_MARK_CONSUME) ? 1u : 0u;
+        a.kind = CC_TASK_MARKED_CKPT;
+        break;
+    case CC_DISC_VERSIONS:
+        if (!z.version || !z.committed || ((uintptr_t)z.version & 7) || ((uintptr_t)z.committed & 7)) return CC_ERR_INVALID;
+        a.disc = CC_DISC_VERSIONS;
+        a.version = z.version;
+        a.committed = z.committed;
+        a.kind = CC_TASK_VERSION_CKPT;
+        break;
+    default:
+        a.disc = CC_DISC_ALL;
+        a.kind = CC_TASK_SNAPSHOT;
+        break;
+    }
+    if (z.discovery == CC_DISC_MARKS_VERIFY) return CC_ERR_INVALID;      // (spelled CC_DISC_MARKS + CC_MARK_VERIFY)
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    const bool can_pass = cc_pass_supported(r.n_pages, z.run_pages);
+    bool pass;
+    if (z.path == CC_PATH_SINGLE_PASS) {
+        if (!can_pass) return CC_ERR_INVALID;
+        pass = true;
+    } else if (z.path == CC_PATH_PHASES) pass = false;
+    else {
+        // AUTO, from measurements (profiles/r02_pass_probe.md): the single pass wins where the log
+        // crosses the host link (the transfer overlaps the scan: C2 11.7 vs 13.8 ms, C5b 111 vs 160 us per task);
+        // with a device log the separately sized kernels win at every size (64 MiB: 70 vs 90 us, 8 GiB: 2.8 vs 3.2 ms).
+        pass = can_pass && ctx->log_is_host;
+    }
+    return pass ? launch_pass(ctx, slot, a, (cudaStream_t)stream, out) : launch_phases(ctx, slot, a, (cudaStream_t)stream, out);
+}
+
+static int32_t checkpoint_opts(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out, uint32_t disc,
+                               uint32_t path, uint32_t run_pages, uint32_t* marks, uint32_t mark_flags, const uint64_t* version,
+                               uint64_t* committed) {
+    cc_ckpt_opts o;
+    memset(&o, 0, sizeof(o));
+    o.discovery = disc; o.path = path; o.run_pages = run_pages; o.dirty_bitmap = marks; o.mark_flags = mark_flags;
+    o.version = version; o.committed = committed;
+    return cc_checkpoint_ex(ctx, region_id, epoch, &o, stream, out);
+}
+
+extern "C" int32_t cc_checkpoint_delta(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out) {
+    return checkpoint_opts(ctx, region_id, epoch, stream, out, CC_DISC_SCAN, CC_PATH_AUTO, 0, nullptr, 0, nullptr, nullptr);
+}
+
+extern "C" int32_t cc_checkpoint_delta_fused(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out) {
+    return checkpoint_opts(ctx, region_id, epoch, stream, out, CC_DISC_SCAN, CC_PATH_SINGLE_PASS, 0, nullptr, 0, nullptr, nullptr);
 }
 
 extern "C" int32_t cc_checkpoint_delta_rle(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, uint32_t run_pages, void* stream,
                                            cc_result* out) {
-    if (!ctx || run_pages == 0) return CC_ERR_INVALID;
-    CC_NO_WORKER(ctx);
-    int slot = find_slot(ctx, region_id);
-    if (slot < 0) return CC_ERR_NOT_REGISTERED;
-    const cc_region_dev& r = ctx->regions[slot].dev;
-    if (!r.shadow || (uint64_t)run_pages * r.page_bytes > 0xFFFFFFFFull) return CC_ERR_INVALID;
-    CC_CUDA(ctx, cudaSetDevice(ctx->device));
-    cudaStream_t st = (cudaStream_t)stream;
-    cudaEvent_t ec = ctx->ev_after_compact;
-    ctx->ev_after_compact = nullptr;                    // the trace event goes after the whole ranking
-    int32_t rc = launch_scan_compact(ctx, slot, CC_MODE_SCAN_ONLY, epoch, st, nullptr);
-    ctx->ev_after_compact = ec;
-    if (rc != CC_OK) return rc;
-    const uint64_t n_tiles = (r.n_words + CC_COMPACT_TILE_WORDS - 1) / CC_COMPACT_TILE_WORDS;
-    const unsigned g2 = (unsigned)(n_tiles < (uint64_t)ctx->sm_count * 4 ? n_tiles : (uint64_t)ctx->sm_count * 4);
-    cc_rle_starts_kernel<<<small_grid(ctx, r.n_words, 8), 256, 0, st>>>(ctx->d_dev, slot, run_pages);
-    cc_rle_rank_kernel<<<g2, CC_COMPACT_THREADS, 0, st>>>(ctx->d_dev, slot);
-    cc_rle_plan_kernel<<<small_grid(ctx, r.n_pages, 256), 256, 0, st>>>(ctx->d_dev, slot, epoch);
-    if (ec) cudaEventRecord(ec, st);
-    cc_rle_gather_kernel<<<(unsigned)(ctx->sm_count * ctx->gather_bps), CC_GATHER_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, slot, out);
-    ctx->launches += 4;
-    CC_CUDA(ctx, cudaGetLastError());
-    return CC_OK;
+    if (run_pages == 0) return CC_ERR_INVALID;
+    return checkpoint_opts(ctx, region_id, epoch, stream, out, CC_DISC_SCAN, run_pages <= 32 ? CC_PATH_AUTO : CC_PATH_PHASES, run_pages,
+                           nullptr, 0, nullptr, nullptr);
+}
+
+extern "C" int32_t cc_checkpoint_marked(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, uint32_t* dirty_bitmap,
+                                        uint32_t flags, void* stream, cc_result* out) {
+    if (!dirty_bitmap) return CC_ERR_INVALID;
+    return checkpoint_opts(ctx, region_id, epoch, stream, out, CC_DISC_MARKS, CC_PATH_AUTO, 0, dirty_bitmap, flags, nullptr, nullptr);
+}
+
+extern "C" int32_t cc_checkpoint_versions(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, const uint64_t* version,
+                                          uint64_t* committed, void* stream, cc_result* out) {
+    if (!version || !committed) return CC_ERR_INVALID;
+    return checkpoint_opts(ctx, region_id, epoch, stream, out, CC_DISC_VERSIONS, CC_PATH_AUTO, 0, nullptr, 0, version, committed);
+}
+
+extern "C" int32_t cc_snapshot_region(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out) {
+    return checkpoint_opts(ctx, region_id, epoch, stream, out, CC_DISC_ALL, CC_PATH_AUTO, 0, nullptr, 0, nullptr, nullptr);
 }
 
 extern "C" int32_t cc_checkpoint_all(cc_ctx* ctx, uint64_t epoch, void* stream, cc_result* out) {
@@ -832,20 +991,16 @@ extern "C" int32_t cc_checkpoint_all(cc_ctx* ctx, uint64_t epoch, void* stream, 
     return CC_OK;
 }
 
-extern "C" int32_t cc_snapshot_region(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, void* stream, cc_result* out) {
-    if (!ctx) return CC_ERR_INVALID;
-    CC_NO_WORKER(ctx);
-    int slot = find_slot(ctx, region_id);
-    if (slot < 0) return CC_ERR_NOT_REGISTERED;
-    const cc_region_dev& r = ctx->regions[slot].dev;
-    CC_CUDA(ctx, cudaSetDevice(ctx->device));
-    cudaStream_t st = (cudaStream_t)stream;
-    cc_snapshot_plan_kernel<<<small_grid(ctx, r.n_pages, 256), 256, 0, st>>>(ctx->d_dev, slot, epoch);
-    ctx->launches += 1;
-    if (ctx->ev_after_scan) cudaEventRecord(ctx->ev_after_scan, st);
-    if (ctx->ev_after_compact) cudaEventRecord(ctx->ev_after_compact, st);
-    CC_CUDA(ctx, cudaGetLastError());
-    return launch_gather(ctx, slot, st, out);
+// the three parse launches (candidates, walks, serial fallback)
+static void launch_parse(cc_ctx* ctx, const u8* lg, uint64_t nbytes, cudaStream_t st) {
+    const uint64_t ranges = ((nbytes >> 4) + (1u << 13) - 1) >> 13;                 // 128 KiB ranges (fewer, larger ones on huge logs)
+    uint64_t gc = ranges < 1 ? 1 : ranges;
+    const uint64_t capc = (uint64_t)ctx->sm_count * 8;
+    if (gc > capc) gc = capc;
+    cc_apply_cand_kernel<<<(unsigned)gc, CC_CAND_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, lg, nbytes);
+    cc_apply_walk_kernel<<<(unsigned)(ctx->sm_count * 4), CC_WALK_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, lg, nbytes);
+    cc_apply_parse_kernel<<<1, CC_PARSE_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, lg, nbytes);
+    ctx->launches += 3;
 }
 
 extern "C" int32_t cc_compact_log(cc_ctx* ctx, const void* in_log, uint64_t in_bytes, void* out_log, uint64_t out_capacity,
@@ -859,14 +1014,14 @@ extern "C" int32_t cc_compact_log(cc_ctx* ctx, const void* in_log, uint64_t in_b
     cudaStream_t st = (cudaStream_t)stream;
     const u8* lg = stage_log(ctx, in_log, in_bytes, st);
     const unsigned gv = (unsigned)(ctx->sm_count * ctx->validate_bps);
-    cc_apply_parse_kernel<<<1, CC_PARSE_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, lg, in_bytes);
+    launch_parse(ctx, lg, in_bytes, st);
     cc_apply_validate_kernel<<<gv, CC_APPLY_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, ctx->tabs, lg);
     cc_compactor_mark_kernel<<<(unsigned)ctx->sm_count, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs);
     cc_compactor_rank_kernel<<<(unsigned)ctx->sm_count, CC_COMPACT_THREADS, 0, st>>>(ctx->d_dev);
     cc_compactor_plan_kernel<<<1, CC_MAX_REGIONS, 0, st>>>(ctx->d_dev, out_capacity);
     cc_compactor_copy_kernel<<<gv, CC_APPLY_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, ctx->tabs, lg, (u8*)out_log);
     cc_compactor_cleanup_kernel<<<(unsigned)ctx->sm_count, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, out);
-    ctx->launches += 7;
+    ctx->launches += 6;
     CC_CUDA(ctx, cudaGetLastError());
     return CC_OK;
 }
@@ -900,16 +1055,17 @@ extern "C" int32_t cc_dirty_list(cc_ctx* ctx, uint32_t region_id, const uint32_t
 }
 
 extern "C" uint64_t cc_apply_scratch_bytes(uint64_t max_records) {
-    if (max_records == 0 || max_records > 0xFFFFFFF0ull) return 0;
-    return align_up(max_records * sizeof(cc_rec), 256) + align_up(max_records * sizeof(cc_epoch_ent), 256) +
-           align_up(max_records * 8, 256) + align_up((max_records + 1) * 4, 256);
+    if (max_records == 0 || max_records >= 0x7FFFFFF0ull) return 0;      // record numbers travel in 31 bits
+    return align_up(max_records * sizeof(cc_rec), 256) + align_up((max_records + 1) * sizeof(cc_epoch_ent), 256) +
+           align_up(max_records * 8, 256) + align_up((max_records + 1) * 4, 256) +
+           align_up((max_records + 1) * 4, 256) + align_up((max_records + 2) * 8, 256);
 }
 
 extern "C" int32_t cc_apply_attach(cc_ctx* ctx, void* scratch, uint64_t scratch_bytes) {
     if (!ctx || !scratch || ((uintptr_t)scratch & 255)) return CC_ERR_INVALID;
     if (ctx->worker_running) return CC_ERR_WORKER;
     // largest max_records whose tables fit
-    uint64_t lo = 0, hi = scratch_bytes / 32 + 1;
+    uint64_t lo = 0, hi = scratch_bytes / 64 + 2;
     while (lo + 1 < hi) {
         uint64_t mid = (lo + hi) / 2;
         uint64_t need = cc_apply_scratch_bytes(mid);
@@ -921,9 +1077,11 @@ extern "C" int32_t cc_apply_attach(cc_ctx* ctx, void* scratch, uint64_t scratch_
     cc_apply_tabs T;
     T.max_records = m;
     T.recs = (cc_rec*)p; p += align_up(m * sizeof(cc_rec), 256);
-    T.epochs = (cc_epoch_ent*)p; p += align_up(m * sizeof(cc_epoch_ent), 256);
+    T.epochs = (cc_epoch_ent*)p; p += align_up((m + 1) * sizeof(cc_epoch_ent), 256);
     T.rec_state = (u64*)p; p += align_up(m * 8, 256);
-    T.seg_begin = (u32*)p;
+    T.seg_begin = (u32*)p; p += align_up((m + 1) * 4, 256);
+    T.cand = (u32*)p; p += align_up((m + 1) * 4, 256);
+    T.span_status = (u64*)p;
     ctx->tabs = T;
     ctx->apply_attached = true;
     return CC_OK;
@@ -957,12 +1115,12 @@ extern "C" int32_t cc_apply_log(cc_ctx* ctx, const void* log, uint64_t nbytes, v
     const u8* lg = stage_log(ctx, log, nbytes, st);
     const unsigned gv = (unsigned)(ctx->sm_count * ctx->validate_bps);
     const unsigned gs = (unsigned)(ctx->sm_count * 8);
-    cc_apply_parse_kernel<<<1, CC_PARSE_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, lg, nbytes);
+    launch_parse(ctx, lg, nbytes, st);
     cc_apply_validate_kernel<<<gv, CC_APPLY_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, ctx->tabs, lg);
     cc_apply_latest_kernel<<<(unsigned)ctx->sm_count, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs);
     cc_apply_scatter_kernel<<<gs, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, lg);
     cc_apply_cleanup_kernel<<<(unsigned)ctx->sm_count, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, out);
-    ctx->launches += 5;
+    ctx->launches += 4;
     CC_CUDA(ctx, cudaGetLastError());
     return CC_OK;
 }
@@ -976,6 +1134,17 @@ static inline volatile u64* ring_tail(cc_ctx* c) { return c->ring_words + 0; }
 static inline volatile u64* ring_completed(cc_ctx* c) { return c->ring_words + 8; }
 static inline volatile u64* ring_heartbeat(cc_ctx* c) { return c->ring_words + 16; }
 
+// Worker CTAs: the configured number; CC_WORKER_BLOCKS_ALL = as many as are co-resident; 0 = the default footprint
+// CC_WORKER_BLOCKS_DEFAULT (about a ninth of the SMs: a bandwidth-bound application kernel next to an idle worker of
+// that size keeps ~96 % of its throughput and a 256 MiB checkpoint task takes ~0.26 ms -- profiles/r02_overlap.txt;
+// the paper runs ONE block = 0.53 % of its SMs, which on B200 moves ~70 GB/s).
+static uint32_t worker_block_count(cc_ctx* ctx, int bps) {
+    const uint32_t max = (uint32_t)(bps * ctx->sm_count);
+    if (ctx->cfg.worker_blocks == CC_WORKER_BLOCKS_ALL) return max;
+    if (ctx->cfg.worker_blocks == 0) return CC_WORKER_BLOCKS_DEFAULT < max ? CC_WORKER_BLOCKS_DEFAULT : max;
+    return ctx->cfg.worker_blocks;
+}
+
 extern "C" int32_t cc_worker_start(cc_ctx* ctx) {
     if (!ctx) return CC_ERR_INVALID;
     if (ctx->worker_running) return CC_ERR_WORKER;
@@ -987,7 +1156,7 @@ extern "C" int32_t cc_worker_start(cc_ctx* ctx) {
     int bps = 0;
     CC_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, cc_worker_kernel, threads, sizeof(cc_crc_smem)));
     if (bps < 1) return CC_ERR_WORKER;
-    uint32_t blocks = ctx->cfg.worker_blocks ? ctx->cfg.worker_blocks : (uint32_t)(bps * ctx->sm_count);
+    const uint32_t blocks = worker_block_count(ctx, bps);
     if (blocks > (uint32_t)(bps * ctx->sm_count)) return CC_ERR_INVALID;   // must all be co-resident (grid barrier)
     // reset barrier / doorbell state and the host-side ring words
     struct { u32 bar_count, bar_gen; u64 doorbell; } z = {0, 0, 0};
@@ -1177,7 +1346,7 @@ extern "C" int32_t cc_worker_footprint(cc_ctx* ctx, uint32_t* blocks, uint32_t* 
     if (!ctx->worker_running) {
         int bps = 0;
         CC_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, cc_worker_kernel, th, sizeof(cc_crc_smem)));
-        b = ctx->cfg.worker_blocks ? ctx->cfg.worker_blocks : (uint32_t)(bps * ctx->sm_count);
+        b = worker_block_count(ctx, bps);
     }
     if (blocks) *blocks = b;
     if (threads) *threads = (uint32_t)th;
