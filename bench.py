@@ -702,35 +702,46 @@ def ring_on_region(cc, env, cur, shadow, P, k_exp, log_bytes, mutate, blocks_lis
 
 # ------------------------------------------------------- generic timed checkpoints --
 
-def timed_checkpoints(ctx, cc, env, rid, K, Wm, rearm, k_expect, cold, call=None, reset=True):
+def timed_checkpoints(ctx, cc, env, rid, K, Wm, rearm, k_expect, cold, call=None, reset=True, phases=True, ahead=False):
     """W warm-ups, then K checkpoints of region `rid`, each timed on its own with CUDA events on the launch stream
     (re-arming the mutation and the optional L2 flush are NOT inside the events).  Returns per-step lists of ms:
-    total, discovery (scan + compaction), writer (gather + commit + shadow)."""
+    total, discovery (scan + compaction), writer (gather + commit + shadow), and the device time between the
+    %globaltimer stamps of the result.
+    phases=False: no event is recorded between the kernels of a call (an event there also keeps the kernels of the
+    phases path from overlapping by programmatic dependent launch); discovery / writer are then 0.
+    ahead=True: a ~150 us spin kernel is queued in front of the first event, so that the host has issued the whole call
+    before the GPU reaches it -- the events then bracket GPU time only (an idle GPU would otherwise sit between the two
+    events waiting for the interpreter to marshal the call, which is 10-20 us of a 60 us checkpoint)."""
     torch, stream = env.torch, env.stream
     res = cc.Result()
     call = call or (lambda it, res: ctx.checkpoint_delta(rid, it, res))
-    tot, disc, wr = [], [], []
+    tot, disc, wr, devt = [], [], [], []
     for it in range(Wm + K):
         rearm(it)
         if cold:
             env.flush_l2(it)
         evs = [env.ev() for _ in range(4)]
         torch.cuda.synchronize()
+        if ahead:
+            torch.cuda._sleep(300000)
         evs[0].record(stream)
-        ctx.trace_events(evs[1], evs[2])
+        if phases:
+            ctx.trace_events(evs[1], evs[2])
         call(it, res)
         evs[3].record(stream)
         torch.cuda.synchronize()
-        ctx.trace_events(None, None)
+        if phases:
+            ctx.trace_events(None, None)
         r = res.read()
         assert r.status == 0 and r.n_dirty == k_expect, (r.as_dict(), k_expect)
         if reset:
             ctx.log_reset()
         if it >= Wm:
             tot.append(evs[0].elapsed_time(evs[3]))
-            disc.append(evs[0].elapsed_time(evs[2]))
-            wr.append(evs[2].elapsed_time(evs[3]))
-    return tot, disc, wr
+            disc.append(evs[0].elapsed_time(evs[2]) if phases else 0.0)
+            wr.append(evs[2].elapsed_time(evs[3]) if phases else 0.0)
+            devt.append((r.t_end_ns - r.t_start_ns) / 1e6)
+    return tot, disc, wr, devt
 
 
 def small_region_workload(args, env, name):
@@ -797,11 +808,14 @@ def small_region_workload(args, env, name):
     sampler = ClockSampler(env.local).start()
     launches0 = ctx.kernel_launches()
     env.barrier()
-    tot, disc, wr = timed_checkpoints(ctx, cc, env, 1, K, Wm, rearm, k, cold=True)
+    tot, _, _, devt = timed_checkpoints(ctx, cc, env, 1, K, Wm, rearm, k, cold=True, phases=False, ahead=True)
     env.barrier()
     launches = (ctx.kernel_launches() - launches0) * K // (K + Wm)
     clocks = sampler.stop()
-    tot_w, disc_w, wr_w = timed_checkpoints(ctx, cc, env, 1, K, Wm, rearm, k, cold=False)
+    tot_w, _, _, devt_w = timed_checkpoints(ctx, cc, env, 1, K, Wm, rearm, k, cold=False, phases=False, ahead=True)
+    # the split into discovery / writer needs events between the kernels (which cost the kernels their overlap), and the
+    # call issued to an idle GPU shows what the interpreter adds: both reported beside the headline, not in it
+    tot_p, disc, wr, _ = timed_checkpoints(ctx, cc, env, 1, K, Wm, rearm, k, cold=True, phases=True, ahead=False)
     # ---- e2e: pinned host log, the mutation bytes come from host memory, result read on the host ----
     e2e = None
     if not args.no_e2e:
@@ -830,14 +844,19 @@ def small_region_workload(args, env, name):
         line = base_line(env, K, Wm, env.world * N / (ms * 1e-3) / 1e9, ms, desc + "; log in device memory",
                          {"page_bytes": P, "region_bytes_per_gpu": N, "dirty_pages": k, "dirty_bytes": k * P,
                           "l2": "flushed: 512 MiB written between timed iterations (outside the events); each step timed on its own",
-                          "timing": "CUDA events around each cc_checkpoint_delta; the re-arming byte flips and the flush are not timed"},
+                          "timing": "CUDA events around each cc_checkpoint_delta, the call queued behind a 150 us spin kernel so that the "
+                                    "events bracket GPU time only; the re-arming byte flips and the flush are not timed"},
                          "u8 (bitwise compare/copy; CRC32C in u32)")
         line["gpu_launches"] = int(launches)
         line["clocks"] = clocks
         line["parity"] = parity
-        line["phases_ms"] = {"discovery": round(statistics.mean(disc), 4), "writer": round(statistics.mean(wr), 4),
-                             "checkpoint_total": round(ms, 4), "best_checkpoint_total": round(min(tot), 4),
-                             "warm_l2_checkpoint_total": round(statistics.mean(tot_w), 4), "warm_l2_best": round(min(tot_w), 4)}
+        line["phases_ms"] = {"checkpoint_total": round(ms, 4), "best_checkpoint_total": round(min(tot), 4),
+                             "device_stamps_total": round(statistics.mean(devt), 4),
+                             "warm_l2_checkpoint_total": round(statistics.mean(tot_w), 4), "warm_l2_best": round(min(tot_w), 4),
+                             "warm_l2_device_stamps_total": round(statistics.mean(devt_w), 4),
+                             "issued_to_idle_gpu_with_events_between_kernels": {
+                                 "total": round(statistics.mean(tot_p), 4), "discovery": round(statistics.mean(disc), 4),
+                                 "writer": round(statistics.mean(wr), 4)}}
         line["roofline"] = roofline("cc_checkpoint_delta (whole call: launch- and latency-bound at this size)", algo, ms, args.workload)
         line["roofline"]["note"] = "64 MiB regions are launch/latency-bound, not HBM-bound; HBM-fraction claims are made on c2 / c4"
         if e2e:
@@ -916,7 +935,7 @@ def run_c4_sparse(args, env):
             sampler = ClockSampler(env.local).start()
             launches0 = ctx.kernel_launches()
         env.barrier()
-        tot, disc, wr = timed_checkpoints(ctx, cc, env, rid, K if P == Ps[0] else max(3, K // 4), Wm,
+        tot, disc, wr, _ = timed_checkpoints(ctx, cc, env, rid, K if P == Ps[0] else max(3, K // 4), Wm,
                                           lambda it: synth.toggle_flips(cur, offs, masks), k, cold=False)
         env.barrier()
         if P == Ps[0]:
@@ -1048,12 +1067,12 @@ def run_c4_full(args, env):
             sampler = ClockSampler(env.local).start()
             launches0 = ctx.kernel_launches()
         env.barrier()
-        tot, disc, wr = timed_checkpoints(ctx, cc, env, 1, K, Wm, lambda it: synth.toggle_flips(cur, offs, masks), n_pages, cold=False)
+        tot, disc, wr, _ = timed_checkpoints(ctx, cc, env, 1, K, Wm, lambda it: synth.toggle_flips(cur, offs, masks), n_pages, cold=False)
         env.barrier()
         if P == Ps[0]:
             clocks = sampler.stop()
             launches = (ctx.kernel_launches() - launches0) * K // (K + Wm)
-        totf, _, _ = timed_checkpoints(ctx, cc, env, 1, K, 2, lambda it: synth.toggle_flips(cur, offs, masks), n_pages, cold=False,
+        totf, _, _, _ = timed_checkpoints(ctx, cc, env, 1, K, 2, lambda it: synth.toggle_flips(cur, offs, masks), n_pages, cold=False,
                                        call=lambda it, res: ctx.checkpoint_delta_fused(1, it, res))
         ms = statistics.mean(tot)
         sweep["%dKiB" % (P >> 10)] = {"dirty_pages": n_pages, "ms_total": round(ms, 4), "ms_scan_compact": round(statistics.mean(disc), 4),

@@ -224,8 +224,13 @@ int32_t cc_log_drain_stop(cc_ctx* ctx);
  *               classic phases behind grid barriers instead (all-or-nothing needs the count first).
  *               CC_PATH_PHASES: the classic phases as separate launches (discovery, ordered compaction,
  *               [run ranking,] gather + commit), each sized for its own work.
- *               CC_PATH_AUTO: single pass when the attached log is pinned host memory (the host-link transfer then
- *               overlaps the scan); phases otherwise (with a device log they are faster at every size measured).
+ *               CC_PATH_SMALL: ONE kernel launch with one grid-wide rendezvous, for regions of at most 131,072 pages
+ *               (CC_DISC_SCAN, one record per page; CC_ERR_INVALID otherwise): scan, then every block ranks the
+ *               whole dirty bitmap by itself and the record writer follows at once -- the low-latency path of small
+ *               regions (Table 6: the cost of a boundary is flat in the dirty count).
+ *               CC_PATH_AUTO: CC_PATH_SMALL where it applies and the region is small enough to be latency-bound;
+ *               else the single pass when the attached log is pinned host memory (the host-link transfer then overlaps
+ *               the scan), and the phases otherwise (with a device log they are faster at every larger size measured).
  * Every path writes the same bytes.  Result, asynchrony, CC_ERR_LOG_FULL rule: as cc_checkpoint_delta below. */
 #define CC_DISC_SCAN 0u
 #define CC_DISC_MARKS 1u
@@ -234,6 +239,7 @@ int32_t cc_log_drain_stop(cc_ctx* ctx);
 #define CC_PATH_AUTO 0u
 #define CC_PATH_SINGLE_PASS 1u
 #define CC_PATH_PHASES 2u
+#define CC_PATH_SMALL 3u
 typedef struct {
     uint32_t discovery;        /* CC_DISC_* */
     uint32_t path;             /* CC_PATH_* */

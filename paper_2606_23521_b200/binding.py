@@ -47,7 +47,7 @@ CC_TASKF_RLE = 2
 CC_WORKER_BLOCKS_DEFAULT = 16
 CC_WORKER_BLOCKS_ALL = 0xFFFFFFFF
 CC_DISC_SCAN, CC_DISC_MARKS, CC_DISC_VERSIONS, CC_DISC_ALL = 0, 1, 3, 4
-CC_PATH_AUTO, CC_PATH_SINGLE_PASS, CC_PATH_PHASES = 0, 1, 2
+CC_PATH_AUTO, CC_PATH_SINGLE_PASS, CC_PATH_PHASES, CC_PATH_SMALL = 0, 1, 2, 3
 
 EXPORTS = [
     "cc_init", "cc_shutdown", "cc_last_cuda_error", "cc_kernel_launches", "cc_workspace_bytes",

@@ -150,21 +150,6 @@ __device__ __forceinline__ void cc_batch_plan_phase(cc_dev* dev, u64 epoch) {
     }
 }
 
-__device__ __forceinline__ void cc_batch_write_result(cc_dev* dev, cc_result* out, u32 kind) {
-    const cc_batch_state* B = &dev->batch;
-    if (!out) return;
-    out->n_dirty = B->k_total;
-    out->bytes = B->bytes_total;
-    out->log_offset_after = B->W_final;
-    out->epoch = B->epoch;
-    out->status = B->status;
-    out->flags = kind;
-    out->t_start_ns = B->t_start_ns;
-    out->t_end_ns = globaltimer_ns();
-    __threadfence_system();
-    st_release_sys_u64(&out->seq_done, 1ull);
-}
-
 // cs must already hold the CRC tables.
 __device__ __forceinline__ void cc_batch_gather_phase(cc_dev* dev, cc_crc_smem* cs, cc_batch_tab* T, cc_grid g, cc_result* out,
                                                       u32 kind) {
@@ -184,27 +169,35 @@ __device__ __forceinline__ void cc_batch_gather_phase(cc_dev* dev, cc_crc_smem* 
             if (first < T->n_items[s]) cc_gather_items(dev->regions[s], dev, cs, first, nw);
         }
     }
-    // ---- one completion for the whole boundary ----
+    // ---- one completion for the whole boundary (same fence chain as cc_gather_complete: gpu-scope per block, ONE
+    //      system-scope fence in the last block behind every commit record) ----
     __shared__ u32 s_last;
-    __threadfence_system();
     __syncthreads();
     if (threadIdx.x == 0) {
-        __threadfence_system();
+        __threadfence();
         s_last = (atomicAdd(&B->done, 1u) == g.nblocks - 1) ? 1u : 0u;
+        if (s_last) __threadfence();
     }
     __syncthreads();
     if (!s_last) return;
-    __threadfence_system();
     if (threadIdx.x < CC_MAX_REGIONS && cc_batch_takes_part(dev, (int)threadIdx.x))
         cc_gather_commit_record(dev->regions[threadIdx.x], dev);
-    __threadfence_system();
     __syncthreads();
     if (threadIdx.x == 0) {
-        __threadfence_system();
         cc_log_dev* log = &dev->log;
-        if (B->bytes_total != 0) cc_log_publish(log, B->W_final);
         B->done = 0;
-        cc_batch_write_result(dev, out, kind);
-        __threadfence();
+        if (out) {
+            out->n_dirty = B->k_total;
+            out->bytes = B->bytes_total;
+            out->log_offset_after = B->W_final;
+            out->epoch = B->epoch;
+            out->status = B->status;
+            out->flags = kind;
+            out->t_start_ns = B->t_start_ns;
+            out->t_end_ns = globaltimer_ns();
+        }
+        __threadfence_system();
+        if (B->bytes_total != 0) cc_log_publish_fenced(log, B->W_final);
+        if (out) st_relaxed_sys_u64(&out->seq_done, 1ull);
     }
 }

@@ -259,70 +259,74 @@ __device__ __forceinline__ void st_u32x4(u8* p, u32 a, u32 b, u32 c, u32 d) {
     st_stream(reinterpret_cast<uint4*>(p), v);
 }
 
+// One (record, segment) item of the record writer: segment c of page p, which is record i of the checkpoint that starts
+// at log offset W0.  The warp reads the segment ONCE; log payload, shadow and CRC contribution come from that read; the
+// warp that completes the record's last segment writes its header.
+__device__ __forceinline__ void cc_gather_segment(const cc_region_dev& r, cc_dev* dev, cc_crc_smem* cs, u64 W0, u32 i, u32 c, u32 p,
+                                                  u32 lane) {
+    constexpr int U = 8;
+    cc_log_dev* log = &dev->log;
+    const u32 P = r.page_bytes;
+    const u64 plen = page_len_dev(r, p);
+    const u64 so = (u64)c * CC_SEG_BYTES;
+    if (so >= plen) return;
+    const u64 rem = plen - so;
+    const u32 seg_len = (u32)(rem < CC_SEG_BYTES ? rem : CC_SEG_BYTES);
+    const u32 nv = seg_len >> 4;
+    const u64 after = rem - seg_len;
+    const u32 nseg = (u32)((plen + CC_SEG_BYTES - 1) / CC_SEG_BYTES);
+    const u64 src_off = (u64)p * P + so;
+    const uint4* src = reinterpret_cast<const uint4*>(r.base + src_off);
+    const bool has_shadow = r.shadow != nullptr;      // allocator-aware regions may have none (cc_mark.cuh)
+    uint4* dsh = reinterpret_cast<uint4*>(r.shadow + src_off);
+    u8* rec = log->buf + W0 + (u64)i * ((u64)P + CC_RECORD_HEADER_BYTES);
+    uint4* dlog = reinterpret_cast<uint4*>(rec + CC_RECORD_HEADER_BYTES + so);
+    uint4 v[U];
+    if (nv == CC_SEG_VECS) {
+#pragma unroll
+        for (int u = 0; u < U; u++) v[u] = ld_stream(src + lane + 32 * u);
+#pragma unroll
+        for (int u = 0; u < U; u++) st_stream(dlog + lane + 32 * u, v[u]);
+        if (has_shadow) {
+#pragma unroll
+            for (int u = 0; u < U; u++) st_stream(dsh + lane + 32 * u, v[u]);
+        }
+    } else {
+#pragma unroll
+        for (int u = 0; u < U; u++) {
+            const u32 j = lane + 32 * u;
+            if (j < nv) {
+                v[u] = ld_stream(src + j);
+                st_stream(dlog + j, v[u]);
+                if (has_shadow) st_stream(dsh + j, v[u]);
+            } else {
+                v[u] = make_uint4(0, 0, 0, 0);
+            }
+        }
+    }
+    const u32 contrib = crc_segment_warp<U>(cs, &dev->crc, v, nv, after, lane);
+    if (lane == 0) {
+        u32 acc = 0;
+        const bool finish = crc_record_combine(&r.rec_state[i], nseg, c, contrib, &acc);
+        if (finish) st_u32x4(rec, r.region_id, p, (u32)plen,
+                             crc_finalize(acc, plen == P ? r.crc_init_full : r.crc_init_tail));
+    }
+}
+
 // The record writer proper (no synchronisation with other blocks): items first, first + step, ... of the
 // region's k_eff * spp (record, segment) items.  cs must hold the CRC tables.
 __device__ __forceinline__ void cc_gather_items(const cc_region_dev& r, cc_dev* dev, cc_crc_smem* cs, u64 first, u64 step) {
-    constexpr int U = 8;
     cc_ws_hdr* h = r.hdr;
-    cc_log_dev* log = &dev->log;
     const u32 k_eff = h->k_eff;
     const u32 lane = threadIdx.x & 31u;
-    const u32 P = r.page_bytes;
     const u64 W0 = h->W_start;
-    {
-        const u32 spp = r.spp;
-        const u64 n_items = (u64)k_eff * spp;
-        const u64 rec_stride = (u64)P + CC_RECORD_HEADER_BYTES;
-        for (u64 item = first; item < n_items; item += step) {
-            u32 i, c;
-            if (r.spp_shift >= 0) { i = (u32)(item >> r.spp_shift); c = (u32)(item & (spp - 1)); }
-            else { i = (u32)(item / spp); c = (u32)(item - (u64)i * spp); }
-            const u32 p = r.D[i];
-            const u64 plen = page_len_dev(r, p);
-            const u64 so = (u64)c * CC_SEG_BYTES;
-            if (so >= plen) continue;
-            const u64 rem = plen - so;
-            const u32 seg_len = (u32)(rem < CC_SEG_BYTES ? rem : CC_SEG_BYTES);
-            const u32 nv = seg_len >> 4;
-            const u64 after = rem - seg_len;
-            const u32 nseg = (u32)((plen + CC_SEG_BYTES - 1) / CC_SEG_BYTES);
-            const u64 src_off = (u64)p * P + so;
-            const uint4* src = reinterpret_cast<const uint4*>(r.base + src_off);
-            const bool has_shadow = r.shadow != nullptr;      // allocator-aware regions may have none (cc_mark.cuh)
-            uint4* dsh = reinterpret_cast<uint4*>(r.shadow + src_off);
-            u8* rec = log->buf + W0 + (u64)i * rec_stride;
-            uint4* dlog = reinterpret_cast<uint4*>(rec + CC_RECORD_HEADER_BYTES + so);
-            uint4 v[U];
-            if (nv == CC_SEG_VECS) {
-#pragma unroll
-                for (int u = 0; u < U; u++) v[u] = ld_stream(src + lane + 32 * u);
-#pragma unroll
-                for (int u = 0; u < U; u++) st_stream(dlog + lane + 32 * u, v[u]);
-                if (has_shadow) {
-#pragma unroll
-                    for (int u = 0; u < U; u++) st_stream(dsh + lane + 32 * u, v[u]);
-                }
-            } else {
-#pragma unroll
-                for (int u = 0; u < U; u++) {
-                    const u32 j = lane + 32 * u;
-                    if (j < nv) {
-                        v[u] = ld_stream(src + j);
-                        st_stream(dlog + j, v[u]);
-                        if (has_shadow) st_stream(dsh + j, v[u]);
-                    } else {
-                        v[u] = make_uint4(0, 0, 0, 0);
-                    }
-                }
-            }
-            const u32 contrib = crc_segment_warp<U>(cs, &dev->crc, v, nv, after, lane);
-            if (lane == 0) {
-                u32 acc = 0;
-                const bool finish = crc_record_combine(&r.rec_state[i], nseg, c, contrib, &acc);
-                if (finish) st_u32x4(rec, r.region_id, p, (u32)plen,
-                                     crc_finalize(acc, plen == P ? r.crc_init_full : r.crc_init_tail));
-            }
-        }
+    const u32 spp = r.spp;
+    const u64 n_items = (u64)k_eff * spp;
+    for (u64 item = first; item < n_items; item += step) {
+        u32 i, c;
+        if (r.spp_shift >= 0) { i = (u32)(item >> r.spp_shift); c = (u32)(item & (spp - 1)); }
+        else { i = (u32)(item / spp); c = (u32)(item - (u64)i * spp); }
+        cc_gather_segment(r, dev, cs, W0, i, c, r.D[i], lane);
     }
 }
 
@@ -362,11 +366,15 @@ __device__ __forceinline__ u64 cc_gather_commit_record(const cc_region_dev& r, c
     return W_after;
 }
 
-// Completion of a region's record writer: every block fences its stores at system scope and counts itself
-// done; the last block appends the commit record, fences, publishes the committed offset with a system-scope
-// release store (L263) and fills the result.
+// Completion of a region's record writer.  Every block that wrote records orders its stores before one gpu-scope
+// atomic on the region's counter (bar.sync, then ONE thread: fence.gpu + atomicAdd -- the fence is cumulative over what
+// the barrier ordered before it); the block that counts last has, by that chain, every block's record bytes behind it:
+// it appends the commit record, fills the result, executes the ONE system-scope fence of the call and only then stores
+// the publishing words (L263 "a commit marker publishes the epoch only after all bytes are visible").  System-scope
+// fences cost microseconds each (more with host-link stores in flight); a chain of four of them per call -- every
+// thread, then one thread per block, then two in the last block -- was 15-20 us of a 55 us checkpoint of a 64 MiB region.
 // Only the blocks that had items take part (n_items = items of the record writer; at least block 0): with a
-// small dirty set the other blocks leave at once instead of queueing fences and atomics on one counter.
+// small dirty set the other blocks leave at once instead of queueing atomics on one counter.
 __device__ __forceinline__ void cc_gather_complete(const cc_region_dev& r, cc_dev* dev, cc_grid g, cc_result* out, u32 kind,
                                                    u64 n_items) {
     cc_ws_hdr* h = r.hdr;
@@ -377,16 +385,15 @@ __device__ __forceinline__ void cc_gather_complete(const cc_region_dev& r, cc_de
     if (n_work == 0) n_work = 1;
     if (g.block >= n_work) return;
     __shared__ u32 s_last;
-    __threadfence_system();
     __syncthreads();
     if (threadIdx.x == 0) {
-        __threadfence_system();
+        __threadfence();
         s_last = (atomicAdd(&h->gather_done, 1u) == (u32)n_work - 1) ? 1u : 0u;
     }
     __syncthreads();
     if (s_last && threadIdx.x == 0) {
         CC_TRACE(dev, 6);
-        __threadfence_system();                 // (acquire side of the counter: every block's record bytes are behind us)
+        __threadfence();                        // (acquire side of the counter: every block's record bytes are behind us)
         const bool appended = h->k_eff != 0;
         const u64 W_after = cc_gather_commit_record(r, dev);
         CC_TRACE(dev, 7);
@@ -400,13 +407,12 @@ __device__ __forceinline__ void cc_gather_complete(const cc_region_dev& r, cc_de
             out->t_start_ns = h->t_start_ns;
             out->t_end_ns = globaltimer_ns();
         }
-        // ONE fence behind the commit record and the result fields, then the publishing words (L263: "a commit marker
-        // publishes the epoch only after all bytes are visible")
+        // ONE system-scope fence behind the record bytes (all blocks'), the commit record and the result fields, then
+        // the publishing words
         __threadfence_system();
         if (appended) cc_log_publish_fenced(log, W_after);
         if (out) st_relaxed_sys_u64(&out->seq_done, 1ull);
         CC_TRACE(dev, 8);
-        __threadfence();
     }
 }
 

@@ -288,28 +288,23 @@ __device__ __forceinline__ u32 ld_relaxed_sys_u32(const u32* p) {
     return v;
 }
 
-// One thread, after the commit record's bytes have been fenced at system scope ("a commit marker publishes
-// the epoch only after all bytes are visible"): advance the write offset and publish the committed offset -- to the
-// caller's word and to the library's own (generation-tagged) word.
-__device__ __forceinline__ void cc_log_publish(cc_log_dev* log, u64 W_after) {
-    if (log->committed_off) st_release_sys_u64(log->committed_off, W_after);
-    if (log->pub) st_release_sys_u64(log->pub, (log->gen << CC_PUB_SHIFT) | W_after);
-    log->W = W_after;
-}
-// The same after the CALLER has issued __threadfence_system() behind the commit record (and whatever else must be visible
-// first): plain system-scope stores -- every release store would be another full fence, ~2 us each with host-memory
-// stores in flight.
+// One thread, after the CALLER has executed __threadfence_system() behind the commit record ("a commit
+// marker publishes the epoch only after all bytes are visible") and whatever else must be visible first: advance the
+// write offset and publish the committed offset -- to the caller's word and to the library's own (generation-tagged)
+// word -- with plain system-scope stores (every release store would be another full fence, ~2 us each with host-memory
+// stores in flight).
 __device__ __forceinline__ void cc_log_publish_fenced(cc_log_dev* log, u64 W_after) {
     if (log->committed_off) st_relaxed_sys_u64(log->committed_off, W_after);
     if (log->pub) st_relaxed_sys_u64(log->pub, (log->gen << CC_PUB_SHIFT) | W_after);
     log->W = W_after;
 }
-// W := 0: a new generation of the log (cc_log_reset*, CC_TASK_LOG_RESET).
+// W := 0: a new generation of the log (cc_log_reset*, CC_TASK_LOG_RESET).  One fence, then the two words.
 __device__ __forceinline__ void cc_log_rewind(cc_log_dev* log) {
     log->gen = log->gen + 1;
     log->W = 0;
-    if (log->committed_off) st_release_sys_u64(log->committed_off, 0ull);
-    if (log->pub) st_release_sys_u64(log->pub, log->gen << CC_PUB_SHIFT);
+    __threadfence_system();
+    if (log->committed_off) st_relaxed_sys_u64(log->committed_off, 0ull);
+    if (log->pub) st_relaxed_sys_u64(log->pub, log->gen << CC_PUB_SHIFT);
 }
 
 __device__ __forceinline__ u64 page_len_dev(const cc_region_dev& r, u64 p) {

@@ -15,9 +15,9 @@
 //               PAPER.md:L221 "contiguous dirty ranges use run-length encoding" -- one RUN of consecutive dirty pages.
 //               Runs are cut at tile boundaries, and tiles are whole multiples of run_pages, so no run crosses a tile
 //               and the bytes are exactly those of the oracle's run records;
-//   leaves      every warp fences what it stored and counts itself out (per block in shared memory, then one atomic
-//               per block); the LAST warp of the grid appends the commit record, fences, publishes the committed
-//               offset and fills the result (L263).
+//   leaves      every warp counts itself out (per block in shared memory, then one gpu-scope atomic per block); the
+//               LAST warp of the grid appends the commit record, fills the result, executes the call's one
+//               system-scope fence and publishes the committed offset (L263).
 // All-or-nothing (reading #10) is decided up front: records are written inline only if the WORST case (every page
 // dirty) fits behind the write offset.  Otherwise the same kernel falls back to the classic phases (scan, compaction,
 // [run ranking,] gather) separated by grid barriers -- which is why it is launched cooperatively.
@@ -132,15 +132,19 @@ __device__ __forceinline__ bool cc_pass_page_dirty(const cc_region_dev& r, u64 p
 }
 
 // Completion of a single-pass call: every warp of the grid comes here once.  s_warps_left: shared counter of the
-// block, preset to its warp count.  Returns true in the ONE warp of the grid that leaves last.
+// block, preset to its warp count.  Returns true in the ONE warp of the grid that leaves last.  No system-scope fence
+// here: a warp orders its record / shadow stores before its count-out at block scope, the block's last warp before the
+// grid counter at gpu scope, and the grid's last warp executes the call's one system-scope fence behind the commit
+// record (cc_pass_commit) -- fences are cumulative along that chain.
 __device__ __forceinline__ bool cc_pass_leave(cc_ws_hdr* h, u32* s_warps_left, bool wrote, u32 nblocks, u32 lane) {
-    if (wrote) __threadfence_system();                        // this warp's record / shadow bytes, before it counts out
+    __syncwarp();
     u32 last = 0;
     if (lane == 0) {
+        if (wrote) __threadfence_block();
         if (atomicSub(s_warps_left, 1u) == 1u) {              // last warp of the block
-            __threadfence_system();
+            __threadfence();
             last = (atomicAdd(&h->gather_done, 1u) == nblocks - 1) ? 1u : 0u;
-            if (last) __threadfence_system();
+            if (last) __threadfence();
         }
     }
     return __shfl_sync(0xFFFFFFFFu, last, 0) != 0;
@@ -357,10 +361,9 @@ __device__ __forceinline__ void cc_pass_commit(const cc_region_dev& r, cc_dev* d
         out->t_start_ns = h->t_start_ns;
         out->t_end_ns = globaltimer_ns();
     }
-    __threadfence_system();                                   // one fence behind commit record + result, then the publishing words
+    __threadfence_system();                                   // the call's ONE system-scope fence: behind every warp's records, the commit record and the result
     if (appended) cc_log_publish_fenced(log, W_after);
     if (out) st_relaxed_sys_u64(&out->seq_done, 1ull);
-    __threadfence();
 }
 
 // worst case of one checkpoint of the region: every page dirty, one record per page
