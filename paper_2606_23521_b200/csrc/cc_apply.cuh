@@ -26,6 +26,7 @@ struct cc_apply_tabs {      // carved out of the attached scratch
     u64* rec_state;         // per-record {done-mask or count | CRC accumulator} (crc_record_combine)
     u32* seg_begin;         // per-record first segment number (+ one trailing total)
     u32* cand;              // max_records + 1: candidate commit records, log offset / 16, ascending
+    u32* cand_raw;          // max_records + 1: the same as found (unordered)
     u64* span_status;       // max_records + 2: look-back words of the epoch walk
     u64 max_records;
 };

@@ -3,8 +3,8 @@
 // The sequential definition walks record by record; every epoch ends in a 32-byte commit record.  Here the epochs
 // are parsed CONCURRENTLY, with exactly the sequential result:
 //   candidates  every 16-byte-aligned position of the log is tested for a commit record's signature
-//               {0xFFFFFFFF, 0xFFFFFFFF, 16, crc32c(next 16 bytes)}; the positions that pass are listed in ascending
-//               order (contiguous ranges per block by ticket, per-warp ordered lists, look-back over the tickets).
+//               {0xFFFFFFFF, 0xFFFFFFFF, 16, crc32c(next 16 bytes)}; the positions that pass are appended to a list,
+//               which a ranking step then puts in ascending order.
 //               Every real commit record is on the list; a payload that happens to contain the image of a commit
 //               record puts a FALSE candidate on it.
 //   walk        span j = [end of candidate j-1, candidate j) is walked by one block from its start, as the sequential
@@ -35,97 +35,73 @@ __device__ __forceinline__ u32 sp_segs(u64 w) { return (u32)((w >> 31) & 0x7FFFF
 __device__ __forceinline__ u32 sp_flag(u64 w) { return (u32)(w >> 62); }
 
 // ---------------------------------------------------------------------------- candidates --
-// grid-wide; scratch: T.cand[0 .. max_records], T.span_status[0 .. max_records + 1]
-__device__ __forceinline__ void cc_parse_cand_phase(cc_dev* dev, cc_parse_ctl* C, u32* cand, u64* span_status, u64 max_records,
-                                                    const u8* log, u64 n, bool first_block) {
-    __shared__ u32 s_list[CC_CAND_THREADS / 32][CC_CAND_WARP_CAP];
-    __shared__ u32 s_cnt[CC_CAND_THREADS / 32];
-    __shared__ u32 s_ticket, s_base, s_over;
-    const u32 tid = threadIdx.x, lane = tid & 31u, wid = tid >> 5;
-    constexpr u32 NW = CC_CAND_THREADS / 32;
+// grid-wide, no block barrier, no ordering: a warp tests 4 KiB of the log per step (8 independent 16-byte loads per
+// lane, the scanner's loop) and appends the rare hits to an UNORDERED list with one atomic each; cc_parse_sort_phase
+// then ranks the list.  (The first version kept the list ordered as it went -- ticketed ranges per block, per-warp
+// ordered sub-lists, look-back over the tickets: three block barriers per 128 KiB and 78 registers held it at 2.7 TB/s,
+// profiles/r02_apply_ncu.md.)  scratch: T.cand_raw[0 .. max_records].
+__device__ __forceinline__ void cc_parse_cand_phase(cc_dev* dev, cc_parse_ctl* C, u32* cand_raw, u64 max_records, const u8* log, u64 n,
+                                                    cc_grid g) {
+    const u32 lane = threadIdx.x & 31u;
     const u64 units = n >> 4;                                    // 16-byte units of the log
-    // ranges of whole 4 KiB steps per warp, at most CC_CAND_TICKETS of them, at least 128 KiB each (fine ranges spread
-    // a few-hundred-MB log evenly over the SMs: 1 MiB ranges left half of them with twice the work of the rest)
-    u64 range_units = (units + CC_CAND_TICKETS - 1) / CC_CAND_TICKETS;
-    if (range_units < (1u << 13)) range_units = 1u << 13;
-    range_units = (range_units + 2047) / 2048 * 2048;            // a multiple of NW warps x 256 units
-    const u32 n_ranges = (u32)((units + range_units - 1) / range_units);
-    const u64 warp_units = range_units / NW;
-    const u32 run = C->run & 0x3FFFFFFFu;
-    if (n_ranges == 0) {                                         // a log shorter than 16 bytes: nothing to find
-        if (first_block && tid == 0) { cc_apply_reset_state(dev); C->n_cand = 0; span_status[0] = 0; }
-        return;
+    if (g.block == 0 && threadIdx.x == 0) cc_apply_reset_state(dev);     // (read by the walk phase, two launches later)
+    const uint4* L = reinterpret_cast<const uint4*>(log);
+    for (u64 ub = (u64)g.warp() * 256u; ub < units; ub += (u64)g.nwarps() * 256u) {
+        uint4 v[8];
+#pragma unroll
+        for (int q = 0; q < 8; q++) {
+            const u64 u = ub + 32u * q + lane;
+            v[q] = (u < units) ? ld_v4(L + u) : make_uint4(0, 0, 0, 0);
+        }
+#pragma unroll
+        for (int q = 0; q < 8; q++) {
+            const u64 u = ub + 32u * q + lane;
+            if ((v[q].x == CC_COMMIT_ID) && (v[q].y == CC_COMMIT_ID) && (v[q].z == 16u) && (u + 2 <= units)) {
+                // rare: check the commit payload's CRC
+                const uint4 pl = ld_v4(L + u + 1);
+                u32 c = 0xFFFFFFFFu;
+                const u32 pay[4] = {pl.x, pl.y, pl.z, pl.w};
+#pragma unroll
+                for (int w = 0; w < 4; w++) {
+                    c ^= pay[w];
+                    for (int b = 0; b < 32; b++) c = gf_mulx(c);
+                }
+                if ((c ^ 0xFFFFFFFFu) == v[q].w) {
+                    const u32 pos = atomicAdd(&C->n_raw, 1u);
+                    if ((u64)pos <= max_records) cand_raw[pos] = (u32)u;
+                    else C->cand_overflow = 1;
+                }
+            }
+        }
     }
-    for (;;) {
-        if (tid == 0) { s_ticket = atomicAdd(&C->ticket, 1u); s_over = 0; }
-        if (lane == 0) s_cnt[wid] = 0;
-        __syncthreads();
-        const u32 t = s_ticket;
-        if (t >= n_ranges) break;
-        // warp `wid` owns the contiguous part [u0, u1) of the range and keeps its hits in ascending order
-        const u64 u0 = (u64)t * range_units + (u64)wid * warp_units;
-        u64 u1 = u0 + warp_units;
-        if (u1 > units) u1 = units;
-        u32 cnt = 0;
-        for (u64 ub = u0; ub < u1; ub += 256) {
-            uint4 v[8];
-#pragma unroll
-            for (int q = 0; q < 8; q++) {
-                const u64 u = ub + 32u * q + lane;
-                v[q] = (u < u1) ? ld_v4(reinterpret_cast<const uint4*>(log) + u) : make_uint4(0, 0, 0, 0);
-            }
-#pragma unroll
-            for (int q = 0; q < 8; q++) {
-                const u64 u = ub + 32u * q + lane;
-                bool hit = (v[q].x == CC_COMMIT_ID) && (v[q].y == CC_COMMIT_ID) && (v[q].z == 16u) && (u + 2 <= units) && (u < u1);
-                if (hit) {                                       // rare: check the commit payload's CRC
-                    const uint4 pl = ld_v4(reinterpret_cast<const uint4*>(log) + u + 1);
-                    u32 pay[4] = {pl.x, pl.y, pl.z, pl.w};
-                    hit = crc_serial(&dev->crc, reinterpret_cast<const u8*>(pay), 16) == v[q].w;
-                }
-                const u32 b = __ballot_sync(0xFFFFFFFFu, hit);
-                if (hit) {
-                    const u32 pos = cnt + __popc(b & ((1u << lane) - 1u));
-                    if (pos < CC_CAND_WARP_CAP) s_list[wid][pos] = (u32)u;
-                }
-                cnt += __popc(b);
-            }
+}
+
+// ---------------------------------------------------------------------------------- sort --
+// Ascending order of the candidate list by ranking: position = number of smaller candidates (they are distinct log
+// offsets).  n^2 / threads comparisons out of shared-memory tiles: a hundred candidates are a few microseconds of one
+// block, a hundred thousand ~0.1 ms of the whole grid -- either way far below the serial walk the ordered list saves.
+// Also arms the look-back words of the walk.  scratch: T.cand[0 .. max_records], T.span_status[0 .. max_records + 1].
+#define CC_SORT_THREADS 256
+__device__ __forceinline__ void cc_parse_sort_phase(cc_parse_ctl* C, const u32* cand_raw, u32* cand, u64* span_status, u64 max_records,
+                                                    cc_grid g) {
+    __shared__ u32 s_tile[CC_SORT_THREADS];
+    const u32 tid = threadIdx.x;
+    u64 n64 = C->n_raw;
+    if (n64 > max_records + 1) n64 = max_records + 1;
+    const u32 n = (u32)n64;
+    if (g.block == 0 && tid == 0) { C->n_cand = n; span_status[0] = 0; }
+    for (u32 base = g.block * CC_SORT_THREADS; base < n; base += g.nblocks * CC_SORT_THREADS) {
+        const u32 i = base + tid;
+        const u32 mine = i < n ? cand_raw[i] : 0xFFFFFFFFu;
+        u32 rank = 0;
+        for (u32 t0 = 0; t0 < n; t0 += CC_SORT_THREADS) {
+            __syncthreads();
+            s_tile[tid] = (t0 + tid < n) ? cand_raw[t0 + tid] : 0xFFFFFFFFu;
+            __syncthreads();
+            const u32 m = n - t0 < CC_SORT_THREADS ? n - t0 : CC_SORT_THREADS;
+            for (u32 q = 0; q < m; q++) rank += (s_tile[q] < mine) ? 1u : 0u;
         }
-        if (lane == 0) { s_cnt[wid] = cnt; if (cnt > CC_CAND_WARP_CAP) s_over = 1; }
-        __syncthreads();
-        u32 before = 0, total = 0;
-        for (u32 w = 0; w < NW; w++) { const u32 c = s_cnt[w]; if (w < wid) before += c; total += c; }
-        if (tid == 0) {
-            u32 excl = 0;
-            if (t == 0) {
-                cc_apply_reset_state(dev);                       // (read by the walk phase, which starts after this one)
-                span_status[0] = 0;
-                st_release_gpu_u64(&C->cand_status[0], lb_pack(run, CC_LB_INC, total));
-            } else {
-                st_release_gpu_u64(&C->cand_status[t], lb_pack(run, CC_LB_AGG, total));
-                int j = (int)t - 1;
-                while (j >= 0) {
-                    const u64 s = ld_acquire_gpu_u64(&C->cand_status[j]);
-                    if ((u32)(s >> 34) != run || ((s >> 32) & 3ull) == 0) { __nanosleep(20); continue; }
-                    excl += (u32)s;
-                    if (((s >> 32) & 3ull) == CC_LB_INC) break;
-                    j--;
-                }
-                st_release_gpu_u64(&C->cand_status[t], lb_pack(run, CC_LB_INC, excl + total));
-            }
-            s_base = excl;
-            if (s_over) C->cand_overflow = 1;
-            if (t == n_ranges - 1) C->n_cand = excl + total;     // every earlier range has published
-        }
-        __syncthreads();
-        const u32 base = s_base + before;
-        const u32 mine = cnt < CC_CAND_WARP_CAP ? cnt : CC_CAND_WARP_CAP;
-        for (u32 i = lane; i < mine; i += 32) {
-            const u64 idx = (u64)base + i;
-            if (idx <= max_records) { cand[idx] = s_list[wid][i]; span_status[idx + 1] = 0; }
-            else C->cand_overflow = 1;
-        }
-        __syncthreads();
+        if (i < n) { cand[rank] = mine; span_status[rank + 1] = 0; }
     }
 }
 
@@ -252,7 +228,7 @@ __device__ __forceinline__ void cc_parse_walk_phase(cc_dev* dev, cc_parse_ctl* C
     __shared__ cc_walk_smem S;
     cc_apply_state* A = &dev->apply;
     const u32 tid = threadIdx.x;
-    if (first_block && tid == 0) { C->ticket = 0; C->run = C->run + 1; }      // (the candidate search is over) for the next parse
+    if (first_block && tid == 0) C->n_raw = 0;                    // (the candidate list is sorted and counted) for the next parse
     if (C->cand_overflow) {                                       // the list is incomplete: the serial parser does it all
         if (first_block && tid == 0) C->need_serial = 1;
         return;

@@ -15,7 +15,9 @@ typedef uint64_t u64;
 #define CC_COMPACT_THREADS 256
 #define CC_COMPACT_WORDS_PER_THREAD 4
 #define CC_COMPACT_TILE_WORDS (CC_COMPACT_THREADS * CC_COMPACT_WORDS_PER_THREAD)   // 1024 words = 32768 pages
-#define CC_FUSED_TILE_BYTES (32u * 1024u)    // fused pass: one WARP scans (and gathers) this much of the region per ticket
+#ifndef CC_FUSED_TILE_BYTES
+#define CC_FUSED_TILE_BYTES (32u * 1024u)
+#endif    // fused pass: one WARP scans (and gathers) this much of the region per ticket
 #define CC_FUSED_MAX_TP 32u                  // ... but at most this many pages (the tile's dirty mask is one register)
 
 // Per-region control block in the workspace (device memory).
@@ -134,16 +136,13 @@ struct cc_batch_state {
     u32 pad;
 };
 
-#define CC_CAND_TICKETS 4096u            // look-back slots of the applier's candidate search (ranges of >= 1 MiB)
 struct cc_parse_ctl {                    // control block of the parallel parse (cc_apply_parse.cuh)
-    u32 ticket;                          // candidate search: range ticket (reset by the walk phase)
-    u32 run;                             // tag of the candidate look-back words (bumped by the walk phase)
-    u32 n_cand;                          // candidates found
+    u32 n_raw;                           // candidate search: hits appended so far (reset by the walk phase)
+    u32 n_cand;                          // candidates on the ordered list
     u32 cand_overflow;                   // reset by the validation's resolver
     u32 need_serial;                     // the serial parser must redo the parse (reset by the validation's resolver)
     u32 wticket;                         // walk: span ticket (reset by the validation phase)
-    u32 pad[2];
-    u64 cand_status[CC_CAND_TICKETS];    // look-back over the range tickets (lb_pack)
+    u32 pad[3];
 };
 
 struct alignas(16) cc_crc_tables {

@@ -48,7 +48,7 @@ struct cc_pass_args {
 // Pages per warp tile for this call: about one tile per warp of the grid for small regions (every tile costs one atomic
 // on the ticket counter), at most ~32 KiB of region per tile (a warp that finds a dirty page waits for its
 // predecessors: a 256 MiB / 4 KiB-page task took 179 us with 64 KiB tiles and 116 us with 16-32 KiB tiles), at most
-// CC_PASS_MAX_TILES tiles, and a whole multiple of run_pages.
+// CC_PASS_MAX_TILES tiles, and a whole multiple of run_pages.  (profiles/r02_pass_probe.md: 8 / 16 / 32 / 64 KiB tiles.)
 __device__ __forceinline__ u32 cc_pass_tile_pages(const cc_region_dev& r, u32 run_pages, u32 nwarps) {
     const u64 n = r.n_pages;
     u64 tp = (n + nwarps - 1) / nwarps;
@@ -174,11 +174,11 @@ struct cc_pass_smem { u32 unused; };
 
 // The inline single pass over the tiles (see the file header).  Whole warps call this; no block barrier inside.
 // Tiles are handed out by an atomic TICKET, so that a tile's predecessors have always started -- and, being taken in
-// time order, have mostly FINISHED: the look-back then finds an inclusive sum within a step or two.  (Measured
-// alternatives, profiles/r02_pass_probe.md: dealing the tiles round-robin without a ticket leaves thousands of tiles in
-// flight at once, none of which can publish an inclusive sum yet, and a dirty tile walks back through hundreds of
-// aggregate-only words -- 192 us instead of 148 us on a 256 MiB region; ranking per block with two block barriers per
-// round costs 154-167 us.)  The next ticket is drawn before the current tile is processed, which hides its latency.
+// time order, have mostly FINISHED: the look-back then finds an inclusive sum within a step or two.  A ticket is drawn
+// only when the warp is ready for the tile: drawing the next one ahead of time (to hide the atomic's latency) hands out
+// every tile in the first microseconds -- a static deal in disguise, in which a dirty tile waits on predecessors that
+// sit in some other warp's queue (profiles/r02_pass_probe.md: a 256 MiB ring task took 156 us instead of 109 us, an
+// 8 GiB checkpoint into a pinned log 16.2 ms instead of 12.0 ms).
 // Returns whether this warp stored record or shadow bytes.
 __device__ __forceinline__ bool cc_pass_tiles(const cc_region_dev& r, cc_dev* dev, cc_crc_smem* cs, u32* s_crc_state, cc_pass_smem*,
                                               const cc_pass_args& a, u32 TP, u64 W0, cc_grid) {
@@ -196,12 +196,11 @@ __device__ __forceinline__ bool cc_pass_tiles(const cc_region_dev& r, cc_dev* de
     u32 cut = 0xFFFFFFFFu;
     if (rle) { cut = 0; for (u32 q = 0; q < 32; q += a.run_pages) cut |= 1u << q; }
     bool wrote = false;
-    u32 t_next = 0;
-    if (lane == 0) t_next = atomicAdd(&h->fticket, 1u);
     for (;;) {
-        const u32 t = __shfl_sync(0xFFFFFFFFu, t_next, 0);
+        u32 t = 0;
+        if (lane == 0) t = atomicAdd(&h->fticket, 1u);
+        t = __shfl_sync(0xFFFFFFFFu, t, 0);
         if (t >= nt) break;
-        if (lane == 0) t_next = atomicAdd(&h->fticket, 1u);      // the next tile's ticket is on its way while this one is processed
         const u64 p0 = (u64)t * TP;
         const u32 np = (u32)((r.n_pages - p0) < TP ? (r.n_pages - p0) : TP);
         const u32 tile_bits = np == 32 ? 0xFFFFFFFFu : ((1u << np) - 1u);

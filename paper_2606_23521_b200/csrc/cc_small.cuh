@@ -12,7 +12,7 @@
 //   rank      EVERY block reads the whole bitmap (a few KiB out of L2) and ranks it by itself: per-thread popcounts, one
 //             block-wide exclusive scan, the per-thread offsets kept in shared memory.  Record i's page is then found
 //             by a search in shared memory plus one 64-byte look at the bitmap: no dirty list has to be produced
-//             first and waited for (block 0 still writes D[] for cc_dirty_list);
+//             first and waited for (one block still writes D[] for cc_dirty_list);
 //   write     (record, 4 KiB segment) items round-robin over all warps -- cc_gather_segment, the same record writer;
 //   commit    every block counts itself out (gpu-scope); the last one clears the bitmap, appends the commit record, fills
 //             the result, executes the call's one system-scope fence and publishes (L263).
@@ -105,7 +105,13 @@ __device__ __forceinline__ void cc_small_checkpoint(cc_dev* dev, const cc_region
         }
     }
     if (init_tables) cc_crc_smem_init(cs, &dev->crc);
+    // what the plan needs from the log does not depend on the scan: loaded while the block waits
+    const u64 W0 = log->W;
+    const u64 log_cap = log->capacity;
+    const bool have_log = log->buf != nullptr;
+    const u64 last_page = r.n_pages - 1;
     if (tid == 0) {
+        S->last_dirty = 0;
         while (ld_acquire_gpu_u32(&dev->bar_gen) == gen) __nanosleep(32);
         __threadfence();
     }
@@ -121,6 +127,11 @@ __device__ __forceinline__ void cc_small_checkpoint(cc_dev* dev, const cc_region
         if (wi < padded_words) {
             const uint4 w = ld_relaxed_gpu_v4(&r.bitmap[wi]);
             cnt += __popc(w.x) + __popc(w.y) + __popc(w.z) + __popc(w.w);
+            if ((u32)(last_page >> 7) == (wi >> 2)) {            // this 16-byte group holds the region's last page
+                const u32 sel = (u32)(last_page >> 5) & 3u;
+                const u32 lw = sel == 0 ? w.x : sel == 1 ? w.y : sel == 2 ? w.z : w.w;
+                if ((lw >> (last_page & 31u)) & 1u) S->last_dirty = 1;
+            }
         }
     }
     u32 inc = cnt;
@@ -130,6 +141,7 @@ __device__ __forceinline__ void cc_small_checkpoint(cc_dev* dev, const cc_region
         if (lane >= (u32)o) inc += n;
     }
     if (lane == 31) S->warp_tot[wid] = inc;
+    const u32 my_excl_in_warp = inc - cnt;
     __syncthreads();
     u32 warp_base = 0, k = 0;
     for (u32 w = 0; w < (blockDim.x >> 5); w++) {
@@ -137,30 +149,15 @@ __device__ __forceinline__ void cc_small_checkpoint(cc_dev* dev, const cc_region
         if (w < wid) warp_base += v;
         k += v;
     }
-    const u32 my_excl = warp_base + inc - cnt;
+    const u32 my_excl = warp_base + my_excl_in_warp;
     S->excl[tid] = my_excl;
     // the plan, identical in every block: record count, byte need, all-or-nothing log-full decision (reading #10)
-    const u64 last_page = r.n_pages - 1;
-    const bool last_dirty = (ld_relaxed_gpu_u32(&r.bitmap[last_page >> 5]) >> (last_page & 31u)) & 1u;
-    const u64 W0 = log->W;
+    const bool last_dirty = S->last_dirty != 0;
     u64 need = (u64)k * (CC_RECORD_HEADER_BYTES + (u64)r.page_bytes) + CC_COMMIT_RECORD_BYTES;
     if (last_dirty) need -= (u64)r.page_bytes - page_len_dev(r, last_page);
-    const bool fits = k != 0 && log->buf != nullptr && W0 + need <= log->capacity;
+    const bool fits = k != 0 && have_log && W0 + need <= log_cap;
     const u32 k_eff = fits ? k : 0u;
     __syncthreads();
-    // ---- D[] for cc_dirty_list (block 0; nobody inside this call reads it) ----
-    if (g.block == 0 && cnt != 0) {
-        u32 pos = my_excl;
-        for (u32 q = 0; q < wpt; q++) {
-            const u32 wi = tid * wpt + q;
-            u32 w = wi < padded_words ? ld_relaxed_gpu_u32(&r.bitmap[wi]) : 0u;
-            while (w) {
-                const u32 bit = (u32)__ffs(w) - 1u;
-                w &= w - 1;
-                r.D[pos++] = (wi << 5) + bit;
-            }
-        }
-    }
     // ---- write: (record, segment) items round-robin over the grid's warps ----
     {
         const u32 spp = r.spp;
@@ -171,6 +168,19 @@ __device__ __forceinline__ void cc_small_checkpoint(cc_dev* dev, const cc_region
             else { i = (u32)(item / spp); c = (u32)(item - (u64)i * spp); }
             const u32 p = cc_small_select(r, S, wpt, padded_words, i, lane);
             cc_gather_segment(r, dev, cs, W0, i, c, p, lane);
+        }
+    }
+    // ---- D[] for cc_dirty_list (the grid's last block: round-robin items reach it last; nobody inside this call reads D) ----
+    if (g.block == g.nblocks - 1 && cnt != 0) {
+        u32 pos = my_excl;
+        for (u32 q = 0; q < wpt; q++) {
+            const u32 wi = tid * wpt + q;
+            u32 w = wi < padded_words ? ld_relaxed_gpu_u32(&r.bitmap[wi]) : 0u;
+            while (w) {
+                const u32 bit = (u32)__ffs(w) - 1u;
+                w &= w - 1;
+                r.D[pos++] = (wi << 5) + bit;
+            }
         }
     }
     // ---- commit: every block counts out (all of them read the bitmap); the last one finishes the call ----

@@ -187,30 +187,52 @@ __global__ void __launch_bounds__(256) cc_mark_finish_kernel(const cc_dev* dev, 
 
 // parse: candidate commit records (whole log, grid-wide) -> epoch walks (one block per epoch, chained by look-back)
 // -> the one-block serial walk, which returns at once unless the parallel parse asked for it
+// Every launch of the chain carries the programmatic-serialization attribute: a kernel lets its successor be scheduled at
+// once (cc_pdl_trigger) and waits for its predecessor's results itself (cc_pdl_wait), so the launch latencies of the eight
+// short kernels overlap the kernels before them.
 __global__ void __launch_bounds__(CC_CAND_THREADS) cc_apply_cand_kernel(cc_dev* dev, cc_apply_tabs tabs, const u8* log, u64 n) {
-    cc_parse_cand_phase(dev, &dev->parse, tabs.cand, tabs.span_status, tabs.max_records, log, n, blockIdx.x == 0);
+    cc_pdl_trigger();                           // (launched normally: ordered behind whatever the stream held before)
+    cc_parse_cand_phase(dev, &dev->parse, tabs.cand_raw, tabs.max_records, log, n, cc_hw_grid());
+}
+__global__ void __launch_bounds__(CC_SORT_THREADS) cc_apply_sort_kernel(cc_dev* dev, cc_apply_tabs tabs) {
+    cc_pdl_trigger();
+    cc_pdl_wait();
+    cc_parse_sort_phase(&dev->parse, tabs.cand_raw, tabs.cand, tabs.span_status, tabs.max_records, cc_hw_grid());
 }
 __global__ void __launch_bounds__(CC_WALK_THREADS) cc_apply_walk_kernel(cc_dev* dev, cc_apply_tabs tabs, const u8* log, u64 n) {
+    cc_pdl_trigger();
+    cc_pdl_wait();
     cc_parse_walk_phase(dev, &dev->parse, tabs, log, n, blockIdx.x == 0);
 }
 __global__ void __launch_bounds__(CC_PARSE_THREADS) cc_apply_parse_kernel(cc_dev* dev, cc_apply_tabs tabs, const u8* log, u64 n) {
+    cc_pdl_trigger();
+    cc_pdl_wait();
     cc_apply_parse_phase(dev, tabs, log, n, false);
 }
 
 __global__ void __launch_bounds__(CC_APPLY_THREADS) cc_apply_validate_kernel(cc_dev* dev, cc_apply_tabs tabs, const u8* log) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    cc_apply_validate_phase(dev, tabs, reinterpret_cast<cc_crc_smem*>(smem_raw), log, cc_hw_grid(), true);
+    cc_crc_smem* cs = reinterpret_cast<cc_crc_smem*>(smem_raw);
+    cc_pdl_trigger();
+    cc_crc_smem_init(cs, &dev->crc);            // (does not depend on the parse: filled while it is still running)
+    cc_pdl_wait();
+    cc_apply_validate_phase(dev, tabs, cs, log, cc_hw_grid(), false);
 }
 
 __global__ void __launch_bounds__(CC_APPLY_THREADS) cc_apply_latest_kernel(cc_dev* dev, cc_apply_tabs tabs) {
+    cc_pdl_trigger();
+    cc_pdl_wait();
     cc_apply_latest_phase(dev, tabs, cc_hw_grid());
 }
 
 __global__ void __launch_bounds__(CC_APPLY_THREADS) cc_apply_scatter_kernel(cc_dev* dev, cc_apply_tabs tabs, const u8* log) {
+    cc_pdl_trigger();
+    cc_pdl_wait();
     cc_apply_scatter_phase(dev, tabs, log, cc_hw_grid());
 }
 
 __global__ void __launch_bounds__(CC_APPLY_THREADS) cc_apply_cleanup_kernel(cc_dev* dev, cc_apply_tabs tabs, cc_result* out) {
+    cc_pdl_wait();
     cc_apply_cleanup_phase(dev, tabs, cc_hw_grid(), out, CC_TASK_RESTORE);
 }
 
@@ -253,7 +275,7 @@ struct cc_ctx {
     uint64_t stage_bytes;
     int last_cuda;
     uint64_t launches;
-    int scan_bps, gather_bps, validate_bps, fused_bps, small_bps;     // blocks per SM from the occupancy API
+    int scan_bps, gather_bps, validate_bps, fused_bps, small_bps, cand_bps;     // blocks per SM from the occupancy API
     // ring + worker (pinned host)
     cc_task* ring_slots;
     cc_result* ring_results;
@@ -376,6 +398,7 @@ extern "C" int32_t cc_init(cc_ctx** out, int32_t device, const cc_config* cfg) {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_worker_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->scan_bps, cc_scan_kernel, CC_SCAN_THREADS, 0);
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->gather_bps, cc_gather_kernel, CC_GATHER_THREADS, sizeof(cc_crc_smem));
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->cand_bps, cc_apply_cand_kernel, CC_CAND_THREADS, 0);
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->validate_bps, cc_apply_validate_kernel, CC_APPLY_THREADS, sizeof(cc_crc_smem));
     // ring + completion slots + control words: pinned, device-mapped host memory
     if (e == cudaSuccess) e = cudaHostAlloc((void**)&ctx->ring_slots, (size_t)cap * sizeof(cc_task), cudaHostAllocMapped | cudaHostAllocPortable);
@@ -395,6 +418,7 @@ extern "C" int32_t cc_init(cc_ctx** out, int32_t device, const cc_config* cfg) {
     if (ctx->validate_bps < 1) ctx->validate_bps = 1;
     if (ctx->fused_bps < 1) ctx->fused_bps = 1;
     if (ctx->small_bps < 1) ctx->small_bps = 1;
+    if (ctx->cand_bps < 1) ctx->cand_bps = 1;
     *out = ctx;
     return CC_OK;
 }
@@ -1035,16 +1059,18 @@ extern "C" int32_t cc_checkpoint_all(cc_ctx* ctx, uint64_t epoch, void* stream, 
     return CC_OK;
 }
 
-// the three parse launches (candidates, walks, serial fallback)
+// the four parse launches (candidates, their ordering, walks, serial fallback)
 static void launch_parse(cc_ctx* ctx, const u8* lg, uint64_t nbytes, cudaStream_t st) {
-    const uint64_t ranges = ((nbytes >> 4) + (1u << 13) - 1) >> 13;                 // 128 KiB ranges (fewer, larger ones on huge logs)
-    uint64_t gc = ranges < 1 ? 1 : ranges;
-    const uint64_t capc = (uint64_t)ctx->sm_count * 8;
+    const uint64_t chunks = ((nbytes >> 4) + 255) >> 8;                              // 4 KiB per warp and step
+    uint64_t gc = (chunks + CC_CAND_THREADS / 32 - 1) / (CC_CAND_THREADS / 32);
+    const uint64_t capc = (uint64_t)ctx->sm_count * ctx->cand_bps;
     if (gc > capc) gc = capc;
+    if (gc < 1) gc = 1;
     cc_apply_cand_kernel<<<(unsigned)gc, CC_CAND_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, lg, nbytes);
-    cc_apply_walk_kernel<<<(unsigned)(ctx->sm_count * 4), CC_WALK_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, lg, nbytes);
-    cc_apply_parse_kernel<<<1, CC_PARSE_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, lg, nbytes);
-    ctx->launches += 3;
+    launch_dependent(cc_apply_sort_kernel, (unsigned)ctx->sm_count, CC_SORT_THREADS, 0, st, ctx->d_dev, ctx->tabs);
+    launch_dependent(cc_apply_walk_kernel, (unsigned)(ctx->sm_count * 4), CC_WALK_THREADS, 0, st, ctx->d_dev, ctx->tabs, lg, nbytes);
+    launch_dependent(cc_apply_parse_kernel, 1u, CC_PARSE_THREADS, 0, st, ctx->d_dev, ctx->tabs, lg, nbytes);
+    ctx->launches += 4;
 }
 
 extern "C" int32_t cc_compact_log(cc_ctx* ctx, const void* in_log, uint64_t in_bytes, void* out_log, uint64_t out_capacity,
@@ -1059,7 +1085,7 @@ extern "C" int32_t cc_compact_log(cc_ctx* ctx, const void* in_log, uint64_t in_b
     const u8* lg = stage_log(ctx, in_log, in_bytes, st);
     const unsigned gv = (unsigned)(ctx->sm_count * ctx->validate_bps);
     launch_parse(ctx, lg, in_bytes, st);
-    cc_apply_validate_kernel<<<gv, CC_APPLY_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, ctx->tabs, lg);
+    launch_dependent(cc_apply_validate_kernel, gv, CC_APPLY_THREADS, sizeof(cc_crc_smem), st, ctx->d_dev, ctx->tabs, lg);
     cc_compactor_mark_kernel<<<(unsigned)ctx->sm_count, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs);
     cc_compactor_rank_kernel<<<(unsigned)ctx->sm_count, CC_COMPACT_THREADS, 0, st>>>(ctx->d_dev);
     cc_compactor_plan_kernel<<<1, CC_MAX_REGIONS, 0, st>>>(ctx->d_dev, out_capacity);
@@ -1102,7 +1128,7 @@ extern "C" uint64_t cc_apply_scratch_bytes(uint64_t max_records) {
     if (max_records == 0 || max_records >= 0x7FFFFFF0ull) return 0;      // record numbers travel in 31 bits
     return align_up(max_records * sizeof(cc_rec), 256) + align_up((max_records + 1) * sizeof(cc_epoch_ent), 256) +
            align_up(max_records * 8, 256) + align_up((max_records + 1) * 4, 256) +
-           align_up((max_records + 1) * 4, 256) + align_up((max_records + 2) * 8, 256);
+           2 * align_up((max_records + 1) * 4, 256) + align_up((max_records + 2) * 8, 256);
 }
 
 extern "C" int32_t cc_apply_attach(cc_ctx* ctx, void* scratch, uint64_t scratch_bytes) {
@@ -1125,6 +1151,7 @@ extern "C" int32_t cc_apply_attach(cc_ctx* ctx, void* scratch, uint64_t scratch_
     T.rec_state = (u64*)p; p += align_up(m * 8, 256);
     T.seg_begin = (u32*)p; p += align_up((m + 1) * 4, 256);
     T.cand = (u32*)p; p += align_up((m + 1) * 4, 256);
+    T.cand_raw = (u32*)p; p += align_up((m + 1) * 4, 256);
     T.span_status = (u64*)p;
     ctx->tabs = T;
     ctx->apply_attached = true;
@@ -1160,10 +1187,10 @@ extern "C" int32_t cc_apply_log(cc_ctx* ctx, const void* log, uint64_t nbytes, v
     const unsigned gv = (unsigned)(ctx->sm_count * ctx->validate_bps);
     const unsigned gs = (unsigned)(ctx->sm_count * 8);
     launch_parse(ctx, lg, nbytes, st);
-    cc_apply_validate_kernel<<<gv, CC_APPLY_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, ctx->tabs, lg);
-    cc_apply_latest_kernel<<<(unsigned)ctx->sm_count, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs);
-    cc_apply_scatter_kernel<<<gs, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, lg);
-    cc_apply_cleanup_kernel<<<(unsigned)ctx->sm_count, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs, out);
+    launch_dependent(cc_apply_validate_kernel, gv, CC_APPLY_THREADS, sizeof(cc_crc_smem), st, ctx->d_dev, ctx->tabs, lg);
+    launch_dependent(cc_apply_latest_kernel, (unsigned)ctx->sm_count, CC_APPLY_THREADS, 0, st, ctx->d_dev, ctx->tabs);
+    launch_dependent(cc_apply_scatter_kernel, gs, CC_APPLY_THREADS, 0, st, ctx->d_dev, ctx->tabs, lg);
+    launch_dependent(cc_apply_cleanup_kernel, (unsigned)ctx->sm_count, CC_APPLY_THREADS, 0, st, ctx->d_dev, ctx->tabs, out);
     ctx->launches += 4;
     CC_CUDA(ctx, cudaGetLastError());
     return CC_OK;
