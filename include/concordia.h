@@ -226,11 +226,10 @@ int32_t cc_log_drain_stop(cc_ctx* ctx);
  *               [run ranking,] gather + commit), each sized for its own work.
  *               CC_PATH_SMALL: ONE kernel launch with one grid-wide rendezvous, for regions of at most 131,072 pages
  *               (CC_DISC_SCAN, one record per page; CC_ERR_INVALID otherwise): scan, then every block ranks the
- *               whole dirty bitmap by itself and the record writer follows at once -- the low-latency path of small
- *               regions (Table 6: the cost of a boundary is flat in the dirty count).
- *               CC_PATH_AUTO: CC_PATH_SMALL where it applies and the region is small enough to be latency-bound;
- *               else the single pass when the attached log is pinned host memory (the host-link transfer then overlaps
- *               the scan), and the phases otherwise (with a device log they are faster at every larger size measured).
+ *               whole dirty bitmap by itself and the record writer follows at once.  It is what the persistent worker
+ *               runs for a plain CC_TASK_DELTA_CKPT on such a region; host-launched it ties with the phases.
+ *               CC_PATH_AUTO: the phases, except with a pinned host log on regions of 128 MiB and more, where the single
+ *               pass sends the records over the host link while it scans.
  * Every path writes the same bytes.  Result, asynchrony, CC_ERR_LOG_FULL rule: as cc_checkpoint_delta below. */
 #define CC_DISC_SCAN 0u
 #define CC_DISC_MARKS 1u

@@ -16,7 +16,7 @@ typedef uint64_t u64;
 #define CC_COMPACT_WORDS_PER_THREAD 4
 #define CC_COMPACT_TILE_WORDS (CC_COMPACT_THREADS * CC_COMPACT_WORDS_PER_THREAD)   // 1024 words = 32768 pages
 #ifndef CC_FUSED_TILE_BYTES
-#define CC_FUSED_TILE_BYTES (32u * 1024u)
+#define CC_FUSED_TILE_BYTES (16u * 1024u)
 #endif    // fused pass: one WARP scans (and gathers) this much of the region per ticket
 #define CC_FUSED_MAX_TP 32u                  // ... but at most this many pages (the tile's dirty mask is one register)
 

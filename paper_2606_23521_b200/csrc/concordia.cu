@@ -37,8 +37,7 @@ static_assert(sizeof(cc_rec) == 32, "cc_rec must be 32 bytes");
 #endif
 
 #define CC_SCAN_THREADS 256
-#define CC_SMALL_AUTO_BYTES (512ull << 20)           // CC_PATH_AUTO takes the small-region path up to this size (device log)
-#define CC_SMALL_AUTO_BYTES_HOSTLOG (128ull << 20)   // ... and up to this size with a pinned host log
+#define CC_PASS_AUTO_MIN_BYTES (128ull << 20)        // CC_PATH_AUTO: single pass for pinned host logs from this region size on
 #define CC_GATHER_THREADS 256
 #define CC_APPLY_THREADS 256
 #define CC_PARSE_THREADS 1024
@@ -59,7 +58,10 @@ __global__ void __launch_bounds__(CC_COMPACT_THREADS) cc_compact_kernel(cc_dev* 
     if (blockIdx.x == 0 && threadIdx.x == 0) CC_TRACE(dev, 3);
 }
 
-__global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_gather_kernel(cc_dev* dev, int slot, cc_result* out) {
+#ifndef CC_GATHER_MIN_BLOCKS
+#define CC_GATHER_MIN_BLOCKS 4
+#endif
+__global__ void __launch_bounds__(CC_GATHER_THREADS, CC_GATHER_MIN_BLOCKS) cc_gather_kernel(cc_dev* dev, int slot, cc_result* out) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (blockIdx.x == 0 && threadIdx.x == 0) CC_TRACE(dev, 4);
     // the CRC tables do not depend on the plan: filled while the compaction is still running (programmatic dependent
@@ -210,7 +212,10 @@ __global__ void __launch_bounds__(CC_PARSE_THREADS) cc_apply_parse_kernel(cc_dev
     cc_apply_parse_phase(dev, tabs, log, n, false);
 }
 
-__global__ void __launch_bounds__(CC_APPLY_THREADS) cc_apply_validate_kernel(cc_dev* dev, cc_apply_tabs tabs, const u8* log) {
+#ifndef CC_VALIDATE_MIN_BLOCKS
+#define CC_VALIDATE_MIN_BLOCKS 4
+#endif
+__global__ void __launch_bounds__(CC_APPLY_THREADS, CC_VALIDATE_MIN_BLOCKS) cc_apply_validate_kernel(cc_dev* dev, cc_apply_tabs tabs, const u8* log) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cc_crc_smem* cs = reinterpret_cast<cc_crc_smem*>(smem_raw);
     cc_pdl_trigger();
@@ -982,22 +987,19 @@ extern "C" int32_t cc_checkpoint_ex(cc_ctx* ctx, uint32_t region_id, uint64_t ep
         if (!can_small) return CC_ERR_INVALID;
         return launch_small(ctx, slot, epoch, (cudaStream_t)stream, out);
     }
-    // AUTO, small regions: one launch, one rendezvous (64 MiB: 38 us against 55 us as three kernels).
-    // Past CC_SMALL_AUTO_BYTES the scan is long enough for the separately sized kernels (47 resident warps per SM in
-    // the scan) to win back their launch gaps; with a pinned host log the single pass takes over earlier, because it
-    // sends the records over the host link while it scans.
-    if (z.path == CC_PATH_AUTO && can_small && r.bytes <= (ctx->log_is_host ? CC_SMALL_AUTO_BYTES_HOSTLOG : CC_SMALL_AUTO_BYTES))
-        return launch_small(ctx, slot, epoch, (cudaStream_t)stream, out);
     bool pass;
     if (z.path == CC_PATH_SINGLE_PASS) {
         if (!can_pass) return CC_ERR_INVALID;
         pass = true;
     } else if (z.path == CC_PATH_PHASES) pass = false;
     else {
-        // AUTO, from measurements (profiles/r02_pass_probe.md): the single pass wins where the log
-        // crosses the host link (the transfer overlaps the scan: C2 11.7 vs 13.8 ms, C5b 111 vs 160 us per task);
-        // with a device log the separately sized kernels win at every size (64 MiB: 70 vs 90 us, 8 GiB: 2.8 vs 3.2 ms).
-        pass = can_pass && ctx->log_is_host;
+        // AUTO, from measurements (profiles/r02_small_region.md, profiles/r02_pass_probe.md): with a
+        // device log the separately sized kernels, chained by programmatic dependent launch, win or tie at every size
+        // (64 MiB: 54 us against 55 us for the one-launch small path and 62 us for the single pass; 8 GiB: 2.77 vs
+        // 3.2 ms); the single pass wins where the records cross the host link while it scans (8 GiB: 12.0 vs 13.8 ms,
+        // 256 MiB ring task: 110 vs 150 us) -- but not on regions so small that its per-tile ranking costs more than the
+        // transfer (64 MiB: 66 vs 56 us).
+        pass = can_pass && ctx->log_is_host && r.bytes >= CC_PASS_AUTO_MIN_BYTES;
     }
     return pass ? launch_pass(ctx, slot, a, (cudaStream_t)stream, out) : launch_phases(ctx, slot, a, (cudaStream_t)stream, out);
 }

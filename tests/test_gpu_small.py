@@ -136,9 +136,9 @@ def test_small_path_log_full_then_retry_and_chained_epochs():
 
 
 @pytest.mark.parametrize("name", ["c1", "c3"])
-def test_small_path_full_configs_and_auto_selects_it(name):
-    """BASELINE.json configs[0] and configs[2] at full size through CC_PATH_SMALL and through cc_checkpoint_delta (AUTO
-    takes the small path at this size: one kernel launch per call), then applied back onto the old snapshot."""
+def test_small_path_full_configs_one_launch_same_bytes_as_auto(name):
+    """BASELINE.json configs[0] and configs[2] at full size through CC_PATH_SMALL (ONE kernel launch) and through
+    cc_checkpoint_delta (AUTO: the three chained kernels): same bytes; then applied back onto the old snapshot."""
     if name == "c1":
         P = 4096
         cur = synth.raw_region(64 << 20, 1001, "cuda")
@@ -151,15 +151,23 @@ def test_small_path_full_configs_and_auto_selects_it(name):
         pages = synth.lora_update(cur, P, 0.05, 1003)
     ctx, glog, shadow, res, olog, W = _parity(cur.view(torch.uint8).view(-1), old.view(torch.uint8).view(-1), P, rid=1, epoch=7)
     assert ctx.dirty_list(1).tolist() == pages.tolist()
-    # the same through cc_checkpoint_delta: one launch, same bytes
+    # one launch for the small path ...
     ctx.log_reset()
     shadow.copy_(old.view(torch.uint8).view(-1))
     glog.zero_()
     n0 = ctx.kernel_launches()
     res.clear()
-    ctx.checkpoint_delta(1, 7, res)
+    ctx.checkpoint_ex(1, 7, res, path=cc.CC_PATH_SMALL)
     torch.cuda.synchronize()
     assert ctx.kernel_launches() - n0 == 1
+    assert res.read().n_dirty == len(pages) and np.array_equal(glog.cpu().numpy(), olog)
+    # ... and the same bytes through cc_checkpoint_delta
+    ctx.log_reset()
+    shadow.copy_(old.view(torch.uint8).view(-1))
+    glog.zero_()
+    res.clear()
+    ctx.checkpoint_delta(1, 7, res)
+    torch.cuda.synchronize()
     assert res.read().n_dirty == len(pages) and np.array_equal(glog.cpu().numpy(), olog)
     # apply onto the old snapshot
     new = cur.clone()
