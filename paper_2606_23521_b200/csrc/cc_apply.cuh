@@ -260,11 +260,93 @@ __device__ __forceinline__ u32 cc_find_rec(const u32* seg_begin, u32 n, u32 item
     return lo;
 }
 
+// CRC32C contribution of segment c of record ri; the warp that completes the record compares with the header's CRC.
+template <class SM>
+__device__ __forceinline__ void cc_apply_validate_segment(cc_dev* dev, const cc_apply_tabs& T, SM* cs, const u8* log, u32 ri,
+                                                          const cc_rec& rec, u32 c, u32 lane) {
+    constexpr int U = 8;
+    const u64 so = (u64)c * CC_SEG_BYTES;
+    const u64 rem = rec.len - so;
+    const u32 seg_len = (u32)(rem < CC_SEG_BYTES ? rem : CC_SEG_BYTES);
+    const u32 nv = seg_len >> 4;
+    const u32 nseg = (rec.len + CC_SEG_BYTES - 1) / CC_SEG_BYTES;
+    const uint4* src = reinterpret_cast<const uint4*>(log + rec.off + CC_RECORD_HEADER_BYTES + so);
+    uint4 v[U];
+#pragma unroll
+    for (int u = 0; u < U; u++) {
+        const u32 j = lane + 32 * u;
+        v[u] = (j < nv) ? ld_v4(src + j) : make_uint4(0, 0, 0, 0);
+    }
+    const u32 contrib = crc_segment_warp<U>(cs, &dev->crc, v, nv, rem - seg_len, lane);
+    if (lane == 0) {
+        u32 acc = 0;
+        const bool finish = crc_record_combine(&T.rec_state[ri], nseg, c, contrib, &acc);
+        if (finish) {
+            const u32 it = cc_crc_init_term(dev, dev->regions[rec.slot], rec.len);
+            if (crc_finalize(acc, it) != rec.crc) atomicMin(&dev->apply.first_bad_rec, ri);
+        }
+    }
+}
+
+// Segment c of record ri into the live page and the shadow -- if the record is the page's LATEST one.  A segment lies
+// inside one page when pages are whole multiples of 4 KiB (or the record is a single page); otherwise the check is per
+// 16-byte vector.
+__device__ __forceinline__ void cc_apply_scatter_segment(cc_dev* dev, const u8* log, u32 ri, const cc_rec& rec, u32 c, u32 lane) {
+    constexpr int U = 8;
+    const cc_region_dev& r = dev->regions[rec.slot];
+    const u64 so = (u64)c * CC_SEG_BYTES;
+    const u64 rem = rec.len - so;
+    const u32 nv = (u32)(rem < CC_SEG_BYTES ? rem : CC_SEG_BYTES) >> 4;
+    const bool one_page = (r.page_bytes % CC_SEG_BYTES == 0) || rec.len <= r.page_bytes;
+    if (one_page && r.latest[rec.page_idx + (u32)(so / r.page_bytes)] != ri + 1) return;
+    const uint4* src = reinterpret_cast<const uint4*>(log + rec.off + CC_RECORD_HEADER_BYTES + so);
+    const u64 dst_off = (u64)rec.page_idx * r.page_bytes + so;
+    uint4* d0 = reinterpret_cast<uint4*>(r.base + dst_off);
+    uint4* d1 = reinterpret_cast<uint4*>(r.shadow + dst_off);
+    uint4 v[U];
+    bool take[U];
+#pragma unroll
+    for (int u = 0; u < U; u++) {
+        const u32 j = lane + 32 * u;
+        take[u] = j < nv;
+        if (take[u] && !one_page) take[u] = r.latest[rec.page_idx + (u32)((so + 16ull * j) / r.page_bytes)] == ri + 1;
+        if (take[u]) v[u] = ld_v4(src + j);
+    }
+#pragma unroll
+    for (int u = 0; u < U; u++) {
+        const u32 j = lane + 32 * u;
+        if (take[u]) { st_stream(d0 + j, v[u]); if (r.shadow) st_stream(d1 + j, v[u]); }
+    }
+}
+
 #define CC_APPLY_CHUNK 4u       // consecutive 4 KiB segments one warp takes per search of the record table
 
-__device__ __forceinline__ void cc_apply_validate_phase(cc_dev* dev, const cc_apply_tabs& T, cc_crc_smem* cs,
+// One thread, once every CRC verdict is in: the committed prefix = the epochs whose records all precede the first failed
+// check; status; and the parallel parse re-armed for the next log.
+__device__ __forceinline__ void cc_apply_resolve(cc_dev* dev, const cc_apply_tabs& T) {
+    cc_apply_state* A = &dev->apply;
+    const u32 f = A->first_bad_rec;           // 0xFFFFFFFF if every CRC matched
+    const u32 ne = A->n_epochs;
+    u32 lo = 0, hi = ne;                      // epochs are ordered by rec_end: count those with rec_end <= f
+    while (lo < hi) {
+        const u32 mid = (lo + hi) >> 1;
+        if (T.epochs[mid].rec_end <= f) lo = mid + 1; else hi = mid;
+    }
+    int32_t st = CC_OK;
+    if (f != 0xFFFFFFFFu || A->struct_fail) st = CC_ERR_CORRUPT;
+    u32 E = lo;
+    if (A->scratch_overflow) { st = CC_ERR_SCRATCH; E = 0; }
+    A->n_commit_epochs = E;
+    A->n_commit_recs = E ? T.epochs[E - 1].rec_end : 0;
+    A->consumed = E ? T.epochs[E - 1].off_after : 0;
+    A->status = st;
+    dev->parse.cand_overflow = 0;             // re-arm the parallel parse for the next log
+    dev->parse.need_serial = 0;
+}
+
+template <class SM>
+__device__ __forceinline__ void cc_apply_validate_phase(cc_dev* dev, const cc_apply_tabs& T, SM* cs,
                                                         const u8* log, cc_grid g, bool init_tables) {
-    constexpr int U = 8;
     cc_apply_state* A = &dev->apply;
     const u32 n_recs = A->n_recs;
     const u32 lane = threadIdx.x & 31u;
@@ -283,28 +365,7 @@ __device__ __forceinline__ void cc_apply_validate_phase(cc_dev* dev, const cc_ap
             u32 sb = T.seg_begin[ri], next = T.seg_begin[ri + 1];
             for (u32 item = item0; item < item1; item++) {
                 while (item >= next) { ri++; rec = T.recs[ri]; sb = next; next = T.seg_begin[ri + 1]; }
-                const u32 c = item - sb;
-                const u64 so = (u64)c * CC_SEG_BYTES;
-                const u64 rem = rec.len - so;
-                const u32 seg_len = (u32)(rem < CC_SEG_BYTES ? rem : CC_SEG_BYTES);
-                const u32 nv = seg_len >> 4;
-                const u32 nseg = (rec.len + CC_SEG_BYTES - 1) / CC_SEG_BYTES;
-                const uint4* src = reinterpret_cast<const uint4*>(log + rec.off + CC_RECORD_HEADER_BYTES + so);
-                uint4 v[U];
-#pragma unroll
-                for (int u = 0; u < U; u++) {
-                    const u32 j = lane + 32 * u;
-                    v[u] = (j < nv) ? ld_v4(src + j) : make_uint4(0, 0, 0, 0);
-                }
-                const u32 contrib = crc_segment_warp<U>(cs, &dev->crc, v, nv, rem - seg_len, lane);
-                if (lane == 0) {
-                    u32 acc = 0;
-                    const bool finish = crc_record_combine(&T.rec_state[ri], nseg, c, contrib, &acc);
-                    if (finish) {
-                        const u32 it = cc_crc_init_term(dev, dev->regions[rec.slot], rec.len);
-                        if (crc_finalize(acc, it) != rec.crc) atomicMin(&A->first_bad_rec, ri);
-                    }
-                }
+                cc_apply_validate_segment(dev, T, cs, log, ri, rec, item - sb, lane);
             }
         }
     }
@@ -316,24 +377,8 @@ __device__ __forceinline__ void cc_apply_validate_phase(cc_dev* dev, const cc_ap
     __syncthreads();
     if (s_last && threadIdx.x == 0) {
         __threadfence();
-        const u32 f = A->first_bad_rec;           // 0xFFFFFFFF if every CRC matched
-        const u32 ne = A->n_epochs;
-        u32 lo = 0, hi = ne;                      // epochs are ordered by rec_end: count those with rec_end <= f
-        while (lo < hi) {
-            const u32 mid = (lo + hi) >> 1;
-            if (T.epochs[mid].rec_end <= f) lo = mid + 1; else hi = mid;
-        }
-        int32_t st = CC_OK;
-        if (f != 0xFFFFFFFFu || A->struct_fail) st = CC_ERR_CORRUPT;
-        u32 E = lo;
-        if (A->scratch_overflow) { st = CC_ERR_SCRATCH; E = 0; }
-        A->n_commit_epochs = E;
-        A->n_commit_recs = E ? T.epochs[E - 1].rec_end : 0;
-        A->consumed = E ? T.epochs[E - 1].off_after : 0;
-        A->status = st;
+        cc_apply_resolve(dev, T);
         A->validate_done = 0;
-        dev->parse.cand_overflow = 0;             // re-arm the parallel parse for the next log
-        dev->parse.need_serial = 0;
         __threadfence();
     }
 }
@@ -349,7 +394,6 @@ __device__ __forceinline__ void cc_apply_latest_phase(cc_dev* dev, const cc_appl
 }
 
 __device__ __forceinline__ void cc_apply_scatter_phase(cc_dev* dev, const cc_apply_tabs& T, const u8* log, cc_grid g) {
-    constexpr int U = 8;
     const u32 n = dev->apply.n_commit_recs;
     if (n == 0) return;
     const u32 lane = threadIdx.x & 31u;
@@ -363,33 +407,7 @@ __device__ __forceinline__ void cc_apply_scatter_phase(cc_dev* dev, const cc_app
         u32 sb = T.seg_begin[ri], next = T.seg_begin[ri + 1];
         for (u32 item = item0; item < item1; item++) {
             while (item >= next) { ri++; rec = T.recs[ri]; sb = next; next = T.seg_begin[ri + 1]; }
-            const cc_region_dev& r = dev->regions[rec.slot];
-            const u32 c = item - sb;
-            const u64 so = (u64)c * CC_SEG_BYTES;
-            const u64 rem = rec.len - so;
-            const u32 nv = (u32)(rem < CC_SEG_BYTES ? rem : CC_SEG_BYTES) >> 4;
-            // a page takes its bytes from its LATEST record only.  A segment lies inside one page when pages are
-            // whole multiples of 4 KiB (or the record is a single page); otherwise the check is per 16-byte vector.
-            const bool one_page = (r.page_bytes % CC_SEG_BYTES == 0) || rec.len <= r.page_bytes;
-            if (one_page && r.latest[rec.page_idx + (u32)(so / r.page_bytes)] != ri + 1) continue;
-            const uint4* src = reinterpret_cast<const uint4*>(log + rec.off + CC_RECORD_HEADER_BYTES + so);
-            const u64 dst_off = (u64)rec.page_idx * r.page_bytes + so;
-            uint4* d0 = reinterpret_cast<uint4*>(r.base + dst_off);
-            uint4* d1 = reinterpret_cast<uint4*>(r.shadow + dst_off);
-            uint4 v[U];
-            bool take[U];
-#pragma unroll
-            for (int u = 0; u < U; u++) {
-                const u32 j = lane + 32 * u;
-                take[u] = j < nv;
-                if (take[u] && !one_page) take[u] = r.latest[rec.page_idx + (u32)((so + 16ull * j) / r.page_bytes)] == ri + 1;
-                if (take[u]) v[u] = ld_v4(src + j);
-            }
-#pragma unroll
-            for (int u = 0; u < U; u++) {
-                const u32 j = lane + 32 * u;
-                if (take[u]) { st_stream(d0 + j, v[u]); if (r.shadow) st_stream(d1 + j, v[u]); }
-            }
+            cc_apply_scatter_segment(dev, log, ri, rec, item - sb, lane);
         }
     }
 }

@@ -147,6 +147,7 @@ struct cc_parse_ctl {                    // control block of the parallel parse 
 
 struct alignas(16) cc_crc_tables {
     u32 t0[256];            // byte table of the reflected polynomial
+    u32 t0k[3][256];        // t0k[k-1]: the same for a byte followed by k zero bytes (slicing-by-4, cc_crc_smem4)
     alignas(16) u32 s512[4][256];       // multiply by x^(8*512) mod G, one table per register byte
     u32 lane_mul[32];       // x^(8*16*(31-lane))
     u32 seg_mul[CC_SEG_POW_MAX + 1];   // x^(8*4096*m), m = 0..CC_SEG_POW_MAX
@@ -222,9 +223,10 @@ __device__ __forceinline__ void st_stream(uint4* p, const uint4& v) {
 // Programmatic dependent launch (sm_90+): a kernel launched with the programmatic-stream-serialization attribute may
 // start while its predecessor in the stream is still running; it must execute cc_pdl_wait() before it touches anything
 // the predecessor writes (no-op when launched normally).  cc_pdl_trigger() in the predecessor lets the dependent grid
-// be scheduled as soon as SM resources free up.  -DCC_PDL=0 builds without it (A/B).
+// be scheduled as soon as SM resources free up.  OFF by default (-DCC_PDL=1 builds with it): measured with the calls
+// queued ahead of the GPU, plain stream order is faster (C5a replay 0.382 vs 0.400 ms, C1 checkpoint 51.9 vs 53.9 us).
 #ifndef CC_PDL
-#define CC_PDL 1
+#define CC_PDL 0
 #endif
 __device__ __forceinline__ void cc_pdl_wait() {
 #if CC_PDL

@@ -46,6 +46,11 @@ static inline void cc_crc_build_tables(cc_crc_tables* t) {
         for (int b = 0; b < 8; b++) c = gf_mulx(c);
         t->t0[i] = c;
     }
+    for (int k = 1; k < 4; k++)                   // t0k[k-1][b]: byte b followed by k zero bytes (slicing-by-4)
+        for (u32 i = 0; i < 256; i++) {
+            const u32 prev = k == 1 ? t->t0[i] : t->t0k[k - 2][i];
+            t->t0k[k - 1][i] = (prev >> 8) ^ t->t0[prev & 0xFFu];
+        }
     u32 x8 = 0x80000000u;
     for (int b = 0; b < 8; b++) x8 = gf_mulx(x8);
     t->xp[0] = x8;
@@ -106,7 +111,8 @@ __device__ __forceinline__ u32 crc_step_z(const char* t0, u32 lane4, u32 z) {
 }
 
 // raw register (init 0) over one 16-byte vector, memory order; returns the UNrotated register
-__device__ __forceinline__ u32 crc_vec16(const char* t0, u32 lane4, const uint4& v) {
+__device__ __forceinline__ u32 crc_vec16(const cc_crc_smem* s, u32 lane4, const uint4& v) {
+    const char* t0 = reinterpret_cast<const char*>(s->t0);
     const u32 w[4] = {v.x, v.y, v.z, v.w};
     u32 z = 0;
 #pragma unroll
@@ -118,13 +124,61 @@ __device__ __forceinline__ u32 crc_vec16(const char* t0, u32 lane4, const uint4&
     return rotr32(z, 7);
 }
 
+// ---- slicing-by-4 variant (the applier's validation, which is bound by instruction issue) ----
+// Four byte tables T3..T0 (byte followed by 3..0 zero bytes), each replicated per lane, laid out so that ONE byte-permute
+// forms a lookup address: entry b of slice q sits at byte offset (q >> 1) * 65536 + b * 256 + (q & 1) * 128 + lane * 4 --
+// PRMT(z, laneoff) puts byte k of the register into address bits 8..15 above the lane offset, no shift, no mask.
+// A 32-bit step is 4 PRMT + 4 LDS + 2 LOP3 = 2.5 instructions per byte against 4.5 for the single table; 128 KiB of
+// shared memory, so one 1,024-thread block per SM.
+struct alignas(16) cc_crc_smem4 {
+    u32 t[2 * 256 * 64];                    // 128 KiB
+    alignas(16) u32 lane_nib[8 * 16 * 32];
+    alignas(16) u32 s512[4 * 256];
+};
+
+__device__ __forceinline__ void cc_crc_smem_init(cc_crc_smem4* s, const cc_crc_tables* g) {
+    const u32 lane = threadIdx.x & 31u, w = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    // slice q uses table T(3-q): the FIRST message byte of a word is followed by three more
+    for (u32 job = w; job < 4u * 8u; job += nw) {             // 4 slices x 8 groups of 32 entries
+        const u32 q = job >> 3, e0 = (job & 7u) * 32u;
+        const u32* src = q == 3 ? g->t0 : g->t0k[2 - q];
+        const u32 mine = src[e0 + lane];
+        u32* base = s->t + (q >> 1) * (256u * 64u) + (q & 1u) * 32u;
+#pragma unroll
+        for (u32 e = 0; e < 32u; e++) base[(e0 + e) * 64u + lane] = __shfl_sync(0xFFFFFFFFu, mine, e);
+    }
+    const uint4* nib = reinterpret_cast<const uint4*>(g->lane_nib);
+    uint4* dn = reinterpret_cast<uint4*>(s->lane_nib);
+    for (u32 i = threadIdx.x; i < 8 * 16 * 32 / 4; i += blockDim.x) dn[i] = nib[i];
+    const uint4* s5 = reinterpret_cast<const uint4*>(&g->s512[0][0]);
+    uint4* d5 = reinterpret_cast<uint4*>(s->s512);
+    for (u32 i = threadIdx.x; i < 4 * 256 / 4; i += blockDim.x) d5[i] = s5[i];
+    __syncthreads();
+}
+
+// one 32-bit step: the register after feeding the four bytes of z (already XORed with the message word)
+__device__ __forceinline__ u32 crc_step32(const char* t, u32 lo, u32 hi, u32 z) {
+    const u32 a0 = __byte_perm(z, lo, 0x5504), a1 = __byte_perm(z, hi, 0x5514);
+    const u32 a2 = __byte_perm(z, lo, 0x5524), a3 = __byte_perm(z, hi, 0x5534);
+    return *reinterpret_cast<const u32*>(t + a0) ^ *reinterpret_cast<const u32*>(t + a1) ^
+           *reinterpret_cast<const u32*>(t + 65536 + a2) ^ *reinterpret_cast<const u32*>(t + 65536 + a3);
+}
+__device__ __forceinline__ u32 crc_vec16(const cc_crc_smem4* s, u32 lane4, const uint4& v) {
+    const char* t = reinterpret_cast<const char*>(s->t);
+    const u32 lo = lane4, hi = lane4 + 128u;
+    u32 z = crc_step32(t, lo, hi, v.x);
+    z = crc_step32(t, lo, hi, z ^ v.y);
+    z = crc_step32(t, lo, hi, z ^ v.z);
+    return crc_step32(t, lo, hi, z ^ v.w);
+}
+
 __device__ __forceinline__ u32 crc_shift512(const u32* s512, u32 v) {
     return s512[v & 0xFFu] ^ s512[256 + ((v >> 8) & 0xFFu)] ^ s512[512 + ((v >> 16) & 0xFFu)] ^ s512[768 + (v >> 24)];
 }
 
 // acc * lane_mul[lane] through the lane-replicated nibble tables (conflict-free, 8 lookups)
-__device__ __forceinline__ u32 crc_lane_mul(const cc_crc_smem* s, u32 lane4, u32 acc) {
-    const char* nb = reinterpret_cast<const char*>(s->lane_nib);
+__device__ __forceinline__ u32 crc_lane_mul(const u32* lane_nib, u32 lane4, u32 acc) {
+    const char* nb = reinterpret_cast<const char*>(lane_nib);
     u32 r = 0;
 #pragma unroll
     for (int n = 0; n < 8; n++) {
@@ -137,25 +191,25 @@ __device__ __forceinline__ u32 crc_lane_mul(const cc_crc_smem* s, u32 lane4, u32
 // Warp-level raw CRC contribution of one segment of nv (<= 256) 16-byte vectors held as
 // v[u] = vector (lane + 32u); `after` = bytes of the message that follow this segment.
 // Returns (in every lane) raw(segment, 0) * x^(8*after).
-template <int U>
-__device__ __forceinline__ u32 crc_segment_warp(const cc_crc_smem* s, const cc_crc_tables* g, const uint4 (&v)[U],
+// SM: the shared-memory table set (cc_crc_smem: one byte table, 4 instructions per byte; cc_crc_smem4: slicing-by-4).
+template <int U, class SM>
+__device__ __forceinline__ u32 crc_segment_warp(const SM* s, const cc_crc_tables* g, const uint4 (&v)[U],
                                                 u32 nv, u64 after, u32 lane) {
-    const char* t0 = reinterpret_cast<const char*>(s->t0);
     const u32 lane4 = lane << 2;
     u32 acc = 0;
     if (nv == 32u * U) {
         u32 part[U];
 #pragma unroll
-        for (int u = 0; u < U; u++) part[u] = crc_vec16(t0, lane4, v[u]);     // U independent chains
+        for (int u = 0; u < U; u++) part[u] = crc_vec16(s, lane4, v[u]);      // U independent chains
 #pragma unroll
         for (int u = 0; u < U; u++) acc = (u ? crc_shift512(s->s512, acc) : 0u) ^ part[u];
-        acc = crc_lane_mul(s, lane4, acc);
+        acc = crc_lane_mul(s->lane_nib, lane4, acc);
     } else {
         int last = -1;
 #pragma unroll
         for (int u = 0; u < U; u++) {
             if (lane + 32u * u < nv) {
-                acc = crc_shift512(s->s512, acc) ^ crc_vec16(t0, lane4, v[u]);
+                acc = crc_shift512(s->s512, acc) ^ crc_vec16(s, lane4, v[u]);
                 last = u;
             }
         }

@@ -189,9 +189,9 @@ __global__ void __launch_bounds__(256) cc_mark_finish_kernel(const cc_dev* dev, 
 
 // parse: candidate commit records (whole log, grid-wide) -> epoch walks (one block per epoch, chained by look-back)
 // -> the one-block serial walk, which returns at once unless the parallel parse asked for it
-// Every launch of the chain carries the programmatic-serialization attribute: a kernel lets its successor be scheduled at
-// once (cc_pdl_trigger) and waits for its predecessor's results itself (cc_pdl_wait), so the launch latencies of the eight
-// short kernels overlap the kernels before them.
+// (In a -DCC_PDL=1 build every launch of the chain carries the programmatic-serialization attribute: a kernel lets its
+// successor be scheduled at once, cc_pdl_trigger, and waits for its predecessor's results itself, cc_pdl_wait.  Off by
+// default: measured slower than plain stream order, see cc_common.cuh.)
 __global__ void __launch_bounds__(CC_CAND_THREADS) cc_apply_cand_kernel(cc_dev* dev, cc_apply_tabs tabs, const u8* log, u64 n) {
     cc_pdl_trigger();                           // (launched normally: ordered behind whatever the stream held before)
     cc_parse_cand_phase(dev, &dev->parse, tabs.cand_raw, tabs.max_records, log, n, cc_hw_grid());
@@ -212,14 +212,14 @@ __global__ void __launch_bounds__(CC_PARSE_THREADS) cc_apply_parse_kernel(cc_dev
     cc_apply_parse_phase(dev, tabs, log, n, false);
 }
 
-#ifndef CC_VALIDATE_MIN_BLOCKS
-#define CC_VALIDATE_MIN_BLOCKS 4
-#endif
-__global__ void __launch_bounds__(CC_APPLY_THREADS, CC_VALIDATE_MIN_BLOCKS) cc_apply_validate_kernel(cc_dev* dev, cc_apply_tabs tabs, const u8* log) {
+// The validation is bound by instruction issue: it runs the slicing-by-4 CRC (cc_crc_smem4: 128 KiB of lane-replicated
+// tables, 2.5 instead of 4.5 instructions per payload byte and lane) as ONE block of 1,024 threads per SM.
+#define CC_VALIDATE_THREADS 1024
+__global__ void __launch_bounds__(CC_VALIDATE_THREADS, 1) cc_apply_validate_kernel(cc_dev* dev, cc_apply_tabs tabs, const u8* log) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    cc_crc_smem* cs = reinterpret_cast<cc_crc_smem*>(smem_raw);
+    cc_crc_smem4* cs = reinterpret_cast<cc_crc_smem4*>(smem_raw);
     cc_pdl_trigger();
-    cc_crc_smem_init(cs, &dev->crc);            // (does not depend on the parse: filled while it is still running)
+    cc_crc_smem_init(cs, &dev->crc);            // (does not depend on the parse)
     cc_pdl_wait();
     cc_apply_validate_phase(dev, tabs, cs, log, cc_hw_grid(), false);
 }
@@ -399,12 +399,12 @@ extern "C" int32_t cc_init(cc_ctx** out, int32_t device, const cc_config* cfg) {
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->fused_bps, cc_pass_kernel, CC_GATHER_THREADS, sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->small_bps, cc_small_kernel, CC_GATHER_THREADS, sizeof(cc_crc_smem));
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_apply_validate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_apply_validate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem4));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_worker_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->scan_bps, cc_scan_kernel, CC_SCAN_THREADS, 0);
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->gather_bps, cc_gather_kernel, CC_GATHER_THREADS, sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->cand_bps, cc_apply_cand_kernel, CC_CAND_THREADS, 0);
-    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->validate_bps, cc_apply_validate_kernel, CC_APPLY_THREADS, sizeof(cc_crc_smem));
+    if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->validate_bps, cc_apply_validate_kernel, CC_VALIDATE_THREADS, sizeof(cc_crc_smem4));
     // ring + completion slots + control words: pinned, device-mapped host memory
     if (e == cudaSuccess) e = cudaHostAlloc((void**)&ctx->ring_slots, (size_t)cap * sizeof(cc_task), cudaHostAllocMapped | cudaHostAllocPortable);
     if (e == cudaSuccess) e = cudaHostAlloc((void**)&ctx->ring_results, (size_t)cap * sizeof(cc_result), cudaHostAllocMapped | cudaHostAllocPortable);
@@ -1087,7 +1087,7 @@ extern "C" int32_t cc_compact_log(cc_ctx* ctx, const void* in_log, uint64_t in_b
     const u8* lg = stage_log(ctx, in_log, in_bytes, st);
     const unsigned gv = (unsigned)(ctx->sm_count * ctx->validate_bps);
     launch_parse(ctx, lg, in_bytes, st);
-    launch_dependent(cc_apply_validate_kernel, gv, CC_APPLY_THREADS, sizeof(cc_crc_smem), st, ctx->d_dev, ctx->tabs, lg);
+    launch_dependent(cc_apply_validate_kernel, gv, CC_VALIDATE_THREADS, sizeof(cc_crc_smem4), st, ctx->d_dev, ctx->tabs, lg);
     cc_compactor_mark_kernel<<<(unsigned)ctx->sm_count, CC_APPLY_THREADS, 0, st>>>(ctx->d_dev, ctx->tabs);
     cc_compactor_rank_kernel<<<(unsigned)ctx->sm_count, CC_COMPACT_THREADS, 0, st>>>(ctx->d_dev);
     cc_compactor_plan_kernel<<<1, CC_MAX_REGIONS, 0, st>>>(ctx->d_dev, out_capacity);
@@ -1189,7 +1189,7 @@ extern "C" int32_t cc_apply_log(cc_ctx* ctx, const void* log, uint64_t nbytes, v
     const unsigned gv = (unsigned)(ctx->sm_count * ctx->validate_bps);
     const unsigned gs = (unsigned)(ctx->sm_count * 8);
     launch_parse(ctx, lg, nbytes, st);
-    launch_dependent(cc_apply_validate_kernel, gv, CC_APPLY_THREADS, sizeof(cc_crc_smem), st, ctx->d_dev, ctx->tabs, lg);
+    launch_dependent(cc_apply_validate_kernel, gv, CC_VALIDATE_THREADS, sizeof(cc_crc_smem4), st, ctx->d_dev, ctx->tabs, lg);
     launch_dependent(cc_apply_latest_kernel, (unsigned)ctx->sm_count, CC_APPLY_THREADS, 0, st, ctx->d_dev, ctx->tabs);
     launch_dependent(cc_apply_scatter_kernel, gs, CC_APPLY_THREADS, 0, st, ctx->d_dev, ctx->tabs, lg);
     launch_dependent(cc_apply_cleanup_kernel, (unsigned)ctx->sm_count, CC_APPLY_THREADS, 0, st, ctx->d_dev, ctx->tabs, out);

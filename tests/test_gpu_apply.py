@@ -210,3 +210,38 @@ def test_long_single_epoch_many_parse_steps():
     r = _gpu_apply(ctx, torch.from_numpy(olog).cuda(), nb)
     assert (r.status, r.n_dirty, r.bytes) == (0, n_pages, nb)
     assert torch.equal(reg, cur)
+
+
+@pytest.mark.parametrize("bad_epoch", [0, 1, 2, 3, 4])
+def test_failed_check_falls_back_to_the_latest_committed_record(bad_epoch):
+    """Five epochs rewrite overlapping pages; one payload bit of epoch `bad_epoch` is flipped.  Pages whose LATEST record
+    lies in or behind the damaged epoch must end up with their latest COMMITTED record (or untouched) -- the case in which
+    the applier's side-by-side validation + scatter has to rebuild its last-wins table over the committed prefix.  The same
+    context then applies the undamaged log (the tables must have been left clean)."""
+    P, n_pages = 4096, 64
+    N = P * n_pages
+    rng = np.random.default_rng(17)
+    old = rng.integers(0, 256, N, dtype=np.uint8)
+    cur, sh = old.copy(), old.copy()
+    log = np.zeros(1 << 20, dtype=np.uint8)
+    W, ends = 0, []
+    for e in range(5):
+        for p in sorted(set(rng.integers(0, n_pages, 12).tolist()) | {5, 6 + e}):     # page 5 in every epoch
+            cur[p * P + int(rng.integers(0, P))] ^= 0x3C
+        st, D, nb, W = oracle.checkpoint(cur, sh, P, 3, 200 + e, log, W)
+        assert st == 0
+        ends.append(W)
+    good = log.copy()
+    start = ends[bad_epoch - 1] if bad_epoch else 0
+    log[start + 16 + 100] ^= 0x04                      # first record's payload of the damaged epoch
+    ctx, reg, sh_t, r = _compare(old, log, W, P)
+    assert r.status == cc.CC_ERR_CORRUPT and r.epoch == bad_epoch
+    # the same context, the undamaged log, from scratch
+    reg.copy_(torch.from_numpy(old).cuda())
+    sh_t.copy_(torch.from_numpy(old).cuda())
+    r2 = _gpu_apply(ctx, torch.from_numpy(good).cuda(), W)
+    reg_o, sh_o = old.copy(), old.copy()
+    exp = oracle.apply_log(good, W, [oracle.Region(3, P, reg_o, sh_o)])
+    assert (r2.status, r2.n_dirty, r2.bytes) == exp and r2.status == 0 and r2.epoch == 5
+    assert np.array_equal(reg.cpu().numpy(), reg_o) and np.array_equal(sh_t.cpu().numpy(), sh_o)
+    assert np.array_equal(reg_o, cur)
