@@ -349,3 +349,41 @@ def test_library_side_drainer_thread_follows_commits_and_resets():
         ctx.worker_stop()
     ctx.log_drain_stop()
     ctx.shutdown()
+
+
+@pytest.mark.parametrize("path", ["phases", "single", "small"])
+def test_host_sees_every_record_byte_once_the_committed_offset_moves(path):
+    """PAPER.md:L263 "a commit marker publishes the epoch only after all bytes are visible": records go straight into a
+    PINNED HOST log; the host never synchronises with the stream -- it polls the committed-offset word and, the moment it
+    moves, replays the newly committed bytes with the oracle's applier (every record's CRC32C is checked there) onto its own
+    copy of the region.  The record bytes are written by hundreds of blocks; only the last one executes a system-scope fence
+    (the others release at gpu scope), so this is the test of that fence chain."""
+    P, n_pages, per_step, steps = 4096, 4096, 384, 40
+    N = P * n_pages
+    cur = _region(N, 77)
+    host = cur.cpu().numpy().copy()                     # what the host has recovered so far
+    ctx = cc.Context()
+    ctx.register_region(1, cur, P)
+    cap = steps * (per_step * (16 + P) + 32) + 4096
+    hlog = torch.zeros(cap, dtype=torch.uint8, pin_memory=True)
+    committed = torch.zeros(1, dtype=torch.int64, pin_memory=True)
+    ctx.log_attach(hlog, committed)
+    log_np, com_np = hlog.numpy(), committed.numpy()
+    kw = {"phases": cc.CC_PATH_PHASES, "single": cc.CC_PATH_SINGLE_PASS, "small": cc.CC_PATH_SMALL}[path]
+    rng = np.random.default_rng(9)
+    import time
+    W = 0
+    for it in range(steps):
+        pages = torch.from_numpy(rng.choice(n_pages, per_step, replace=False)).cuda()
+        offs = pages * P + torch.from_numpy(rng.integers(0, P, per_step)).cuda()
+        cur[offs] ^= 0x5A
+        ctx.checkpoint_ex(1, it, None, path=kw)         # no result, no synchronize
+        need = per_step * (16 + P) + 32
+        t0 = time.time()
+        while int(com_np[0]) < W + need:
+            assert time.time() - t0 < 20, "committed offset never moved"
+        st, nrec, consumed = oracle.apply_log(log_np[W:W + need], need, [oracle.Region(1, P, host)])
+        assert (st, nrec, consumed) == (0, per_step, need), (it, st, nrec, consumed)
+        W += need
+    torch.cuda.synchronize()
+    assert np.array_equal(host, cur.cpu().numpy())
