@@ -255,23 +255,35 @@ __device__ __forceinline__ void cc_parse_walk_phase(cc_dev* dev, cc_parse_ctl* C
         const u64 target = has_target ? ((u64)T.cand[j] << 4) : 0ull;
         cc_walk_span<false>(T, log, n, &S, start, target, has_target, j, 0, 0);
         const u32 oc = S.outcome, nrec = S.nrec, nseg = S.nseg;
-        // ---- chain: records / segments of all earlier spans; dead if an earlier span stopped the parse ----
-        if (tid == 0) {
-            u32 br = 0, bs = 0, dead = 0;
-            if (j != 0) {
+        // ---- chain: records / segments of all earlier spans; dead if an earlier span stopped the parse.  Warp-wide
+        //      look-back: 32 predecessors per step (one thread walking back word by word made span 99 wait through up to
+        //      99 dependent loads) ----
+        if (tid < 32) {
+            const u32 lane = tid;
+            if (j != 0 && lane == 0)
                 st_release_gpu_u64(&T.span_status[j], sp_pack(oc == CC_WO_COMMIT ? CC_SP_AGG : CC_SP_STOP, nrec, nseg));
-                int q = (int)j - 1;
-                while (q >= 0) {
-                    const u64 s = ld_acquire_gpu_u64(&T.span_status[q]);
-                    const u32 f = sp_flag(s);
-                    if (f == 0) { __nanosleep(20); continue; }
-                    if (f == CC_SP_STOP) { dead = 1; break; }
-                    br += sp_recs(s); bs += sp_segs(s);
-                    if (f == CC_SP_INC) break;
-                    q--;
-                }
+            u32 br = 0, bs = 0, dead = 0;
+            int base = (int)j - 1;
+            while (base >= 0) {
+                const int q = base - (int)lane;
+                u64 s = sp_pack(CC_SP_INC, 0, 0);                 // virtual span -1: inclusive (0, 0)
+                if (q >= 0) s = ld_acquire_gpu_u64(&T.span_status[q]);
+                const u32 f = sp_flag(s);
+                const u32 nr = __ballot_sync(0xFFFFFFFFu, f == 0);
+                const u32 term = __ballot_sync(0xFFFFFFFFu, f == CC_SP_INC || f == CC_SP_STOP);
+                const u32 first_nr = nr ? (u32)__ffs(nr) - 1u : 32u;
+                const u32 first_t = term ? (u32)__ffs(term) - 1u : 32u;
+                if (first_nr < first_t) { __nanosleep(20); continue; }     // a nearer predecessor has not published yet
+                const u32 upto = first_t < 32u ? first_t : 31u;
+                const bool in = lane <= upto;
+                const u32 tf = __shfl_sync(0xFFFFFFFFu, f, upto);
+                if (first_t < 32u && tf == CC_SP_STOP) { dead = 1; break; }
+                br += __reduce_add_sync(0xFFFFFFFFu, in ? sp_recs(s) : 0u);
+                bs += __reduce_add_sync(0xFFFFFFFFu, in ? sp_segs(s) : 0u);
+                if (first_t < 32u) break;                         // reached an inclusive word
+                base -= 32;
             }
-            S.base_recs = br; S.base_segs = bs; S.dead = dead;
+            if (lane == 0) { S.base_recs = br; S.base_segs = bs; S.dead = dead; }
         }
         __syncthreads();
         if (S.dead) {                                             // something before this span ended the parse
