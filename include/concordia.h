@@ -110,7 +110,8 @@ typedef struct {
 
 /* Completion / result record, exactly 64 bytes.  Written by the GPU. */
 typedef struct {
-    uint64_t seq_done;         /* worker path: task seq + 1, release-stored LAST; host-launched path: 1 */
+    uint64_t seq_done;         /* worker path: task seq + 1; host-launched path: 1.  Stored LAST, at system scope, behind a
+                                  system-scope fence that covers every other field and every log byte of the call */
     uint64_t n_dirty;          /* checkpoint: k;  apply: page records applied (duplicates counted) */
     uint64_t bytes;            /* checkpoint: bytes appended;  apply: bytes consumed (end of last applied commit) */
     uint64_t log_offset_after; /* checkpoint: log write offset W after the call;  apply: same as bytes */
@@ -170,7 +171,10 @@ int32_t cc_unregister_region(cc_ctx* ctx, uint32_t region_id);
 
 /* Attach the append-only log: log_buf (device or pinned host, 16-byte aligned), capacity bytes.
  * committed_off (pinned host or device, 8 bytes, may be NULL) receives the committed write
- * offset with a system-scope release store after every commit record.  W := 0.
+ * offset after every commit record: a system-scope store behind ONE system-scope fence that, by cumulativity, covers
+ * every record byte the call wrote, whichever block wrote it ("a commit marker publishes the epoch
+ * only after all bytes are visible").  A host thread that reads the word with acquire semantics may read the log up to
+ * that offset without synchronising with the stream.  W := 0.
  * Only while the worker is stopped. */
 int32_t cc_log_attach(cc_ctx* ctx, void* log_buf, uint64_t capacity, uint64_t* committed_off);
 /* W := 0 and *committed_off := 0 (synchronous; only while the worker is stopped -- use CC_TASK_LOG_RESET otherwise). */

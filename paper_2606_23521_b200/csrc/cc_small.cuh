@@ -28,7 +28,7 @@
 struct cc_small_smem {
     u32 excl[CC_SMALL_MAX_THREADS];         // records before thread t's words
     u32 warp_tot[CC_SMALL_MAX_THREADS / 32];
-    u32 k, last_dirty, is_last;
+    u32 last_dirty, is_last;
 };
 
 __host__ __device__ __forceinline__ bool cc_small_supported(u64 n_words) { return n_words <= CC_SMALL_MAX_WORDS; }
