@@ -183,8 +183,10 @@ struct cc_dev {
 #endif
 #if CC_TRACE_ON
 #define CC_TRACE(dev, i) do { (dev)->trace[i] = globaltimer_ns(); } while (0)
+#define CC_TRACE_MAX(dev, i, lane) do { if ((lane) == 0) atomicMax(reinterpret_cast<unsigned long long*>(&(dev)->trace[i]), (unsigned long long)globaltimer_ns()); } while (0)
 #else
 #define CC_TRACE(dev, i) do { } while (0)
+#define CC_TRACE_MAX(dev, i, lane) do { } while (0)
 #endif
 
 // ------------------------------------------------------------------ PTX helpers --

@@ -229,6 +229,7 @@ __device__ __forceinline__ bool cc_pass_tiles(const cc_region_dev& r, cc_dev* de
         }
         // ---- a2: rank of this tile's dirty pages (and records) among all ----
         const u32 cnt = __popc(mask);
+        CC_TRACE_MAX(dev, cnt ? 20 : 23, lane);
         const u32 starts = rle ? (mask & (~(mask << 1) | cut)) : mask;
         const u32 nrec = __popc(starts);
         const bool last = (t == nt - 1);
@@ -273,6 +274,7 @@ __device__ __forceinline__ bool cc_pass_tiles(const cc_region_dev& r, cc_dev* de
             if ((mask >> lane) & 1u) a.committed[p0 + lane] = a.version[p0 + lane];
         } else if (a.consume && lane == 0) cc_pass_clear_marks(r, a, p0, np, last);
         if (cnt == 0) continue;
+        CC_TRACE_MAX(dev, 21, lane);
         // ---- a3 + a5: this warp writes its own records (one read -> log payload, shadow, CRC) ----
         cc_crc_smem_lazy(cs, &dev->crc, s_crc_state, lane);
         wrote = true;
@@ -339,6 +341,7 @@ __device__ __forceinline__ bool cc_pass_tiles(const cc_region_dev& r, cc_dev* de
             rank += npg;
             m &= ~(((npg == 32 ? 0u : (1u << npg)) - 1u) << s);
         }
+        CC_TRACE_MAX(dev, 22, lane);
     }
     return wrote;
 }

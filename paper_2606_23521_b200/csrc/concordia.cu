@@ -64,12 +64,18 @@ __global__ void __launch_bounds__(CC_COMPACT_THREADS) cc_compact_kernel(cc_dev* 
 __global__ void __launch_bounds__(CC_GATHER_THREADS, CC_GATHER_MIN_BLOCKS) cc_gather_kernel(cc_dev* dev, int slot, cc_result* out) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (blockIdx.x == 0 && threadIdx.x == 0) CC_TRACE(dev, 4);
+    cc_crc_smem* cs = reinterpret_cast<cc_crc_smem*>(smem_raw);
+#if CC_PDL
     // the CRC tables do not depend on the plan: filled while the compaction is still running (programmatic dependent
     // launch), then wait for the plan
-    cc_crc_smem* cs = reinterpret_cast<cc_crc_smem*>(smem_raw);
     cc_crc_smem_init(cs, &dev->crc);
     cc_pdl_wait();
     cc_gather_phase(dev->regions[slot], dev, cs, cc_hw_grid(), out, CC_TASK_DELTA_CKPT, false);
+#else
+    // plain stream order: only the blocks that have records to write fill the tables (a sparse checkpoint keeps 20 of
+    // 592 blocks busy; the other 572 fetching 52 KiB each out of L2 delayed those 20)
+    cc_gather_phase(dev->regions[slot], dev, cs, cc_hw_grid(), out, CC_TASK_DELTA_CKPT, true);
+#endif
 }
 
 // The whole checkpoint of one region in ONE launch (cc_pass.cuh).  Cooperative: when the worst case does not fit
