@@ -317,6 +317,14 @@ int32_t cc_checkpoint_versions(cc_ctx* ctx, uint32_t region_id, uint64_t epoch, 
  * no part.  ASYNCHRONOUS on `stream`. */
 int32_t cc_checkpoint_all(cc_ctx* ctx, uint64_t epoch, void* stream, cc_result* out);
 
+/* The same boundary with RUN-LENGTH records (reading #38): the bytes of calling
+ * cc_checkpoint_delta_rle(region, epoch, run_pages) region by region in ascending region_id order.  One launch per
+ * region (the single pass for run_pages <= 32, the phases above that) plus one that sums up the result; the committed
+ * offset moves region by region, always to the end of a whole epoch.  Skipping rule, result and the regions that
+ * take part: as cc_checkpoint_all.  run_pages >= 1 and run_pages * page_bytes < 2^32 for every region taking part
+ * (CC_ERR_INVALID otherwise, nothing launched). */
+int32_t cc_checkpoint_all_rle(cc_ctx* ctx, uint64_t epoch, uint32_t run_pages, void* stream, cc_result* out);
+
 /* Base snapshot ("The initial base snapshot captured all 8,192 pages of the full region";
  * L257: immutable regions "are included in the base snapshot but do not keep GPU shadows"): append EVERY
  * page of the region, ascending, as one committed epoch in the same record format -- no discovery pass.

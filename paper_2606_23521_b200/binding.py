@@ -53,7 +53,7 @@ EXPORTS = [
     "cc_init", "cc_shutdown", "cc_last_cuda_error", "cc_kernel_launches", "cc_workspace_bytes",
     "cc_register_region", "cc_unregister_region", "cc_log_attach", "cc_log_reset", "cc_log_reset_async", "cc_log_mirror_attach", "cc_log_drain", "cc_log_drain_start", "cc_log_drain_wait", "cc_log_drain_stop",
     "cc_checkpoint_ex", "cc_checkpoint_delta", "cc_checkpoint_delta_fused", "cc_checkpoint_delta_rle", "cc_checkpoint_marked", "cc_checkpoint_versions",
-    "cc_checkpoint_all", "cc_snapshot_region", "cc_compact_log", "cc_scan_only", "cc_trace_events", "cc_dirty_list", "cc_apply_scratch_bytes", "cc_apply_attach", "cc_apply_stage_attach", "cc_apply_log",
+    "cc_checkpoint_all", "cc_checkpoint_all_rle", "cc_snapshot_region", "cc_compact_log", "cc_scan_only", "cc_trace_events", "cc_dirty_list", "cc_apply_scratch_bytes", "cc_apply_attach", "cc_apply_stage_attach", "cc_apply_log",
     "cc_worker_start", "cc_worker_stop", "cc_worker_alive", "cc_worker_footprint", "cc_peek_queue", "cc_submit", "cc_measure_submit_cost", "cc_measure_launch_cost", "cc_poll", "cc_wait",
 ]
 
@@ -133,6 +133,7 @@ def load_library():
         "cc_checkpoint_marked": (i32, [vp, u32, u64, vp, u32, vp, vp]),
         "cc_checkpoint_versions": (i32, [vp, u32, u64, vp, vp, vp, vp]),
         "cc_checkpoint_all": (i32, [vp, u64, vp, vp]),
+        "cc_checkpoint_all_rle": (i32, [vp, u64, u32, vp, vp]),
         "cc_snapshot_region": (i32, [vp, u32, u64, vp, vp]),
         "cc_compact_log": (i32, [vp, vp, u64, vp, u64, vp, vp]),
         "cc_scan_only": (i32, [vp, u32, vp, vp]),
@@ -336,6 +337,10 @@ class Context:
     def checkpoint_all(self, epoch: int, result: Result = None, stream=None):
         self._check("cc_checkpoint_all", self.lib.cc_checkpoint_all(
             self.h, epoch, _stream_ptr(stream), ctypes.c_void_p(result.ptr) if result else None))
+
+    def checkpoint_all_rle(self, epoch: int, run_pages: int, result: Result = None, stream=None):
+        self._check("cc_checkpoint_all_rle", self.lib.cc_checkpoint_all_rle(
+            self.h, epoch, run_pages, _stream_ptr(stream), ctypes.c_void_p(result.ptr) if result else None))
 
     def snapshot_region(self, region_id: int, epoch: int, result: Result = None, stream=None):
         self._check("cc_snapshot_region", self.lib.cc_snapshot_region(

@@ -177,6 +177,30 @@ __global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_batch_gather_kernel(c
     cc_batch_gather_phase(dev, cs, &tab, cc_hw_grid(), out, CC_TASK_CKPT_ALL);
 }
 
+// cc_checkpoint_all_rle: the per-region calls have run (stream order); one thread sums their plans up into the result
+struct cc_slot_list { int n; int slot[CC_MAX_REGIONS]; };
+__global__ void cc_batch_collect_kernel(cc_dev* dev, cc_slot_list L, u64 epoch, u64 t_start_ns, cc_result* out) {
+    if (!out) return;
+    u64 k = 0, bytes = 0;
+    int32_t st = CC_OK;
+    for (int i = 0; i < L.n; i++) {                    // ascending region_id
+        const cc_ws_hdr* h = dev->regions[L.slot[i]].hdr;
+        k += h->k;
+        bytes += h->need;
+        if (st == CC_OK && h->status != CC_OK) st = h->status;
+    }
+    out->n_dirty = k;
+    out->bytes = bytes;
+    out->log_offset_after = dev->log.W;
+    out->epoch = epoch;
+    out->status = st;
+    out->flags = CC_TASK_CKPT_ALL;
+    out->t_start_ns = L.n ? dev->regions[L.slot[0]].hdr->t_start_ns : t_start_ns;
+    out->t_end_ns = globaltimer_ns();
+    __threadfence_system();
+    st_relaxed_sys_u64(&out->seq_done, 1ull);
+}
+
 // allocator-aware discovery (cc_mark.cuh)
 __global__ void __launch_bounds__(256) cc_mark_load_kernel(const cc_dev* dev, int slot, const u32* marks) {
     cc_mark_load_phase(dev->regions[slot], marks, cc_hw_grid());
@@ -1063,6 +1087,39 @@ extern "C" int32_t cc_checkpoint_all(cc_ctx* ctx, uint64_t epoch, void* stream, 
     if (ctx->ev_after_compact) cudaEventRecord(ctx->ev_after_compact, st);
     cc_batch_gather_kernel<<<(unsigned)(ctx->sm_count * ctx->gather_bps), CC_GATHER_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, out);
     ctx->launches += 4;
+    CC_CUDA(ctx, cudaGetLastError());
+    return CC_OK;
+}
+
+extern "C" int32_t cc_checkpoint_all_rle(cc_ctx* ctx, uint64_t epoch, uint32_t run_pages, void* stream, cc_result* out) {
+    if (!ctx || run_pages == 0) return CC_ERR_INVALID;
+    CC_NO_WORKER(ctx);
+    // the regions that take part, in ascending region_id order
+    cc_slot_list L;
+    L.n = 0;
+    for (int s = 0; s < CC_MAX_REGIONS; s++) {
+        if (!ctx->regions[s].used || !ctx->regions[s].dev.shadow) continue;
+        if ((uint64_t)run_pages * ctx->regions[s].dev.page_bytes > 0xFFFFFFFFull) return CC_ERR_INVALID;
+        int i = L.n++;
+        while (i > 0 && ctx->regions[L.slot[i - 1]].dev.region_id > ctx->regions[s].dev.region_id) { L.slot[i] = L.slot[i - 1]; i--; }
+        L.slot[i] = s;
+    }
+    CC_CUDA(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    cc_pass_args a;
+    memset(&a, 0, sizeof(a));
+    a.epoch = epoch;
+    a.disc = CC_DISC_SCAN;
+    a.run_pages = run_pages;
+    a.kind = CC_TASK_DELTA_CKPT;
+    for (int i = 0; i < L.n; i++) {
+        const cc_region_dev& r = ctx->regions[L.slot[i]].dev;
+        const int32_t rc = cc_pass_supported(r.n_pages, run_pages) ? launch_pass(ctx, L.slot[i], a, st, nullptr)
+                                                                   : launch_phases(ctx, L.slot[i], a, st, nullptr);
+        if (rc != CC_OK) return rc;
+    }
+    cc_batch_collect_kernel<<<1, 1, 0, st>>>(ctx->d_dev, L, epoch, 0ull, out);
+    ctx->launches += 1;
     CC_CUDA(ctx, cudaGetLastError());
     return CC_OK;
 }

@@ -146,3 +146,105 @@ def test_worker_ckpt_all_task_and_no_regions():
     r = res.read()
     assert (r.seq_done, r.status, r.n_dirty, r.bytes) == (1, 0, 0, 0)
     ctx.shutdown()
+
+
+def _oracle_all_rle(regs, epoch, run_pages, olog, W):
+    """reading #37 + #38: the regions that have a shadow, ascending region_id, each as oracle.checkpoint_rle; a region that
+    does not fit is skipped whole, the ones after it are still tried; status = the first failure's."""
+    st_all, k_tot, b_tot = 0, 0, 0
+    for rg in sorted((r for r in regs if r.shadow is not None), key=lambda r: r.region_id):
+        st, D, _runs, nb, W2 = oracle.checkpoint_rle(rg.base, rg.shadow, rg.page_bytes, rg.region_id, epoch, run_pages, olog, W)
+        k_tot += D.size
+        if st == 0:
+            b_tot += nb
+            W = W2
+        elif st_all == 0:
+            st_all = st
+    return st_all, k_tot, b_tot, W
+
+
+def _mutate_runs(regs, tensors, rng, skip=()):
+    """runs of 1..9 consecutive dirty pages (so that run-length records have something to join)"""
+    for r in regs:
+        if r.region_id in skip:
+            continue
+        N, P = r.base.size, r.page_bytes
+        n_pages = (N + P - 1) // P
+        cur = tensors[r.region_id][0]
+        pages = {n_pages - 1}
+        for s in rng.integers(0, n_pages, max(1, n_pages // 40)).tolist():
+            pages |= set(range(s, min(n_pages, s + int(rng.integers(1, 10)))))
+        for p in pages:
+            off = p * P + int(rng.integers(0, min(P, N - p * P)))
+            r.base[off] ^= 0x31
+            cur[off] ^= 0x31
+
+
+@pytest.mark.parametrize("run_pages", [1, 4, 32, 64])
+def test_checkpoint_all_rle_equals_the_oracle_sequence(run_pages):
+    """cc_checkpoint_all_rle: run-length records at a multi-region boundary (run_pages <= 32: the single pass per region,
+    64: the phases), incl. boundaries where some or all regions are clean; the log replays through the applier."""
+    cap = 64 << 20
+    ctx, regs, tensors, log, committed, rng = _setup(11 + run_pages, cap)
+    start = {rid: t[0].clone() for rid, t in tensors.items()}
+    olog = np.zeros(cap, np.uint8)
+    W = 0
+    res = cc.Result()
+    for epoch in range(4):
+        if epoch == 2:
+            _mutate_runs(regs, tensors, rng, skip=(2, 9, 30))
+        elif epoch < 3:
+            _mutate_runs(regs, tensors, rng)
+        st, kt, bt, W = _oracle_all_rle(regs, 70 + epoch, run_pages, olog, W)
+        res.clear()
+        ctx.checkpoint_all_rle(70 + epoch, run_pages, res)
+        torch.cuda.synchronize()
+        r = res.read()
+        assert (r.status, r.n_dirty, r.bytes, r.log_offset_after, r.epoch, r.seq_done) == (st, kt, bt, W, 70 + epoch, 1), r.as_dict()
+        assert int(committed.item()) == W
+    assert np.array_equal(log.cpu().numpy(), olog)
+    for rg in regs:
+        if rg.shadow is not None:
+            assert np.array_equal(tensors[rg.region_id][1].cpu().numpy(), rg.shadow)
+    # replay onto the starting state
+    final = {rid: t[0].clone() for rid, t in tensors.items()}
+    for rid, (cur, sh) in tensors.items():
+        if sh is not None:
+            cur.copy_(start[rid])
+            sh.copy_(start[rid])
+    ctx.apply_attach(50000)
+    res.clear()
+    ctx.apply_log(log, W, res)
+    torch.cuda.synchronize()
+    assert res.read().status == 0
+    for rid, (cur, sh) in tensors.items():
+        if sh is not None:
+            assert torch.equal(cur, final[rid]) and torch.equal(sh, final[rid])
+
+
+def test_checkpoint_all_rle_skips_a_region_that_does_not_fit_and_checks_arguments():
+    """A middle region whose records do not fit is skipped whole (shadow untouched), the later ones are still logged;
+    status = that region's; a retry after a reset logs exactly the skipped region."""
+    ctx, regs, tensors, log, committed, rng = _setup(23, 5 << 19)
+    _mutate_runs(regs, tensors, rng)
+    # make region 9 (64 KiB pages) too big for what is left: dirty every page
+    big = next(r for r in regs if r.region_id == 9)
+    big.base[::4096] ^= 0x01
+    tensors[9][0][::4096] ^= 0x01
+    cap = log.numel()
+    olog = np.zeros(cap, np.uint8)
+    st, kt, bt, W = _oracle_all_rle(regs, 5, 8, olog, 0)
+    assert st == cc.CC_ERR_LOG_FULL and W > 0
+    res = cc.Result()
+    ctx.checkpoint_all_rle(5, 8, res)
+    torch.cuda.synchronize()
+    r = res.read()
+    assert (r.status, r.n_dirty, r.bytes, r.log_offset_after) == (st, kt, bt, W), r.as_dict()
+    assert np.array_equal(log.cpu().numpy(), olog)
+    assert np.array_equal(tensors[9][1].cpu().numpy(), big.shadow)             # untouched
+    with pytest.raises(cc.ConcordiaError) as e:
+        ctx.checkpoint_all_rle(6, 0, res)
+    assert e.value.code == cc.CC_ERR_INVALID
+    with pytest.raises(cc.ConcordiaError) as e:
+        ctx.checkpoint_all_rle(6, 1 << 20, res)                                 # run_pages * 81920 >= 2^32
+    assert e.value.code == cc.CC_ERR_INVALID
