@@ -37,14 +37,14 @@ def _two_epoch_setup(P=64, n_pages=12, tail=32):
     return old, log, nb1, nb2, P
 
 
-def _compare(old, log_np, nbytes, P, region_id=3, pinned=False):
+def _compare(old, log_np, nbytes, P, region_id=3, pinned=False, max_records=1024):
     """Apply log_np[:nbytes] to `old` on both sides and compare everything."""
     reg_o, sh_o = old.copy(), old.copy()
     exp = oracle.apply_log(log_np, nbytes, [oracle.Region(region_id, P, reg_o, sh_o)])
     ctx = cc.Context()
     reg = torch.from_numpy(old.copy()).cuda()
     sh = ctx.register_region(region_id, reg, P)
-    ctx.apply_attach(1024)
+    ctx.apply_attach(max_records)
     lt = torch.from_numpy(log_np.copy())
     lt = lt.pin_memory() if pinned else lt.cuda()
     r = _gpu_apply(ctx, lt, nbytes)
@@ -245,3 +245,63 @@ def test_failed_check_falls_back_to_the_latest_committed_record(bad_epoch):
     assert (r2.status, r2.n_dirty, r2.bytes) == exp and r2.status == 0 and r2.epoch == 5
     assert np.array_equal(reg.cpu().numpy(), reg_o) and np.array_equal(sh_t.cpu().numpy(), sh_o)
     assert np.array_equal(reg_o, cur)
+
+
+def _commit_image(epoch, region_id, k):
+    """the 32 bytes of a VALID commit record (signature, length 16, CRC32C of its payload)"""
+    pay = struct.pack("<QII", epoch, region_id, k)
+    return struct.pack("<IIII", 0xFFFFFFFF, 0xFFFFFFFF, 16, oracle.crc32c(np.frombuffer(pay, np.uint8))) + pay
+
+
+@pytest.mark.parametrize("n_false,max_records", [(1, 1024), (7, 1024), (300, 64)])
+def test_payloads_that_contain_valid_commit_record_images(n_false, max_records):
+    """The parallel parse finds commit records by signature + CRC; a page whose BYTES contain a valid commit record puts a
+    false candidate on its list.  The epoch walks must notice (they run past the false one) and hand the log to the serial
+    parser: same result as the sequential definition.  (300 false candidates with tables for 64 records: the candidate list
+    overflows, which must end the same way.)"""
+    P, n_pages = 4096, 48
+    N = P * n_pages
+    rng = np.random.default_rng(n_false)
+    old = rng.integers(0, 256, N, dtype=np.uint8)
+    cur, sh = old.copy(), old.copy()
+    log = np.zeros(1 << 20, dtype=np.uint8)
+    W, placed = 0, 0
+    for e in range(6):
+        pages = sorted(set(rng.integers(0, n_pages, 5).tolist()))
+        for p in pages:
+            cur[p * P + int(rng.integers(0, P))] ^= 0x42
+            per_page = min(n_false - placed, 60) if e % 2 == 0 else 0
+            for q in range(per_page):                     # images at 16-byte-aligned offsets of the page
+                off = p * P + 64 * q + 16 * (q % 2)
+                img = np.frombuffer(_commit_image(int(rng.integers(0, 1 << 40)), int(rng.integers(1, 9)), int(rng.integers(0, 9))), np.uint8)
+                cur[off:off + 32] = img
+            placed += per_page
+        st, D, nb, W = oracle.checkpoint(cur, sh, P, 3, 300 + e, log, W)
+        assert st == 0
+    assert placed == n_false
+    ctx, reg, sh_t, r = _compare(old, log, W, P, max_records=max_records)
+    assert r.status == 0 and r.epoch == 6
+    # a torn tail behind the false candidates, and a damaged real commit record
+    _compare(old, log, W - 40, P, max_records=max_records)
+    bad = log.copy()
+    bad[W - 4] ^= 0x80                                     # k of the last commit record
+    _compare(old, bad, W, P, max_records=max_records)
+
+
+def test_thousands_of_one_record_epochs():
+    """3,000 epochs of one or two 64-byte-page records: 3,000 candidates ranked over several tiles, 3,000 epoch walks
+    chained by look-back."""
+    P, n_pages, E = 64, 512, 3000
+    N = P * n_pages
+    rng = np.random.default_rng(12)
+    old = rng.integers(0, 256, N, dtype=np.uint8)
+    cur, sh = old.copy(), old.copy()
+    log = np.zeros(E * (2 * (16 + P) + 32) + 64, dtype=np.uint8)
+    W = 0
+    for e in range(E):
+        for p in rng.integers(0, n_pages, 1 + e % 2).tolist():
+            cur[p * P + int(rng.integers(0, P))] ^= 0x01
+        st, D, nb, W = oracle.checkpoint(cur, sh, P, 3, e, log, W)
+    ctx, reg, sh_t, r = _compare(old, log, W, P, max_records=8192)
+    assert r.status == 0 and r.epoch >= E - 600 and np.array_equal(reg.cpu().numpy(), cur)
+    _compare(old, log, W // 2 + 8, P, max_records=8192)    # torn in the middle
