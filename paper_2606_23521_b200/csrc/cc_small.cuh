@@ -84,40 +84,20 @@ __device__ __forceinline__ u32 cc_small_select(const cc_region_dev& r, const cc_
     return page;
 }
 
-// All blocks of a co-resident grid.  gen: the caller's grid-barrier generation (cc_tasks.cuh), advanced by one.
-// cs: shared-memory CRC tables, filled here while the block waits for the others if init_tables.
-__device__ __forceinline__ void cc_small_checkpoint(cc_dev* dev, const cc_region_dev& r, cc_crc_smem* cs, cc_small_smem* S, u64 epoch,
-                                                    u32 kind, cc_grid g, u32& gen, cc_result* out, bool init_tables) {
+// Everything behind the scan: rank, write, commit.  All blocks of the grid call it once the bitmap is complete (behind the
+// rendezvous of cc_small_checkpoint, or as a kernel of its own behind cc_scan_kernel: cc_small_tail_kernel).
+// tables_ready: cs already holds the CRC tables; otherwise a block fills them once it knows that it has records to write.
+__device__ __forceinline__ void cc_small_tail(cc_dev* dev, const cc_region_dev& r, cc_crc_smem* cs, cc_small_smem* S, u64 epoch,
+                                              u32 kind, cc_grid g, cc_result* out, bool tables_ready) {
     const u32 tid = threadIdx.x, lane = tid & 31u, wid = tid >> 5;
     cc_ws_hdr* h = r.hdr;
     cc_log_dev* log = &dev->log;
-    // ---- scan ----
-    if (g.block == 0 && tid == 0) { h->t_start_ns = globaltimer_ns(); CC_TRACE(dev, 10); }
-    cc_scan_items<8>(r, g.warp(), g.nwarps());
-    // ---- meet: arrive, fill the tables, wait ----
-    __syncthreads();
-    if (tid == 0) {
-        __threadfence();
-        if (atomicAdd(&dev->bar_count, 1u) == g.nblocks - 1) {
-            atomicExch(&dev->bar_count, 0u);
-            __threadfence();
-            atomicAdd(&dev->bar_gen, 1u);
-        }
-    }
-    if (init_tables) cc_crc_smem_init(cs, &dev->crc);
-    // what the plan needs from the log does not depend on the scan: loaded while the block waits
     const u64 W0 = log->W;
     const u64 log_cap = log->capacity;
     const bool have_log = log->buf != nullptr;
     const u64 last_page = r.n_pages - 1;
-    if (tid == 0) {
-        S->last_dirty = 0;
-        while (ld_acquire_gpu_u32(&dev->bar_gen) == gen) __nanosleep(32);
-        __threadfence();
-    }
-    gen++;
+    if (tid == 0) S->last_dirty = 0;
     __syncthreads();
-    if (g.block == 0 && tid == 0) CC_TRACE(dev, 11);
     // ---- rank: every block, the whole bitmap ----
     const u32 wpt = cc_small_wpt(r);
     const u32 padded_words = (u32)((r.n_words + CC_COMPACT_TILE_WORDS - 1) / CC_COMPACT_TILE_WORDS * CC_COMPACT_TILE_WORDS);
@@ -162,6 +142,7 @@ __device__ __forceinline__ void cc_small_checkpoint(cc_dev* dev, const cc_region
     {
         const u32 spp = r.spp;
         const u64 n_items = (u64)k_eff * spp;
+        if (!tables_ready && (u64)g.block * (blockDim.x >> 5) < n_items) cc_crc_smem_init(cs, &dev->crc);   // (block-uniform)
         for (u64 item = g.warp(); item < n_items; item += g.nwarps()) {
             u32 i, c;
             if (r.spp_shift >= 0) { i = (u32)(item >> r.spp_shift); c = (u32)(item & (spp - 1)); }
@@ -218,4 +199,32 @@ __device__ __forceinline__ void cc_small_checkpoint(cc_dev* dev, const cc_region
         if (out) st_relaxed_sys_u64(&out->seq_done, 1ull);
         CC_TRACE(dev, 13);
     }
+}
+
+// One launch: scan, ONE grid-wide rendezvous (all blocks co-resident: cooperative launch / the resident worker; a block
+// fills its CRC tables while it waits), then cc_small_tail.  gen: the caller's grid-barrier generation (cc_tasks.cuh),
+// advanced by one.
+__device__ __forceinline__ void cc_small_checkpoint(cc_dev* dev, const cc_region_dev& r, cc_crc_smem* cs, cc_small_smem* S, u64 epoch,
+                                                    u32 kind, cc_grid g, u32& gen, cc_result* out, bool init_tables) {
+    const u32 tid = threadIdx.x;
+    if (g.block == 0 && tid == 0) { r.hdr->t_start_ns = globaltimer_ns(); CC_TRACE(dev, 10); }
+    cc_scan_items<8>(r, g.warp(), g.nwarps());
+    __syncthreads();
+    if (tid == 0) {
+        __threadfence();
+        if (atomicAdd(&dev->bar_count, 1u) == g.nblocks - 1) {
+            atomicExch(&dev->bar_count, 0u);
+            __threadfence();
+            atomicAdd(&dev->bar_gen, 1u);
+        }
+    }
+    if (init_tables) cc_crc_smem_init(cs, &dev->crc);
+    if (tid == 0) {
+        while (ld_acquire_gpu_u32(&dev->bar_gen) == gen) __nanosleep(32);
+        __threadfence();
+    }
+    gen++;
+    __syncthreads();
+    if (g.block == 0 && tid == 0) CC_TRACE(dev, 11);
+    cc_small_tail(dev, r, cs, S, epoch, kind, g, out, true);
 }

@@ -37,31 +37,32 @@ static_assert(sizeof(cc_rec) == 32, "cc_rec must be 32 bytes");
 #endif
 
 #define CC_SCAN_THREADS 256
+#define CC_SMALL_TAIL_MAX_BYTES (1ull << 30)         // phases path: up to this region size the compaction kernel is replaced by in-block ranking
 #define CC_PASS_AUTO_MIN_BYTES (128ull << 20)        // CC_PATH_AUTO: single pass for pinned host logs from this region size on
 #define CC_GATHER_THREADS 256
 #define CC_APPLY_THREADS 256
 #define CC_PARSE_THREADS 1024
 
-__global__ void __launch_bounds__(CC_SCAN_THREADS) cc_scan_kernel(cc_dev* dev, int slot) {
+__global__ void __launch_bounds__(CC_SCAN_THREADS) cc_scan_kernel(cc_dev* dev, const __grid_constant__ cc_region_dev rg) {
     cc_pdl_trigger();                       // the compaction (and behind it the gather) may queue up behind this grid
     if (blockIdx.x == 0 && threadIdx.x == 0) CC_TRACE(dev, 0);
-    cc_scan_phase<8>(dev->regions[slot], cc_hw_grid());
+    cc_scan_phase<8>(rg, cc_hw_grid());
     if (blockIdx.x == 0 && threadIdx.x == 0) CC_TRACE(dev, 1);
 }
 
-__global__ void __launch_bounds__(CC_COMPACT_THREADS) cc_compact_kernel(cc_dev* dev, int slot, u32 mode, u64 epoch,
+__global__ void __launch_bounds__(CC_COMPACT_THREADS) cc_compact_kernel(cc_dev* dev, const __grid_constant__ cc_region_dev rg, u32 mode, u64 epoch,
                                                                         cc_result* out) {
     cc_pdl_trigger();
     cc_pdl_wait();                          // the bitmap is complete
     if (blockIdx.x == 0 && threadIdx.x == 0) CC_TRACE(dev, 2);
-    cc_compact_phase(dev->regions[slot], &dev->log, mode, epoch, out);
+    cc_compact_phase(rg, &dev->log, mode, epoch, out);
     if (blockIdx.x == 0 && threadIdx.x == 0) CC_TRACE(dev, 3);
 }
 
 #ifndef CC_GATHER_MIN_BLOCKS
 #define CC_GATHER_MIN_BLOCKS 4
 #endif
-__global__ void __launch_bounds__(CC_GATHER_THREADS, CC_GATHER_MIN_BLOCKS) cc_gather_kernel(cc_dev* dev, int slot, cc_result* out) {
+__global__ void __launch_bounds__(CC_GATHER_THREADS, CC_GATHER_MIN_BLOCKS) cc_gather_kernel(cc_dev* dev, const __grid_constant__ cc_region_dev rg, cc_result* out) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (blockIdx.x == 0 && threadIdx.x == 0) CC_TRACE(dev, 4);
     cc_crc_smem* cs = reinterpret_cast<cc_crc_smem*>(smem_raw);
@@ -70,22 +71,22 @@ __global__ void __launch_bounds__(CC_GATHER_THREADS, CC_GATHER_MIN_BLOCKS) cc_ga
     // launch), then wait for the plan
     cc_crc_smem_init(cs, &dev->crc);
     cc_pdl_wait();
-    cc_gather_phase(dev->regions[slot], dev, cs, cc_hw_grid(), out, CC_TASK_DELTA_CKPT, false);
+    cc_gather_phase(rg, dev, cs, cc_hw_grid(), out, CC_TASK_DELTA_CKPT, false);
 #else
     // plain stream order: only the blocks that have records to write fill the tables (a sparse checkpoint keeps 20 of
     // 592 blocks busy; the other 572 fetching 52 KiB each out of L2 delayed those 20)
-    cc_gather_phase(dev->regions[slot], dev, cs, cc_hw_grid(), out, CC_TASK_DELTA_CKPT, true);
+    cc_gather_phase(rg, dev, cs, cc_hw_grid(), out, CC_TASK_DELTA_CKPT, true);
 #endif
 }
 
 // The whole checkpoint of one region in ONE launch (cc_pass.cuh).  Cooperative: when the worst case does not fit
 // behind the write offset the classic phases run instead, separated by grid barriers.
-__global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_pass_kernel(cc_dev* dev, int slot, cc_pass_args a, cc_result* out) {
+__global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_pass_kernel(cc_dev* dev, const __grid_constant__ cc_region_dev rg, cc_pass_args a, cc_result* out) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cc_crc_smem* cs = reinterpret_cast<cc_crc_smem*>(smem_raw);
     __shared__ u32 s_crc_state, s_warps_left;
     __shared__ cc_pass_smem s_pass;
-    const cc_region_dev& r = dev->regions[slot];
+    const cc_region_dev& r = rg;
     const cc_grid g = cc_hw_grid();
     if (threadIdx.x == 0) { s_crc_state = 0; s_warps_left = blockDim.x >> 5; }
     if (g.block == 0 && threadIdx.x == 0) { r.hdr->t_start_ns = globaltimer_ns(); CC_TRACE(dev, 10); }
@@ -116,16 +117,26 @@ __global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_pass_kernel(cc_dev* d
 }
 
 // The low-latency checkpoint of a small region in ONE launch (cc_small.cuh).  Cooperative: one grid-wide rendezvous.
-__global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_small_kernel(cc_dev* dev, int slot, u64 epoch, cc_result* out) {
+__global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_small_kernel(cc_dev* dev, const __grid_constant__ cc_region_dev rg, u64 epoch, cc_result* out) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ cc_small_smem s_small;
     u32 gen = ld_acquire_gpu_u32(&dev->bar_gen);
-    cc_small_checkpoint(dev, dev->regions[slot], reinterpret_cast<cc_crc_smem*>(smem_raw), &s_small, epoch, CC_TASK_DELTA_CKPT,
+    cc_small_checkpoint(dev, rg, reinterpret_cast<cc_crc_smem*>(smem_raw), &s_small, epoch, CC_TASK_DELTA_CKPT,
                         cc_hw_grid(), gen, out, true);
 }
 
-__global__ void __launch_bounds__(256) cc_snapshot_plan_kernel(const cc_dev* dev, int slot, u64 epoch) {
-    cc_snapshot_plan_phase(dev->regions[slot], &dev->log, epoch, cc_hw_grid());
+// The same path as TWO launches for host-launched calls: cc_scan_kernel at its own occupancy (47 resident warps per SM),
+// then rank + write + commit -- no compaction kernel, no dirty list to wait for (a plain launch: no block waits on another).
+__global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_small_tail_kernel(cc_dev* dev, const __grid_constant__ cc_region_dev rg, u64 epoch,
+                                                                            cc_result* out) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ cc_small_smem s_small;
+    if (blockIdx.x == 0 && threadIdx.x == 0) CC_TRACE(dev, 11);
+    cc_small_tail(dev, rg, reinterpret_cast<cc_crc_smem*>(smem_raw), &s_small, epoch, CC_TASK_DELTA_CKPT, cc_hw_grid(), out, false);
+}
+
+__global__ void __launch_bounds__(256) cc_snapshot_plan_kernel(const cc_dev* dev, const __grid_constant__ cc_region_dev rg, u64 epoch) {
+    cc_snapshot_plan_phase(rg, &dev->log, epoch, cc_hw_grid());
 }
 
 // log compactor (cc_compactor.cuh)
@@ -145,18 +156,18 @@ __global__ void __launch_bounds__(CC_APPLY_THREADS) cc_compactor_cleanup_kernel(
 }
 
 // run-length records (cc_rle.cuh)
-__global__ void __launch_bounds__(256) cc_rle_starts_kernel(const cc_dev* dev, int slot, u32 run_pages) {
-    cc_rle_starts_phase(dev->regions[slot], run_pages, cc_hw_grid());
+__global__ void __launch_bounds__(256) cc_rle_starts_kernel(const cc_dev* dev, const __grid_constant__ cc_region_dev rg, u32 run_pages) {
+    cc_rle_starts_phase(rg, run_pages, cc_hw_grid());
 }
-__global__ void __launch_bounds__(CC_COMPACT_THREADS) cc_rle_rank_kernel(const cc_dev* dev, int slot) {
-    cc_rle_rank_phase(dev->regions[slot], &dev->log);
+__global__ void __launch_bounds__(CC_COMPACT_THREADS) cc_rle_rank_kernel(const cc_dev* dev, const __grid_constant__ cc_region_dev rg) {
+    cc_rle_rank_phase(rg, &dev->log);
 }
-__global__ void __launch_bounds__(256) cc_rle_plan_kernel(const cc_dev* dev, int slot, u64 epoch) {
-    cc_rle_plan_phase(dev->regions[slot], &dev->log, epoch, cc_hw_grid());
+__global__ void __launch_bounds__(256) cc_rle_plan_kernel(const cc_dev* dev, const __grid_constant__ cc_region_dev rg, u64 epoch) {
+    cc_rle_plan_phase(rg, &dev->log, epoch, cc_hw_grid());
 }
-__global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_rle_gather_kernel(cc_dev* dev, int slot, cc_result* out) {
+__global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_rle_gather_kernel(cc_dev* dev, const __grid_constant__ cc_region_dev rg, cc_result* out) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    cc_rle_gather_phase(dev->regions[slot], dev, reinterpret_cast<cc_crc_smem*>(smem_raw), cc_hw_grid(), out,
+    cc_rle_gather_phase(rg, dev, reinterpret_cast<cc_crc_smem*>(smem_raw), cc_hw_grid(), out,
                         CC_TASK_DELTA_CKPT, true);
 }
 
@@ -202,19 +213,19 @@ __global__ void cc_batch_collect_kernel(cc_dev* dev, cc_slot_list L, u64 epoch, 
 }
 
 // allocator-aware discovery (cc_mark.cuh)
-__global__ void __launch_bounds__(256) cc_mark_load_kernel(const cc_dev* dev, int slot, const u32* marks) {
-    cc_mark_load_phase(dev->regions[slot], marks, cc_hw_grid());
+__global__ void __launch_bounds__(256) cc_mark_load_kernel(const cc_dev* dev, const __grid_constant__ cc_region_dev rg, const u32* marks) {
+    cc_mark_load_phase(rg, marks, cc_hw_grid());
 }
-__global__ void __launch_bounds__(256) cc_mark_versions_kernel(const cc_dev* dev, int slot, const u64* version,
+__global__ void __launch_bounds__(256) cc_mark_versions_kernel(const cc_dev* dev, const __grid_constant__ cc_region_dev rg, const u64* version,
                                                                const u64* committed) {
-    cc_mark_versions_phase(dev->regions[slot], version, committed, cc_hw_grid());
+    cc_mark_versions_phase(rg, version, committed, cc_hw_grid());
 }
-__global__ void __launch_bounds__(CC_SCAN_THREADS) cc_mark_verify_kernel(const cc_dev* dev, int slot) {
-    cc_mark_verify_phase(dev->regions[slot], cc_hw_grid());
+__global__ void __launch_bounds__(CC_SCAN_THREADS) cc_mark_verify_kernel(const cc_dev* dev, const __grid_constant__ cc_region_dev rg) {
+    cc_mark_verify_phase(rg, cc_hw_grid());
 }
-__global__ void __launch_bounds__(256) cc_mark_finish_kernel(const cc_dev* dev, int slot, u32* marks_to_clear,
+__global__ void __launch_bounds__(256) cc_mark_finish_kernel(const cc_dev* dev, const __grid_constant__ cc_region_dev rg, u32* marks_to_clear,
                                                              const u64* version, u64* committed) {
-    cc_mark_finish_phase(dev->regions[slot], marks_to_clear, version, committed, cc_hw_grid());
+    cc_mark_finish_phase(rg, marks_to_clear, version, committed, cc_hw_grid());
 }
 
 // parse: candidate commit records (whole log, grid-wide) -> epoch walks (one block per epoch, chained by look-back)
@@ -428,6 +439,7 @@ extern "C" int32_t cc_init(cc_ctx** out, int32_t device, const cc_config* cfg) {
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->fused_bps, cc_pass_kernel, CC_GATHER_THREADS, sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_small_tail_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&ctx->small_bps, cc_small_kernel, CC_GATHER_THREADS, sizeof(cc_crc_smem));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_apply_validate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem4));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(cc_worker_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(cc_crc_smem));
@@ -828,7 +840,7 @@ static int32_t launch_compact(cc_ctx* ctx, int slot, u32 mode, uint64_t epoch, c
     const cc_region_dev& r = ctx->regions[slot].dev;
     const uint64_t n_tiles = (r.n_words + CC_COMPACT_TILE_WORDS - 1) / CC_COMPACT_TILE_WORDS;
     uint64_t g2 = n_tiles < (uint64_t)ctx->sm_count * 4 ? n_tiles : (uint64_t)ctx->sm_count * 4;
-    CC_CUDA(ctx, launch_dependent(cc_compact_kernel, (unsigned)g2, CC_COMPACT_THREADS, 0, st, ctx->d_dev, slot, mode, epoch, out));
+    CC_CUDA(ctx, launch_dependent(cc_compact_kernel, (unsigned)g2, CC_COMPACT_THREADS, 0, st, ctx->d_dev, ctx->regions[slot].dev, mode, epoch, out));
     if (ctx->ev_after_compact) cudaEventRecord(ctx->ev_after_compact, st);
     ctx->launches += 1;
     return CC_OK;
@@ -841,7 +853,7 @@ static int32_t launch_scan_compact(cc_ctx* ctx, int slot, u32 mode, uint64_t epo
     uint64_t g1 = (n_items + wpb - 1) / wpb;
     const uint64_t cap1 = (uint64_t)ctx->sm_count * ctx->scan_bps;
     if (g1 > cap1) g1 = cap1;
-    cc_scan_kernel<<<(unsigned)g1, CC_SCAN_THREADS, 0, st>>>(ctx->d_dev, slot);
+    cc_scan_kernel<<<(unsigned)g1, CC_SCAN_THREADS, 0, st>>>(ctx->d_dev, ctx->regions[slot].dev);
     if (ctx->ev_after_scan) cudaEventRecord(ctx->ev_after_scan, st);
     ctx->launches += 1;
     return launch_compact(ctx, slot, mode, epoch, st, out);
@@ -849,7 +861,7 @@ static int32_t launch_scan_compact(cc_ctx* ctx, int slot, u32 mode, uint64_t epo
 
 static int32_t launch_gather(cc_ctx* ctx, int slot, cudaStream_t st, cc_result* out) {
     const unsigned g3 = (unsigned)(ctx->sm_count * ctx->gather_bps);
-    CC_CUDA(ctx, launch_dependent(cc_gather_kernel, g3, CC_GATHER_THREADS, sizeof(cc_crc_smem), st, ctx->d_dev, slot, out));
+    CC_CUDA(ctx, launch_dependent(cc_gather_kernel, g3, CC_GATHER_THREADS, sizeof(cc_crc_smem), st, ctx->d_dev, ctx->regions[slot].dev, out));
     ctx->launches += 1;
     return CC_OK;
 }
@@ -874,13 +886,14 @@ static int32_t launch_pass(cc_ctx* ctx, int slot, const cc_pass_args& a, cudaStr
     if (g > cap) g = cap;
     cc_dev* d = ctx->d_dev;
     cc_pass_args aa = a;
-    void* args[] = {&d, &slot, &aa, &out};
+    cc_region_dev rgv = ctx->regions[slot].dev;
+    void* args[] = {&d, &rgv, &aa, &out};
 #if CC_PASS_COOP
     CC_CUDA(ctx, cudaLaunchCooperativeKernel((const void*)cc_pass_kernel, dim3((unsigned)g), dim3(CC_GATHER_THREADS), args,
                                              sizeof(cc_crc_smem), st));
 #else
     (void)args;
-    cc_pass_kernel<<<(unsigned)g, CC_GATHER_THREADS, sizeof(cc_crc_smem), st>>>(d, slot, aa, out);
+    cc_pass_kernel<<<(unsigned)g, CC_GATHER_THREADS, sizeof(cc_crc_smem), st>>>(d, rgv, aa, out);
     CC_CUDA(ctx, cudaGetLastError());
 #endif
     ctx->launches += 1;
@@ -898,7 +911,8 @@ static int32_t launch_small(cc_ctx* ctx, int slot, uint64_t epoch, cudaStream_t 
     if (g > cap) g = cap;
     if (g < 1) g = 1;
     cc_dev* d = ctx->d_dev;
-    void* args[] = {&d, &slot, &epoch, &out};
+    cc_region_dev rgv = ctx->regions[slot].dev;
+    void* args[] = {&d, &rgv, &epoch, &out};
     CC_CUDA(ctx, cudaLaunchCooperativeKernel((const void*)cc_small_kernel, dim3((unsigned)g), dim3(CC_GATHER_THREADS), args,
                                              sizeof(cc_crc_smem), st));
     ctx->launches += 1;
@@ -914,26 +928,45 @@ static int32_t launch_phases(cc_ctx* ctx, int slot, const cc_pass_args& a, cudaS
     const u32 final_mode = rle ? CC_MODE_SCAN_ONLY : CC_MODE_CHECKPOINT;
     cudaEvent_t ec = ctx->ev_after_compact;
     int32_t rc = CC_OK;
+    if (a.disc == CC_DISC_SCAN && !rle && cc_small_supported(r.n_words) && r.bytes <= CC_SMALL_TAIL_MAX_BYTES) {
+        // latency-bound sizes: the scan kernel, then ONE kernel in which every block ranks the bitmap by itself and the
+        // records follow at once (cc_small.cuh) -- the compaction kernel and its launch gap are 8 us of a 50 us call
+        const uint64_t n_items = r.n_pages * (uint64_t)r.spp;
+        uint64_t g1 = (n_items + CC_SCAN_THREADS / 32 - 1) / (CC_SCAN_THREADS / 32);
+        const uint64_t cap1 = (uint64_t)ctx->sm_count * ctx->scan_bps;
+        if (g1 > cap1) g1 = cap1;
+        cc_scan_kernel<<<(unsigned)g1, CC_SCAN_THREADS, 0, st>>>(ctx->d_dev, r);
+        if (ctx->ev_after_scan) cudaEventRecord(ctx->ev_after_scan, st);
+        if (ec) cudaEventRecord(ec, st);
+        uint64_t g2 = (n_items + CC_GATHER_THREADS / 32 - 1) / (CC_GATHER_THREADS / 32);
+        const uint64_t cap2 = (uint64_t)ctx->sm_count * ctx->small_bps;
+        if (g2 > cap2) g2 = cap2;
+        if (g2 < 1) g2 = 1;
+        cc_small_tail_kernel<<<(unsigned)g2, CC_GATHER_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, r, a.epoch, out);
+        ctx->launches += 2;
+        CC_CUDA(ctx, cudaGetLastError());
+        return CC_OK;
+    }
     if (a.disc == CC_DISC_SCAN) {
         if (rle) ctx->ev_after_compact = nullptr;             // the trace event goes after the whole ranking
         rc = launch_scan_compact(ctx, slot, final_mode, a.epoch, st, nullptr);
         ctx->ev_after_compact = ec;
     } else if (a.disc == CC_DISC_ALL) {
-        cc_snapshot_plan_kernel<<<small_grid(ctx, r.n_pages, 256), 256, 0, st>>>(ctx->d_dev, slot, a.epoch);
+        cc_snapshot_plan_kernel<<<small_grid(ctx, r.n_pages, 256), 256, 0, st>>>(ctx->d_dev, ctx->regions[slot].dev, a.epoch);
         ctx->launches += 1;
         if (ctx->ev_after_scan) cudaEventRecord(ctx->ev_after_scan, st);
         if (ec && !rle) cudaEventRecord(ec, st);
     } else {
         if (a.disc == CC_DISC_VERSIONS)
-            cc_mark_versions_kernel<<<small_grid(ctx, r.n_words, 8), 256, 0, st>>>(ctx->d_dev, slot, a.version, a.committed);
+            cc_mark_versions_kernel<<<small_grid(ctx, r.n_words, 8), 256, 0, st>>>(ctx->d_dev, ctx->regions[slot].dev, a.version, a.committed);
         else
-            cc_mark_load_kernel<<<small_grid(ctx, r.n_words, 256), 256, 0, st>>>(ctx->d_dev, slot, a.marks);
+            cc_mark_load_kernel<<<small_grid(ctx, r.n_words, 256), 256, 0, st>>>(ctx->d_dev, ctx->regions[slot].dev, a.marks);
         ctx->launches += 1;
         ctx->ev_after_compact = nullptr;                      // the trace events bracket discovery as a whole
         if (a.disc == CC_DISC_MARKS_VERIFY) {
             rc = launch_compact(ctx, slot, CC_MODE_SCAN_ONLY, a.epoch, st, nullptr);
             if (rc == CC_OK) {
-                cc_mark_verify_kernel<<<(unsigned)(ctx->sm_count * ctx->scan_bps), CC_SCAN_THREADS, 0, st>>>(ctx->d_dev, slot);
+                cc_mark_verify_kernel<<<(unsigned)(ctx->sm_count * ctx->scan_bps), CC_SCAN_THREADS, 0, st>>>(ctx->d_dev, ctx->regions[slot].dev);
                 ctx->launches += 1;
             }
         }
@@ -946,11 +979,11 @@ static int32_t launch_phases(cc_ctx* ctx, int slot, const cc_pass_args& a, cudaS
     if (rle) {
         const uint64_t n_tiles = (r.n_words + CC_COMPACT_TILE_WORDS - 1) / CC_COMPACT_TILE_WORDS;
         const unsigned g2 = (unsigned)(n_tiles < (uint64_t)ctx->sm_count * 4 ? n_tiles : (uint64_t)ctx->sm_count * 4);
-        cc_rle_starts_kernel<<<small_grid(ctx, r.n_words, 8), 256, 0, st>>>(ctx->d_dev, slot, a.run_pages);
-        cc_rle_rank_kernel<<<g2, CC_COMPACT_THREADS, 0, st>>>(ctx->d_dev, slot);
-        cc_rle_plan_kernel<<<small_grid(ctx, r.n_pages, 256), 256, 0, st>>>(ctx->d_dev, slot, a.epoch);
+        cc_rle_starts_kernel<<<small_grid(ctx, r.n_words, 8), 256, 0, st>>>(ctx->d_dev, ctx->regions[slot].dev, a.run_pages);
+        cc_rle_rank_kernel<<<g2, CC_COMPACT_THREADS, 0, st>>>(ctx->d_dev, ctx->regions[slot].dev);
+        cc_rle_plan_kernel<<<small_grid(ctx, r.n_pages, 256), 256, 0, st>>>(ctx->d_dev, ctx->regions[slot].dev, a.epoch);
         if (ec) cudaEventRecord(ec, st);
-        cc_rle_gather_kernel<<<(unsigned)(ctx->sm_count * ctx->gather_bps), CC_GATHER_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, slot, out);
+        cc_rle_gather_kernel<<<(unsigned)(ctx->sm_count * ctx->gather_bps), CC_GATHER_THREADS, sizeof(cc_crc_smem), st>>>(ctx->d_dev, ctx->regions[slot].dev, out);
         ctx->launches += 4;
         CC_CUDA(ctx, cudaGetLastError());
     } else {
@@ -958,10 +991,10 @@ static int32_t launch_phases(cc_ctx* ctx, int slot, const cc_pass_args& a, cudaS
         if (rc != CC_OK) return rc;
     }
     if ((a.disc == CC_DISC_MARKS || a.disc == CC_DISC_MARKS_VERIFY) && a.consume) {
-        cc_mark_finish_kernel<<<small_grid(ctx, r.n_words, 256), 256, 0, st>>>(ctx->d_dev, slot, a.marks, nullptr, nullptr);
+        cc_mark_finish_kernel<<<small_grid(ctx, r.n_words, 256), 256, 0, st>>>(ctx->d_dev, ctx->regions[slot].dev, a.marks, nullptr, nullptr);
         ctx->launches += 1;
     } else if (a.disc == CC_DISC_VERSIONS) {
-        cc_mark_finish_kernel<<<small_grid(ctx, r.n_pages, 256), 256, 0, st>>>(ctx->d_dev, slot, nullptr, a.version, a.committed);
+        cc_mark_finish_kernel<<<small_grid(ctx, r.n_pages, 256), 256, 0, st>>>(ctx->d_dev, ctx->regions[slot].dev, nullptr, a.version, a.committed);
         ctx->launches += 1;
     }
     CC_CUDA(ctx, cudaGetLastError());
