@@ -227,11 +227,13 @@ int32_t cc_log_drain_stop(cc_ctx* ctx);
  *               worst case (every page dirty) does not fit behind the log's write offset, the same launch runs the
  *               classic phases behind grid barriers instead (all-or-nothing needs the count first).
  *               CC_PATH_PHASES: the classic phases as separate launches (discovery, ordered compaction,
- *               [run ranking,] gather + commit), each sized for its own work.
+ *               [run ranking,] gather + commit), each sized for its own work.  For page records on a region of at most
+ *               131,072 pages and 1 GiB it is two launches: the scan, then one kernel in which every block ranks the
+ *               dirty bitmap by itself and writes its share of the records (no compaction launch).
  *               CC_PATH_SMALL: ONE kernel launch with one grid-wide rendezvous, for regions of at most 131,072 pages
  *               (CC_DISC_SCAN, one record per page; CC_ERR_INVALID otherwise): scan, then every block ranks the
  *               whole dirty bitmap by itself and the record writer follows at once.  It is what the persistent worker
- *               runs for a plain CC_TASK_DELTA_CKPT on such a region; host-launched it ties with the phases.
+ *               runs for a plain CC_TASK_DELTA_CKPT on such a region; host-launched the two-launch phases are faster.
  *               CC_PATH_AUTO: the phases, except with a pinned host log on regions of 128 MiB and more, where the single
  *               pass sends the records over the host link while it scans.
  * Every path writes the same bytes.  Result, asynchrony, CC_ERR_LOG_FULL rule: as cc_checkpoint_delta below. */

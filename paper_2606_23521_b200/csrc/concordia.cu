@@ -1057,9 +1057,8 @@ extern "C" int32_t cc_checkpoint_ex(cc_ctx* ctx, uint32_t region_id, uint64_t ep
     } else if (z.path == CC_PATH_PHASES) pass = false;
     else {
         // AUTO, from measurements (profiles/r02_small_region.md, profiles/r02_pass_probe.md): with a
-        // device log the separately sized kernels, chained by programmatic dependent launch, win or tie at every size
-        // (64 MiB: 54 us against 55 us for the one-launch small path and 62 us for the single pass; 8 GiB: 2.77 vs
-        // 3.2 ms); the single pass wins where the records cross the host link while it scans (8 GiB: 12.0 vs 13.8 ms,
+        // device log the separately sized kernels win at every size (64 MiB: 46 us as scan + tail kernel against 55 us for
+        // the one-launch small path and 62 us for the single pass; 8 GiB: 2.75 vs 3.2 ms); the single pass wins where the records cross the host link while it scans (8 GiB: 12.0 vs 13.8 ms,
         // 256 MiB ring task: 110 vs 150 us) -- but not on regions so small that its per-tile ranking costs more than the
         // transfer (64 MiB: 66 vs 56 us).
         pass = can_pass && ctx->log_is_host && r.bytes >= CC_PASS_AUTO_MIN_BYTES;
