@@ -245,6 +245,8 @@ __device__ __forceinline__ void cc_snapshot_plan_phase(const cc_region_dev& r, c
     }
 }
 
+#define CC_GATHER_CHUNK 4u      // consecutive 4 KiB segments of a record one warp takes at a time (cc_gather_items)
+
 // ------------------------------------------------- a3-a5: gather + CRC + commit + shadow --
 // For record i < k_eff: header {region_id, D[i], len, crc32c(payload)} + payload at
 // W_start + i*(16+P), and shadow[page] := cur[page] (L264).  One warp moves
@@ -260,21 +262,20 @@ __device__ __forceinline__ void st_u32x4(u8* p, u32 a, u32 b, u32 c, u32 d) {
 }
 
 // One (record, segment) item of the record writer: segment c of page p, which is record i of the checkpoint that starts
-// at log offset W0.  The warp reads the segment ONCE; log payload, shadow and CRC contribution come from that read; the
-// warp that completes the record's last segment writes its header.
-__device__ __forceinline__ void cc_gather_segment(const cc_region_dev& r, cc_dev* dev, cc_crc_smem* cs, u64 W0, u32 i, u32 c, u32 p,
-                                                  u32 lane) {
+// at log offset W0.  The warp reads the segment ONCE; log payload, shadow and CRC contribution come from that read.
+// Returns the segment's CRC contribution (in every lane); 0 for a segment beyond the page's end.
+__device__ __forceinline__ u32 cc_gather_segment_copy(const cc_region_dev& r, cc_dev* dev, cc_crc_smem* cs, u64 W0, u32 i, u32 c, u32 p,
+                                                      u32 lane) {
     constexpr int U = 8;
     cc_log_dev* log = &dev->log;
     const u32 P = r.page_bytes;
     const u64 plen = page_len_dev(r, p);
     const u64 so = (u64)c * CC_SEG_BYTES;
-    if (so >= plen) return;
+    if (so >= plen) return 0u;
     const u64 rem = plen - so;
     const u32 seg_len = (u32)(rem < CC_SEG_BYTES ? rem : CC_SEG_BYTES);
     const u32 nv = seg_len >> 4;
     const u64 after = rem - seg_len;
-    const u32 nseg = (u32)((plen + CC_SEG_BYTES - 1) / CC_SEG_BYTES);
     const u64 src_off = (u64)p * P + so;
     const uint4* src = reinterpret_cast<const uint4*>(r.base + src_off);
     const bool has_shadow = r.shadow != nullptr;      // allocator-aware regions may have none (cc_mark.cuh)
@@ -304,13 +305,30 @@ __device__ __forceinline__ void cc_gather_segment(const cc_region_dev& r, cc_dev
             }
         }
     }
-    const u32 contrib = crc_segment_warp<U>(cs, &dev->crc, v, nv, after, lane);
-    if (lane == 0) {
-        u32 acc = 0;
-        const bool finish = crc_record_combine(&r.rec_state[i], nseg, c, contrib, &acc);
-        if (finish) st_u32x4(rec, r.region_id, p, (u32)plen,
-                             crc_finalize(acc, plen == P ? r.crc_init_full : r.crc_init_tail));
+    return crc_segment_warp<U>(cs, &dev->crc, v, nv, after, lane);
+}
+
+// Segments c0 .. c0 + cn - 1 of record i are in place (contrib = XOR of their contributions; segments beyond the page's
+// end count as done): the warp that completes the record writes its header.
+__device__ __forceinline__ void cc_gather_record_done(const cc_region_dev& r, cc_dev* dev, u64 W0, u32 i, u32 p, u32 c0, u32 cn,
+                                                      u32 contrib, u32 lane) {
+    if (lane != 0) return;
+    const u32 P = r.page_bytes;
+    const u64 plen = page_len_dev(r, p);
+    const u32 nseg = (u32)((plen + CC_SEG_BYTES - 1) / CC_SEG_BYTES);
+    if (c0 >= nseg) return;
+    if (c0 + cn > nseg) cn = nseg - c0;
+    u32 acc = 0;
+    if (crc_record_combine_n(&r.rec_state[i], nseg, c0, cn, contrib, &acc)) {
+        u8* rec = dev->log.buf + W0 + (u64)i * ((u64)P + CC_RECORD_HEADER_BYTES);
+        st_u32x4(rec, r.region_id, p, (u32)plen, crc_finalize(acc, plen == P ? r.crc_init_full : r.crc_init_tail));
     }
+}
+
+__device__ __forceinline__ void cc_gather_segment(const cc_region_dev& r, cc_dev* dev, cc_crc_smem* cs, u64 W0, u32 i, u32 c, u32 p,
+                                                  u32 lane) {
+    const u32 contrib = cc_gather_segment_copy(r, dev, cs, W0, i, c, p, lane);
+    cc_gather_record_done(r, dev, W0, i, p, c, 1u, contrib, lane);
 }
 
 // The record writer proper (no synchronisation with other blocks): items first, first + step, ... of the
@@ -322,11 +340,30 @@ __device__ __forceinline__ void cc_gather_items(const cc_region_dev& r, cc_dev* 
     const u64 W0 = h->W_start;
     const u32 spp = r.spp;
     const u64 n_items = (u64)k_eff * spp;
-    for (u64 item = first; item < n_items; item += step) {
-        u32 i, c;
-        if (r.spp_shift >= 0) { i = (u32)(item >> r.spp_shift); c = (u32)(item & (spp - 1)); }
-        else { i = (u32)(item / spp); c = (u32)(item - (u64)i * spp); }
-        cc_gather_segment(r, dev, cs, W0, i, c, r.D[i], lane);
+    // A warp takes CC_GATHER_CHUNK consecutive segments of one record at a time when pages have that many and there are
+    // chunks enough to go round (>= 4 per warp): one look at D[], one 64-bit atomic on the record's state word per chunk
+    // instead of per segment.  Item numbering (first, first + step, ...) then counts chunks.
+    u32 G = 1;
+    if (r.spp_shift >= 2 && n_items / CC_GATHER_CHUNK >= 4 * step) G = CC_GATHER_CHUNK;
+    if (G == 1) {
+        for (u64 item = first; item < n_items; item += step) {
+            u32 i, c;
+            if (r.spp_shift >= 0) { i = (u32)(item >> r.spp_shift); c = (u32)(item & (spp - 1)); }
+            else { i = (u32)(item / spp); c = (u32)(item - (u64)i * spp); }
+            cc_gather_segment(r, dev, cs, W0, i, c, r.D[i], lane);
+        }
+        return;
+    }
+    const u64 n_chunks = n_items / G;                          // spp is a power of two >= G: whole chunks
+    const u32 cps_shift = (u32)r.spp_shift - 2u;               // log2(chunks per page), G == 4
+    for (u64 ch = first; ch < n_chunks; ch += step) {
+        const u32 i = (u32)(ch >> cps_shift);
+        const u32 c0 = (u32)(ch & ((1u << cps_shift) - 1u)) * G;
+        const u32 p = r.D[i];
+        u32 contrib = 0;
+#pragma unroll 1
+        for (u32 q = 0; q < G; q++) contrib ^= cc_gather_segment_copy(r, dev, cs, W0, i, c0 + q, p, lane);
+        cc_gather_record_done(r, dev, W0, i, p, c0, G, contrib, lane);
     }
 }
 

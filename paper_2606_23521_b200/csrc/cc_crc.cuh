@@ -256,21 +256,26 @@ __device__ inline u32 crc_serial(const cc_crc_tables*, const u8* p, u32 n) {
 // thread that sees every other bit already set is the finisher and the returned old value holds
 // the XOR of all other contributions.  Longer records fall back to XOR + fence + counter.
 // Returns true for the finisher, with *acc = XOR of all contributions; the state word is left zero.
-__device__ __forceinline__ bool crc_record_combine(u64* state, u32 nseg, u32 c, u32 contrib, u32* acc) {
-    if (nseg == 1) { *acc = contrib; return true; }
+// Segments c0 .. c0 + cn - 1 at once (contrib = XOR of their contributions).
+__device__ __forceinline__ bool crc_record_combine_n(u64* state, u32 nseg, u32 c0, u32 cn, u32 contrib, u32* acc) {
+    if (cn == nseg) { *acc = contrib; return true; }
     if (nseg <= 32) {
         const u32 full = nseg == 32 ? 0xFFFFFFFFu : ((1u << nseg) - 1u);
-        const u64 old = atomicXor(reinterpret_cast<unsigned long long*>(state), ((u64)(1u << c) << 32) | contrib);
-        if (((u32)(old >> 32) | (1u << c)) != full) return false;
+        const u32 mine = (cn == 32 ? 0xFFFFFFFFu : ((1u << cn) - 1u)) << c0;
+        const u64 old = atomicXor(reinterpret_cast<unsigned long long*>(state), ((u64)mine << 32) | contrib);
+        if (((u32)(old >> 32) | mine) != full) return false;
         *acc = (u32)old ^ contrib;
         *state = 0;
         return true;
     }
     atomicXor(reinterpret_cast<unsigned long long*>(state), (u64)contrib);
     __threadfence();
-    const u64 old = atomicAdd(reinterpret_cast<unsigned long long*>(state), 1ull << 32);
-    if ((u32)(old >> 32) != nseg - 1) return false;
+    const u64 old = atomicAdd(reinterpret_cast<unsigned long long*>(state), (u64)cn << 32);
+    if ((u32)(old >> 32) != nseg - cn) return false;
     __threadfence();
     *acc = (u32)atomicExch(reinterpret_cast<unsigned long long*>(state), 0ull);
     return true;
+}
+__device__ __forceinline__ bool crc_record_combine(u64* state, u32 nseg, u32 c, u32 contrib, u32* acc) {
+    return crc_record_combine_n(state, nseg, c, 1u, contrib, acc);
 }
