@@ -260,16 +260,14 @@ __device__ __forceinline__ u32 cc_find_rec(const u32* seg_begin, u32 n, u32 item
     return lo;
 }
 
-// CRC32C contribution of segment c of record ri; the warp that completes the record compares with the header's CRC.
+// CRC32C contribution of segment c of record ri (in every lane).
 template <class SM>
-__device__ __forceinline__ void cc_apply_validate_segment(cc_dev* dev, const cc_apply_tabs& T, SM* cs, const u8* log, u32 ri,
-                                                          const cc_rec& rec, u32 c, u32 lane) {
+__device__ __forceinline__ u32 cc_apply_segment_crc(cc_dev* dev, SM* cs, const u8* log, const cc_rec& rec, u32 c, u32 lane) {
     constexpr int U = 8;
     const u64 so = (u64)c * CC_SEG_BYTES;
     const u64 rem = rec.len - so;
     const u32 seg_len = (u32)(rem < CC_SEG_BYTES ? rem : CC_SEG_BYTES);
     const u32 nv = seg_len >> 4;
-    const u32 nseg = (rec.len + CC_SEG_BYTES - 1) / CC_SEG_BYTES;
     const uint4* src = reinterpret_cast<const uint4*>(log + rec.off + CC_RECORD_HEADER_BYTES + so);
     uint4 v[U];
 #pragma unroll
@@ -277,14 +275,18 @@ __device__ __forceinline__ void cc_apply_validate_segment(cc_dev* dev, const cc_
         const u32 j = lane + 32 * u;
         v[u] = (j < nv) ? ld_v4(src + j) : make_uint4(0, 0, 0, 0);
     }
-    const u32 contrib = crc_segment_warp<U>(cs, &dev->crc, v, nv, rem - seg_len, lane);
-    if (lane == 0) {
-        u32 acc = 0;
-        const bool finish = crc_record_combine(&T.rec_state[ri], nseg, c, contrib, &acc);
-        if (finish) {
-            const u32 it = cc_crc_init_term(dev, dev->regions[rec.slot], rec.len);
-            if (crc_finalize(acc, it) != rec.crc) atomicMin(&dev->apply.first_bad_rec, ri);
-        }
+    return crc_segment_warp<U>(cs, &dev->crc, v, nv, rem - seg_len, lane);
+}
+// Segments c0 .. c0 + cn - 1 of record ri are checked (contrib = XOR of their contributions): the warp that completes the
+// record compares with the header's CRC.
+__device__ __forceinline__ void cc_apply_record_verdict(cc_dev* dev, const cc_apply_tabs& T, u32 ri, const cc_rec& rec, u32 c0, u32 cn,
+                                                        u32 contrib, u32 lane) {
+    if (lane != 0) return;
+    const u32 nseg = (rec.len + CC_SEG_BYTES - 1) / CC_SEG_BYTES;
+    u32 acc = 0;
+    if (crc_record_combine_n(&T.rec_state[ri], nseg, c0, cn, contrib, &acc)) {
+        const u32 it = cc_crc_init_term(dev, dev->regions[rec.slot], rec.len);
+        if (crc_finalize(acc, it) != rec.crc) atomicMin(&dev->apply.first_bad_rec, ri);
     }
 }
 
@@ -363,10 +365,18 @@ __device__ __forceinline__ void cc_apply_validate_phase(cc_dev* dev, const cc_ap
             u32 ri = cc_find_rec(T.seg_begin, n_recs, item0, lane);
             cc_rec rec = T.recs[ri];
             u32 sb = T.seg_begin[ri], next = T.seg_begin[ri + 1];
+            // consecutive segments of one record are handed in together: one 64-bit combine per record and chunk
+            u32 c0 = item0 - sb, cn = 0, contrib = 0;
             for (u32 item = item0; item < item1; item++) {
-                while (item >= next) { ri++; rec = T.recs[ri]; sb = next; next = T.seg_begin[ri + 1]; }
-                cc_apply_validate_segment(dev, T, cs, log, ri, rec, item - sb, lane);
+                if (item >= next) {
+                    cc_apply_record_verdict(dev, T, ri, rec, c0, cn, contrib, lane);
+                    while (item >= next) { ri++; rec = T.recs[ri]; sb = next; next = T.seg_begin[ri + 1]; }
+                    c0 = item - sb; cn = 0; contrib = 0;
+                }
+                contrib ^= cc_apply_segment_crc(dev, cs, log, rec, item - sb, lane);
+                cn++;
             }
+            cc_apply_record_verdict(dev, T, ri, rec, c0, cn, contrib, lane);
         }
     }
     // last block resolves the committed prefix
