@@ -245,7 +245,10 @@ __device__ __forceinline__ void cc_snapshot_plan_phase(const cc_region_dev& r, c
     }
 }
 
-#define CC_GATHER_CHUNK 4u      // consecutive 4 KiB segments of a record one warp takes at a time (cc_gather_items)
+#ifndef CC_GATHER_CHUNK_LOG2
+#define CC_GATHER_CHUNK_LOG2 2u
+#endif
+#define CC_GATHER_CHUNK (1u << CC_GATHER_CHUNK_LOG2)      // consecutive 4 KiB segments of a record one warp takes at a time (cc_gather_items)
 
 // ------------------------------------------------- a3-a5: gather + CRC + commit + shadow --
 // For record i < k_eff: header {region_id, D[i], len, crc32c(payload)} + payload at
@@ -344,7 +347,7 @@ __device__ __forceinline__ void cc_gather_items(const cc_region_dev& r, cc_dev* 
     // chunks enough to go round (>= 4 per warp): one look at D[], one 64-bit atomic on the record's state word per chunk
     // instead of per segment.  Item numbering (first, first + step, ...) then counts chunks.
     u32 G = 1;
-    if (r.spp_shift >= 2 && n_items / CC_GATHER_CHUNK >= 4 * step) G = CC_GATHER_CHUNK;
+    if (r.spp_shift >= (int)CC_GATHER_CHUNK_LOG2 && n_items / CC_GATHER_CHUNK >= 4 * step) G = CC_GATHER_CHUNK;
     if (G == 1) {
         for (u64 item = first; item < n_items; item += step) {
             u32 i, c;
@@ -355,7 +358,7 @@ __device__ __forceinline__ void cc_gather_items(const cc_region_dev& r, cc_dev* 
         return;
     }
     const u64 n_chunks = n_items / G;                          // spp is a power of two >= G: whole chunks
-    const u32 cps_shift = (u32)r.spp_shift - 2u;               // log2(chunks per page), G == 4
+    const u32 cps_shift = (u32)r.spp_shift - CC_GATHER_CHUNK_LOG2;      // log2(chunks per page)
     for (u64 ch = first; ch < n_chunks; ch += step) {
         const u32 i = (u32)(ch >> cps_shift);
         const u32 c0 = (u32)(ch & ((1u << cps_shift) - 1u)) * G;
