@@ -166,9 +166,12 @@ def ncu_traffic(kernel, workload):
             with open(os.path.join(pdir, name), newline="") as fh:
                 for row in csv.DictReader(fh):
                     if row.get("Kernel Name", "").split("(")[0].strip() == kernel:
-                        rd = float(row["dram__bytes_read.sum [Gbyte]"])
-                        wr = float(row["dram__bytes_write.sum [Gbyte]"])
-                        return int(round((rd + wr) * 1e9)), "profiles/%s (one ncu --set full launch of %s)" % (name, kernel)
+                        tot = 0.0
+                        for col, val in row.items():                       # ncu picks the unit per column
+                            if col.startswith("dram__bytes_read.sum") or col.startswith("dram__bytes_write.sum"):
+                                unit = col[col.index("[") + 1:col.index("]")].lower()
+                                tot += float(val) * {"byte": 1.0, "kbyte": 1e3, "mbyte": 1e6, "gbyte": 1e9, "tbyte": 1e12}[unit]
+                        return int(round(tot)), "profiles/%s (one ncu --set full launch of %s)" % (name, kernel)
         except Exception:
             continue
     return None, "no tracked ncu --set full capture of %s on this workload" % kernel
