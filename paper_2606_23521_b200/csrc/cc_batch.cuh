@@ -31,10 +31,11 @@ __device__ __forceinline__ bool cc_batch_takes_part(const cc_dev* dev, int s) {
 struct cc_batch_tab {
     u64 n_items[CC_MAX_REGIONS];
     u64 cum[CC_MAX_REGIONS + 1];
+    u32 mod[CC_MAX_REGIONS];            // cum[s] % nwarps: a warp's first item of a region is one subtraction away
 };
 
 // call with all threads of the block; n_items[] filled by threads < CC_MAX_REGIONS beforehand
-__device__ __forceinline__ void cc_batch_tab_finish(cc_batch_tab* T) {
+__device__ __forceinline__ void cc_batch_tab_finish(cc_batch_tab* T, u64 nwarps) {
     __syncthreads();
     if (threadIdx.x == 0) {
         u64 c = 0;
@@ -42,12 +43,16 @@ __device__ __forceinline__ void cc_batch_tab_finish(cc_batch_tab* T) {
         T->cum[CC_MAX_REGIONS] = c;
     }
     __syncthreads();
+    // one 64-bit remainder per slot and BLOCK, not per slot and warp (7,104 warps x 64 slots of software division were
+    // most of the 38 M instructions cc_batch_scan_kernel executed on 48 small regions)
+    if (threadIdx.x < CC_MAX_REGIONS) T->mod[threadIdx.x] = (u32)(T->cum[threadIdx.x] % nwarps);
+    __syncthreads();
 }
 
-// first local item of region slot s for this warp (>= n_items[s] if none)
+// first local item of region slot s for this warp (>= n_items[s] if none); warp < nwarps < 2^32
 __device__ __forceinline__ u64 cc_batch_first(const cc_batch_tab* T, int s, u64 warp, u64 nwarps) {
-    const u64 m = T->cum[s] % nwarps;
-    return (warp + nwarps - m) % nwarps;
+    const u32 w = (u32)warp, m = T->mod[s];
+    return w >= m ? (u64)(w - m) : (u64)(w + (u32)nwarps - m);
 }
 
 __device__ __forceinline__ void cc_batch_scan_phase(cc_dev* dev, cc_batch_tab* T, cc_grid g) {
@@ -69,7 +74,7 @@ __device__ __forceinline__ void cc_batch_scan_phase(cc_dev* dev, cc_batch_tab* T
         }
         T->n_items[s] = n;
     }
-    cc_batch_tab_finish(T);
+    cc_batch_tab_finish(T, g.nwarps());
     const u64 w = g.warp(), nw = g.nwarps();
     for (int s = 0; s < CC_MAX_REGIONS; s++) {
         if (T->n_items[s] == 0) continue;
@@ -172,7 +177,7 @@ __device__ __forceinline__ void cc_batch_gather_phase(cc_dev* dev, cc_crc_smem* 
         if (cc_batch_takes_part(dev, s)) n = (u64)dev->regions[s].hdr->k_eff * dev->regions[s].spp;
         T->n_items[s] = n;
     }
-    cc_batch_tab_finish(T);
+    cc_batch_tab_finish(T, g.nwarps());
     {
         const u64 w = g.warp(), nw = g.nwarps();
         for (int s = 0; s < CC_MAX_REGIONS; s++) {
