@@ -65,6 +65,7 @@ extern "C" {
 #define CC_ERR_CUDA (-8)           /* a CUDA call failed: cc_last_cuda_error() */
 #define CC_ERR_TIMEOUT (-9)
 #define CC_ERR_SCRATCH (-10)       /* apply: log holds more records/epochs than the attached scratch; nothing applied */
+#define CC_ERR_STATIC_LIMIT (-11)  /* cc_dirty_pages_static: the region has more than CC_STATIC_MAX_PAGES pages */
 
 #define CC_MAX_REGIONS 64
 #define CC_COMMIT_ID 0xFFFFFFFFu
@@ -406,6 +407,45 @@ int32_t cc_submit(cc_ctx* ctx, const cc_task* task, uint64_t* seq_out);
 int32_t cc_poll(cc_ctx* ctx, uint64_t seq, cc_result* out);
 /* Spin (host) until done or timeout_ns elapsed (CC_ERR_TIMEOUT). */
 int32_t cc_wait(cc_ctx* ctx, uint64_t seq, uint64_t timeout_ns, cc_result* out);
+
+/* ---- dirty list without any allocation ---------------------------------------------------- */
+
+/* Steps a1-a2 for callers that cannot allocate: compare `cur` with `shadow` page by page
+ * and write the ascending list of the pages that differ -- the list cc_scan_only + cc_dirty_list give -- with
+ * NO context, NO registered region, NO workspace, and no cudaMalloc / cudaFree / allocating library routine
+ * anywhere in the call.  It is meant for code that runs beside a resident persistent kernel (device allocation
+ * synchronises the GPU and can wait forever on a kernel that never exits), for servers whose
+ * memory pool took all of HBM at start-up (a later cudaMalloc just fails), and for fault handlers that want to
+ * see what changed before they touch any allocator.
+ *
+ * The scratch (one bit per page + a counter) is a fixed array inside the library image, 2 MiB + 256 bytes,
+ * enough for CC_STATIC_MAX_PAGES pages: every GPU that loads libconcordia.so holds it until the process exits.
+ * A region with more pages is refused with CC_ERR_STATIC_LIMIT and nothing is launched; use a larger page
+ * size, call per sub-range, or use the workspace path.
+ *
+ *   device         CUDA device ordinal (0 ... 63) that owns every pointer and the stream; made current for the
+ *                  duration of the call and the previous device restored
+ *   cur, shadow    device memory, `bytes` bytes each, 16-byte aligned; only read
+ *   bytes          multiple of 16, > 0;   page_bytes  multiple of 16, > 0;  the last page may be short
+ *   d_list         device, u32[list_capacity], caller-owned: receives min(k, list_capacity) ascending page indices
+ *                  (may be NULL when list_capacity is 0: count only)
+ *   d_count        device (or pinned host), one u32, caller-owned: receives k, the number of dirty pages, even
+ *                  when k > list_capacity -- that is how a too-short list shows
+ *   stream         cudaStream_t of `device` (0 = legacy default stream).  ASYNCHRONOUS: one memset of the scratch
+ *                  and one kernel are queued; outputs are valid once the stream has reached that point
+ *   cuda_error     may be NULL; receives the cudaError_t when the return value is CC_ERR_CUDA
+ *
+ * FIRST CALL ON A DEVICE does the set-up: it resolves the array's device address (cudaGetSymbolAddress) and the
+ * launch geometry, which can make the runtime load the library's GPU code.  Make that first call outside any
+ * stream capture and before anything that must not stall; later calls only queue work.
+ * ONE ARRAY, SHARED: all calls on a GPU use the same scratch and it keeps the previous call's bits, so every call
+ * begins by zeroing the part it will read.  Calls queued on one stream are safe back to back.  Two calls that can
+ * run at the same time on one GPU (different streams, different host threads, different contexts of this process)
+ * race on it and both results are garbage: serialise them yourself.  The regular workspace path has no such limit. */
+#define CC_STATIC_MAX_PAGES (1u << 24)
+int32_t cc_dirty_pages_static(int32_t device, const void* cur, const void* shadow, uint64_t bytes, uint32_t page_bytes,
+                              uint32_t* d_list, uint32_t list_capacity, uint32_t* d_count, void* stream,
+                              int32_t* cuda_error);
 
 /* ============================ BENCH / TEST HOOKS -- not part of the product API ============================
  * Measurement and test instrumentation used by bench.py and tests/ only.  They change no result.  Compiled in by

@@ -4,4 +4,4 @@ CUDA kernels + C ABI: csrc/ and include/concordia.h.  This package is the thin P
 It never imports oracle/ (the CPU oracle is test infrastructure) and has no CPU fallback.
 """
 from .binding import *  # noqa: F401,F403
-from .binding import Context, Result, load_library, lib_path, EXPORTS  # noqa: F401
+from .binding import Context, Result, load_library, lib_path, dirty_pages_static, EXPORTS  # noqa: F401

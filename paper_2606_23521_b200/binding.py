@@ -24,6 +24,8 @@ CC_ERR_WORKER = -7
 CC_ERR_CUDA = -8
 CC_ERR_TIMEOUT = -9
 CC_ERR_SCRATCH = -10
+CC_ERR_STATIC_LIMIT = -11
+CC_STATIC_MAX_PAGES = 1 << 24
 
 CC_REG_SNAPSHOT_NOW = 1
 CC_REG_NO_SHADOW = 2
@@ -55,6 +57,7 @@ EXPORTS = [
     "cc_checkpoint_ex", "cc_checkpoint_delta", "cc_checkpoint_delta_fused", "cc_checkpoint_delta_rle", "cc_checkpoint_marked", "cc_checkpoint_versions",
     "cc_checkpoint_all", "cc_checkpoint_all_rle", "cc_snapshot_region", "cc_compact_log", "cc_scan_only", "cc_trace_events", "cc_dirty_list", "cc_apply_scratch_bytes", "cc_apply_attach", "cc_apply_stage_attach", "cc_apply_log",
     "cc_worker_start", "cc_worker_stop", "cc_worker_alive", "cc_worker_footprint", "cc_peek_queue", "cc_submit", "cc_measure_submit_cost", "cc_measure_launch_cost", "cc_poll", "cc_wait",
+    "cc_dirty_pages_static",
 ]
 
 
@@ -153,6 +156,7 @@ def load_library():
         "cc_measure_launch_cost": (i32, [vp, u32, vp, P(ctypes.c_double), P(ctypes.c_double)]),
         "cc_poll": (i32, [vp, u64, P(cc_result)]),
         "cc_wait": (i32, [vp, u64, u64, P(cc_result)]),
+        "cc_dirty_pages_static": (i32, [i32, vp, vp, u64, u32, vp, u32, vp, vp, P(i32)]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -172,6 +176,32 @@ def _stream_ptr(stream):
     if stream is None:
         stream = torch.cuda.current_stream()
     return ctypes.c_void_p(stream.cuda_stream)
+
+
+def dirty_pages_static(cur: torch.Tensor, shadow: torch.Tensor, page_bytes: int, d_list: torch.Tensor,
+                       d_count: torch.Tensor, stream=None):
+    """cc_dirty_pages_static: the ascending dirty page list of `cur` against `shadow` for callers that cannot
+    allocate -- no Context, no registered region, no workspace; the scratch is a fixed array inside the library
+    (at most CC_STATIC_MAX_PAGES pages, else ConcordiaError with code CC_ERR_STATIC_LIMIT).  Every tensor is the
+    caller's: cur / shadow contiguous CUDA tensors of equal byte size, d_list an int32 CUDA tensor that receives
+    min(k, d_list.numel()) page indices, d_count an int32 CUDA (or pinned) tensor of one element that receives
+    k.  Asynchronous on `stream` (default: torch's current stream).  Calls that can overlap on one GPU race on the
+    shared scratch; the first call on a device does the one-time set-up and belongs outside stream capture.
+    This wrapper marshals arguments and allocates no device memory either."""
+    assert cur.is_cuda and cur.is_contiguous() and shadow.is_cuda and shadow.is_contiguous()
+    nbytes = cur.numel() * cur.element_size()
+    assert shadow.numel() * shadow.element_size() == nbytes and shadow.device == cur.device
+    assert d_list.dtype == torch.int32 and d_list.is_cuda and d_list.is_contiguous()
+    assert d_count.dtype == torch.int32 and d_count.numel() == 1 and (d_count.is_cuda or d_count.is_pinned())
+    lib = load_library()
+    err = ctypes.c_int32(0)
+    if stream is None:
+        stream = torch.cuda.current_stream(cur.device)
+    rc = lib.cc_dirty_pages_static(cur.device.index, cur.data_ptr(), shadow.data_ptr(), nbytes, page_bytes,
+                                   d_list.data_ptr() if d_list.numel() else None, d_list.numel(), d_count.data_ptr(),
+                                   ctypes.c_void_p(stream.cuda_stream), ctypes.byref(err))
+    if rc != CC_OK:
+        raise ConcordiaError("cc_dirty_pages_static", rc, err.value)
 
 
 class Result:

@@ -5,7 +5,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libconcordia.so")
-SOURCES = ["concordia.cu"]
+SOURCES = ["concordia.cu", "cc_static.cu"]
 HEADERS = ["cc_common.cuh", "cc_crc.cuh", "cc_ckpt.cuh", "cc_mark.cuh", "cc_fused.cuh", "cc_pass.cuh", "cc_small.cuh", "cc_tasks.cuh", "cc_rle.cuh", "cc_apply.cuh",
            "cc_apply_parse.cuh", "cc_compactor.cuh", "cc_batch.cuh", "cc_worker.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
