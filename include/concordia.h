@@ -224,7 +224,8 @@ int32_t cc_log_drain_stop(cc_ctx* ctx);
  *               that is a multiple of run_pages (run_pages * page_bytes < 2^32)
  *   path        CC_PATH_SINGLE_PASS: ONE kernel launch -- warp tiles of pages are discovered, ranked by decoupled
  *               look-back and written (records, CRC32C, shadow) by the same warp, the last warp of the grid commits
- *               and publishes; needs run_pages <= 32 and at most 2^25 pages (CC_ERR_INVALID otherwise).  When the
+ *               and publishes; needs run_pages <= 32 and at most 2^20 * (32 rounded down to a multiple of run_pages) pages -- 2^25 for
+ *               page records (CC_ERR_INVALID otherwise).  When the
  *               worst case (every page dirty) does not fit behind the log's write offset, the same launch runs the
  *               classic phases behind grid barriers instead (all-or-nothing needs the count first).
  *               CC_PATH_PHASES: the classic phases as separate launches (discovery, ordered compaction,

@@ -59,13 +59,21 @@ __device__ __forceinline__ u32 cc_pass_tile_pages(const cc_region_dev& r, u32 ru
     if (tp < 1) tp = 1;
     if (tp > 32) tp = 32;
     if (run_pages > 1) {
-        tp = tp / run_pages * run_pages;
-        if (tp < run_pages) tp = run_pages;
+        u64 t = tp / run_pages * run_pages;
+        if (t < run_pages) t = run_pages;
+        // rounding down must not undo the lower bound: more than CC_PASS_MAX_TILES tiles would run past the look-back
+        // words the workspace holds.  Rounding `lo` UP stays <= 32 for every shape cc_pass_supported admits.
+        if (t < lo) t = (lo + run_pages - 1) / run_pages * run_pages;
+        tp = t;
     }
     return (u32)tp;
 }
+// The single pass takes a region iff it can be cut into at most CC_PASS_MAX_TILES tiles: a tile has at most 32 pages
+// (one mask register) and is a whole multiple of run_pages, so at most 32 / run_pages * run_pages pages.
 __host__ __device__ __forceinline__ bool cc_pass_supported(u64 n_pages, u32 run_pages) {
-    return run_pages <= 32 && n_pages <= 32ull * CC_PASS_MAX_TILES;
+    if (run_pages > 32) return false;
+    const u64 tmax = run_pages > 1 ? 32u / run_pages * run_pages : 32u;
+    return n_pages <= tmax * CC_PASS_MAX_TILES;
 }
 
 // Shared-memory CRC tables, filled on first use by the warp that needs them (most blocks of a sparse checkpoint
@@ -267,6 +275,10 @@ __device__ __forceinline__ bool cc_pass_tiles(const cc_region_dev& r, cc_dev* de
                 h->W_start = W0;
                 h->need = k ? need : 0;
                 h->inline_done = 1;
+                // The grid's last warp (cc_pass_commit) reads the plan.  This warp may leave without having written a
+                // record (a clean last tile), so cc_pass_leave would not fence for it: order the plan stores before
+                // this thread's count-out here, at gpu scope (one warp per call).
+                __threadfence();
             }
         }
         // ---- allocator metadata handed back (the checkpoint cannot fail any more: the worst case fits) ----

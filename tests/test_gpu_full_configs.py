@@ -280,3 +280,41 @@ def test_c4_full_64gib_arena_as_8_regions_through_one_pinned_log():
     out = bench.c4_full_arena(A, bench.Env(), cc, 65536, verify=True)
     assert out["parity"].startswith("arena: all 8 x 131072 records"), out
     assert out["host_link_GBps_log"] > 20.0, out
+
+
+@pytest.mark.parametrize("R", [3, 5])
+def test_single_pass_run_records_16gib_region_odd_run_length(R):
+    """16 GiB at 4 KiB pages (2^22 + 3 pages) with a run length that is no power of two, forced onto the single pass: the
+    tile size has a lower bound of ceil(n_pages / 2^20) pages (the look-back table has 2^20 words) that rounding to a
+    multiple of run_pages must not undercut -- rounded DOWN, 4 -> 3 pages gave 1.4 M tiles and writes past the workspace.
+    Mostly-zero contents (the host copies stay virtual); the dirty pages carry seeded bytes."""
+    _need(36, 12)
+    P, n_pages = 4096, (1 << 22) + 3
+    N = n_pages * P
+    rng = np.random.default_rng(160 + R)
+    starts = rng.choice(n_pages - 16, 2000, replace=False)
+    pages = np.unique(np.concatenate([starts + j for j in range(R + 2)] + [np.array([0, n_pages - 2, n_pages - 1])]))
+    idx = pages * P + rng.integers(0, P, pages.size)
+    vals = rng.integers(1, 256, pages.size).astype(np.uint8)
+    cur = torch.zeros(N, dtype=torch.uint8, device="cuda")
+    shadow = torch.zeros(N, dtype=torch.uint8, device="cuda")
+    cur[torch.from_numpy(idx).cuda()] = torch.from_numpy(vals).cuda()
+    cur_h, sh_h = np.zeros(N, np.uint8), np.zeros(N, np.uint8)
+    cur_h[idx] = vals
+    cap = pages.size * (16 + P) + 4096
+    olog = np.zeros(cap, np.uint8)
+    st, D, runs, nb, W = oracle.checkpoint_rle(cur_h, sh_h, P, 4, 9, R, olog, 0)
+    assert st == 0 and D.tolist() == pages.tolist() and 0 < runs < pages.size
+    ctx = cc.Context()
+    ctx.register_region(4, cur, P, shadow=shadow, snapshot_now=False)
+    glog = torch.zeros(cap, dtype=torch.uint8, device="cuda")
+    ctx.log_attach(glog)
+    res = cc.Result()
+    ctx.checkpoint_ex(4, 9, res, path=cc.CC_PATH_SINGLE_PASS, run_pages=R)
+    torch.cuda.synchronize()
+    r = res.read()
+    assert (r.status, r.n_dirty, r.bytes, r.log_offset_after) == (0, D.size, nb, W), r.as_dict()
+    assert ctx.dirty_list(4).tolist() == D.tolist()
+    assert np.array_equal(glog.cpu().numpy(), olog)
+    assert _equal_chunked(shadow, cur)                      # every dirty page refreshed, nothing else touched
+    ctx.shutdown()

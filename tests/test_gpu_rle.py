@@ -298,3 +298,21 @@ def test_rle_prefill_shaped_c2_full_size():
         assert crc == oracle.crc32c(payload) and np.array_equal(payload, cur[p0 * P:p0 * P + ln].cpu().numpy())
         off += 16 + ln
     ctx.shutdown()
+
+
+@pytest.mark.parametrize("R", [3, 5, 7])
+def test_rle_millions_of_small_pages_with_odd_run_lengths(R):
+    """More than 2^22 pages with a run length that is no power of two: the single pass must still cut the region into at
+    most 2^20 warp tiles (its look-back table), i.e. round the tile size UP to a multiple of R, not down."""
+    P, n_pages = 16, (1 << 22) + 37
+    N = n_pages * P
+    cur = synth.raw_region(N, 77 + R, "cuda")
+    sh = cur.clone()
+    rng = np.random.default_rng(R)
+    starts = rng.choice(n_pages - 16, 3000, replace=False)
+    pages = np.unique(np.concatenate([starts + j for j in range(int(R) + 2)] + [np.array([0, n_pages - 1, n_pages - 2])]))
+    idx = torch.from_numpy(pages * P + rng.integers(0, P, pages.size)).cuda()
+    sh[idx] = sh[idx] ^ 0x40
+    ctx, r, runs, glog, nb = _rle_parity(cur, sh, P, R, cap=pages.size * (16 + P) + 4096)
+    assert r.n_dirty == pages.size and 0 < runs < pages.size
+    ctx.shutdown()
