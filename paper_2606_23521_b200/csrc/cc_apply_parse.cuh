@@ -44,7 +44,12 @@ __device__ __forceinline__ void cc_parse_cand_phase(cc_dev* dev, cc_parse_ctl* C
                                                     cc_grid g) {
     const u32 lane = threadIdx.x & 31u;
     const u64 units = n >> 4;                                    // 16-byte units of the log
-    if (g.block == 0 && threadIdx.x == 0) cc_apply_reset_state(dev);     // (read by the walk phase, two launches later)
+    if (g.block == 0 && threadIdx.x == 0) {
+        cc_apply_reset_state(dev);                               // (read by the walk phase, two launches later)
+        // candidates are kept as u32 counts of 16-byte units: a log of 64 GiB or more does not fit them, and wrapped
+        // offsets could coincide (the ranking below needs distinct values).  Such a log goes to the serial parser.
+        if (units > 0xFFFFFFFFull) C->cand_overflow = 1;
+    }
     const uint4* L = reinterpret_cast<const uint4*>(log);
     for (u64 ub = (u64)g.warp() * 256u; ub < units; ub += (u64)g.nwarps() * 256u) {
         uint4 v[8];
@@ -81,12 +86,20 @@ __device__ __forceinline__ void cc_parse_cand_phase(cc_dev* dev, cc_parse_ctl* C
 // offsets).  n^2 / threads comparisons out of shared-memory tiles: a hundred candidates are a few microseconds of one
 // block, a hundred thousand ~0.1 ms of the whole grid -- either way far below the serial walk the ordered list saves.
 // Also arms the look-back words of the walk.  scratch: T.cand[0 .. max_records], T.span_status[0 .. max_records + 1].
+// The ranking is quadratic in the number of candidates (= commit records): beyond CC_SORT_MAX_CAND of them -- 2^17,
+// ~0.3 ms of the whole grid -- the list is declared overflowed and the linear serial parser takes the log instead, so
+// that recovery time grows with the log's bytes, not with the square of its epoch count.
 #define CC_SORT_THREADS 256
+#define CC_SORT_MAX_CAND (1u << 17)
 __device__ __forceinline__ void cc_parse_sort_phase(cc_parse_ctl* C, const u32* cand_raw, u32* cand, u64* span_status, u64 max_records,
                                                     cc_grid g) {
     __shared__ u32 s_tile[CC_SORT_THREADS];
     const u32 tid = threadIdx.x;
     u64 n64 = C->n_raw;
+    if (n64 > CC_SORT_MAX_CAND || C->cand_overflow) {             // (every block takes the same decision from n_raw)
+        if (g.block == 0 && tid == 0) { C->cand_overflow = 1; C->n_cand = 0; }
+        return;
+    }
     if (n64 > max_records + 1) n64 = max_records + 1;
     const u32 n = (u32)n64;
     if (g.block == 0 && tid == 0) { C->n_cand = n; span_status[0] = 0; }

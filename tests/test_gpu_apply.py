@@ -305,3 +305,32 @@ def test_thousands_of_one_record_epochs():
     ctx, reg, sh_t, r = _compare(old, log, W, P, max_records=8192)
     assert r.status == 0 and r.epoch >= E - 600 and np.array_equal(reg.cpu().numpy(), cur)
     _compare(old, log, W // 2 + 8, P, max_records=8192)    # torn in the middle
+
+
+def test_more_epochs_than_the_candidate_ranking_takes_go_to_the_serial_parser():
+    """140,000 one-record epochs of 16-byte pages: more commit records than the quadratic ranking of the parallel parse
+    accepts (2^17), so the whole log is parsed by the linear serial parser -- same result as the oracle, and the same
+    context then takes a short log through the parallel parse again (the overflow flag was re-armed)."""
+    P, n_pages, E = 16, 64, 140_000
+    N = P * n_pages
+    rng = np.random.default_rng(140)
+    old = rng.integers(0, 256, N, dtype=np.uint8)
+    cur, sh = old.copy(), old.copy()
+    log = np.zeros(E * (16 + P + 32) + 64, dtype=np.uint8)
+    W = 0
+    where = rng.integers(0, N, E)
+    for e in range(E):
+        cur[where[e]] ^= 0x01 + (e & 0x7E)
+        st, D, nb, W = oracle.checkpoint(cur, sh, P, 3, e, log, W)
+        assert D.size == 1
+    ctx, reg, sh_t, r = _compare(old, log, W, P, max_records=E + 64)
+    assert (r.status, r.n_dirty, r.epoch, r.bytes) == (0, E, E, W) and np.array_equal(reg.cpu().numpy(), cur)
+    short = 50 * (16 + P + 32)
+    reg_o, sh_o = old.copy(), old.copy()
+    exp = oracle.apply_log(log, short, [oracle.Region(3, P, reg_o, sh_o)])
+    reg.copy_(torch.from_numpy(old))
+    sh_t.copy_(torch.from_numpy(old))
+    r = _gpu_apply(ctx, torch.from_numpy(log[:short].copy()).cuda(), short)
+    assert (r.status, r.n_dirty, r.bytes) == exp == (0, 50, short)
+    assert np.array_equal(reg.cpu().numpy(), reg_o) and np.array_equal(sh_t.cpu().numpy(), sh_o)
+    ctx.shutdown()
