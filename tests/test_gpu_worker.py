@@ -262,3 +262,47 @@ def test_wait_and_submit_notice_a_worker_that_left_by_itself():
     assert time.time() - t0 < 5.0                           # not the 20 s timeout
     assert not ctx.worker_alive()
     ctx.shutdown()
+
+
+def test_two_host_threads_submitting_at_once(tmp_path):
+    """SURVEY.md section 5 row 2 / PAPER.md:L119, L249: the ring has ONE producer.  Two native threads call cc_submit
+    on the same context as fast as they can (100,000 NOP tasks in all, the ring mostly full): a thread that finds the
+    other one inside is refused with CC_ERR_INVALID and tries again; no sequence number is handed out twice or skipped,
+    each thread's numbers ascend, every task completes, and the completion records of the last ring's worth of tasks
+    carry the tag of the thread that really submitted them."""
+    import ctypes
+    import os
+    import subprocess
+    so = str(tmp_path / "libring_stress.so")
+    subprocess.run(["gcc", "-O2", "-pthread", "-shared", "-fPIC", "-o", so,
+                    os.path.join(os.path.dirname(os.path.abspath(__file__)), "helpers", "ring_stress.c")], check=True)
+    h = ctypes.CDLL(so)
+    h.ring_stress.restype = ctypes.c_int32
+    h.ring_stress.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint32, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+    n, cap = 50_000, 256
+    ctx = cc.Context(ring_capacity=cap)
+    ctx.worker_start()
+    try:
+        sa, sb = np.zeros(n, np.uint64), np.zeros(n, np.uint64)
+        cnt = np.zeros(4, np.uint64)
+        submit = ctypes.cast(ctx.lib.cc_submit, ctypes.c_void_p)
+        rc = h.ring_stress(submit, ctx.h, n, sa.ctypes.data, sb.ctypes.data, cnt.ctypes.data)
+        assert rc == 0, rc
+        assert np.all(np.diff(sa.astype(np.int64)) > 0) and np.all(np.diff(sb.astype(np.int64)) > 0)
+        both = np.sort(np.concatenate([sa, sb]))
+        assert np.array_equal(both, np.arange(2 * n, dtype=np.uint64)), "a sequence number was lost or handed out twice"
+        last = ctx.wait(2 * n - 1, 30.0)
+        assert last.status == 0 and last.seq_done == 2 * n
+        assert ctx.peek_queue() == (2 * n, 2 * n)
+        owner = {int(s): (1, i) for i, s in enumerate(sa)}
+        owner.update({int(s): (2, i) for i, s in enumerate(sb)})
+        for seq in range(2 * n - cap, 2 * n):
+            r = ctx.poll(seq)
+            tag, i = owner[seq]
+            assert r is not None and r.seq_done == seq + 1 and r.epoch == (tag << 32) | i, (seq, r.as_dict())
+        if (os.cpu_count() or 1) >= 2:
+            assert int(cnt[0] + cnt[1]) > 0, "the two producers never met inside cc_submit: %s" % cnt.tolist()
+        assert ctx.worker_alive()
+    finally:
+        ctx.worker_stop()
+        ctx.shutdown()
