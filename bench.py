@@ -1011,28 +1011,14 @@ def c4_e2e(args, env, ctx, cc, cur, shadow, P, rid, sparse):
                     "H2D of the new bytes, launch, synchronize and reading the result"}
 
 
-def all_dirty_flips(torch, synth, N, P, seed, dev):
-    n_pages = N // P
-    g = synth.gen(seed, dev)
-    offs = torch.arange(n_pages, device=dev) * P + torch.randint(0, P, (n_pages,), generator=g, device=dev)
-    masks = torch.randint(1, 256, (n_pages,), generator=g, device=dev, dtype=torch.int64).to(torch.uint8)
-    return offs, masks
-
-
-def verify_all_dirty(torch, cc, ctx, rid, cur, log, offs, masks, P, epoch, N, chunk=1 << 30, threads=16, log_is_host=False):
-    """Every record of an all-dirty checkpoint against oracle.checkpoint, chunk by chunk."""
-    import numpy as np
-    from oracle import chunked
-    o_cpu, m_cpu = offs.cpu().numpy(), masks.cpu().numpy()
-
-    def fetch_shadow0(o, n):
-        a = cur[o:o + n].cpu().numpy()
-        lo, hi = (o // P), ((o + n) // P)                          # one flip per page, ascending
-        a[o_cpu[lo:hi] - o] ^= m_cpu[lo:hi]
-        return a
-    fl = (lambda o, n: log[o:o + n].numpy()) if log_is_host else (lambda o, n: log[o:o + n].cpu().numpy())
-    return chunked.verify_checkpoint_chunked(N, P, rid, epoch, lambda o, n: cur[o:o + n].cpu().numpy(), fetch_shadow0, fl,
-                                             chunk_bytes=chunk, threads=threads)
+def _tests_util():
+    """The C4 all-dirty checker lives with the tests (tests/gpu_util.py: it calls oracle/chunked.py); the untimed parity
+    legs below borrow it from there."""
+    tdir = os.path.join(ROOT, "tests")
+    if tdir not in sys.path:
+        sys.path.insert(0, tdir)
+    import gpu_util
+    return gpu_util
 
 
 def run_c4_full(args, env):
@@ -1051,14 +1037,14 @@ def run_c4_full(args, env):
         shadow = ctx.register_region(1, cur, P)
         log = torch.empty(n_pages * (16 + P) + 32, dtype=torch.uint8, device=dev)
         ctx.log_attach(log)
-        offs, masks = all_dirty_flips(torch, synth, N, P, 1004 + P, dev)
+        offs, masks = synth.all_dirty_flips(N, P, 1004 + P, dev)
         if not args.no_parity and env.rank == 0:
             synth.toggle_flips(cur, offs, masks)
             res = cc.Result()
             ctx.checkpoint_delta(1, 6, res)
             torch.cuda.synchronize()
             r = res.read()
-            kk, nb, D = verify_all_dirty(torch, cc, ctx, 1, cur, log, offs, masks, P, 6, N)
+            kk, nb, D = _tests_util().verify_all_dirty(cur, log, offs, masks, P, 1, 6)
             assert (r.status, r.n_dirty, r.bytes) == (0, n_pages, nb) and kk == n_pages
             assert all(torch.equal(shadow[o:o + (1 << 30)], cur[o:o + (1 << 30)]) for o in range(0, N, 1 << 30))
             parity = parity or {"checked": [], "ok": True}
@@ -1141,7 +1127,7 @@ def c4_full_arena(args, env, cc, P, verify, regions=8, region_gib=8):
     committed = torch.zeros(1, dtype=torch.int64, pin_memory=True)
     ctx.log_attach(hlog, committed)
     res = cc.Result()
-    flips = [all_dirty_flips(torch, synth, R, P, 7000 + i, dev) for i in range(regions)]
+    flips = [synth.all_dirty_flips(R, P, 7000 + i, dev) for i in range(regions)]
     times, ok = [], 0
     for rnd in range(2):                                             # round 0 warms up and verifies; round 1 is timed
         for i in range(regions):
@@ -1155,7 +1141,7 @@ def c4_full_arena(args, env, cc, P, verify, regions=8, region_gib=8):
             dt = (time.perf_counter() - t0) * 1e3
             assert r.status == 0 and r.n_dirty == n_pages and r.bytes == cap and int(committed.item()) == cap, r.as_dict()
             if rnd == 0 and verify:
-                kk, nb, D = verify_all_dirty(torch, cc, ctx, i + 1, v, hlog, flips[i][0], flips[i][1], P, i, R, log_is_host=True)
+                kk, nb, D = _tests_util().verify_all_dirty(v, hlog, flips[i][0], flips[i][1], P, i + 1, i, log_is_host=True)
                 assert kk == n_pages and nb == cap and torch.equal(shadows[i], v)
                 ok += 1
             if rnd == 1:
@@ -1166,10 +1152,10 @@ def c4_full_arena(args, env, cc, P, verify, regions=8, region_gib=8):
     out = {"value": round(regions * R / (total * 1e-3) / 1e9, 2), "unit": UNIT, "h2d_bytes_per_step": 0,
            "d2h_bytes_per_step": regions * cap + 64 * regions, "ms_per_step": round(total, 3),
            "host_link_GBps_log": round(regions * cap / (total * 1e-3) / 1e9, 2),
-           "path": "SURVEY.md 8d fallback (i): the %d GiB arena as %d x %d GiB regions (64 KiB pages, every page dirty), "
+           "path": "SURVEY.md 8d fallback (i): the %d GiB arena as %d x %d GiB regions (%d KiB pages, every page dirty), "
                    "cc_checkpoint_delta of each into ONE pinned %.1f GiB host log, result read on the host and the log rewound "
                    "between regions; one step = the whole arena; host wall clock; link-bound (SM stores cap at 52.7 GB/s)"
-                   % (regions * region_gib, regions, region_gib, cap / 2**30)}
+                   % (regions * region_gib, regions, region_gib, P >> 10, cap / 2**30)}
     if verify:
         out["parity"] = ("arena: all %d x %d records of the pinned host log and the shadows bit-exact with the oracle (chunk-wise), %d regions"
                          % (ok, n_pages, ok))

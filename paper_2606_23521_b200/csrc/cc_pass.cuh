@@ -177,9 +177,6 @@ __device__ __forceinline__ void cc_pass_clear_marks(const cc_region_dev& r, cons
     }
 }
 
-// (kept for the kernels' signatures: the tile pass itself needs no shared scratch)
-struct cc_pass_smem { u32 unused; };
-
 // The inline single pass over the tiles (see the file header).  Whole warps call this; no block barrier inside.
 // Tiles are handed out by an atomic TICKET, so that a tile's predecessors have always started -- and, being taken in
 // time order, have mostly FINISHED: the look-back then finds an inclusive sum within a step or two.  A ticket is drawn
@@ -188,7 +185,7 @@ struct cc_pass_smem { u32 unused; };
 // sit in some other warp's queue (profiles/r02_pass_probe.md: a 256 MiB ring task took 156 us instead of 109 us, an
 // 8 GiB checkpoint into a pinned log 16.2 ms instead of 12.0 ms).
 // Returns whether this warp stored record or shadow bytes.
-__device__ __forceinline__ bool cc_pass_tiles(const cc_region_dev& r, cc_dev* dev, cc_crc_smem* cs, u32* s_crc_state, cc_pass_smem*,
+__device__ __forceinline__ bool cc_pass_tiles(const cc_region_dev& r, cc_dev* dev, cc_crc_smem* cs, u32* s_crc_state,
                                               const cc_pass_args& a, u32 TP, u64 W0, cc_grid) {
     constexpr int U = 8;
     cc_ws_hdr* h = r.hdr;

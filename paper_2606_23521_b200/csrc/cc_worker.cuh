@@ -99,7 +99,7 @@ __device__ __noinline__ void cc_worker_compact_task(cc_dev* dev, const cc_apply_
 // the classic phases -- the same device code as the host-launched calls.  Out of line, like the recovery-side
 // tasks below: the dispatch loop stays small and every task body gets the register file to itself.
 __device__ __noinline__ void cc_worker_ckpt_task(cc_dev* dev, const cc_region_dev& r, cc_crc_smem* cs, u32* s_crc_ready,
-                                                 cc_pass_smem* s_pass, cc_small_smem* s_small, const cc_task& task, u64 t_start,
+                                                 cc_small_smem* s_small, const cc_task& task, u64 t_start,
                                                  cc_grid g, u32& gen) {
     cc_pass_args a;
     a.epoch = task.epoch; a.kind = task.kind; a.run_pages = 0; a.marks = nullptr; a.consume = 0;
@@ -121,7 +121,7 @@ __device__ __noinline__ void cc_worker_ckpt_task(cc_dev* dev, const cc_region_de
     if (single) {
         if (g.block == 0 && threadIdx.x == 0) r.hdr->t_start_ns = t_start;
         const u32 TP = cc_pass_tile_pages(r, a.run_pages, g.nwarps());
-        cc_pass_tiles(r, dev, cs, s_crc_ready, s_pass, a, TP, W0, g);
+        cc_pass_tiles(r, dev, cs, s_crc_ready, a, TP, W0, g);
         if (g.block == 0 && threadIdx.x == 0) CC_TRACE(dev, 11);
         cc_grid_barrier(dev, g.nblocks, gen);                 // (gpu-scope fences: every block's record bytes are behind block 0 now)
         if (g.block == 0 && threadIdx.x == 0) CC_TRACE(dev, 12);
@@ -153,7 +153,6 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
     cc_crc_smem* cs = reinterpret_cast<cc_crc_smem*>(smem_raw);
     __shared__ __align__(16) cc_task s_task;
     __shared__ cc_batch_tab s_btab;
-    __shared__ cc_pass_smem s_pass;
     __shared__ cc_small_smem s_small;
     __shared__ u32 s_crc_ready;             // the CRC tables are filled once, at kernel start: always "ready"
     if (threadIdx.x == 0) s_crc_ready = 2u;
@@ -254,7 +253,7 @@ cc_worker_kernel(cc_dev* dev, cc_ring_dev ring, cc_apply_tabs tabs) {
             case CC_TASK_MARKED_CKPT:
             case CC_TASK_VERSION_CKPT:
             case CC_TASK_SNAPSHOT:
-                cc_worker_ckpt_task(dev, dev->regions[slot], cs, &s_crc_ready, &s_pass, &s_small, task, t_start, g, gen);
+                cc_worker_ckpt_task(dev, dev->regions[slot], cs, &s_crc_ready, &s_small, task, t_start, g, gen);
                 break;
             case CC_TASK_CKPT_ALL:
                 cc_worker_ckpt_all_task(dev, cs, &s_btab, task, g, gen);

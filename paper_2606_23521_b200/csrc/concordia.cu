@@ -85,7 +85,6 @@ __global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_pass_kernel(cc_dev* d
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cc_crc_smem* cs = reinterpret_cast<cc_crc_smem*>(smem_raw);
     __shared__ u32 s_crc_state, s_warps_left;
-    __shared__ cc_pass_smem s_pass;
     const cc_region_dev& r = rg;
     const cc_grid g = cc_hw_grid();
     if (threadIdx.x == 0) { s_crc_state = 0; s_warps_left = blockDim.x >> 5; }
@@ -103,7 +102,7 @@ __global__ void __launch_bounds__(CC_GATHER_THREADS, 4) cc_pass_kernel(cc_dev* d
         __syncthreads();
 #endif
         const u32 TP = cc_pass_tile_pages(r, a.run_pages, g.nwarps());
-        const bool wrote = cc_pass_tiles(r, dev, cs, &s_crc_state, &s_pass, a, TP, W0, g);
+        const bool wrote = cc_pass_tiles(r, dev, cs, &s_crc_state, a, TP, W0, g);
         if (g.block == 0 && threadIdx.x == 0) CC_TRACE(dev, 11);
         if (cc_pass_leave(r.hdr, &s_warps_left, wrote, g.nblocks, lane)) {
             if (lane == 0) CC_TRACE(dev, 12);
@@ -1304,7 +1303,7 @@ static inline volatile u64* ring_heartbeat(cc_ctx* c) { return c->ring_words + 1
 
 // Worker CTAs: the configured number; CC_WORKER_BLOCKS_ALL = as many as are co-resident; 0 = the default footprint
 // CC_WORKER_BLOCKS_DEFAULT (about a ninth of the SMs: a bandwidth-bound application kernel next to an idle worker of
-// that size keeps ~96 % of its throughput and a 256 MiB checkpoint task takes ~0.26 ms -- profiles/r02_overlap.txt;
+// that size keeps ~96 % of its throughput and a 256 MiB checkpoint task takes ~0.26 ms -- profiles/r02_bench_overlap.txt;
 // the paper runs ONE block = 0.53 % of its SMs, which on B200 moves ~70 GB/s).
 static uint32_t worker_block_count(cc_ctx* ctx, int bps) {
     const uint32_t max = (uint32_t)(bps * ctx->sm_count);
@@ -1494,8 +1493,10 @@ extern "C" int32_t cc_worker_alive(cc_ctx* ctx) {
     if (cudaEventQuery(ctx->worker_done) != cudaErrorNotReady) return 0;    // kernel has left (or failed)
     const u64 hb0 = __atomic_load_n(ctx->ring_words + 16, __ATOMIC_ACQUIRE);
     const u64 t0 = now_ns();
+    const struct timespec nap = {0, 20000};                                   // 20 us: the heartbeat moves every few us
     while (now_ns() - t0 < 1000000000ull) {
         if (__atomic_load_n(ctx->ring_words + 16, __ATOMIC_ACQUIRE) != hb0) return 1;
+        nanosleep(&nap, nullptr);                                             // a dead worker costs a sleeping second, not a spinning core
     }
     return 0;
 }

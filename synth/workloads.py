@@ -12,7 +12,7 @@ import torch
 
 __all__ = [
     "gen", "choose_pages", "raw_region", "mutate_byte_flips", "kv_cache_region", "kv_decode_step",
-    "lora_region", "lora_update", "bf16_normal_region", "sparse_xor_flips", "toggle_flips",
+    "lora_region", "lora_update", "bf16_normal_region", "sparse_xor_flips", "toggle_flips", "all_dirty_flips",
     "RecoveryEpoch", "recovery_epochs", "worker_mutation_pages", "C5A_REGIONS",
 ]
 
@@ -231,3 +231,13 @@ def worker_mutation_pages(task_no: int, n_pages: int, n_mut: int, seed: int):
     A = 2 * ((seed * 7919 + 12345) % 100000) + 1
     h = (seed * 2654435761 + task_no * 40503) & 0xFFFFFFFF
     return [((j * A + h) % n_pages) for j in range(n_mut)], h
+
+
+def all_dirty_flips(n_bytes: int, page_bytes: int, seed: int, device):
+    """Config 4, 100 % dirty leg: one seeded byte flip in EVERY page (n_bytes a multiple of page_bytes).  Returns
+    (offsets int64, masks uint8) for toggle_flips, ascending -- offsets[p] lies in page p."""
+    n_pages = n_bytes // page_bytes
+    g = gen(seed, device)
+    offs = torch.arange(n_pages, device=device) * page_bytes + torch.randint(0, page_bytes, (n_pages,), generator=g, device=device)
+    masks = torch.randint(1, 256, (n_pages,), generator=g, device=device, dtype=torch.int64).to(torch.uint8)
+    return offs, masks

@@ -48,3 +48,21 @@ def check_checkpoint_parity(cur: torch.Tensor, shadow0: torch.Tensor, P: int, re
     assert np.array_equal(shadow.cpu().numpy(), sh_h), "shadow differs"
     assert np.array_equal(cur.cpu().numpy(), cur_h), "live region was modified"
     return ctx, glog, r, olog, nb
+
+
+def verify_all_dirty(cur, log, offs, masks, P, region_id, epoch, chunk=1 << 30, threads=16, log_is_host=False):
+    """Every record of an all-dirty checkpoint (one seeded flip per page: synth.all_dirty_flips) against oracle.checkpoint,
+    1 GiB chunk by chunk (oracle/chunked.py).  cur: the live region AFTER the flips; the shadow the checkpoint started
+    from is cur with the flips undone.  Returns (k, log bytes, D) as the oracle sees them; raises on the first mismatch."""
+    from oracle import chunked
+    N = cur.numel()
+    o_cpu, m_cpu = offs.cpu().numpy(), masks.cpu().numpy()
+
+    def fetch_shadow0(o, n):
+        a = cur[o:o + n].cpu().numpy()
+        lo, hi = (o // P), ((o + n) // P)                          # one flip per page, ascending
+        a[o_cpu[lo:hi] - o] ^= m_cpu[lo:hi]
+        return a
+    fl = (lambda o, n: log[o:o + n].numpy()) if log_is_host else (lambda o, n: log[o:o + n].cpu().numpy())
+    return chunked.verify_checkpoint_chunked(N, P, region_id, epoch, lambda o, n: cur[o:o + n].cpu().numpy(), fetch_shadow0, fl,
+                                             chunk_bytes=chunk, threads=threads)

@@ -15,7 +15,7 @@ import torch
 import oracle
 import synth
 import paper_2606_23521_b200 as cc
-from gpu_util import gpu_checkpoint
+from gpu_util import gpu_checkpoint, verify_all_dirty
 
 pytestmark = pytest.mark.gpu
 
@@ -247,7 +247,6 @@ def test_c4_full_32gib_all_dirty_every_record_against_the_oracle(P):
     and shadow, SURVEY.md 8d fallback ii), every page dirty, at 4 / 16 / 64 KiB pages.  EVERY record of the 32 GiB
     device log -- header, CRC32C, payload -- and the commit record are compared with oracle.checkpoint run on every
     1 GiB chunk of the region (oracle/chunked.py); shadow == region afterwards."""
-    import bench
     _need(100, 60)
     N = 32 << 30
     cur = synth.bf16_normal_region(N, 1004, "cuda")
@@ -256,11 +255,11 @@ def test_c4_full_32gib_all_dirty_every_record_against_the_oracle(P):
     n_pages = N // P
     log = torch.empty(n_pages * (16 + P) + 32, dtype=torch.uint8, device="cuda")
     ctx.log_attach(log)
-    offs, masks = bench.all_dirty_flips(torch, synth, N, P, 1004 + P, "cuda")
+    offs, masks = synth.all_dirty_flips(N, P, 1004 + P, "cuda")
     synth.toggle_flips(cur, offs, masks)
     r = gpu_checkpoint(ctx, 1, 6)
     assert (r.status, r.n_dirty, r.bytes) == (0, n_pages, log.numel())
-    k, nb, D = bench.verify_all_dirty(torch, cc, ctx, 1, cur, log, offs, masks, P, 6, N)
+    k, nb, D = verify_all_dirty(cur, log, offs, masks, P, 1, 6)
     assert (k, nb) == (n_pages, log.numel())
     assert _equal_chunked(shadow, cur)
     r = gpu_checkpoint(ctx, 1, 7)
@@ -268,18 +267,32 @@ def test_c4_full_32gib_all_dirty_every_record_against_the_oracle(P):
     ctx.shutdown()
 
 
-def test_c4_full_64gib_arena_as_8_regions_through_one_pinned_log():
-    """SURVEY.md 8d capacity fallback (i): the 64 GiB arena registered as 8 x 8 GiB regions, every page dirty, each
-    checkpointed into ONE pinned 8.1 GiB host log that the harness verifies against the oracle (every record,
-    chunk-wise) and rewinds between regions."""
-    import bench
-
-    class A:
-        steps = 4
+@pytest.mark.parametrize("P", [4096, 16384, 65536])
+def test_c4_full_64gib_arena_as_8_regions_through_one_pinned_log(P):
+    """SURVEY.md 8d capacity fallback (i), BASELINE.json configs[3] "100 % pages dirty ... sweeping page size over
+    4/16/64 KiB": the 64 GiB arena registered as 8 x 8 GiB regions, every page dirty, each checkpointed into ONE pinned
+    8.0-8.1 GiB host log; every record of every region (16.8 M records in all at 4 KiB pages) is checked against the
+    oracle chunk-wise, the shadows against the regions, and the log is rewound between regions."""
     _need(140, 40)
-    out = bench.c4_full_arena(A, bench.Env(), cc, 65536, verify=True)
-    assert out["parity"].startswith("arena: all 8 x 131072 records"), out
-    assert out["host_link_GBps_log"] > 20.0, out
+    R, regions = 8 << 30, 8
+    arena = synth.bf16_normal_region(regions * R, 1004, "cuda")
+    ctx = cc.Context()
+    shadows = [ctx.register_region(i + 1, arena[i * R:(i + 1) * R], P) for i in range(regions)]
+    n_pages = R // P
+    cap = n_pages * (16 + P) + 32
+    hlog = torch.empty(cap, dtype=torch.uint8, pin_memory=True)
+    committed = torch.zeros(1, dtype=torch.int64, pin_memory=True)
+    ctx.log_attach(hlog, committed)
+    for i in range(regions):
+        v = arena[i * R:(i + 1) * R]
+        offs, masks = synth.all_dirty_flips(R, P, 7000 + i, "cuda")
+        synth.toggle_flips(v, offs, masks)
+        r = gpu_checkpoint(ctx, i + 1, i)
+        assert (r.status, r.n_dirty, r.bytes, int(committed.item())) == (0, n_pages, cap, cap), r.as_dict()
+        kk, nb, D = verify_all_dirty(v, hlog, offs, masks, P, i + 1, i, log_is_host=True)
+        assert (kk, nb) == (n_pages, cap) and _equal_chunked(shadows[i], v)
+        ctx.log_reset()
+    ctx.shutdown()
 
 
 @pytest.mark.parametrize("R", [3, 5])
