@@ -331,3 +331,67 @@ def test_single_pass_run_records_16gib_region_odd_run_length(R):
     assert np.array_equal(glog.cpu().numpy(), olog)
     assert _equal_chunked(shadow, cur)                      # every dirty page refreshed, nothing else touched
     ctx.shutdown()
+
+
+def test_replay_of_a_base_snapshot_larger_than_64gib():
+    """PAPER.md:L227 "replays the latest base snapshot and committed AOF suffix" at config 4's own size: the base
+    snapshot of a 64 GiB region (64 KiB pages, allocator-aware: no shadow) is a 64.016 GiB log -- more than 2^36 bytes,
+    so its commit record lies beyond what the parallel parse's 32-bit candidate offsets reach and the whole log takes
+    the serial parser.  Too large for the host oracle in one piece, so: result fields against the closed form; every
+    header field and every payload byte against the region on the device (exact); the CRC32C of sampled records
+    (first, middle, the first one past 2^36, last) and the commit record against the oracle; then the region is zeroed
+    and replayed from the log and must equal the payloads again; finally one flipped payload byte in the LAST record
+    (past 2^36) must give CC_ERR_CORRUPT with nothing applied (single epoch)."""
+    _need(136, 4)
+    P, N = 65536, 64 << 30
+    n_pages = N // P
+    nbytes = n_pages * (16 + P) + 32
+    assert nbytes > (1 << 36)
+    region = synth.bf16_normal_region(N, 2036, "cuda")
+    ctx = cc.Context()
+    ctx.register_region(9, region, P, no_shadow=True)
+    log = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    ctx.log_attach(log)
+    ctx.apply_attach(n_pages + 64)
+    res = cc.Result()
+    ctx.snapshot_region(9, 41, res)
+    torch.cuda.synchronize()
+    r = res.read()
+    assert (r.status, r.n_dirty, r.bytes, r.log_offset_after, r.epoch) == (0, n_pages, nbytes, nbytes, 41), r.as_dict()
+    recs = log[:n_pages * (16 + P)].view(n_pages, 16 + P)
+    step = 16384                                                    # pages per 1 GiB chunk
+
+    def region_equals_payloads():
+        return all(torch.equal(recs[a:a + step, 16:], region[a * P:(a + step) * P].view(-1, P)) for a in range(0, n_pages, step))
+
+    assert region_equals_payloads()
+    hdr = recs[:, :16].contiguous().view(torch.int32).view(n_pages, 4)
+    assert bool((hdr[:, 0] == 9).all()) and bool((hdr[:, 2] == P).all())
+    assert torch.equal(hdr[:, 1], torch.arange(n_pages, dtype=torch.int32, device="cuda"))
+    past = (1 << 36) // (16 + P) + 1                                # first record that starts beyond 2^36 bytes
+    assert past < n_pages
+    for i in (0, 1, n_pages // 2, past, n_pages - 1):
+        page = region[i * P:(i + 1) * P].cpu().numpy()
+        assert int(hdr[i, 3].item()) & 0xFFFFFFFF == oracle.crc32c(page), i
+    tail = log[nbytes - 32:].cpu().numpy().tobytes()
+    cid, cid2, clen, ccrc, epoch, rid, k = struct.unpack("<IIIIQII", tail)
+    assert (cid, cid2, clen, epoch, rid, k) == (0xFFFFFFFF, 0xFFFFFFFF, 16, 41, 9, n_pages)
+    assert ccrc == oracle.crc32c(np.frombuffer(tail[16:], np.uint8))
+    # replay into the zeroed region
+    region.zero_()
+    res.clear()
+    ctx.apply_log(log, nbytes, res)
+    torch.cuda.synchronize()
+    r = res.read()
+    assert (r.status, r.n_dirty, r.bytes, r.epoch) == (0, n_pages, nbytes, 1), r.as_dict()
+    assert region_equals_payloads()
+    # damage the last record (its bytes lie past 2^36): the only epoch fails its check, nothing is applied
+    region.zero_()
+    log[nbytes - 32 - 100] ^= 0x20
+    res.clear()
+    ctx.apply_log(log, nbytes, res)
+    torch.cuda.synchronize()
+    r = res.read()
+    assert (r.status, r.n_dirty, r.bytes, r.epoch) == (cc.CC_ERR_CORRUPT, 0, 0, 0), r.as_dict()
+    assert not any(bool(region[o:o + (1 << 30)].any()) for o in range(0, N, 1 << 30))
+    ctx.shutdown()
