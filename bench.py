@@ -69,6 +69,7 @@ def parse_args():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-parity", action="store_true", help="skip the untimed oracle comparison (profiling runs)")
     ap.add_argument("--no-extras", action="store_true", help="c2: skip the allocator-aware and ring legs")
+    ap.add_argument("--no-configs", action="store_true", help="c2: skip the short legs of the other configs (c1, c3, c5a, c5b)")
     return ap.parse_args()
 
 
@@ -154,7 +155,11 @@ def measured_peak():
 
 def ncu_traffic(kernel, workload):
     """dram__bytes_read.sum + dram__bytes_write.sum of one launch of `kernel`, read at run time from the newest tracked
-    `ncu --set full` summary of this workload (profiles/rNN_ncu_full[_<workload>].csv).  Returns (bytes or None, source)."""
+    `ncu --set full` summary of this workload (profiles/rNN_ncu_full[_<workload>].csv).  `kernel` may be a tuple of names or
+    name prefixes ending in '*': then the sum over the FIRST launch of every kernel that matches (a call that is several
+    launches; a capture file holds one call).  Returns (bytes or None, source)."""
+    if isinstance(kernel, (tuple, list)):
+        return _ncu_traffic_sum(tuple(kernel), workload)
     pdir = os.path.join(ROOT, "profiles")
     suffix = "" if workload == "c2" else "_" + workload.replace("-", "_")
     try:
@@ -177,10 +182,39 @@ def ncu_traffic(kernel, workload):
     return None, "no tracked ncu --set full capture of %s on this workload" % kernel
 
 
-def roofline(kernel, algo_bytes, ms, workload):
+def _ncu_traffic_sum(patterns, workload):
+    pdir = os.path.join(ROOT, "profiles")
+    suffix = "" if workload == "c2" else "_" + workload.replace("-", "_")
+    try:
+        names = sorted(f for f in os.listdir(pdir) if f.endswith("_ncu_full%s.csv" % suffix) and f[0] == "r" and f[1:3].isdigit())
+    except OSError:
+        names = []
+    hit = lambda k: any(k == p or (p.endswith("*") and k.startswith(p[:-1])) for p in patterns)
+    for name in reversed(names):
+        try:
+            seen, tot = [], 0.0
+            with open(os.path.join(pdir, name), newline="") as fh:
+                for row in csv.DictReader(fh):
+                    k = row.get("Kernel Name", "").split("(")[0].strip()
+                    if not hit(k) or k in seen:
+                        continue
+                    seen.append(k)
+                    for col, val in row.items():
+                        if col.startswith("dram__bytes_read.sum") or col.startswith("dram__bytes_write.sum"):
+                            unit = col[col.index("[") + 1:col.index("]")].lower()
+                            tot += float(val) * {"byte": 1.0, "kbyte": 1e3, "mbyte": 1e6, "gbyte": 1e9, "tbyte": 1e12}[unit]
+            if seen:
+                return int(round(tot)), "profiles/%s (ncu --set full, one launch each of %s)" % (name, ", ".join(seen))
+        except Exception:
+            continue
+    return None, "no tracked ncu --set full capture of %s on this workload" % (patterns,)
+
+
+def roofline(kernel, algo_bytes, ms, workload, kernels=None):
+    """kernel: the name reported; kernels: the launches whose DRAM traffic is summed (default: `kernel` itself)."""
     peak, peak_src = measured_peak()
     ach = algo_bytes / (ms * 1e-3) / 1e9
-    traffic, tsrc = ncu_traffic(kernel, workload)
+    traffic, tsrc = ncu_traffic(kernels if kernels is not None else kernel, workload)
     return {"bound": "hbm", "kernel": kernel, "achieved": round(ach, 1), "peak": peak, "unit": "GB/s",
             "frac": round(ach / peak, 4), "frac_of_8000": round(ach / 8000, 4), "traffic": traffic, "traffic_source": tsrc,
             "peak_source": peak_src, "algorithmic_bytes_per_launch": int(algo_bytes), "avg_launch_ms": round(ms, 4)}
@@ -233,6 +267,15 @@ class Env:
         if self.dist is not None:
             self.dist.barrier()
             self.dist.destroy_process_group()
+
+
+def emit(args, line):
+    """Print the workload's JSON line -- or hand it to the caller that runs this workload as a short leg of another line."""
+    sink = getattr(args, "collect", None)
+    if sink is not None:
+        sink.append(line)
+    else:
+        print(json.dumps(line), flush=True)
 
 
 def base_line(env, K, Wm, value, ms_per_step, workload_desc, extra_cfg, dtype):
@@ -658,11 +701,47 @@ def run_c2(args, env):
                            "other_paths_ms_per_step": {k2: round(v / K, 4) for k2, v in e2e["extras"].items()},
                            "other_paths": "the record writer storing straight into the pinned host log (SM stores cap at 52.7 GB/s): "
                                           "fused single pass / three kernels"}
+        if args.workload == "c2" and world == 1 and not args.no_extras and not args.no_configs:
+            ctx.shutdown()                                           # (idempotent; the legs make their own contexts)
+            torch.cuda.empty_cache()
+            line["configs"] = short_config_legs(args, env)
         if not args.no_cpu_baseline:
             torch.cuda.empty_cache()
             line["cpu_baseline"] = oracle_leg(args.workload, args)
         print(json.dumps(line), flush=True)
     ctx.shutdown()
+
+
+def short_config_legs(args, env):
+    """BASELINE.json's other single-GPU configs as SHORT legs of the default line, so that the driver's record of
+    `python bench.py` carries a number and a parity flag for each (the full lines: --workload c1|c3|c5a|c5b).  Same code
+    as those workloads, fewer steps / tasks, no CPU baseline, no end-to-end leg."""
+    import argparse
+    legs = {}
+    for name, fn, over in (("c1", lambda a: small_region_workload(a, env, "c1"), {"steps": 10}),
+                           ("c3", lambda a: small_region_workload(a, env, "c3"), {"steps": 10}),
+                           ("c5a", lambda a: run_c5a(a, env), {"steps": 5}),
+                           ("c5b", lambda a: run_c5b(a, env), {"tasks": 1000})):
+        sub = argparse.Namespace(**vars(args))
+        sub.workload, sub.warmup, sub.no_cpu_baseline, sub.no_e2e, sub.collect = name, 3, True, True, []
+        for k2, v in over.items():
+            setattr(sub, k2, v)
+        t0 = time.perf_counter()
+        try:
+            fn(sub)
+            ln = sub.collect[0]
+            rf = ln.get("roofline", {})
+            legs[name] = {"workload": ln["config"]["workload"], "metric": ln["metric"], "value": ln["value"], "unit": ln["unit"],
+                          "ms_per_step": ln["ms_per_step"], "steps": ln["steps"], "parity": ln.get("parity"),
+                          "roofline": {k2: rf.get(k2) for k2 in ("kernel", "achieved", "peak", "frac", "traffic", "algorithmic_bytes_per_launch")},
+                          "gpu_launches": ln.get("gpu_launches"), "leg_wall_s": round(time.perf_counter() - t0, 1)}
+            if name == "c5b":
+                legs[name]["checkpoint_task_device_us"] = {m: v["device_us"] for m, v in ln["checkpoint_task"].items()}
+                legs[name]["nop_round_trip_us"] = ln["trigger_latency"]["nop_round_trip_us"]
+        except Exception as e:                                       # a failed leg must not take the headline line with it
+            legs[name] = {"error": "%s: %s" % (type(e).__name__, e), "leg_wall_s": round(time.perf_counter() - t0, 1)}
+        env.torch.cuda.empty_cache()
+    return legs
 
 
 def ring_on_region(cc, env, cur, shadow, P, k_exp, log_bytes, mutate, blocks_list=(1, 8, 32, 148), tasks=6):
@@ -860,7 +939,8 @@ def small_region_workload(args, env, name):
                              "issued_to_idle_gpu_with_events_between_kernels": {
                                  "total": round(statistics.mean(tot_p), 4), "discovery": round(statistics.mean(disc), 4),
                                  "writer": round(statistics.mean(wr), 4)}}
-        line["roofline"] = roofline("cc_checkpoint_delta (whole call: launch- and latency-bound at this size)", algo, ms, args.workload)
+        line["roofline"] = roofline("cc_checkpoint_delta (whole call: launch- and latency-bound at this size)", algo, ms, name,
+                                    kernels=("cc_scan_kernel", "cc_small_tail_kernel"))
         line["roofline"]["note"] = "64 MiB regions are launch/latency-bound, not HBM-bound; HBM-fraction claims are made on c2 / c4"
         if e2e:
             line["e2e"] = {"value": round(env.world * N / (e2e["ms"] * 1e-3) / 1e9, 2), "unit": UNIT, "h2d_bytes_per_step": e2e["h2d"],
@@ -869,7 +949,7 @@ def small_region_workload(args, env, name):
                                    "new bytes, launch, synchronize and reading the result"}
         if not args.no_cpu_baseline:
             line["cpu_baseline"] = oracle_leg(name, args)
-        print(json.dumps(line), flush=True)
+        emit(args, line)
     ctx.shutdown()
 
 
@@ -1229,7 +1309,7 @@ def run_c5a(args, env):
         t_pin2 = timed(log_pin, 3, 1)
         e2e = (statistics.mean(t_pin), statistics.mean(t_pin2))
     if env.rank == 0:
-        algo = 4 * W                                                 # validate reads the log, scatter reads it again and writes live + shadow
+        algo = 3 * W                                                 # the method's own bytes: the log read once, live page + shadow written
         line = base_line(env, K, Wm, env.world * W / (ms * 1e-3) / 1e9, ms,
                          "BASELINE.json configs[4], recovery half: replay of a committed log of %d page records in 100 epochs (mixed 4 / 16 / 64 KiB "
                          "pages, %d bytes, written by the oracle's record writer) into an 8 GiB arena registered as three regions; log in "
@@ -1243,8 +1323,10 @@ def run_c5a(args, env):
         line["clocks"] = clocks
         line["parity"] = parity
         line["phases_ms"] = {"apply_total": round(ms, 4), "best": round(min(t_dev), 4), "records_per_s": round(n_rec / (ms * 1e-3))}
-        line["roofline"] = roofline("cc_apply_* (whole replay: parse + validate + scatter)", algo, ms, args.workload)
-        line["roofline"]["note"] = "algorithmic bytes = 4 x log bytes: the log is read by the validation and by the scatter, every payload byte is written to the live page and to the shadow"
+        line["roofline"] = roofline("cc_apply_* (whole replay: parse + validate + scatter)", algo, ms, "c5a", kernels=("cc_apply_*",))
+        line["roofline"]["note"] = ("algorithmic bytes = 3 x log bytes (SURVEY.md 8d: the method reads the log once and writes every payload byte to the "
+                                    "live page and to the shadow); the implementation reads the log three times (candidate search, validation, "
+                                    "scatter) -- that shows in `traffic`, not here")
         if e2e:
             line["e2e"] = {"value": round(env.world * W / (e2e[0] * 1e-3) / 1e9, 2), "unit": UNIT, "h2d_bytes_per_step": W,
                            "d2h_bytes_per_step": 64, "ms_per_step": round(e2e[0], 4),
@@ -1253,7 +1335,7 @@ def run_c5a(args, env):
                            "ms_without_stage_buffer": round(e2e[1], 4)}
         if not args.no_cpu_baseline:
             line["cpu_baseline"] = oracle_leg("c5a", args)
-        print(json.dumps(line), flush=True)
+        emit(args, line)
     ctx.shutdown()
 
 
@@ -1390,14 +1472,16 @@ def run_c5b(args, env):
                                                     "round trip ~80 us for a trivial op (L307)"}
         line["checkpoint_task"] = out
         line["worker_footprint"] = footprint
-        line["roofline"] = roofline("cc_worker_kernel (one %s checkpoint task)" % best, 2 * N + 3 * n_mut * P, ms, args.workload)
+        line["roofline"] = roofline("cc_worker_kernel (one %s checkpoint task)" % best, 2 * N + 3 * n_mut * P, ms, "c5b", kernels=("cc_pass_kernel",))
+        line["roofline"]["traffic_note"] = ("traffic is that of the host-launched equivalent of the fused task (cc_pass_kernel on the same region and "
+                                            "pinned log): a never-ending worker kernel cannot be profiled launch by launch")
         line["e2e"] = {"value": round(N / (out[best]["round_trip_us"]["p50"] * 1e-6) / 1e9, 2), "unit": UNIT,
                        "h2d_bytes_per_step": 64, "d2h_bytes_per_step": per + 64, "ms_per_step": round(out[best]["round_trip_us"]["p50"] / 1e3, 4),
                        "path": "host clock around cc_submit + cc_wait (p50): the 64-byte descriptor crosses the host link, the records go "
                                "straight into the pinned host log, the 64-byte completion record is read on the host"}
         if not args.no_cpu_baseline:
             line["cpu_baseline"] = oracle_leg("c5b", args)
-        print(json.dumps(line), flush=True)
+        emit(args, line)
 
 
 # -------------------------------------------------------------------- overlap --
@@ -1440,7 +1524,7 @@ def run_overlap(args, env):
         ctx.log_attach(log)
         stream.synchronize()
         ctx.worker_start()
-        row = {"worker_blocks": B, "sm_share_pct": round(100.0 * B / 148, 2)}
+        row = {"worker_blocks": B, "sm_share_pct": ctx.worker_footprint()["sm_share_pct"]}
         print("overlap: worker_blocks", B, file=sys.stderr, flush=True)
         try:
             row["copy_alone_GBps"] = round(copy_gbps(), 1)

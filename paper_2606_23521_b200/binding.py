@@ -448,8 +448,11 @@ class Context:
         v = [ctypes.c_uint32() for _ in range(5)]
         self._check("cc_worker_footprint", self.lib.cc_worker_footprint(self.h, *[ctypes.byref(x) for x in v]))
         b, t, sm, rg, sms = [x.value for x in v]
+        # CTAs of this shape one SM holds (B200: 64 Ki registers, 2,048 threads, 227 KiB of shared memory + 1 KiB reserved per CTA);
+        # the worker's share of the GPU = its CTAs / the CTA slots of the whole device
+        fit = max(1, min(65536 // max(1, rg * t), 2048 // max(1, t), (227 * 1024) // (sm + 1024)))
         return {"blocks": b, "threads_per_block": t, "smem_bytes_per_block": sm, "registers_per_thread": rg, "sm_count": sms,
-                "sm_share_pct": round(100.0 * min(b, sms) / sms, 2)}
+                "blocks_that_fit_per_sm": fit, "sm_share_pct": round(100.0 * min(b, sms * fit) / (sms * fit), 2)}
 
     def peek_queue(self):
         h, t = ctypes.c_uint64(), ctypes.c_uint64()
