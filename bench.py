@@ -1618,8 +1618,23 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def respawn_under_torchrun(a):
+    """`python bench.py --gpus N` with N > 1 and no torchrun environment: start the N ranks ourselves, exactly as the
+    driver would (one process per GPU, rendezvous on 127.0.0.1), and hand back their exit code.  Rank 0 prints the line."""
+    import socket
+    import subprocess
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(a.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
 def main():
     a = parse_args()
+    if a.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(respawn_under_torchrun(a))
     if a.impl == "reference":
         return run_reference(a)
     env = Env()

@@ -67,3 +67,23 @@ def test_two_ranks_shard_without_exchange():
         assert res[r]["max_ms"] == 20.0
         assert res[r]["val"] == pytest.approx(2 * n / 20e-3)
         assert res[r]["mismatch"] is True
+
+
+def test_bench_gpus_2_spawns_its_own_ranks_reference_arm():
+    """`python bench.py --impl reference --gpus 2` with no torchrun environment re-executes itself under
+    torch.distributed.run (two processes, rendezvous on 127.0.0.1): rank 0 alone times the oracle and prints ONE JSON
+    line with n_gpus = 2, rank 1 exits 0 without work.  Runs on CPU (the reference arm is the oracle)."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    p = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--impl", "reference", "--gpus", "2",
+                        "--workload", "c2-small", "--steps", "1", "--warmup", "0"],
+                       cwd=root, env=env, capture_output=True, text=True, timeout=600)
+    assert p.returncode == 0, p.stderr[-2000:]
+    lines = [ln for ln in p.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, p.stdout
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["gpu_launches"] == 0
+    assert d["value"] > 0 and d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
