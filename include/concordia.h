@@ -374,6 +374,12 @@ int32_t cc_apply_attach(cc_ctx* ctx, void* scratch, uint64_t scratch_bytes);
  * read the device copy; results are identical.  Logs that do not fit, device-resident logs and the worker's
  * RESTORE / COMPACT_LOG tasks are unaffected.  Only while the worker is stopped. */
 int32_t cc_apply_stage_attach(cc_ctx* ctx, void* device_buf, uint64_t bytes);
+/* How often the staging buffer was used since cc_init: *staged = host-resident logs that were copied into it,
+ * *bypassed = host-resident logs that were read in place ALTHOUGH a buffer is attached, because they are larger than it
+ * or the copy could not be queued.  A bypassed replay is correct but crosses the host link three times instead of once
+ * (C5a: 16.9 ms instead of 5.5 ms) -- a caller that sees the second counter move should attach a larger buffer.
+ * Either pointer may be NULL. */
+int32_t cc_apply_stage_stats(cc_ctx* ctx, uint64_t* staged, uint64_t* bypassed);
 
 /* Recovery applier: parse log[0, nbytes) (device or pinned host,
  * 16-byte aligned), validate structure and CRC32C of every record, and for every committed epoch

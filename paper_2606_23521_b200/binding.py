@@ -55,7 +55,7 @@ EXPORTS = [
     "cc_init", "cc_shutdown", "cc_last_cuda_error", "cc_kernel_launches", "cc_workspace_bytes",
     "cc_register_region", "cc_unregister_region", "cc_log_attach", "cc_log_reset", "cc_log_reset_async", "cc_log_mirror_attach", "cc_log_drain", "cc_log_drain_start", "cc_log_drain_wait", "cc_log_drain_stop",
     "cc_checkpoint_ex", "cc_checkpoint_delta", "cc_checkpoint_delta_fused", "cc_checkpoint_delta_rle", "cc_checkpoint_marked", "cc_checkpoint_versions",
-    "cc_checkpoint_all", "cc_checkpoint_all_rle", "cc_snapshot_region", "cc_compact_log", "cc_scan_only", "cc_trace_events", "cc_dirty_list", "cc_apply_scratch_bytes", "cc_apply_attach", "cc_apply_stage_attach", "cc_apply_log",
+    "cc_checkpoint_all", "cc_checkpoint_all_rle", "cc_snapshot_region", "cc_compact_log", "cc_scan_only", "cc_trace_events", "cc_dirty_list", "cc_apply_scratch_bytes", "cc_apply_attach", "cc_apply_stage_attach", "cc_apply_stage_stats", "cc_apply_log",
     "cc_worker_start", "cc_worker_stop", "cc_worker_alive", "cc_worker_footprint", "cc_peek_queue", "cc_submit", "cc_measure_submit_cost", "cc_measure_launch_cost", "cc_poll", "cc_wait",
     "cc_dirty_pages_static",
 ]
@@ -145,6 +145,7 @@ def load_library():
         "cc_apply_scratch_bytes": (u64, [u64]),
         "cc_apply_attach": (i32, [vp, vp, u64]),
         "cc_apply_stage_attach": (i32, [vp, vp, u64]),
+        "cc_apply_stage_stats": (i32, [vp, P(u64), P(u64)]),
         "cc_apply_log": (i32, [vp, vp, u64, vp, vp]),
         "cc_worker_start": (i32, [vp]),
         "cc_worker_stop": (i32, [vp]),
@@ -425,6 +426,12 @@ class Context:
         off = (-s.data_ptr()) % 16
         self._check("cc_apply_stage_attach", self.lib.cc_apply_stage_attach(self.h, s.data_ptr() + off, nbytes))
         self._stage = s
+
+    def apply_stage_stats(self):
+        """(staged, bypassed): host-resident logs copied into the staging buffer / read in place although one is attached."""
+        a, b = ctypes.c_uint64(), ctypes.c_uint64()
+        self._check("cc_apply_stage_stats", self.lib.cc_apply_stage_stats(self.h, ctypes.byref(a), ctypes.byref(b)))
+        return a.value, b.value
 
     def apply_log(self, log: torch.Tensor, nbytes: int, result: Result = None, stream=None):
         assert log.dtype == torch.uint8 and log.is_contiguous() and (log.is_cuda or log.is_pinned())

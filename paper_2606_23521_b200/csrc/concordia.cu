@@ -318,6 +318,7 @@ struct cc_ctx {
     bool apply_attached;
     void* stage;                // optional device staging buffer for host-resident logs (cc_apply_stage_attach)
     uint64_t stage_bytes;
+    uint64_t stage_used = 0, stage_bypassed = 0;   // host-resident logs copied into the staging buffer / read in place although one is attached
     int last_cuda;
     uint64_t launches;
     int scan_bps, gather_bps, validate_bps, fused_bps, small_bps, cand_bps;     // blocks per SM from the occupancy API
@@ -1265,12 +1266,27 @@ extern "C" int32_t cc_apply_stage_attach(cc_ctx* ctx, void* device_buf, uint64_t
 // A host-resident log is read twice by the kernels (validate, then scatter / copy): with a staging buffer
 // attached it crosses the host link once, by the copy engine, and the kernels read the device copy.
 static const u8* stage_log(cc_ctx* ctx, const void* log, uint64_t nbytes, cudaStream_t st) {
-    if (!ctx->stage || nbytes == 0 || nbytes > ctx->stage_bytes) return (const u8*)log;
+    if (!ctx->stage || nbytes == 0) return (const u8*)log;
     cudaPointerAttributes at;
     if (cudaPointerGetAttributes(&at, log) != cudaSuccess) { cudaGetLastError(); return (const u8*)log; }
     if (at.type != cudaMemoryTypeHost) return (const u8*)log;
-    if (cudaMemcpyAsync(ctx->stage, log, nbytes, cudaMemcpyHostToDevice, st) != cudaSuccess) { cudaGetLastError(); return (const u8*)log; }
+    // a host-resident log with a staging buffer attached: from here on every way out is counted (cc_apply_stage_stats),
+    // because reading the log in place costs three passes over the host link instead of one
+    if (nbytes > ctx->stage_bytes ||
+        cudaMemcpyAsync(ctx->stage, log, nbytes, cudaMemcpyHostToDevice, st) != cudaSuccess) {
+        cudaGetLastError();
+        ctx->stage_bypassed += 1;
+        return (const u8*)log;
+    }
+    ctx->stage_used += 1;
     return (const u8*)ctx->stage;
+}
+
+extern "C" int32_t cc_apply_stage_stats(cc_ctx* ctx, uint64_t* staged, uint64_t* bypassed) {
+    if (!ctx) return CC_ERR_INVALID;
+    if (staged) *staged = ctx->stage_used;
+    if (bypassed) *bypassed = ctx->stage_bypassed;
+    return CC_OK;
 }
 
 extern "C" int32_t cc_apply_log(cc_ctx* ctx, const void* log, uint64_t nbytes, void* stream, cc_result* out) {

@@ -152,6 +152,15 @@ def test_config5a_scaled_mixed_pages_duplicates(pinned=False):
         assert np.array_equal(work.cpu().numpy(), host)
         for rid, (o, sz, P) in views.items():
             assert np.array_equal(shadows[rid].cpu().numpy(), host[o:o + sz])
+        # the staging buffer's use is visible: only a host-resident log with a buffer attached counts
+        assert ctx.apply_stage_stats() == ((1, 0) if pinned and staged else (0, 0))
+        if pinned and staged:
+            ctx.apply_stage_attach(W - 16)     # one unit too small: the log is read in place -- correct, and counted
+            work.copy_(arena)
+            r = _gpu_apply(ctx, lt, W)
+            assert (r.status, r.n_dirty, r.bytes) == (0, exp[1], W) and np.array_equal(work.cpu().numpy(), host)
+            assert ctx.apply_stage_stats() == (1, 1)
+        ctx.shutdown()
 
 
 def test_scratch_too_small_applies_nothing():
