@@ -457,7 +457,13 @@ int32_t cc_dirty_pages_static(int32_t device, const void* cur, const void* shado
 /* ============================ BENCH / TEST HOOKS -- not part of the product API ============================
  * Measurement and test instrumentation used by bench.py and tests/ only.  They change no result.  Compiled in by
  * default; build with -DCC_BENCH_HOOKS=0 for a library without them (the worker then answers CC_TASK_TEST_MUTATE
- * with CC_ERR_INVALID). */
+ * with CC_ERR_INVALID).
+ * Why the default is ON: the repository builds ONE libconcordia.so and the numbers and parity results it publishes must
+ * come from that very binary -- a second, hook-less build would be a library nobody measured.  What the hooks add for a
+ * ring client is CC_TASK_TEST_MUTATE, which can flip bytes only inside a region the same process registered through
+ * the same context (a ring client already has every pointer).  A deployment that wants them gone sets
+ * CC_NVCC_FLAGS=-DCC_BENCH_HOOKS=0 for paper_2606_23521_b200/build.py (bench.py's c5b workload and the worker tests that
+ * mutate a region from inside the ring need the hooks and do not run against such a build). */
 #ifndef CC_BENCH_HOOKS
 #define CC_BENCH_HOOKS 1
 #endif
